@@ -1,0 +1,199 @@
+/*
+ * pp.h -- C ABI of the B200-native photon propagator ("pp"), the GPU photon-propagation stage of
+ * arXiv:2405.05700 plus the server-side batching that feeds it.
+ *
+ * What the paper fixes (PAPER.md = /root/reference/PAPER.md):
+ *   - light sources: "These losses in the detector volume are then used as light sources for the
+ *     photon propagator" (section 2);
+ *   - medium: "The optical properties of the ice are divided into vertical layers of 10 m thickness
+ *     having different coefficients of scattering and absorption";
+ *   - photon loop: "calculate the distance to the next scatter for each photon and then picking a new
+ *     angle based on the physics of scattering. This process is then repeated until the photon
+ *     intersects a detector or is absorbed";
+ *   - batching: "When the step queue is sufficiently full, a block of steps is sent to the propagation
+ *     server for processing as a batch. The server aggregates steps from multiple events and clients
+ *     in order to keep the GPU as busy as possible" (section 4);
+ *   - hit record: "only stores the ID of the particle that produced it, the time of the hit, and the
+ *     weight";
+ *   - many producers, one server: "multiple instances of IceTray ... sharing a single photon propagator
+ *     server".
+ * Everything the paper leaves open is fixed by the readings R-1..R-14 in DESIGN.md section 3.
+ *
+ * Conventions: metres, nanoseconds, GeV; z up.  All pointers are HOST pointers unless the parameter
+ * name starts with d_ (DEVICE pointer).  The caller owns every pointer it passes; the library copies
+ * what it needs before the call returns unless stated otherwise.  Every call returns PP_OK (0) or a
+ * negative pp_status; no exceptions cross the boundary; after PP_E_CUDA the handle is poisoned (every
+ * later call returns PP_E_CUDA) and pp_last_error() gives the CUDA message.  There is no CPU fallback:
+ * without a CUDA device pp_create fails with PP_E_CUDA.
+ */
+#ifndef PP_H_
+#define PP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum pp_status {
+  PP_OK = 0,
+  PP_E_INVAL = -1,       /* bad argument (NULL, NaN, non-unit direction, non-positive length, ...) */
+  PP_E_NOMEM = -2,       /* workspace too small / allocation failed */
+  PP_E_CUDA = -3,        /* CUDA error (sticky) */
+  PP_E_OVERFLOW = -4,    /* a per-source photon count does not fit 32 bits */
+  PP_E_WOULDBLOCK = -5,  /* non-blocking call could not make progress */
+  PP_E_UNSUPPORTED = -6, /* geometry the fast DOM lookup cannot represent (see pp_geometry) */
+  PP_E_STATE = -7        /* call not valid in this state (e.g. submit after shutdown) */
+} pp_status;
+
+/* A light source ("photon emitting step"): a point cascade that emits
+ * N = floor(double(energy_GeV) * double(photons_per_GeV) + 0.5) photons at (x,y,z), time t_ns, on the
+ * Cherenkov cone about the unit axis (dx,dy,dz) (R-4, R-12b).  32 bytes. */
+typedef struct pp_source {
+  float x, y, z;
+  float dx, dy, dz;
+  float t_ns;
+  float energy_GeV;
+} pp_source;
+
+/* A hit (producing particle, time, weight).  The producing photon is identified by the
+ * Philox counter triple (event_id, source_id, photon_idx), which lets any hit be replayed in isolation;
+ * a single 32-bit photon id would overflow for one C4-size event (5e9 photons).  32 bytes. */
+typedef struct pp_hit {
+  uint32_t event_id;
+  uint32_t source_id;
+  uint32_t photon_idx; /* index of the photon within its source, 0 <= photon_idx < N */
+  uint32_t dom_id;     /* row index into pp_geometry.xyz */
+  double time_ns;      /* source time + path / group velocity */
+  float weight;        /* 1.0 (acceptance == 1, R-4b) */
+  uint32_t n_scatter;  /* number of scatters before the hit (diagnostic; 0 = direct light) */
+} pp_hit;
+
+/* Detector geometry: n_dom spheres of one radius.  dom_id = row index.  The fast lookup needs DOMs
+ * that sit on vertical lines (equal x,y) with a uniform z pitch per line (R-11); anything else makes
+ * pp_create return PP_E_UNSUPPORTED unless PP_FLAG_BRUTE_FORCE_DOMS is set. */
+typedef struct pp_geometry {
+  uint32_t n_dom;
+  const float* xyz; /* [n_dom][3] */
+  float radius;     /* metres, > 0 */
+} pp_geometry;
+
+/* Layered ice.  Layer i spans z in (z_top-(i+1)*dz, z_top-i*dz]; layer 0 extends to
+ * +infinity and layer n_layers-1 to -infinity (R-6).  Lengths in metres; scat_len is the geometric
+ * mean free path between scatters (R-7). */
+typedef struct pp_ice {
+  uint32_t n_layers;     /* 1..PP_MAX_LAYERS */
+  float z_top;
+  float dz;
+  const float* abs_len;  /* [n_layers] > 0 */
+  const float* scat_len; /* [n_layers] > 0 */
+  float g;               /* Henyey-Greenstein asymmetry, |g| < 1 (R-1) */
+  float n_group;         /* group index; photon speed = c / n_group */
+  float cos_cherenkov;   /* cosine of the emission cone half-angle, in [-1, 1] */
+  float photons_per_GeV; /* light yield */
+} pp_ice;
+
+#define PP_MAX_LAYERS 1024u
+
+/* pp_config.flags */
+#define PP_FLAG_BRUTE_FORCE_DOMS 1u /* test every DOM on every flight (validation; any geometry) */
+#define PP_FLAG_NONBLOCKING_SUBMIT 2u /* pp_submit enqueues all n sources or none: PP_E_WOULDBLOCK if the ring lacks space */
+
+/* Sizes and resources.  Zero means "default".  device_workspace / pinned_workspace / streams may be
+ * NULL: the library then allocates them itself (cudaMalloc / cudaHostAlloc / cudaStreamCreate) and
+ * frees them in pp_destroy.  When given (PyTorch supplies them in the Python binding), they stay
+ * owned by the caller and must outlive the handle; pp_workspace_size() says how big they must be. */
+typedef struct pp_config {
+  uint64_t seed;                  /* Philox key (R-3) */
+  uint64_t launch_photons_target; /* photons per GPU launch the server aims for (default 1e8) */
+  uint64_t hit_ring_bytes;        /* total device bytes for the two bounded hit rings (default 256 MiB) */
+  uint64_t source_ring_bytes;     /* pinned host bytes for the source ring (default 64 MiB) */
+  void* device_workspace;
+  uint64_t device_workspace_bytes;
+  void* pinned_workspace;
+  uint64_t pinned_workspace_bytes;
+  void* stream0; /* cudaStream_t */
+  void* stream1; /* cudaStream_t */
+  uint32_t flags;
+  uint32_t max_flights; /* safety cap on flights per photon (default 100000, R-10) */
+  int32_t device;       /* CUDA device ordinal (default: current device) */
+  uint32_t reserved;
+} pp_config;
+
+typedef struct pp_stats_t {
+  uint64_t sources_submitted;
+  uint64_t photons_submitted;
+  uint64_t photons_done;    /* = absorbed + hit + aborted once drained */
+  uint64_t photons_absorbed;
+  uint64_t photons_hit;
+  uint64_t photons_aborted; /* reached max_flights; must be 0 */
+  uint64_t flights;         /* scattering steps (free flights) simulated */
+  uint64_t launches;        /* propagation-kernel launches */
+  uint64_t relaunches;      /* extra launches forced by a full hit ring */
+  uint64_t hits_collected;
+  double kernel_busy_ms;    /* union of the propagation kernels' device intervals (CUDA events) */
+  double wall_ms;           /* first pp_submit .. last drain */
+  uint64_t source_ring_high_water; /* bytes */
+  uint64_t hit_ring_high_water;    /* bytes */
+} pp_stats_t;
+
+typedef struct pp_handle pp_handle;
+
+/* Required workspace sizes for a configuration (cfg may have NULL workspaces). */
+int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, uint64_t* device_bytes,
+                      uint64_t* pinned_bytes);
+
+/* Builds the DOM lookup and ice tables, uploads them, starts the batching server thread. */
+int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, pp_handle** out);
+
+/* Enqueues n light sources ("a block of steps").  event_ids[n] required; source_ids may be
+ * NULL, in which case source i of this call gets id i.  Thread-safe: any number of threads may submit
+ * concurrently.  Copies before returning.  Blocks while the source ring is full unless
+ * PP_FLAG_NONBLOCKING_SUBMIT.  Sources with N == 0 photons are accepted and ignored. */
+int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids, const uint32_t* source_ids,
+              size_t n);
+
+/* Asks the server to launch whatever is queued even if it is less than launch_photons_target. */
+int pp_flush(pp_handle* h);
+
+/* Copies up to cap finished hits into out (unspecified order; hits of one event may span calls).
+ * block != 0: waits until at least one hit is available or everything submitted so far has been
+ * propagated and handed out.  *n_out == 0 with PP_OK then means "drained".  One collector at a time. */
+int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block);
+
+int pp_stats(pp_handle* h, pp_stats_t* out);
+const char* pp_last_error(pp_handle* h);
+void pp_destroy(pp_handle* h);
+
+/* ---- device-resident path (what bench.py times as `value`, and what the parity tests drive) ----
+ * Inputs already in HBM: d_sources[n] (pp_source), d_event_ids[n], d_source_ids[n] (nullable: index)
+ * are DEVICE pointers.  Runs source expansion + propagation for ALL photons of the n sources in
+ * launches of at most launch_photons_target photons, alternating between the two streams,
+ * synchronously; hits go through the bounded device hit ring to the pp_collect queue.  Needs an
+ * idle server (PP_E_STATE otherwise) and n <= source ring capacity (PP_E_NOMEM otherwise).
+ * d_fates, if not NULL, is a DEVICE array with one pp_fate per photon of the batch, indexed by
+ * the batch-global photon number (sources in order, photons in order): validation only.
+ * device_ms_out: device time from the start of expansion to the last status read-back (CUDA events). */
+typedef struct pp_fate {
+  float x, y, z;       /* end point */
+  float path_m;        /* total geometric path */
+  double time_ns;      /* end time */
+  uint32_t n_flights;
+  int32_t dom;         /* hit DOM or -1 */
+  uint32_t fate;       /* 0 absorbed, 1 hit, 2 aborted */
+  uint32_t photon_idx;
+} pp_fate;
+
+int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_event_ids,
+                    const uint32_t* d_source_ids, size_t n, pp_fate* d_fates, uint64_t* photons_out,
+                    double* device_ms_out);
+
+/* Library version and the number of CUDA kernels this library launched so far in this process. */
+const char* pp_version(void);
+uint64_t pp_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PP_H_ */

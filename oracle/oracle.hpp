@@ -285,8 +285,8 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
   const Real two_pi = Real(6.283185307179586476925286766559);
   Real p[3] = {Real(src[0]), Real(src[1]), Real(src[2])};
   Real d[3] = {Real(src[3]), Real(src[4]), Real(src[5])};  // source axis; rotated below (step 2)
-  Real t = Real(src[6]);
-  Real path = 0;
+  double t = double(src[6]);  // time and path are kept in fp64 even in the fp32 diagnostic instantiation
+  double path = 0;
   Real tau_a = 0;
   PhotonResult r{};
   r.dom = -1;
@@ -318,16 +318,16 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
     const int dom = idx ? intersect_lines(geo, *idx, p, d, s, &t_hit) : intersect_brute(geo, p, d, s, &t_hit);
     if (dom >= 0) {
       for (int a = 0; a < 3; ++a) p[a] += d[a] * t_hit;
-      path += t_hit;
-      t += t_hit / v;
+      path += double(t_hit);
+      t += double(t_hit) / double(v);
       r.fate = kHit; r.dom = dom;
       break;
     }
     // step 8: advance
     tau_a -= depth(ice, ice.abs_len, p[2], d[2], s);
     for (int a = 0; a < 3; ++a) p[a] += d[a] * s;
-    path += s;
-    t += s / v;
+    path += double(s);
+    t += double(s) / double(v);
     if (absorbed) { r.fate = kAbsorbed; break; }
   }
   r.x = double(p[0]); r.y = double(p[1]); r.z = double(p[2]);

@@ -1,0 +1,290 @@
+"""Thin ctypes binding of the C ABI in ``include/pp.h`` (argument marshalling only).
+
+PyTorch is used for exactly three things here: device memory (the workspace and the resident
+input arrays), pinned host memory, and the two CUDA streams.  Every step of the hot path runs in
+the library's own kernels; there is no CPU or PyTorch fallback: if ``libpp.so`` is missing or
+no CUDA device is present, construction fails loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpp.so")
+
+PP_OK = 0
+ERRORS = {-1: "PP_E_INVAL", -2: "PP_E_NOMEM", -3: "PP_E_CUDA", -4: "PP_E_OVERFLOW", -5: "PP_E_WOULDBLOCK",
+          -6: "PP_E_UNSUPPORTED", -7: "PP_E_STATE"}
+FLAG_BRUTE_FORCE_DOMS = 1
+FLAG_NONBLOCKING_SUBMIT = 2
+
+SOURCE_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("dx", "<f4"), ("dy", "<f4"), ("dz", "<f4"),
+                         ("t_ns", "<f4"), ("energy_GeV", "<f4")])
+HIT_DTYPE = np.dtype([("event_id", "<u4"), ("source_id", "<u4"), ("photon_idx", "<u4"), ("dom_id", "<u4"),
+                      ("time_ns", "<f8"), ("weight", "<f4"), ("n_scatter", "<u4")])
+FATE_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("path_m", "<f4"), ("time_ns", "<f8"),
+                       ("n_flights", "<u4"), ("dom", "<i4"), ("fate", "<u4"), ("photon_idx", "<u4")])
+assert SOURCE_DTYPE.itemsize == 32 and HIT_DTYPE.itemsize == 32 and FATE_DTYPE.itemsize == 40
+
+
+class PPError(RuntimeError):
+    def __init__(self, code: int, msg: str = ""):
+        self.code = code
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+
+
+class _Geometry(C.Structure):
+    _fields_ = [("n_dom", C.c_uint32), ("xyz", C.POINTER(C.c_float)), ("radius", C.c_float)]
+
+
+class _Ice(C.Structure):
+    _fields_ = [("n_layers", C.c_uint32), ("z_top", C.c_float), ("dz", C.c_float),
+                ("abs_len", C.POINTER(C.c_float)), ("scat_len", C.POINTER(C.c_float)), ("g", C.c_float),
+                ("n_group", C.c_float), ("cos_cherenkov", C.c_float), ("photons_per_GeV", C.c_float)]
+
+
+class _Config(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("launch_photons_target", C.c_uint64), ("hit_ring_bytes", C.c_uint64),
+                ("source_ring_bytes", C.c_uint64), ("device_workspace", C.c_void_p),
+                ("device_workspace_bytes", C.c_uint64), ("pinned_workspace", C.c_void_p),
+                ("pinned_workspace_bytes", C.c_uint64), ("stream0", C.c_void_p), ("stream1", C.c_void_p),
+                ("flags", C.c_uint32), ("max_flights", C.c_uint32), ("device", C.c_int32), ("reserved", C.c_uint32)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("sources_submitted", C.c_uint64), ("photons_submitted", C.c_uint64), ("photons_done", C.c_uint64),
+                ("photons_absorbed", C.c_uint64), ("photons_hit", C.c_uint64), ("photons_aborted", C.c_uint64),
+                ("flights", C.c_uint64), ("launches", C.c_uint64), ("relaunches", C.c_uint64),
+                ("hits_collected", C.c_uint64), ("kernel_busy_ms", C.c_double), ("wall_ms", C.c_double),
+                ("source_ring_high_water", C.c_uint64), ("hit_ring_high_water", C.c_uint64)]
+
+
+EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
+           "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count"]
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """Loads libpp.so and declares the prototypes of every symbol include/pp.h declares."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} is missing: build it with `python -m paper_2405_05700_b200.build` "
+                                "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp, u32p = C.c_void_p, C.POINTER(C.c_uint32)
+    L.pp_workspace_size.restype = C.c_int
+    L.pp_workspace_size.argtypes = [C.POINTER(_Geometry), C.POINTER(_Ice), C.POINTER(_Config),
+                                    C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.pp_create.restype = C.c_int
+    L.pp_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Ice), C.POINTER(_Config), C.POINTER(vp)]
+    L.pp_submit.restype = C.c_int
+    L.pp_submit.argtypes = [vp, vp, vp, vp, C.c_size_t]
+    L.pp_flush.restype = C.c_int
+    L.pp_flush.argtypes = [vp]
+    L.pp_collect.restype = C.c_int
+    L.pp_collect.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_int]
+    L.pp_stats.restype = C.c_int
+    L.pp_stats.argtypes = [vp, C.POINTER(_Stats)]
+    L.pp_last_error.restype = C.c_char_p
+    L.pp_last_error.argtypes = [vp]
+    L.pp_destroy.restype = None
+    L.pp_destroy.argtypes = [vp]
+    L.pp_run_resident.restype = C.c_int
+    L.pp_run_resident.argtypes = [vp, vp, vp, vp, C.c_size_t, vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+    L.pp_version.restype = C.c_char_p
+    L.pp_kernel_launch_count.restype = C.c_uint64
+    _lib = L
+    return L
+
+
+def kernel_launch_count() -> int:
+    return int(load_library().pp_kernel_launch_count())
+
+
+def pack_sources(src: np.ndarray) -> np.ndarray:
+    """float32 [n, 8] rows (x,y,z,dx,dy,dz,t,E) -> pp_source records (a view when possible)."""
+    a = np.ascontiguousarray(src, dtype=np.float32).reshape(-1, 8)
+    return a.view(SOURCE_DTYPE).reshape(-1)
+
+
+@dataclass
+class Stats:
+    sources_submitted: int
+    photons_submitted: int
+    photons_done: int
+    photons_absorbed: int
+    photons_hit: int
+    photons_aborted: int
+    flights: int
+    launches: int
+    relaunches: int
+    hits_collected: int
+    kernel_busy_ms: float
+    wall_ms: float
+    source_ring_high_water: int
+    hit_ring_high_water: int
+
+
+class Propagator:
+    """pp_create / pp_submit / pp_flush / pp_collect / pp_run_resident over one handle.
+
+    ``geometry`` and ``ice`` are the dataclasses of :mod:`.workloads` (or anything with the same
+    attributes)."""
+
+    def __init__(self, geometry, ice, *, seed: int = 0, launch_photons_target: int = 0, hit_ring_bytes: int = 0,
+                 source_ring_bytes: int = 0, flags: int = 0, max_flights: int = 0, device: int = 0,
+                 use_torch_memory: bool = True):
+        import torch  # device memory, pinned memory and streams only
+
+        if not torch.cuda.is_available():
+            raise PPError(-3, "no CUDA device: the photon propagator has no CPU fallback")
+        self._torch = torch
+        self._L = load_library()
+        self._xyz = np.ascontiguousarray(geometry.xyz, dtype=np.float32).reshape(-1, 3)
+        self._abs = np.ascontiguousarray(ice.abs_len, dtype=np.float32)
+        self._scat = np.ascontiguousarray(ice.scat_len, dtype=np.float32)
+        fp = C.POINTER(C.c_float)
+        self._geo = _Geometry(self._xyz.shape[0], self._xyz.ctypes.data_as(fp), float(geometry.radius))
+        self._ice = _Ice(self._abs.shape[0], float(ice.z_top), float(ice.dz), self._abs.ctypes.data_as(fp),
+                         self._scat.ctypes.data_as(fp), float(ice.g), float(ice.n_group), float(ice.cos_cherenkov),
+                         float(ice.photons_per_GeV))
+        cfg = _Config()
+        cfg.seed = int(seed)
+        cfg.launch_photons_target = int(launch_photons_target)
+        cfg.hit_ring_bytes = int(hit_ring_bytes)
+        cfg.source_ring_bytes = int(source_ring_bytes)
+        cfg.flags = int(flags)
+        cfg.max_flights = int(max_flights)
+        cfg.device = int(device)
+        self.device = torch.device("cuda", device if device else torch.cuda.current_device())
+        self._keep = []
+        if use_torch_memory:
+            dev_b, pin_b = C.c_uint64(0), C.c_uint64(0)
+            with torch.cuda.device(self.device):
+                self._check(self._L.pp_workspace_size(C.byref(self._geo), C.byref(self._ice), C.byref(cfg),
+                                                      C.byref(dev_b), C.byref(pin_b)), None)
+                ws = torch.empty(int(dev_b.value), dtype=torch.uint8, device=self.device)
+                pin = torch.empty(int(pin_b.value), dtype=torch.uint8, pin_memory=True)
+                self.streams = (torch.cuda.Stream(device=self.device), torch.cuda.Stream(device=self.device))
+            self._keep += [ws, pin]
+            cfg.device_workspace, cfg.device_workspace_bytes = ws.data_ptr(), ws.numel()
+            cfg.pinned_workspace, cfg.pinned_workspace_bytes = pin.data_ptr(), pin.numel()
+            cfg.stream0, cfg.stream1 = self.streams[0].cuda_stream, self.streams[1].cuda_stream
+            self.device_workspace_bytes, self.pinned_workspace_bytes = ws.numel(), pin.numel()
+        self._cfg = cfg
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            self._check(self._L.pp_create(C.byref(self._geo), C.byref(self._ice), C.byref(cfg), C.byref(h)), None)
+        self._h = h
+
+    # ---- plumbing ----
+    def _check(self, rc: int, h):
+        if rc != PP_OK:
+            msg = self._L.pp_last_error(h).decode() if h else ""
+            raise PPError(rc, msg)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.pp_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the paper's calls ----
+    def submit(self, sources, event_ids, source_ids=None):
+        """pp_submit: ``sources`` float32 [n, 8] (or SOURCE_DTYPE [n]); host buffers; thread-safe."""
+        rec = pack_sources(sources) if sources.dtype != SOURCE_DTYPE else np.ascontiguousarray(sources)
+        ev = np.ascontiguousarray(event_ids, dtype=np.uint32)
+        sid = None if source_ids is None else np.ascontiguousarray(source_ids, dtype=np.uint32)
+        assert ev.shape[0] == rec.shape[0] and (sid is None or sid.shape[0] == rec.shape[0])
+        rc = self._L.pp_submit(self._h, rec.ctypes.data, ev.ctypes.data, None if sid is None else sid.ctypes.data,
+                               rec.shape[0])
+        self._check(rc, self._h)
+
+    def flush(self):
+        self._check(self._L.pp_flush(self._h), self._h)
+
+    def collect(self, cap: int = 1 << 20, block: bool = True) -> np.ndarray:
+        """pp_collect: up to ``cap`` hits; an empty array from a blocking call means drained."""
+        out = np.empty(cap, dtype=HIT_DTYPE)
+        n = C.c_size_t(0)
+        self._check(self._L.pp_collect(self._h, out.ctypes.data, cap, C.byref(n), 1 if block else 0), self._h)
+        return out[: n.value]
+
+    def collect_all(self, chunk: int = 1 << 20) -> np.ndarray:
+        """flush, then collect until drained."""
+        self.flush()
+        parts = []
+        while True:
+            h = self.collect(chunk, block=True)
+            if len(h) == 0:
+                break
+            parts.append(h.copy())
+        return np.concatenate(parts) if parts else np.empty(0, dtype=HIT_DTYPE)
+
+    def run(self, sources, event_ids, source_ids=None) -> np.ndarray:
+        """End-to-end convenience: submit + flush + collect everything (host buffers in and out)."""
+        self.submit(sources, event_ids, source_ids)
+        return self.collect_all()
+
+    def stats(self) -> Stats:
+        s = _Stats()
+        self._check(self._L.pp_stats(self._h, C.byref(s)), self._h)
+        return Stats(**{f[0]: getattr(s, f[0]) for f in _Stats._fields_})
+
+    # ---- device-resident path ----
+    def upload(self, sources, event_ids, source_ids=None):
+        """Copies a source list into HBM (torch tensors) for :meth:`run_resident`."""
+        torch = self._torch
+        rec = pack_sources(sources) if sources.dtype != SOURCE_DTYPE else np.ascontiguousarray(sources)
+        d_src = torch.from_numpy(rec.view(np.float32).reshape(-1, 8).copy()).to(self.device)
+        d_ev = torch.from_numpy(np.ascontiguousarray(event_ids, dtype=np.uint32).view(np.int32).copy()).to(self.device)
+        d_sid = None if source_ids is None else \
+            torch.from_numpy(np.ascontiguousarray(source_ids, dtype=np.uint32).view(np.int32).copy()).to(self.device)
+        torch.cuda.synchronize(self.device)
+        return d_src, d_ev, d_sid
+
+    def run_resident(self, d_src, d_ev, d_sid=None, want_fates: bool = False, n_photons_hint: int | None = None):
+        """pp_run_resident on tensors from :meth:`upload`.  Returns (photons, device_ms, fates|None);
+        hits are fetched with :meth:`collect` afterwards."""
+        torch = self._torch
+        n = int(d_src.shape[0])
+        fates_t = None
+        if want_fates:
+            assert n_photons_hint is not None, "want_fates needs the total photon count"
+            fates_t = torch.zeros(int(n_photons_hint) * FATE_DTYPE.itemsize, dtype=torch.uint8, device=self.device)
+        ph, ms = C.c_uint64(0), C.c_double(0.0)
+        rc = self._L.pp_run_resident(self._h, d_src.data_ptr(), d_ev.data_ptr(), None if d_sid is None else d_sid.data_ptr(),
+                                     n, None if fates_t is None else fates_t.data_ptr(), C.byref(ph), C.byref(ms))
+        self._check(rc, self._h)
+        fates = None
+        if want_fates:
+            fates = fates_t.cpu().numpy().view(FATE_DTYPE)[: ph.value]
+        return int(ph.value), float(ms.value), fates
+
+    def drain(self, chunk: int = 1 << 20) -> np.ndarray:
+        """Collect whatever is ready without flushing (after run_resident)."""
+        parts = []
+        while True:
+            h = self.collect(chunk, block=False)
+            if len(h) == 0:
+                break
+            parts.append(h.copy())
+        return np.concatenate(parts) if parts else np.empty(0, dtype=HIT_DTYPE)

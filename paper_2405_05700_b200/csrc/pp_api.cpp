@@ -1,0 +1,953 @@
+// Host side of the photon propagator: C ABI (include/pp.h), DOM-lookup construction, launch engine
+// (two slots = two CUDA streams, double-buffered), and the batching server thread that turns a
+// stream of pp_submit() calls from many producer threads into large GPU launches.
+// Product code: shares nothing with oracle/.  No CPU fallback anywhere: every photon is tracked
+// by the kernels in pp_kernels.cu.
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <condition_variable>
+#include <cstdio>
+#include <cstring>
+#include <deque>
+#include <map>
+#include <mutex>
+#include <string>
+#include <thread>
+#include <vector>
+
+#include "pp_internal.h"
+
+using namespace pp;
+
+namespace {
+
+constexpr double kC = 0.299792458;  // m/ns
+constexpr size_t kStageBytes = 4u << 20;  // pinned D2H staging chunk per slot (x2)
+using Clock = std::chrono::steady_clock;
+
+inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+struct Carver {  // hands out aligned pieces of one workspace
+  unsigned char* base;
+  uint64_t off = 0;
+  explicit Carver(void* b) : base(static_cast<unsigned char*>(b)) {}
+  template <class T>
+  T* take(uint64_t count) {
+    off = align_up(off, 256);
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += count * sizeof(T);
+    return p;
+  }
+};
+
+struct HostGeometry {
+  std::vector<StringRec> strings;
+  std::vector<float4> dom_xyzw;
+  std::vector<uint16_t> cell_start, cell_items;
+  uint32_t nx = 1, ny = 1;
+  float gx0 = 0, gy0 = 0, inv_cell = 1;
+  bool fast_ok = false;
+  std::string why;
+};
+
+struct Sizes {
+  uint64_t cap_src = 0;      // records in the pinned source ring == per-slot device source capacity
+  uint64_t max_tiles = 0;    // per launch
+  uint64_t resume_cap = 0;   // WorkItems per resume list
+  uint64_t ring_cap = 0;     // hits per slot ring
+  uint64_t target = 0;       // photons per launch
+};
+
+struct Slot {
+  cudaStream_t stream = nullptr;
+  // device
+  SrcRec* d_src = nullptr;
+  unsigned long long* d_cum = nullptr;
+  uint32_t* d_tile_src = nullptr;
+  Status* d_status = nullptr;
+  WorkItem* d_resume[2] = {nullptr, nullptr};
+  pp_hit* d_ring = nullptr;
+  // pinned host
+  Status* h_status = nullptr;     // D2H target
+  Status* h_status_in = nullptr;  // H2D source for relaunches
+  unsigned char* h_stage[2] = {nullptr, nullptr};
+  cudaEvent_t ev_h2d = nullptr, ev_k0 = nullptr, ev_k1 = nullptr, ev_done = nullptr, ev_stage[2] = {nullptr, nullptr};
+  // state of the launch in flight
+  bool in_flight = false;
+  int resume_sel = 0;  // which of d_resume[] is the OUT list of the launch in flight
+  LaunchParams P;
+  uint64_t seq = 0;
+  bool fates = false;
+};
+
+}  // namespace
+
+struct pp_handle {
+  pp_config cfg{};
+  pp_ice ice{};
+  int device = 0;
+  int n_sm = 0, grid = 0;
+  size_t smem = 0;
+  bool brute = false;
+  Sizes sz;
+  HostGeometry hg;
+  LaunchParams base{};  // medium + geometry filled in once
+
+  // memory
+  void* dev_ws = nullptr; bool own_dev = false;
+  void* pin_ws = nullptr; bool own_pin = false;
+  bool own_streams = false;
+  Slot slot[2];
+  SrcRec* d_res_src = nullptr;            // resident batch
+  unsigned long long* d_res_cum = nullptr;
+  unsigned int* d_res_overflow = nullptr;
+  unsigned long long* h_res_total = nullptr;  // pinned
+  unsigned int* h_res_overflow = nullptr;     // pinned
+  cudaEvent_t ev_base = nullptr, ev_job = nullptr;
+
+  // source ring (pinned), positions are monotonically increasing record numbers
+  SrcRec* ring = nullptr;
+  std::mutex mu;  // protects everything below unless noted
+  std::condition_variable cv_space, cv_work, cv_hits;
+  uint64_t ring_head = 0;     // next record to be written by a producer
+  uint64_t ring_launch = 0;   // first record not yet fully launched
+  uint64_t ring_tail = 0;     // first record still needed
+  uint64_t launch_offset = 0; // photons of record ring_launch already launched
+  uint64_t queued_photons = 0;
+  uint64_t flush_upto = 0;    // records below this position must be launched even if under target
+  bool shutdown = false;
+  bool resident_active = false;
+  int n_in_flight = 0;
+  uint64_t launch_seq = 0;
+  int space_waiters = 0;
+
+  // finished hits waiting for pp_collect
+  std::deque<std::vector<pp_hit>> hitq;
+  size_t hitq_front_off = 0;
+  uint64_t hitq_bytes = 0, hitq_budget = 0;
+
+  // stats
+  pp_stats_t st{};
+  bool wall_started = false;
+  Clock::time_point wall_t0, wall_t1;
+  double busy_end_ms = 0;
+
+  // error state
+  std::atomic<int> sticky{PP_OK};
+  std::string err;
+  std::mutex err_mu;
+
+  std::thread server;
+};
+
+namespace {
+
+int fail(pp_handle* h, int code, const std::string& msg) {
+  if (h) {
+    std::lock_guard<std::mutex> g(h->err_mu);
+    h->err = msg;
+    if (code == PP_E_CUDA) h->sticky.store(PP_E_CUDA);
+  }
+  return code;
+}
+
+#define PP_CUDA(h, call)                                                                        \
+  do {                                                                                          \
+    cudaError_t e__ = (call);                                                                   \
+    if (e__ != cudaSuccess)                                                                     \
+      return fail((h), PP_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__));         \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// validation
+// ---------------------------------------------------------------------------------------------
+bool finite_f(float x) { return std::isfinite(x); }
+
+int validate_inputs(const pp_geometry* geo, const pp_ice* ice, std::string* why) {
+  if (!geo || !ice || !geo->xyz || !ice->abs_len || !ice->scat_len) { *why = "null pointer"; return PP_E_INVAL; }
+  if (geo->n_dom == 0 || !(geo->radius > 0.0f) || !finite_f(geo->radius)) { *why = "bad geometry"; return PP_E_INVAL; }
+  for (uint32_t i = 0; i < 3 * geo->n_dom; ++i)
+    if (!finite_f(geo->xyz[i])) { *why = "non-finite DOM coordinate"; return PP_E_INVAL; }
+  if (ice->n_layers == 0 || ice->n_layers > PP_MAX_LAYERS) { *why = "n_layers out of range"; return PP_E_INVAL; }
+  if (!(ice->dz > 0.0f) || !finite_f(ice->dz) || !finite_f(ice->z_top)) { *why = "bad layer grid"; return PP_E_INVAL; }
+  for (uint32_t i = 0; i < ice->n_layers; ++i)
+    if (!(ice->abs_len[i] > 0.0f) || !(ice->scat_len[i] > 0.0f) || std::isnan(ice->abs_len[i]) ||
+        std::isnan(ice->scat_len[i])) { *why = "non-positive length in ice table"; return PP_E_INVAL; }
+  if (!(std::fabs(ice->g) < 1.0f)) { *why = "|g| must be < 1"; return PP_E_INVAL; }
+  if (!(ice->n_group > 0.0f) || !finite_f(ice->n_group)) { *why = "bad n_group"; return PP_E_INVAL; }
+  if (!(ice->cos_cherenkov >= -1.0f && ice->cos_cherenkov <= 1.0f)) { *why = "bad cos_cherenkov"; return PP_E_INVAL; }
+  if (!(ice->photons_per_GeV >= 0.0f) || !finite_f(ice->photons_per_GeV)) { *why = "bad yield"; return PP_E_INVAL; }
+  return PP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 (host part): group DOMs into vertical lines, build the 2-D cell grid over the footprint
+// ---------------------------------------------------------------------------------------------
+void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
+  const uint32_t n = geo->n_dom;
+  out->fast_ok = false;
+  if (brute) {
+    out->dom_xyzw.resize(n);
+    for (uint32_t j = 0; j < n; ++j) {
+      float4 v;
+      v.x = geo->xyz[3 * j]; v.y = geo->xyz[3 * j + 1]; v.z = geo->xyz[3 * j + 2];
+      std::memcpy(&v.w, &j, 4);
+      out->dom_xyzw[j] = v;
+    }
+    out->cell_start.assign(2, 0);
+    return;
+  }
+  struct Dom { float z; uint32_t id; };
+  std::map<std::pair<uint32_t, uint32_t>, std::vector<Dom>> lines;  // key = bit patterns of (x, y)
+  for (uint32_t j = 0; j < n; ++j) {
+    uint32_t bx, by;
+    float x = geo->xyz[3 * j] + 0.0f, y = geo->xyz[3 * j + 1] + 0.0f;  // +0: fold -0 into +0
+    std::memcpy(&bx, &x, 4); std::memcpy(&by, &y, 4);
+    lines[{bx, by}].push_back(Dom{geo->xyz[3 * j + 2], j});
+  }
+  if (lines.size() > (size_t)kMaxStringsSmem) { out->why = "more than 512 vertical lines of DOMs"; return; }
+  out->dom_xyzw.reserve(n);
+  std::vector<std::pair<float, float>> xy;
+  for (auto& kv : lines) {
+    auto& v = kv.second;
+    std::sort(v.begin(), v.end(), [](const Dom& a, const Dom& b) { return a.z > b.z || (a.z == b.z && a.id < b.id); });
+    float x, y;
+    std::memcpy(&x, &kv.first.first, 4); std::memcpy(&y, &kv.first.second, 4);
+    StringRec r{};
+    r.x = x; r.y = y; r.z0 = v[0].z; r.n = (uint32_t)v.size(); r.base = (uint32_t)out->dom_xyzw.size();
+    double pitch = 1.0;
+    if (v.size() > 1) {
+      pitch = ((double)v.front().z - (double)v.back().z) / (double)(v.size() - 1);
+      if (!(pitch > 0.0)) { out->why = "two DOMs at the same position"; return; }
+      for (size_t k = 0; k < v.size(); ++k)
+        if (std::fabs((double)v[k].z - ((double)v[0].z - k * pitch)) > 1e-3 * pitch + 1e-4) {
+          out->why = "DOMs of a vertical line are not uniformly spaced";
+          return;
+        }
+    }
+    r.pitch = (float)pitch; r.inv_pitch = (float)(1.0 / pitch);
+    out->strings.push_back(r);
+    xy.push_back({x, y});
+    for (auto& d : v) {
+      float4 c; c.x = x; c.y = y; c.z = d.z;
+      std::memcpy(&c.w, &d.id, 4);
+      out->dom_xyzw.push_back(c);
+    }
+  }
+  // cell size ~ median nearest-neighbour distance of the lines (100 m for a single line)
+  const size_t ns = xy.size();
+  double cell = 100.0;
+  if (ns > 1) {
+    std::vector<double> nn(ns, 1e30);
+    for (size_t i = 0; i < ns; ++i)
+      for (size_t j = 0; j < ns; ++j)
+        if (i != j) nn[i] = std::min(nn[i], std::hypot((double)xy[i].first - xy[j].first, (double)xy[i].second - xy[j].second));
+    std::nth_element(nn.begin(), nn.begin() + ns / 2, nn.end());
+    cell = std::max(1.0, nn[ns / 2]);
+  }
+  const double Rm = (double)geo->radius + 5e-3, pad = Rm + 1e-2;
+  double x0 = 1e30, x1 = -1e30, y0 = 1e30, y1 = -1e30;
+  for (auto& p : xy) { x0 = std::min(x0, (double)p.first); x1 = std::max(x1, (double)p.first);
+                       y0 = std::min(y0, (double)p.second); y1 = std::max(y1, (double)p.second); }
+  x0 -= pad; y0 -= pad; x1 += pad; y1 += pad;
+  uint32_t nx, ny;
+  for (;;) {
+    nx = (uint32_t)std::floor((x1 - x0) / cell) + 1; ny = (uint32_t)std::floor((y1 - y0) / cell) + 1;
+    if ((uint64_t)nx * ny <= 4096) break;
+    cell *= 2.0;
+  }
+  std::vector<std::vector<uint16_t>> cells((size_t)nx * ny);
+  for (size_t s = 0; s < ns; ++s) {
+    const int ix0 = std::max(0, (int)std::floor(((double)xy[s].first - pad - x0) / cell));
+    const int ix1 = std::min((int)nx - 1, (int)std::floor(((double)xy[s].first + pad - x0) / cell));
+    const int iy0 = std::max(0, (int)std::floor(((double)xy[s].second - pad - y0) / cell));
+    const int iy1 = std::min((int)ny - 1, (int)std::floor(((double)xy[s].second + pad - y0) / cell));
+    for (int iy = iy0; iy <= iy1; ++iy)
+      for (int ix = ix0; ix <= ix1; ++ix) cells[(size_t)iy * nx + ix].push_back((uint16_t)s);
+  }
+  out->cell_start.assign((size_t)nx * ny + 1, 0);
+  for (size_t c = 0; c < cells.size(); ++c) {
+    out->cell_start[c + 1] = (uint16_t)(out->cell_start[c] + cells[c].size());
+    for (auto s : cells[c]) out->cell_items.push_back(s);
+  }
+  out->nx = nx; out->ny = ny; out->gx0 = (float)x0; out->gy0 = (float)y0; out->inv_cell = (float)(1.0 / cell);
+  out->fast_ok = true;
+}
+
+void fill_sizes(const pp_config& cfg, int n_sm, Sizes* s) {
+  s->target = cfg.launch_photons_target ? cfg.launch_photons_target : 100000000ull;
+  const uint64_t src_bytes = cfg.source_ring_bytes ? cfg.source_ring_bytes : (64ull << 20);
+  s->cap_src = std::max<uint64_t>(64, src_bytes / sizeof(SrcRec));
+  s->max_tiles = (s->target + kTilePhotons - 1) / kTilePhotons + 2;
+  s->resume_cap = (uint64_t)n_sm * 2048ull * 2ull + 4096ull;
+  const uint64_t hit_bytes = cfg.hit_ring_bytes ? cfg.hit_ring_bytes : (256ull << 20);
+  s->ring_cap = std::max<uint64_t>(32, std::min<uint64_t>(hit_bytes / 2 / sizeof(pp_hit), 0xFFFFFF00ull));
+}
+
+// Carve (or, with null base, just measure) the device workspace.
+uint64_t carve_device(pp_handle* h, void* base) {
+  Carver c(base);
+  const HostGeometry& g = h->hg;
+  auto* d_ice = c.take<IceLayer>(h->ice.n_layers);
+  auto* d_strings = c.take<StringRec>(std::max<size_t>(1, g.strings.size()));
+  auto* d_dom = c.take<float4>(g.dom_xyzw.size());
+  auto* d_cs = c.take<uint16_t>(g.cell_start.size());
+  auto* d_ci = c.take<uint16_t>(std::max<size_t>(1, g.cell_items.size()));
+  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.cell_start = d_cs;
+  h->base.cell_items = d_ci;
+  for (int i = 0; i < 2; ++i) {
+    Slot& s = h->slot[i];
+    s.d_src = c.take<SrcRec>(h->sz.cap_src);
+    s.d_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
+    s.d_tile_src = c.take<uint32_t>(h->sz.max_tiles);
+    s.d_status = c.take<Status>(1);
+    s.d_resume[0] = c.take<WorkItem>(h->sz.resume_cap);
+    s.d_resume[1] = c.take<WorkItem>(h->sz.resume_cap);
+    s.d_ring = c.take<pp_hit>(h->sz.ring_cap);
+  }
+  h->d_res_src = c.take<SrcRec>(h->sz.cap_src);
+  h->d_res_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
+  h->d_res_overflow = c.take<unsigned int>(4);
+  return align_up(c.off, 256);
+}
+
+uint64_t carve_pinned(pp_handle* h, void* base) {
+  Carver c(base);
+  h->ring = c.take<SrcRec>(h->sz.cap_src);
+  for (int i = 0; i < 2; ++i) {
+    Slot& s = h->slot[i];
+    s.h_status = c.take<Status>(1);
+    s.h_status_in = c.take<Status>(1);
+    s.h_stage[0] = c.take<unsigned char>(kStageBytes);
+    s.h_stage[1] = c.take<unsigned char>(kStageBytes);
+  }
+  h->h_res_total = c.take<unsigned long long>(2);
+  h->h_res_overflow = c.take<unsigned int>(4);
+  return align_up(c.off, 256);
+}
+
+// ---------------------------------------------------------------------------------------------
+// launch engine
+// ---------------------------------------------------------------------------------------------
+
+// Enqueue tiles + propagate (+ status read-back) for photons [g_begin, g_end) of the batch
+// (src, cum, n_src), which must already be (or be enqueued to become) resident on slot.stream.
+int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long long* cum, uint32_t n_src,
+                   uint64_t g_begin, uint64_t g_end, pp_fate* fates) {
+  const uint64_t n_ph = g_end - g_begin;
+  const uint32_t n_tiles = (uint32_t)((n_ph + kTilePhotons - 1) / kTilePhotons);
+  if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");
+  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, s.d_tile_src, s.stream));
+  LaunchParams P = h->base;
+  P.src = src; P.cum = cum; P.tile_src = s.d_tile_src;
+  P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles;
+  s.resume_sel = 0;
+  P.resume_in = s.d_resume[1]; P.resume_out = s.d_resume[0];
+  P.n_resume_in = 0; P.resume_cap = (uint32_t)h->sz.resume_cap;
+  P.status = s.d_status; P.ring = s.d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap;
+  P.fates = fates;
+  s.fates = fates != nullptr;
+  s.P = P;
+  PP_CUDA(h, cudaMemsetAsync(s.d_status, 0, sizeof(Status), s.stream));
+  PP_CUDA(h, cudaEventRecord(s.ev_k0, s.stream));
+  PP_CUDA(h, launch_propagate(P, h->brute, s.fates, h->grid, h->smem, s.stream));
+  PP_CUDA(h, cudaEventRecord(s.ev_k1, s.stream));
+  PP_CUDA(h, cudaMemcpyAsync(s.h_status, s.d_status, sizeof(Status), cudaMemcpyDeviceToHost, s.stream));
+  PP_CUDA(h, cudaEventRecord(s.ev_done, s.stream));
+  s.in_flight = true;
+  s.seq = ++h->launch_seq;
+  return PP_OK;
+}
+
+// Push finished hits to the collect queue (bounded: blocks the server while the consumer is behind,
+// which in turn back-pressures pp_submit; the resident path fails instead of dead-locking).
+int push_hits(pp_handle* h, std::vector<pp_hit>&& v, bool may_block) {
+  if (v.empty()) return PP_OK;
+  std::unique_lock<std::mutex> lk(h->mu);
+  const uint64_t bytes = v.size() * sizeof(pp_hit);
+  while (h->hitq_bytes + bytes > h->hitq_budget && h->hitq_bytes > 0) {
+    if (!may_block) return fail(h, PP_E_NOMEM, "host hit queue budget exceeded in pp_run_resident; collect more often");
+    if (h->shutdown) break;
+    h->cv_space.wait(lk);
+  }
+  h->hitq_bytes += bytes;
+  h->st.hit_ring_high_water = std::max<uint64_t>(h->st.hit_ring_high_water, bytes);
+  h->hitq.push_back(std::move(v));
+  h->cv_hits.notify_all();
+  return PP_OK;
+}
+
+// Wait for the slot's launch, stream its hits to the host in chunks, relaunch if the ring filled up.
+int finish_slot(pp_handle* h, Slot& s, bool may_block) {
+  PP_CUDA(h, cudaEventSynchronize(s.ev_done));
+  const Status hs = *s.h_status;
+  if (hs.error) return fail(h, PP_E_CUDA, "internal: resume list overflow");
+  float t0 = 0, t1 = 0;
+  PP_CUDA(h, cudaEventElapsedTime(&t0, h->ev_base, s.ev_k0));
+  PP_CUDA(h, cudaEventElapsedTime(&t1, h->ev_base, s.ev_k1));
+  // ---- a9: stream the valid part of the ring to the host through two pinned staging chunks ----
+  const uint64_t n_valid = std::min<uint64_t>(hs.hit_count, h->sz.ring_cap);
+  std::vector<pp_hit> hits(n_valid);
+  {
+    const uint64_t per = kStageBytes / sizeof(pp_hit);
+    uint64_t issued = 0, done = 0;
+    int b = 0;
+    uint64_t cnt[2] = {0, 0};
+    while (done < n_valid) {
+      // keep up to two chunk copies in flight
+      while (issued < n_valid && issued - done < 2 * per) {
+        const int bi = (int)((issued / per) & 1);
+        cnt[bi] = std::min<uint64_t>(per, n_valid - issued);
+        PP_CUDA(h, cudaMemcpyAsync(s.h_stage[bi], s.d_ring + issued, cnt[bi] * sizeof(pp_hit), cudaMemcpyDeviceToHost,
+                                   s.stream));
+        PP_CUDA(h, cudaEventRecord(s.ev_stage[bi], s.stream));
+        issued += cnt[bi];
+      }
+      PP_CUDA(h, cudaEventSynchronize(s.ev_stage[b]));
+      std::memcpy(hits.data() + done, s.h_stage[b], cnt[b] * sizeof(pp_hit));
+      done += cnt[b];
+      b ^= 1;
+    }
+  }
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    h->st.photons_done += hs.photons_started;
+    h->st.photons_hit += hs.photons_hit;
+    h->st.photons_aborted += hs.photons_aborted;
+    h->st.photons_absorbed += hs.photons_started - hs.photons_hit - hs.photons_aborted;
+    h->st.flights += hs.flights;
+    h->st.launches += 1;
+    if (t0 > h->busy_end_ms) h->st.kernel_busy_ms += (double)t1 - t0;
+    else if (t1 > h->busy_end_ms) h->st.kernel_busy_ms += (double)t1 - h->busy_end_ms;
+    h->busy_end_ms = std::max(h->busy_end_ms, (double)t1);
+  }
+  int rc = push_hits(h, std::move(hits), may_block);
+  if (rc != PP_OK) return rc;
+  if (hs.n_resume_out > 0) {
+    // ---- ring filled up: relaunch for the deferred photons, the unfinished tiles and the fresh tiles ----
+    Status ns{};
+    ns.tile_counter = hs.tile_counter;
+    *s.h_status_in = ns;
+    PP_CUDA(h, cudaMemcpyAsync(s.d_status, s.h_status_in, sizeof(Status), cudaMemcpyHostToDevice, s.stream));
+    LaunchParams& P = s.P;
+    P.resume_in = s.d_resume[s.resume_sel];
+    P.n_resume_in = std::min<uint32_t>(hs.n_resume_out, P.resume_cap);
+    s.resume_sel ^= 1;
+    P.resume_out = s.d_resume[s.resume_sel];
+    PP_CUDA(h, cudaEventRecord(s.ev_k0, s.stream));
+    PP_CUDA(h, launch_propagate(P, h->brute, s.fates, h->grid, h->smem, s.stream));
+    PP_CUDA(h, cudaEventRecord(s.ev_k1, s.stream));
+    PP_CUDA(h, cudaMemcpyAsync(s.h_status, s.d_status, sizeof(Status), cudaMemcpyDeviceToHost, s.stream));
+    PP_CUDA(h, cudaEventRecord(s.ev_done, s.stream));
+    std::lock_guard<std::mutex> g(h->mu);
+    h->st.relaunches += 1;
+    return PP_OK;  // still in flight
+  }
+  s.in_flight = false;
+  return PP_OK;
+}
+
+// Finish a slot completely (all relaunches).
+int drain_slot(pp_handle* h, Slot& s, bool may_block) {
+  while (s.in_flight) {
+    int rc = finish_slot(h, s, may_block);
+    if (rc != PP_OK) { s.in_flight = false; return rc; }
+  }
+  return PP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1: the batching server thread
+// ---------------------------------------------------------------------------------------------
+
+// Cut the next launch from the source ring (caller holds h->mu).  Returns false if nothing to launch.
+struct Cut { uint64_t rec_a, rec_b, g_begin, g_end, photons; bool last_partial; };
+
+bool cut_launch(pp_handle* h, bool force, Cut* c) {
+  if (h->queued_photons == 0) {
+    // nothing but zero-photon sources (or nothing at all): drop them
+    h->ring_launch = h->ring_head; h->launch_offset = 0;
+    return false;
+  }
+  const bool ring_pressure = h->space_waiters > 0;
+  if (h->queued_photons < h->sz.target && !force && !ring_pressure) return false;
+  uint64_t pos = h->ring_launch, acc = 0, cum_all = 0;
+  const uint64_t target = h->sz.target;
+  c->rec_a = pos; c->g_begin = h->launch_offset; c->last_partial = false;
+  while (pos < h->ring_head) {
+    const uint64_t np = h->ring[pos % h->sz.cap_src].n_photons;
+    const uint64_t avail = np - (pos == h->ring_launch ? h->launch_offset : 0);
+    if (acc + avail > target) {  // split this source across launches
+      const uint64_t take = target - acc;
+      acc += take; cum_all += np;
+      c->last_partial = true;
+      c->rec_b = pos + 1;
+      c->g_end = (cum_all - np) + (pos == h->ring_launch ? h->launch_offset : 0) + take;
+      c->photons = acc;
+      return true;
+    }
+    acc += avail; cum_all += np;
+    ++pos;
+    if (acc == target) break;
+  }
+  c->rec_b = pos; c->g_end = cum_all; c->photons = acc;
+  return acc > 0;
+}
+
+void server_main(pp_handle* h) {
+  cudaSetDevice(h->device);
+  std::unique_lock<std::mutex> lk(h->mu);
+  int next_slot = 0;
+  for (;;) {
+    if (h->sticky.load() != PP_OK) {  // poisoned: wake everybody, do nothing more
+      h->cv_space.notify_all(); h->cv_hits.notify_all();
+      if (h->shutdown) return;
+      h->cv_work.wait_for(lk, std::chrono::milliseconds(50));
+      continue;
+    }
+    if (h->shutdown) {  // pp_destroy: queued-but-unlaunched work is dropped, launches in flight finish
+      h->ring_launch = h->ring_tail = h->ring_head; h->launch_offset = 0; h->queued_photons = 0;
+    }
+    bool progressed = false;
+    // 1. retire finished launches (oldest first)
+    for (int pass = 0; pass < 2 && !h->resident_active; ++pass) {
+      Slot* oldest = nullptr;
+      for (auto& s : h->slot)
+        if (s.in_flight && (!oldest || s.seq < oldest->seq)) oldest = &s;
+      if (!oldest) break;
+      const cudaError_t q = cudaEventQuery(oldest->ev_done);
+      if (q == cudaErrorNotReady) break;
+      lk.unlock();
+      const int rc = finish_slot(h, *oldest, true);
+      lk.lock();
+      if (rc != PP_OK) { oldest->in_flight = false; }
+      if (!oldest->in_flight) { h->n_in_flight--; h->wall_t1 = Clock::now(); h->cv_hits.notify_all(); }
+      progressed = true;
+    }
+    // 2. launch if a slot is free and enough work is queued
+    if (!h->resident_active && h->n_in_flight < 2 && h->sticky.load() == PP_OK) {
+      Slot& s = h->slot[next_slot].in_flight ? h->slot[next_slot ^ 1] : h->slot[next_slot];
+      Cut c{};
+      const bool force = h->flush_upto > h->ring_launch;
+      if (!s.in_flight && cut_launch(h, force, &c)) {
+        const uint32_t n_src = (uint32_t)(c.rec_b - c.rec_a);
+        // bookkeeping under the lock; the records [rec_a, rec_b) stay valid until ring_tail passes them
+        h->queued_photons -= c.photons;
+        if (c.last_partial) {
+          // the split record stays queued; launch_offset counts its photons already launched
+          uint64_t before = 0;
+          for (uint64_t p = c.rec_a; p + 1 < c.rec_b; ++p) before += h->ring[p % h->sz.cap_src].n_photons;
+          h->ring_launch = c.rec_b - 1;
+          h->launch_offset = c.g_end - before;
+        } else {
+          h->ring_launch = c.rec_b;
+          h->launch_offset = 0;
+        }
+        s.in_flight = true;  // reserve
+        h->n_in_flight++;
+        lk.unlock();
+        int rc = PP_OK;
+        {
+          const uint64_t cap = h->sz.cap_src;
+          const uint64_t a = c.rec_a % cap;
+          const uint64_t first = std::min<uint64_t>(n_src, cap - a);
+          cudaError_t e = cudaMemcpyAsync(s.d_src, h->ring + a, first * sizeof(SrcRec), cudaMemcpyHostToDevice, s.stream);
+          if (e == cudaSuccess && first < n_src)
+            e = cudaMemcpyAsync(s.d_src + first, h->ring, (n_src - first) * sizeof(SrcRec), cudaMemcpyHostToDevice, s.stream);
+          if (e == cudaSuccess) e = cudaEventRecord(s.ev_h2d, s.stream);
+          if (e == cudaSuccess) e = launch_scan(s.d_src, n_src, s.d_cum, s.stream);
+          if (e != cudaSuccess) rc = fail(h, PP_E_CUDA, std::string("upload: ") + cudaGetErrorString(e));
+          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr);
+          if (rc == PP_OK && cudaEventSynchronize(s.ev_h2d) != cudaSuccess) rc = fail(h, PP_E_CUDA, "upload sync failed");
+        }
+        lk.lock();
+        if (rc != PP_OK) { s.in_flight = false; h->n_in_flight--; }
+        // the uploaded records are free again (a split record stays for the next launch)
+        h->ring_tail = h->ring_launch;
+        h->cv_space.notify_all();
+        next_slot ^= 1;
+        progressed = true;
+      }
+    }
+    if (progressed) continue;
+    if (h->shutdown && h->n_in_flight == 0 && h->queued_photons == 0) return;
+    if (h->n_in_flight > 0 && !h->resident_active) {
+      // nothing launchable: sleep briefly (new sources may arrive) -- the GPU is busy meanwhile
+      h->cv_work.wait_for(lk, std::chrono::microseconds(100));
+    } else {
+      h->cv_work.wait_for(lk, std::chrono::milliseconds(20));
+    }
+  }
+}
+
+void destroy_events(Slot& s) {
+  for (cudaEvent_t* e : {&s.ev_h2d, &s.ev_k0, &s.ev_k1, &s.ev_done, &s.ev_stage[0], &s.ev_stage[1]})
+    if (*e) { cudaEventDestroy(*e); *e = nullptr; }
+}
+
+bool idle_locked(pp_handle* h) {
+  return h->n_in_flight == 0 && h->queued_photons == 0 && !h->resident_active;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+const char* pp_version(void) { return "pp 0.1 (sm_100a)"; }
+uint64_t pp_kernel_launch_count(void) { return kernel_launch_count(); }
+
+int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, uint64_t* device_bytes,
+                      uint64_t* pinned_bytes) {
+  std::string why;
+  if (!cfg) return PP_E_INVAL;
+  int rc = validate_inputs(geo, ice, &why);
+  if (rc != PP_OK) return rc;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PP_E_CUDA;
+  if (cfg->device > 0) dev = cfg->device;
+  int n_sm = 0;
+  if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PP_E_CUDA;
+  pp_handle tmp;
+  tmp.cfg = *cfg; tmp.ice = *ice;
+  tmp.brute = (cfg->flags & PP_FLAG_BRUTE_FORCE_DOMS) != 0;
+  build_geometry(geo, tmp.brute, &tmp.hg);
+  if (!tmp.brute && !tmp.hg.fast_ok) return PP_E_UNSUPPORTED;
+  fill_sizes(*cfg, n_sm, &tmp.sz);
+  if (device_bytes) *device_bytes = carve_device(&tmp, nullptr);
+  if (pinned_bytes) *pinned_bytes = carve_pinned(&tmp, nullptr);
+  return PP_OK;
+}
+
+int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, pp_handle** out) {
+  if (!out || !cfg) return PP_E_INVAL;
+  *out = nullptr;
+  std::string why;
+  int rc = validate_inputs(geo, ice, &why);
+  if (rc != PP_OK) return rc;
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return PP_E_CUDA;  // no CPU fallback
+  auto* h = new pp_handle();
+  h->cfg = *cfg;
+  h->ice = *ice;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { delete h; return PP_E_CUDA; }
+  if (cfg->device > 0) dev = cfg->device;
+  h->device = dev;
+  auto bail = [&](int code) { pp_destroy(h); return code; };
+  if (cudaSetDevice(dev) != cudaSuccess) return bail(PP_E_CUDA);
+  if (cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(PP_E_CUDA);
+  h->brute = (cfg->flags & PP_FLAG_BRUTE_FORCE_DOMS) != 0;
+  build_geometry(geo, h->brute, &h->hg);
+  if (!h->brute && !h->hg.fast_ok) return bail(PP_E_UNSUPPORTED);
+  fill_sizes(*cfg, h->n_sm, &h->sz);
+  h->hitq_budget = 1ull << 30;
+
+  // ---- workspaces ----
+  const uint64_t need_dev = carve_device(h, nullptr), need_pin = carve_pinned(h, nullptr);
+  if (cfg->device_workspace) {
+    if (cfg->device_workspace_bytes < need_dev) return bail(PP_E_NOMEM);
+    h->dev_ws = cfg->device_workspace;
+  } else {
+    if (cudaMalloc(&h->dev_ws, need_dev) != cudaSuccess) return bail(PP_E_NOMEM);
+    h->own_dev = true;
+  }
+  if (cfg->pinned_workspace) {
+    if (cfg->pinned_workspace_bytes < need_pin) return bail(PP_E_NOMEM);
+    h->pin_ws = cfg->pinned_workspace;
+  } else {
+    if (cudaHostAlloc(&h->pin_ws, need_pin, cudaHostAllocDefault) != cudaSuccess) return bail(PP_E_NOMEM);
+    h->own_pin = true;
+  }
+  carve_device(h, h->dev_ws);
+  carve_pinned(h, h->pin_ws);
+  if (cfg->stream0 && cfg->stream1) {
+    h->slot[0].stream = (cudaStream_t)cfg->stream0;
+    h->slot[1].stream = (cudaStream_t)cfg->stream1;
+  } else {
+    h->own_streams = true;
+    for (auto& s : h->slot)
+      if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return bail(PP_E_CUDA);
+  }
+  for (auto& s : h->slot) {
+    for (cudaEvent_t* e : {&s.ev_h2d, &s.ev_k0, &s.ev_k1, &s.ev_done, &s.ev_stage[0], &s.ev_stage[1]})
+      if (cudaEventCreate(e) != cudaSuccess) return bail(PP_E_CUDA);
+  }
+  if (cudaEventCreate(&h->ev_base) != cudaSuccess || cudaEventCreate(&h->ev_job) != cudaSuccess) return bail(PP_E_CUDA);
+
+  // ---- medium and geometry constants ----
+  LaunchParams& B = h->base;
+  std::vector<IceLayer> layers(ice->n_layers);
+  for (uint32_t i = 0; i < ice->n_layers; ++i) {
+    layers[i].la = ice->abs_len[i]; layers[i].lb = ice->scat_len[i];
+    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / (double)ice->scat_len[i]);
+  }
+  B.n_layers = ice->n_layers; B.z_top = ice->z_top; B.dz_layer = ice->dz; B.inv_dz_layer = (float)(1.0 / (double)ice->dz);
+  const double g = ice->g;
+  B.hg_one_minus_g = (float)(1.0 - g); B.hg_two_g = (float)(2.0 * g); B.hg_one_minus_g2 = (float)(1.0 - g * g);
+  B.one_minus_cos_c = (float)(1.0 - (double)ice->cos_cherenkov);
+  B.inv_v = (double)ice->n_group / kC;
+  {
+    uint32_t k0 = (uint32_t)cfg->seed, k1 = (uint32_t)(cfg->seed >> 32);
+    for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  }
+  B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
+  B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
+  B.nx = h->hg.nx; B.ny = h->hg.ny; B.gx0 = h->hg.gx0; B.gy0 = h->hg.gy0; B.inv_cell = h->hg.inv_cell;
+  B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
+  auto up = [&](const void* dst, const void* src, size_t bytes) {
+    return bytes == 0 || cudaMemcpy(const_cast<void*>(dst), src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
+  };
+  if (!up(B.ice, layers.data(), layers.size() * sizeof(IceLayer)) ||
+      !up(B.strings, h->hg.strings.data(), h->hg.strings.size() * sizeof(StringRec)) ||
+      !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)) ||
+      !up(B.cell_start, h->hg.cell_start.data(), h->hg.cell_start.size() * sizeof(uint16_t)) ||
+      !up(B.cell_items, h->hg.cell_items.data(), h->hg.cell_items.size() * sizeof(uint16_t)))
+    return bail(PP_E_CUDA);
+
+  // ---- persistent grid: every SM filled to the kernel's occupancy ----
+  h->smem = propagate_smem_bytes(h->hg.nx * h->hg.ny, (uint32_t)h->hg.cell_items.size());
+  {
+    // make the opt-in dynamic shared memory size known before asking for the occupancy
+    int bps = 0;
+    // a zero-work launch sets the function attribute (launch_propagate does it on first use)
+    Status zero{};
+    if (cudaMemcpy(h->slot[0].d_status, &zero, sizeof(zero), cudaMemcpyHostToDevice) != cudaSuccess) return bail(PP_E_CUDA);
+    LaunchParams P = B;
+    P.status = h->slot[0].d_status; P.n_tiles = 0; P.g_begin = P.g_end = 0; P.n_resume_in = 0;
+    P.resume_out = h->slot[0].d_resume[0]; P.resume_in = h->slot[0].d_resume[1]; P.resume_cap = (uint32_t)h->sz.resume_cap;
+    P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
+    P.tile_src = h->slot[0].d_tile_src;
+    for (int f = 0; f < 2; ++f)
+      if (launch_propagate(P, h->brute, f == 1, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
+    if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
+    if (propagate_occupancy(h->brute, false, h->smem, &bps) != cudaSuccess || bps < 1) return bail(PP_E_CUDA);
+    h->grid = h->n_sm * bps;
+  }
+  if (cudaEventRecord(h->ev_base, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
+  if (cudaEventSynchronize(h->ev_base) != cudaSuccess) return bail(PP_E_CUDA);
+  h->server = std::thread(server_main, h);
+  *out = h;
+  return PP_OK;
+}
+
+int pp_submit(pp_handle* h, const pp_source* src, const uint32_t* event_ids, const uint32_t* source_ids, size_t n) {
+  if (!h) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  if (n == 0) return PP_OK;
+  if (!src || !event_ids) return fail(h, PP_E_INVAL, "null sources or event_ids");
+  const float yield = h->ice.photons_per_GeV;
+  // validate everything before enqueueing anything
+  for (size_t i = 0; i < n; ++i) {
+    const pp_source& a = src[i];
+    const float v[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
+    for (float f : v)
+      if (!std::isfinite(f)) return fail(h, PP_E_INVAL, "non-finite field in source " + std::to_string(i));
+    const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
+    if (std::fabs(n2 - 1.0) > 1e-4) return fail(h, PP_E_INVAL, "source direction is not a unit vector");
+    if (a.energy_GeV < 0.0f) return fail(h, PP_E_INVAL, "negative source energy");
+    if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
+      return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
+  }
+  const bool nonblock = (h->cfg.flags & PP_FLAG_NONBLOCKING_SUBMIT) != 0;
+  size_t i = 0;
+  std::unique_lock<std::mutex> lk(h->mu);
+  if (h->shutdown) return PP_E_STATE;
+  if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
+  if (nonblock) {
+    if (n > h->sz.cap_src) return fail(h, PP_E_NOMEM, "batch larger than the source ring");
+    if (h->sz.cap_src - (h->ring_head - h->ring_tail) < n) { h->cv_work.notify_all(); return PP_E_WOULDBLOCK; }
+  }
+  while (i < n) {
+    uint64_t space = h->sz.cap_src - (h->ring_head - h->ring_tail);
+    if (space == 0) {
+      h->space_waiters++;
+      h->cv_work.notify_all();
+      h->cv_space.wait(lk, [&] { return h->sz.cap_src - (h->ring_head - h->ring_tail) > 0 || h->shutdown ||
+                                        h->sticky.load() != PP_OK; });
+      h->space_waiters--;
+      if (h->shutdown) return PP_E_STATE;
+      if (h->sticky.load() != PP_OK) return h->sticky.load();
+      continue;
+    }
+    const size_t m = (size_t)std::min<uint64_t>(space, n - i);
+    uint64_t ph = 0;
+    for (size_t j = 0; j < m; ++j, ++i) {
+      const pp_source& a = src[i];
+      SrcRec& r = h->ring[(h->ring_head + j) % h->sz.cap_src];
+      r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
+      r.event_id = event_ids[i];
+      r.source_id = source_ids ? source_ids[i] : (uint32_t)i;
+      r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
+      r.pad = 0;
+      ph += r.n_photons;
+    }
+    h->ring_head += m;
+    h->queued_photons += ph;
+    h->st.sources_submitted += m;
+    h->st.photons_submitted += ph;
+    h->st.source_ring_high_water =
+        std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_head - h->ring_tail) * sizeof(SrcRec));
+    if (h->queued_photons >= h->sz.target) h->cv_work.notify_all();
+  }
+  return PP_OK;
+}
+
+int pp_flush(pp_handle* h) {
+  if (!h) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  std::lock_guard<std::mutex> g(h->mu);
+  h->flush_upto = h->ring_head;
+  h->cv_work.notify_all();
+  return PP_OK;
+}
+
+int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block) {
+  if (!h || !n_out || (!out && cap)) return PP_E_INVAL;
+  *n_out = 0;
+  std::unique_lock<std::mutex> lk(h->mu);
+  for (;;) {
+    size_t got = 0;
+    while (got < cap && !h->hitq.empty()) {
+      auto& v = h->hitq.front();
+      const size_t m = std::min(cap - got, v.size() - h->hitq_front_off);
+      std::memcpy(out + got, v.data() + h->hitq_front_off, m * sizeof(pp_hit));
+      got += m;
+      h->hitq_front_off += m;
+      if (h->hitq_front_off == v.size()) {
+        h->hitq_bytes -= v.size() * sizeof(pp_hit);
+        h->hitq.pop_front();
+        h->hitq_front_off = 0;
+      }
+    }
+    if (got) {
+      *n_out = got;
+      h->st.hits_collected += got;
+      h->cv_space.notify_all();
+      return PP_OK;
+    }
+    if (h->sticky.load() != PP_OK) return h->sticky.load();
+    if (!block || cap == 0) return PP_OK;
+    if (idle_locked(h) && h->ring_launch == h->ring_head) return PP_OK;  // drained
+    h->cv_hits.wait_for(lk, std::chrono::milliseconds(5));
+  }
+}
+
+int pp_stats(pp_handle* h, pp_stats_t* out) {
+  if (!h || !out) return PP_E_INVAL;
+  std::lock_guard<std::mutex> g(h->mu);
+  *out = h->st;
+  if (h->wall_started) out->wall_ms = std::chrono::duration<double, std::milli>(h->wall_t1 - h->wall_t0).count();
+  return PP_OK;
+}
+
+const char* pp_last_error(pp_handle* h) {
+  if (!h) return "null handle";
+  std::lock_guard<std::mutex> g(h->err_mu);
+  return h->err.c_str();
+}
+
+void pp_destroy(pp_handle* h) {
+  if (!h) return;
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    h->shutdown = true;
+    h->cv_work.notify_all(); h->cv_space.notify_all(); h->cv_hits.notify_all();
+  }
+  if (h->server.joinable()) h->server.join();
+  cudaSetDevice(h->device);
+  for (auto& s : h->slot) {
+    if (s.stream) cudaStreamSynchronize(s.stream);
+    destroy_events(s);
+    if (h->own_streams && s.stream) cudaStreamDestroy(s.stream);
+  }
+  if (h->ev_base) cudaEventDestroy(h->ev_base);
+  if (h->ev_job) cudaEventDestroy(h->ev_job);
+  if (h->own_dev && h->dev_ws) cudaFree(h->dev_ws);
+  if (h->own_pin && h->pin_ws) cudaFreeHost(h->pin_ws);
+  delete h;
+}
+
+int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_event_ids, const uint32_t* d_source_ids,
+                    size_t n, pp_fate* d_fates, uint64_t* photons_out, double* device_ms_out) {
+  if (!h) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  if (photons_out) *photons_out = 0;
+  if (device_ms_out) *device_ms_out = 0.0;
+  if (n == 0) return PP_OK;
+  if (!d_sources || !d_event_ids) return fail(h, PP_E_INVAL, "null device pointer");
+  if (n > h->sz.cap_src) return fail(h, PP_E_NOMEM, "more sources than the source ring holds; raise source_ring_bytes");
+  {
+    std::unique_lock<std::mutex> lk(h->mu);
+    if (h->shutdown) return PP_E_STATE;
+    if (!idle_locked(h) || h->ring_launch != h->ring_head)
+      return fail(h, PP_E_STATE, "pp_run_resident needs an idle server (flush and collect first)");
+    h->resident_active = true;
+    if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
+  }
+  auto leave = [&](int rc) {
+    std::lock_guard<std::mutex> g(h->mu);
+    h->resident_active = false;
+    h->wall_t1 = Clock::now();
+    h->cv_hits.notify_all();
+    return rc;
+  };
+  cudaSetDevice(h->device);
+  Slot& s0 = h->slot[0];
+  cudaStream_t st = s0.stream;
+  // ---- a2: ingest + count + scan, once for the whole resident batch ----
+  cudaError_t e = cudaEventRecord(h->ev_job, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->d_res_overflow, 0, sizeof(unsigned int), st);
+  if (e == cudaSuccess)
+    e = launch_ingest(d_sources, d_event_ids, d_source_ids, (uint32_t)n, h->ice.photons_per_GeV, h->d_res_src,
+                      h->d_res_overflow, st);
+  if (e == cudaSuccess) e = launch_scan(h->d_res_src, (uint32_t)n, h->d_res_cum, st);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(h->h_res_total, h->d_res_cum + n, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(h->h_res_overflow, h->d_res_overflow, sizeof(unsigned int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaEventRecord(s0.ev_h2d, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return leave(fail(h, PP_E_CUDA, std::string("expansion: ") + cudaGetErrorString(e)));
+  if (*h->h_res_overflow) return leave(fail(h, PP_E_OVERFLOW, "a source has more than 2^32-1 photons"));
+  const uint64_t total = *h->h_res_total;
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    h->st.sources_submitted += n;
+    h->st.photons_submitted += total;
+  }
+  // the second stream must see the expansion results
+  if (cudaStreamWaitEvent(h->slot[1].stream, s0.ev_h2d, 0) != cudaSuccess) return leave(fail(h, PP_E_CUDA, "wait event"));
+  // ---- launches of at most `target` photons, alternating between the two slots ----
+  int rc = PP_OK;
+  int which = 0;
+  for (uint64_t g0 = 0; g0 < total && rc == PP_OK; g0 += h->sz.target) {
+    Slot& s = h->slot[which];
+    rc = drain_slot(h, s, false);
+    if (rc != PP_OK) break;
+    const uint64_t g1 = std::min(total, g0 + h->sz.target);
+    rc = enqueue_launch(h, s, h->d_res_src, h->d_res_cum, (uint32_t)n, g0, g1, d_fates);
+    which ^= 1;
+  }
+  // retire in launch order
+  for (int pass = 0; pass < 2; ++pass) {
+    Slot& s = h->slot[which];
+    const int r2 = drain_slot(h, s, false);
+    if (rc == PP_OK) rc = r2;
+    which ^= 1;
+  }
+  if (rc == PP_OK) {
+    float ms0 = 0, ms1 = 0;
+    cudaEventElapsedTime(&ms0, h->ev_job, h->slot[0].ev_done);
+    if (total > h->sz.target) cudaEventElapsedTime(&ms1, h->ev_job, h->slot[1].ev_done);
+    if (device_ms_out) *device_ms_out = std::max(ms0, ms1);
+    if (photons_out) *photons_out = total;
+  }
+  return leave(rc);
+}
+
+}  // extern "C"

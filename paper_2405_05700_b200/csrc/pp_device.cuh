@@ -1,0 +1,87 @@
+// Device-side building blocks of the photon propagator (sm_100a).  Product code: shares nothing
+// with oracle/.  Each function cites the step of DESIGN.md section 2 it implements.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "pp_types.h"
+
+namespace pp {
+
+// ---------------------------------------------------------------------------------------------
+// R-3: Philox4x32-10 with precomputed round keys; counter = (photon, source, event, flight).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3,
+                                              const uint32_t (&rk)[10][2]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[r][0];
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[r][1];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+  }
+}
+
+// u = (x >> 9) * 2^-23 + 2^-24, exactly (R-3): build 1.m from the top 23 bits with one funnel
+// shift, then subtract (1 - 2^-24); both steps are exact in fp32.
+__device__ __forceinline__ float uniform_from_word(uint32_t x) {
+  return __uint_as_float(__funnelshift_r(x, 0x7fu, 9)) - 0.99999994f;
+}
+
+__device__ __forceinline__ float fast_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float fast_rsqrt(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float fast_sqrt(float x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// Step 9a: Henyey-Greenstein, returned as m = 1 - cos(theta) in the cancellation-free form
+//   m = (1-g)(1-u)(q + 1 - g)/(1 - g + 2 g u),  q = (1-g^2)/(1 - g + 2 g u)        (R-1)
+__device__ __forceinline__ float hg_one_minus_cos(float u, float one_minus_g, float two_g, float one_minus_g2) {
+  const float inv = fast_rcp(fmaf(two_g, u, one_minus_g));
+  const float q = one_minus_g2 * inv;
+  return one_minus_g * (1.0f - u) * (q + one_minus_g) * inv;
+}
+
+// Step 2 / 9b: rotate d by polar angle (m = 1 - cos) and azimuth 2*pi*u_az about itself (R-9),
+// then renormalise with one Newton step (|n|^2 is within ~1e-6 of 1).
+__device__ __forceinline__ void rotate(float& dx, float& dy, float& dz, float m, float u_az) {
+  const float cos_t = 1.0f - m;
+  const float sin_t = fast_sqrt(fmaxf(m * (2.0f - m), 0.0f));
+  float sp, cp;
+  sincospif(2.0f * u_az, &sp, &cp);
+  const float rho2 = fmaf(dx, dx, dy * dy);
+  float nx, ny, nz;
+  if (rho2 > kPoleRho2) {
+    const float inv_rho = fast_rsqrt(rho2);
+    const float a = sin_t * inv_rho;
+    const float dzc = dz * cp;
+    nx = fmaf(a, fmaf(dx, dzc, -dy * sp), dx * cos_t);
+    ny = fmaf(a, fmaf(dy, dzc, dx * sp), dy * cos_t);
+    nz = fmaf(-sin_t * cp, rho2 * inv_rho, dz * cos_t);
+  } else {
+    nx = sin_t * cp;
+    ny = sin_t * sp;
+    nz = dz >= 0.0f ? cos_t : -cos_t;
+  }
+  const float n2 = fmaf(nx, nx, fmaf(ny, ny, nz * nz));
+  const float f = fmaf(-0.5f, n2, 1.5f);
+  dx = nx * f;
+  dy = ny * f;
+  dz = nz * f;
+}
+
+}  // namespace pp

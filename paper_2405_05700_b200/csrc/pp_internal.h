@@ -1,0 +1,33 @@
+// Internal interface between the host side of the library (pp_api.cpp) and its kernels
+// (pp_kernels.cu).  Not part of the public ABI.
+#pragma once
+#include <atomic>
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/pp.h"
+#include "pp_types.h"
+
+namespace pp {
+
+uint64_t kernel_launch_count();
+
+cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint32_t* d_sid, uint32_t n, float yield,
+                          SrcRec* d_out, unsigned int* d_overflow, cudaStream_t st);
+cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_cum, cudaStream_t st);
+cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
+                         uint32_t* d_tile_src, cudaStream_t st);
+size_t propagate_smem_bytes(uint32_t n_cells, uint32_t n_items);
+cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st);
+cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm);
+
+// Step 1 on the host (same arithmetic as the device's, exact in fp64).
+inline unsigned long long host_photon_count(float energy, float yield) {
+  const double n = __builtin_floor((double)energy * (double)yield + 0.5);
+  if (!(n > 0.0)) return 0ull;
+  if (n >= 1.8e19) return ~0ull;
+  return (unsigned long long)n;
+}
+
+}  // namespace pp

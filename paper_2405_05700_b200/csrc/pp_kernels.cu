@@ -1,0 +1,519 @@
+// CUDA kernels of the photon propagator (sm_100a): source expansion (a2) and the persistent
+// propagation kernel (a3-a8).  See DESIGN.md sections 2 and 5.  Product code: shares nothing with oracle/.
+#include <cuda_runtime.h>
+
+#include "../../include/pp.h"
+#include "pp_internal.h"
+#include "pp_device.cuh"
+
+namespace pp {
+
+static_assert(sizeof(SrcRec) == 48, "SrcRec layout");
+static_assert(sizeof(pp_hit) == 32, "pp_hit layout");
+static_assert(sizeof(pp_fate) == 40, "pp_fate layout");
+static_assert(sizeof(WorkItem) == 24, "WorkItem layout");
+
+// =============================================================================================
+// a2  Source expansion
+// =============================================================================================
+
+// Step 1 (R-12b): N = floor(double(E) * double(yield) + 0.5); exact in fp64 for fp32 inputs with
+// N < 2^32, so host and device agree bit for bit.  Returns 2^32 or more on overflow.
+__host__ __device__ inline unsigned long long photon_count(float energy, float yield) {
+  const double n = floor((double)energy * (double)yield + 0.5);
+  if (!(n > 0.0)) return 0ull;
+  if (n >= 1.8e19) return ~0ull;
+  return (unsigned long long)n;
+}
+
+// Resident path only: build SrcRec[] from the caller's device arrays and count photons.
+__global__ void ingest_kernel(const pp_source* __restrict__ s, const uint32_t* __restrict__ ev,
+                              const uint32_t* __restrict__ sid, uint32_t n, float yield, SrcRec* __restrict__ out,
+                              unsigned int* __restrict__ overflow) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const pp_source a = s[i];
+  unsigned long long cnt = photon_count(a.energy_GeV, yield);
+  if (cnt > 0xFFFFFFFFull) { atomicExch(overflow, 1u); cnt = 0; }
+  SrcRec r;
+  r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
+  r.event_id = ev[i]; r.source_id = sid ? sid[i] : i; r.n_photons = (uint32_t)cnt; r.pad = 0;
+  out[i] = r;
+}
+
+// Exclusive prefix sum of n_photons into cum[0..n] (64-bit).  One CTA of 1024 threads; each
+// thread owns a contiguous chunk.  n is at most a few 1e5-1e6 per launch, so one CTA suffices
+// (the scan is ~1e-4 of a launch).
+__global__ void __launch_bounds__(1024) scan_kernel(const SrcRec* __restrict__ src, uint32_t n,
+                                                    unsigned long long* __restrict__ cum) {
+  __shared__ unsigned long long part[1024];
+  const uint32_t t = threadIdx.x;
+  const uint32_t per = (n + 1023u) / 1024u;
+  const uint32_t lo = min(n, t * per), hi = min(n, lo + per);
+  unsigned long long s = 0;
+  for (uint32_t i = lo; i < hi; ++i) s += src[i].n_photons;
+  part[t] = s;
+  __syncthreads();
+  // Hillis-Steele inclusive scan over the 1024 partials
+  for (uint32_t off = 1; off < 1024; off <<= 1) {
+    unsigned long long v = (t >= off) ? part[t - off] : 0ull;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  unsigned long long run = (t == 0) ? 0ull : part[t - 1];
+  for (uint32_t i = lo; i < hi; ++i) {
+    cum[i] = run;
+    run += src[i].n_photons;
+  }
+  if (t == 1023) cum[n] = part[1023];
+}
+
+// tile_src[j] = index of the source that holds batch-global photon g_begin + j * kTilePhotons,
+// i.e. the last s with cum[s] <= g (sources with zero photons are skipped by construction).
+__global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_t n_src, unsigned long long g_begin,
+                             uint32_t n_tiles, uint32_t* __restrict__ tile_src) {
+  const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_tiles) return;
+  const unsigned long long g = g_begin + (unsigned long long)j * kTilePhotons;
+  uint32_t lo = 0, hi = n_src;  // invariant: cum[lo] <= g < cum[hi]
+  while (hi - lo > 1) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (cum[mid] <= g) lo = mid; else hi = mid;
+  }
+  tile_src[j] = lo;
+}
+
+// =============================================================================================
+// a3-a8  Persistent propagation kernel
+// =============================================================================================
+constexpr int kBlockThreads = 256;
+
+struct Smem {
+  IceLayer ice[PP_MAX_LAYERS];
+  float4 str_a[kMaxStringsSmem];  // x, y, z0, 1/pitch
+  uint2 str_b[kMaxStringsSmem];   // n, base
+};
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// Step 7 (slow path, rare): the flight passes within the pre-filter radius of the axis of string `si`;
+// test the DOMs whose z lies in the swept interval with the exact ray-sphere solve, using the
+// compensated position (ph + pl).  Updates (best_t, best_row) keeping the smallest t, ties to the
+// smaller public dom id.
+__device__ __noinline__ void test_string(const LaunchParams& P, const Smem& sm, uint32_t si, float phx, float phy,
+                                         float phz, float plx, float ply, float plz, float dx, float dy, float dz,
+                                         float s, float& best_t, uint32_t& best_dom) {
+  const float4 sa = sm.str_a[si];
+  const uint2 sb = sm.str_b[si];
+  const uint32_t n = sb.x, base = sb.y;
+  // interval of the flight inside the infinite cylinder of radius Rm about the axis
+  const float Rm = P.radius_margin;
+  const float ax = (sa.x - phx) - plx, ay = (sa.y - phy) - ply;
+  const float rho2 = fmaf(dx, dx, dy * dy);
+  float ta = 0.0f, tb = s;
+  if (rho2 > 1e-12f) {
+    const float inv = 1.0f / rho2;
+    const float tc = fmaf(ax, dx, ay * dy) * inv;
+    const float cr = fmaf(ax, dy, -ay * dx);
+    const float h2 = fmaf(Rm * Rm, rho2, -cr * cr);
+    if (h2 < 0.0f) return;
+    const float h = sqrtf(h2) * inv;
+    ta = fmaxf(0.0f, tc - h);
+    tb = fminf(s, tc + h);
+    if (ta > tb) return;
+  } else if (fmaf(ax, ax, ay * ay) > Rm * Rm) {
+    return;
+  }
+  const float za = fmaf(dz, ta, phz), zb = fmaf(dz, tb, phz);
+  const float zhi = fmaxf(za, zb) + Rm, zlo = fminf(za, zb) - Rm;
+  int k_lo = (int)ceilf((sa.z - zhi) * sa.w);
+  int k_hi = (int)floorf((sa.z - zlo) * sa.w);
+  k_lo = max(k_lo - 1, 0);  // one extra on each side: the arithmetic lookup is only a candidate filter
+  k_hi = min(k_hi + 1, (int)n - 1);
+  const float R = P.radius;
+  for (int k = k_lo; k <= k_hi; ++k) {
+    const float4 c = __ldg(&P.dom_xyzw[base + k]);
+    const float ox = (phx - c.x) + plx, oy = (phy - c.y) + ply, oz = (phz - c.z) + plz;
+    const float b = fmaf(ox, dx, fmaf(oy, dy, oz * dz));
+    const float qx = fmaf(-b, dx, ox), qy = fmaf(-b, dy, oy), qz = fmaf(-b, dz, oz);  // closest-approach vector
+    const float disc = fmaf(R, R, -fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+    if (disc < 0.0f) continue;
+    const float h = sqrtf(disc);
+    const float t_in = -b - h, t_out = -b + h;
+    if (t_out < 0.0f || t_in > s) continue;
+    const float t = fmaxf(t_in, 0.0f);
+    const uint32_t dom = __float_as_uint(c.w);
+    if (t < best_t || (t == best_t && dom < best_dom)) { best_t = t; best_dom = dom; }
+  }
+}
+
+// Validation variant of step 7: every DOM, every flight.
+__device__ __noinline__ void test_all_doms(const LaunchParams& P, float phx, float phy, float phz, float plx, float ply,
+                                           float plz, float dx, float dy, float dz, float s, float& best_t,
+                                           uint32_t& best_dom) {
+  const float R = P.radius;
+  for (uint32_t j = 0; j < P.n_dom; ++j) {
+    const float4 c = __ldg(&P.dom_xyzw[j]);
+    const float ox = (phx - c.x) + plx, oy = (phy - c.y) + ply, oz = (phz - c.z) + plz;
+    const float b = fmaf(ox, dx, fmaf(oy, dy, oz * dz));
+    const float qx = fmaf(-b, dx, ox), qy = fmaf(-b, dy, oy), qz = fmaf(-b, dz, oz);
+    const float disc = fmaf(R, R, -fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+    if (disc < 0.0f) continue;
+    const float h = sqrtf(disc);
+    const float t_in = -b - h, t_out = -b + h;
+    if (t_out < 0.0f || t_in > s) continue;
+    const float t = fmaxf(t_in, 0.0f);
+    const uint32_t dom = __float_as_uint(c.w);
+    if (t < best_t || (t == best_t && dom < best_dom)) { best_t = t; best_dom = dom; }
+  }
+}
+
+template <bool kBrute, bool kFates>
+__global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __grid_constant__ LaunchParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+  uint16_t* const cell_start = reinterpret_cast<uint16_t*>(smem_raw + sizeof(Smem));
+  uint16_t* const cell_items = cell_start + (P.nx * P.ny + 1);
+
+  // ---- stage the medium and the DOM lookup in shared memory (a4, a5) ----
+  for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) sm.ice[i] = P.ice[i];
+  if (!kBrute) {
+    for (uint32_t i = threadIdx.x; i < P.n_strings; i += blockDim.x) {
+      const StringRec r = P.strings[i];
+      sm.str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
+      sm.str_b[i] = make_uint2(r.n, r.base);
+    }
+    const uint32_t n_cells = P.nx * P.ny;
+    for (uint32_t i = threadIdx.x; i <= n_cells; i += blockDim.x) cell_start[i] = P.cell_start[i];
+    const uint32_t n_items = P.cell_start[n_cells];
+    for (uint32_t i = threadIdx.x; i < n_items; i += blockDim.x) cell_items[i] = P.cell_items[i];
+  }
+  __syncthreads();
+
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned lt = lanemask_lt();
+  Status* const st = P.status;
+
+  // ---- warp-uniform work state ----
+  unsigned long long g_next = 0, g_end = 0;  // current work item
+  uint32_t s_cur = 0;
+  bool more_work = true;                     // global queues may still hold work
+  bool use_resume = P.n_resume_in > 0;
+  bool warp_stop = false;                    // this warp saw the hit ring fill up: no more refills
+  unsigned long long w_started = 0, w_flights = 0;
+  uint32_t w_hits = 0, w_aborted = 0;
+
+  // ---- per-lane photon state ----
+  bool alive = false;
+  float phx = 0, phy = 0, phz = 0, plx = 0, ply = 0, plz = 0;  // position, two-float (hi + lo)
+  float dx = 0, dy = 0, dz = 1;
+  float Lh = 0, Ll = 0;  // path length, two-float
+  float tau_a = 0;
+  uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
+
+  for (;;) {
+    // =========================== refill dead lanes (a2 -> a3) ===========================
+    unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
+    if (need_mask && more_work && !warp_stop) {
+      bool need = !alive;
+      for (;;) {
+        if (g_next == g_end) {
+          // fetch the next work item: resume list first, then fresh tiles
+          unsigned long long a = 0, b = 0;
+          uint32_t sh = 0, res_left = use_resume ? 1u : 0u;
+          if (lane == 0 && *(volatile unsigned int*)&st->stop == 0u) {
+            if (use_resume) {
+              const unsigned r = atomicAdd(&st->resume_counter, 1u);
+              if (r < P.n_resume_in) {
+                const WorkItem w = P.resume_in[r];
+                a = w.g0; b = w.g1; sh = w.src;
+              } else {
+                res_left = 0u;
+              }
+            }
+            if (a == b) {
+              const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
+              if (j < P.n_tiles) {
+                a = P.g_begin + j * kTilePhotons;
+                b = min(a + (unsigned long long)kTilePhotons, P.g_end);
+                sh = __ldg(&P.tile_src[j]);
+                if (*(volatile unsigned int*)&st->stop != 0u) {
+                  // the ring filled up while we were fetching: hand the whole tile to the next launch
+                  const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+                  if (o < P.resume_cap) P.resume_out[o] = WorkItem{a, b, sh, 0u}; else atomicExch(&st->error, 1u);
+                  a = b = 0;
+                }
+              }
+            }
+          }
+          a = __shfl_sync(0xffffffffu, a, 0);
+          b = __shfl_sync(0xffffffffu, b, 0);
+          sh = __shfl_sync(0xffffffffu, sh, 0);
+          use_resume = __shfl_sync(0xffffffffu, res_left, 0) != 0u;
+          if (a == b) { more_work = false; break; }
+          g_next = a; g_end = b; s_cur = sh;
+        }
+        const unsigned long long avail = g_end - g_next;
+        const unsigned n_need = __popc(need_mask);
+        const unsigned take = (unsigned)min((unsigned long long)n_need, avail);
+        const unsigned rank = __popc(need_mask & lt);
+        uint32_t s_new = s_cur;
+        if (need && rank < take) {
+          // ---- a2/a3: initial state of batch-global photon g (fused expansion) ----
+          const unsigned long long g = g_next + rank;
+          uint32_t s = s_cur;
+          while (g >= __ldg(&P.cum[s + 1])) ++s;
+          s_new = s;
+          const float4* rp = reinterpret_cast<const float4*>(P.src + s);
+          const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
+          const uint4 r2 = __ldg(reinterpret_cast<const uint4*>(rp + 2));
+          phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
+          dx = r0.w; dy = r1.x; dz = r1.y;
+          Lh = 0.0f; Ll = 0.0f;
+          ev = r2.x; sid = r2.y;
+          pidx = (uint32_t)(g - __ldg(&P.cum[s]));
+          k = 0; s_mine = s;
+          alive = true;
+          need = false;
+        }
+        s_cur = __reduce_max_sync(0xffffffffu, s_new);
+        g_next += take;
+        w_started += take;
+        need_mask = __ballot_sync(0xffffffffu, need);
+        if (!need_mask) break;
+      }
+    }
+    const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+    if (!alive_mask) break;
+    w_flights += __popc(alive_mask);
+
+    bool hit = false, done = false, aborted = false;
+    uint32_t hit_dom = 0xFFFFFFFFu;
+    if (alive) {
+      // =========================== a7': Philox block k of this photon ===========================
+      uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
+      philox4x32_10(c0, c1, c2, c3, P.rk);
+      const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
+      const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
+      // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
+      const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
+      const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
+      rotate(dx, dy, dz, m, u_az);
+      // =========================== a3: absorption budget (once per photon) ======================
+      const float tau_new = -__logf(u_abs);
+      tau_a = (k == 0) ? tau_new : tau_a;
+      // =========================== a4: free path + fused layer walk =============================
+      float tau_s = -logf(u_dist);
+      int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
+      li = max(0, min(li, (int)P.n_layers - 1));
+      const bool up = dz > 0.0f;
+      const bool flat = fabsf(dz) < 1e-12f;
+      const float inv_dz = flat ? 0.0f : fast_rcp(dz);
+      const int last = (int)P.n_layers - 1;
+      const float zb = P.z_top - P.dz_layer * (float)(li + (up ? 0 : 1));
+      float l = fmaxf((zb - phz) * inv_dz, 0.0f);
+      const float step = P.dz_layer * fabsf(inv_dz);
+      const float inf = __int_as_float(0x7f800000);
+      if (flat || (up ? li == 0 : li == last)) l = inf;
+      float s = 0.0f;
+      bool absorbed;
+      for (;;) {
+        const IceLayer L = sm.ice[li];
+        const float ss = tau_s * L.lb, sa = tau_a * L.la;
+        const float mm = fminf(ss, sa);
+        if (mm <= l) {
+          s += mm;
+          absorbed = sa <= ss;
+          tau_a = fmaxf(0.0f, fmaf(-L.a, mm, tau_a));
+          break;
+        }
+        s += l;
+        tau_s = fmaxf(0.0f, fmaf(-L.b, l, tau_s));
+        tau_a = fmaxf(0.0f, fmaf(-L.a, l, tau_a));
+        li += up ? -1 : 1;
+        l = (up ? li == 0 : li == last) ? inf : step;
+      }
+      // =========================== a5: DOM intersection on [0, s] ===============================
+      float best_t = inf;
+      if (kBrute) {
+        test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best_t, hit_dom);
+      } else {
+        const float Rm = P.radius_margin;
+        const float ex = dx * s, ey = dy * s;
+        const float x_lo = fminf(phx, phx + ex) - Rm, x_hi = fmaxf(phx, phx + ex) + Rm;
+        const float y_lo = fminf(phy, phy + ey) - Rm, y_hi = fmaxf(phy, phy + ey) + Rm;
+        const float fx0 = (x_lo - P.gx0) * P.inv_cell, fx1 = (x_hi - P.gx0) * P.inv_cell;
+        const float fy0 = (y_lo - P.gy0) * P.inv_cell, fy1 = (y_hi - P.gy0) * P.inv_cell;
+        if (fx1 >= 0.0f && fy1 >= 0.0f && fx0 < (float)P.nx && fy0 < (float)P.ny) {
+          const int ix0 = max(0, (int)fx0), ix1 = min((int)P.nx - 1, (int)fx1);
+          const int iy0 = max(0, (int)fy0), iy1 = min((int)P.ny - 1, (int)fy1);
+          const float rho2 = fmaf(dx, dx, dy * dy);
+          const float thr = fmaf(Rm * Rm, rho2, 1e-12f);
+          for (int iy = iy0; iy <= iy1; ++iy) {
+            for (int ix = ix0; ix <= ix1; ++ix) {
+              const int cidx = iy * (int)P.nx + ix;
+              const uint32_t i0 = cell_start[cidx], i1 = cell_start[cidx + 1];
+              for (uint32_t it = i0; it < i1; ++it) {
+                const uint32_t si = cell_items[it];
+                const float4 sa4 = sm.str_a[si];
+                const float ax = sa4.x - phx, ay = sa4.y - phy;
+                const float cr = fmaf(ax, dy, -ay * dx);
+                if (cr * cr <= thr)
+                  test_string(P, sm, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best_t, hit_dom);
+              }
+            }
+          }
+        }
+      }
+      hit = best_t <= s;
+      // =========================== a6: advance / terminate ======================================
+      const float adv = hit ? best_t : s;
+      {
+        // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
+        // more fma (exact unless |p| << |d*adv| ulp-wise, where it is negligible anyway)
+        const float nx_ = fmaf(dx, adv, phx); plx += fmaf(dx, adv, phx - nx_); phx = nx_;
+        const float ny_ = fmaf(dy, adv, phy); ply += fmaf(dy, adv, phy - ny_); phy = ny_;
+        const float nz_ = fmaf(dz, adv, phz); plz += fmaf(dz, adv, phz - nz_); phz = nz_;
+        const float nl = Lh + adv; Ll += adv - (nl - Lh); Lh = nl;
+      }
+      ++k;
+      aborted = !hit && !absorbed && k >= P.max_flights;
+      done = hit || absorbed || aborted;
+    }
+
+    // =========================== a8: hit write (warp-aggregated) ================================
+    bool deferred = false;
+    const unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
+    if (hit_mask) {
+      const unsigned n_hit = __popc(hit_mask);
+      unsigned base = 0;
+      const int leader = __ffs(hit_mask) - 1;
+      if ((int)lane == leader) base = atomicAdd(&st->hit_count, n_hit);
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (hit) {
+        const unsigned slot = base + __popc(hit_mask & lt);
+        if (slot < P.ring_cap) {
+          const double t0 = (double)__ldg(&P.src[s_mine].t);
+          pp_hit h;
+          h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
+          h.time_ns = t0 + ((double)Lh + (double)Ll) * P.inv_v;
+          h.weight = 1.0f; h.n_scatter = k - 1;
+          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
+          const uint4* srcv = reinterpret_cast<const uint4*>(&h);
+          dst[0] = srcv[0];
+          dst[1] = srcv[1];
+        } else {
+          // ring full: this photon is replayed from scratch by the next launch (counter-based RNG)
+          deferred = true;
+          const unsigned long long g = __ldg(&P.cum[s_mine]) + pidx;
+          const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+          if (o < P.resume_cap) P.resume_out[o] = WorkItem{g, g + 1, s_mine, 0u}; else atomicExch(&st->error, 1u);
+          atomicExch(&st->stop, 1u);
+        }
+      }
+      const unsigned def_mask = __ballot_sync(0xffffffffu, deferred);
+      w_hits += n_hit - __popc(def_mask);
+      if (def_mask) {
+        // the replay will count these photons (and their flights) again: take them out here
+        warp_stop = true;
+        w_started -= __popc(def_mask);
+        w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
+      }
+    }
+    if (aborted) ++w_aborted;
+
+    if (kFates) {
+      if (alive && done && !deferred) {
+        const unsigned long long g = __ldg(&P.cum[s_mine]) + pidx;
+        pp_fate f;
+        f.x = phx + plx; f.y = phy + ply; f.z = phz + plz;
+        f.path_m = Lh + Ll;
+        f.time_ns = (double)__ldg(&P.src[s_mine].t) + ((double)Lh + (double)Ll) * P.inv_v;
+        f.n_flights = k;
+        f.dom = hit ? (int32_t)hit_dom : -1;
+        f.fate = hit ? 1u : (aborted ? 2u : 0u);
+        f.photon_idx = pidx;
+        reinterpret_cast<pp_fate*>(P.fates)[g] = f;
+      }
+    }
+    if (done) alive = false;
+  }
+
+  // ---- leftovers of a stopped warp go to the next launch; fold the counters ----
+  if (lane == 0) {
+    if (g_next < g_end) {
+      const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+      if (o < P.resume_cap) P.resume_out[o] = WorkItem{g_next, g_end, s_cur, 0u}; else atomicExch(&st->error, 1u);
+    }
+    atomicAdd(&st->photons_started, w_started);
+    atomicAdd(&st->flights, w_flights);
+    if (w_hits) atomicAdd(&st->photons_hit, (unsigned long long)w_hits);
+  }
+  const unsigned ab = __reduce_add_sync(0xffffffffu, w_aborted);
+  if (lane == 0 && ab) atomicAdd(&st->photons_aborted, (unsigned long long)ab);
+}
+
+// =============================================================================================
+// host-side launch wrappers (declared in pp_internal.h)
+// =============================================================================================
+static std::atomic<uint64_t> g_launches{0};
+uint64_t kernel_launch_count() { return g_launches.load(); }
+
+cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint32_t* d_sid, uint32_t n, float yield,
+                          SrcRec* d_out, unsigned int* d_overflow, cudaStream_t st) {
+  if (n == 0) return cudaSuccess;
+  ingest_kernel<<<(n + 255) / 256, 256, 0, st>>>(d_s, d_ev, d_sid, n, yield, d_out, d_overflow);
+  g_launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_cum, cudaStream_t st) {
+  scan_kernel<<<1, 1024, 0, st>>>(d_src, n, d_cum);
+  g_launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
+                         uint32_t* d_tile_src, cudaStream_t st) {
+  if (n_tiles == 0) return cudaSuccess;
+  tiles_kernel<<<(n_tiles + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, d_tile_src);
+  g_launches++;
+  return cudaGetLastError();
+}
+
+size_t propagate_smem_bytes(uint32_t n_cells, uint32_t n_items) {
+  return sizeof(Smem) + sizeof(uint16_t) * (size_t)(n_cells + 1 + n_items + 8);
+}
+
+template <bool B, bool F>
+static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
+  static std::atomic<size_t> attr_smem{0};  // opt-in dynamic shared memory size set so far
+  if (smem > attr_smem.load()) {
+    cudaError_t e = cudaFuncSetAttribute(propagate_kernel<B, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_smem.store(smem);
+  }
+  propagate_kernel<B, F><<<grid, kBlockThreads, smem, st>>>(P);
+  g_launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
+  if (brute) return fates ? launch_prop_t<true, true>(P, grid, smem, st) : launch_prop_t<true, false>(P, grid, smem, st);
+  return fates ? launch_prop_t<false, true>(P, grid, smem, st) : launch_prop_t<false, false>(P, grid, smem, st);
+}
+
+cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
+  if (brute)
+    return fates ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<true, true>, kBlockThreads, smem)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<true, false>, kBlockThreads, smem);
+  return fates ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<false, true>, kBlockThreads, smem)
+               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<false, false>, kBlockThreads, smem);
+}
+
+}  // namespace pp

@@ -1,0 +1,85 @@
+// Records shared by the host side (pp_api.cpp) and the kernels (pp_kernels.cu) of the library.
+// Not part of the public ABI.  Product code: shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace pp {
+
+// ---------------------------------------------------------------------------------------------
+// Records shared between host and device code of the library (not part of the public ABI).
+// ---------------------------------------------------------------------------------------------
+struct __align__(16) SrcRec {  // 48 B: one light source as the kernels see it
+  float x, y, z, dx;
+  float dy, dz, t, energy;
+  uint32_t event_id, source_id, n_photons, pad;
+};
+
+struct __align__(16) IceLayer {  // per-layer coefficients (1/m) and lengths (m)
+  float a, b, la, lb;
+};
+
+struct __align__(16) StringRec {  // one vertical line of DOMs with uniform pitch
+  float x, y, z0, pitch;          // z0 = z of DOM k = 0 (the highest); DOM k at z0 - k*pitch
+  float inv_pitch;
+  uint32_t n, base, pad;          // n DOMs; rows [base, base+n) of dom_xyzw
+};
+
+struct __align__(8) WorkItem {  // a range of batch-global photon numbers still to be run
+  uint64_t g0, g1;
+  uint32_t src, pad;
+};
+
+struct Status {                 // one per launch slot, device memory, copied back after every launch
+  unsigned long long tile_counter;    // next fresh tile
+  unsigned long long photons_started;
+  unsigned long long photons_hit;
+  unsigned long long photons_aborted;
+  unsigned long long flights;
+  unsigned int hit_count;       // hits reserved in the ring this launch (may exceed ring_cap)
+  unsigned int resume_counter;  // next resume_in item
+  unsigned int n_resume_out;    // items written to resume_out
+  unsigned int stop;            // set when the hit ring filled up
+  unsigned int error;           // internal invariant broken (resume list overflow)
+  unsigned int pad[3];
+};
+
+constexpr int kTilePhotons = 1024;  // photons per fresh work tile
+constexpr int kMaxStringsSmem = 512;
+constexpr float kPoleRho2 = 1e-10f;  // R-9
+
+// Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).
+struct LaunchParams {
+  // work
+  const SrcRec* src;
+  const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons
+  const uint32_t* tile_src;       // [n_tiles] source holding the first photon of each tile
+  unsigned long long g_begin, g_end;
+  uint32_t n_src, n_tiles;
+  const WorkItem* resume_in;
+  WorkItem* resume_out;
+  uint32_t n_resume_in, resume_cap;
+  Status* status;
+  void* ring;         // pp_hit[ring_cap]
+  uint32_t ring_cap;
+  uint32_t max_flights;
+  void* fates;        // pp_fate[g_end] or nullptr
+  // medium
+  const IceLayer* ice;  // [n_layers]
+  uint32_t n_layers;
+  float z_top, dz_layer, inv_dz_layer;
+  float hg_one_minus_g, hg_two_g, hg_one_minus_g2;  // 1-g, 2g, 1-g^2
+  float one_minus_cos_c;                             // 1 - cos(theta_c)
+  double inv_v;                                      // n_group / c  [ns/m]
+  uint32_t rk[10][2];                                // Philox round keys
+  // geometry
+  const StringRec* strings;  // [n_strings]
+  const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
+  const uint16_t* cell_start;  // [nx*ny + 1]
+  const uint16_t* cell_items;  // string indices
+  uint32_t n_strings, n_dom;
+  uint32_t nx, ny;
+  float gx0, gy0, inv_cell, radius, radius_margin;  // radius_margin = R + safety used by the pre-filter
+};
+
+}  // namespace pp
