@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""Benchmark of the photon-propagation hot path (BASELINE.json metric: photons propagated/s on one
+B200, layered ice, 5160 DOMs).
+
+  python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path
+  python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands
+
+A step = one pass of the whole hot path (a1..a9) over one batch of synthetic input: configuration C1
+(BASELINE.json configs[1]: 200 cascades on one 1 km muon, ~1.96e9 photons, 86x60 DOMs, 100 ice layers).
+`value` is measured with the sources already resident in HBM (pp_run_resident) and CUDA events;
+`e2e` goes through pp_submit / pp_flush / pp_collect with host buffers, copies included.
+N > 1 runs N independent replicas ("replicas only", no collective on the data path).
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "photons propagated/s on 1 B200, layered ice 5160 DOMs; % of SM FP32 roofline"
+UNIT = "photons/s"
+WORKLOAD = "C1: BASELINE.json configs[1], 200 cascades E^-1 1 GeV-10 TeV on a 1 km muon, 86x60 DOMs, 100 layers"
+
+# Thread-level instructions the propagation kernel executes per simulated flight (scattering step):
+# smsp__thread_inst_executed.sum / flights from the ncu capture named in profiles/ (DESIGN.md section 6).
+INSTR_PER_FLIGHT_FILE = os.path.join(ROOT, "profiles", "instr_per_flight.json")
+
+
+def load_instr_per_flight():
+    try:
+        with open(INSTR_PER_FLIGHT_FILE) as f:
+            d = json.load(f)
+        return float(d["thread_instructions_per_flight"]), d.get("dram_bytes_per_launch"), d.get("source", "")
+    except Exception:
+        return None, None, ""
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with nvidia-smi while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._th = None
+
+    def _run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip().split("\n")[0]
+                f = [x.strip() for x in out.split(",")]
+                self.samples.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                for nm, v in zip(names, f[2:6]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._th = threading.Thread(target=self._run, daemon=True)
+        self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._th.join(timeout=6)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def workload():
+    from paper_2405_05700_b200 import workloads as W
+    return W.geometry_full(), W.ice_layered(), W.sources_c1()
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------------
+def oracle_rate(geo, ice, src, seed, budget_s):
+    """Times the oracle, as it stands, on a strided sample of the workload sized for ~budget_s."""
+    from oracle import oracle as O
+    t = time.perf_counter()
+    r = O.propagate(geo, ice, src, seed=seed, stride=8192)
+    dt = time.perf_counter() - t
+    rate = r.photons / max(dt, 1e-9)
+    total = sum(O.photon_count(e, ice.photons_per_GeV) for e in src.src[:, 7])
+    stride = 8192
+    while stride > 1 and (total / (stride // 2)) / rate < budget_s:
+        stride //= 2
+    t = time.perf_counter()
+    r = O.propagate(geo, ice, src, seed=seed, stride=stride)
+    dt = time.perf_counter() - t
+    return {"photons": r.photons, "seconds": dt, "value": r.photons / dt, "flights_per_s": r.flights / dt,
+            "stride": stride, "hits": r.hit}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    geo, ice, src = workload()
+    cores = os.cpu_count() or 1
+    per_step_budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(geo, ice, src, 0, 0.5)
+    photons = 0
+    secs = 0.0
+    last = None
+    for k in range(args.steps):
+        last = oracle_rate(geo, ice, src, k, per_step_budget)
+        photons += last["photons"]
+        secs += last["seconds"]
+    value = photons / secs
+    sample = f"C1 photons with photon_idx % {last['stride']} == 0 ({last['photons']} photons per step)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# this repo's CUDA path
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2405_05700_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    from paper_2405_05700_b200 import replicas
+    geo, ice, src = workload()
+    seed = replicas.replica_seed(0, rank)  # independent replicas
+    target = 10 ** 8
+    prop = B.Propagator(geo, ice, seed=seed, launch_photons_target=target)
+    d = prop.upload(src.src, src.event_id, src.source_id)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    def l2_flush():
+        flush_buf.fill_(1)
+
+    s0, s1 = prop.streams
+    # ---- device-resident throughput (`value`) ----
+    for _ in range(args.warmup):
+        prop.run_resident(*d)
+        prop.drain()
+    st_before = prop.stats()
+    launches_before = B.kernel_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    photons = 0
+    hits = 0
+    barrier()
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            l2_flush()
+            torch.cuda.synchronize()
+            ev[k][0].record(s0)
+            ph, _, _ = prop.run_resident(*d)
+            s0.wait_stream(s1)
+            ev[k][1].record(s0)
+            photons += ph
+            hits += len(prop.drain())
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    launches = B.kernel_launch_count() - launches_before
+    st_after = prop.stats()
+    flights = st_after.flights - st_before.flights
+    busy_ms = st_after.kernel_busy_ms - st_before.kernel_busy_ms
+    n_prop_launches = st_after.launches - st_before.launches
+
+    # ---- end to end through pp_submit / pp_flush / pp_collect with host buffers (`e2e`) ----
+    pinned_src = torch.from_numpy(src.src.copy()).pin_memory().numpy()
+    for _ in range(min(args.warmup, 2)):
+        prop.run(pinned_src, src.event_id, src.source_id)
+    barrier()
+    e2e_hits = 0
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        e2e_hits += len(prop.run(pinned_src, src.event_id, src.source_id))
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    st_e2e = prop.stats()
+    e2e_launches = st_e2e.launches - st_after.launches
+
+    # ---- max over ranks ----
+    tmax, wsum = replicas.reduce_results(dist, torch.device("cuda", local), {"dev_ms": dev_ms, "e2e_s": e2e_s},
+                                         {"photons": float(photons)})
+    dev_ms_max, e2e_s_max, photons_all = tmax["dev_ms"], tmax["e2e_s"], wsum["photons"]
+    value = photons_all / (dev_ms_max * 1e-3)
+    e2e_value = photons_all / e2e_s_max
+
+    if rank == 0:
+        peaks = measured_peaks()
+        clocks = clk.summary()
+        ipf, dram_bytes, ipf_src = load_instr_per_flight()
+        sm_max = peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        roofline = None
+        if ipf is not None and busy_ms > 0:
+            # issue-slot roofline: every SM sub-partition issues at most one warp instruction (32 thread
+            # instructions) per clock: peak = SMs * 4 * 32 * f; f = max SM clock.
+            peak = n_sm * 4 * 32 * sm_max * 1e6 / 1e9  # G thread-instr/s
+            achieved = flights * ipf / (busy_ms * 1e-3) / 1e9
+            roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-level)",
+                        "frac": achieved / peak, "traffic": dram_bytes,
+                        "kernel": "pp::propagate_kernel<false,false>",
+                        "kernel_ms_per_launch": busy_ms / max(1, n_prop_launches),
+                        "units_per_launch": {"flights": flights / max(1, n_prop_launches)},
+                        "thread_instructions_per_flight": ipf, "per_unit_source": ipf_src,
+                        "peak_source": f"{n_sm} SMs x 4 issue slots x 32 lanes x {sm_max:.0f} MHz (max SM clock; "
+                                       "MEASURED_PEAKS.json sm_max_mhz)",
+                        "frac_at_observed_clock": (achieved / (n_sm * 4 * 32 * clocks["sm_mhz"] * 1e-3)
+                                                   if clocks.get("sm_mhz") else None)}
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            o = oracle_rate(geo, ice, src, 0, 15.0)
+            cpu = {"value": o["value"], "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                   "sample": f"C1 photons with photon_idx % {o['stride']} == 0 ({o['photons']} photons, {o['seconds']:.1f} s)",
+                   "flights_per_s": o["flights_per_s"]}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOAD, "photons_per_step": photons / args.steps, "launch_photons_target": target,
+                           "l2": "flushed between timed steps (256 MB write); inputs are 9.6 KB, the path is issue-bound",
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "hits_per_step": hits / args.steps},
+                "flights_per_s": flights / (dev_ms * 1e-3) * world, "device_busy_frac_resident": busy_ms / dev_ms,
+                "wall_s_timed_region": t_wall,
+                "e2e": {"value": e2e_value, "unit": UNIT,
+                        "h2d_bytes_per_step": int(len(src) * 48 + 0),
+                        "d2h_bytes_per_step": int(e2e_hits / args.steps * 32 + e2e_launches / args.steps * 64),
+                        "hits_per_step": e2e_hits / args.steps},
+                "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    prop.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

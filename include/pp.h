@@ -189,6 +189,28 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
                     const uint32_t* d_source_ids, size_t n, pp_fate* d_fates, uint64_t* photons_out,
                     double* device_ms_out);
 
+/* ---- host-only helpers (no CUDA call inside; usable and tested on a machine without a GPU) ----
+ * pp_check_inputs: the validation pp_create performs on geometry and ice (PP_E_INVAL), including whether
+ * the fast DOM lookup can represent the geometry (PP_E_UNSUPPORTED unless PP_FLAG_BRUTE_FORCE_DOMS).
+ * pp_photon_count: step 1 of the path, N = floor(double(E)*double(yield)+0.5); PP_E_OVERFLOW if N >= 2^32.
+ * pp_debug_plan_launches: the launch cutting the batching server applies ("when the step
+ * queue is sufficiently full, a block of steps is sent"): given the per-source photon counts in queue
+ * order and the per-launch target, lists the launches a flush of that queue produces.  Launch k covers
+ * sources [first_source, first_source + n_sources) and the photons [g_begin, g_end) of that slice's own
+ * exclusive prefix sum, so a source split across launches appears as the last source of one launch and
+ * the first of the next.  Returns PP_E_NOMEM (with *n_out = launches needed) if cap is too small. */
+typedef struct pp_launch_plan {
+  uint64_t first_source;
+  uint64_t n_sources;
+  uint64_t g_begin;
+  uint64_t g_end;
+} pp_launch_plan;
+
+int pp_check_inputs(const pp_geometry* geo, const pp_ice* ice, uint32_t flags);
+int pp_photon_count(float energy_GeV, float photons_per_GeV, uint64_t* n_out);
+int pp_debug_plan_launches(const uint32_t* photon_counts, size_t n, uint64_t target, pp_launch_plan* out, size_t cap,
+                           size_t* n_out);
+
 /* Library version and the number of CUDA kernels this library launched so far in this process. */
 const char* pp_version(void);
 uint64_t pp_kernel_launch_count(void);

@@ -64,7 +64,13 @@ class _Stats(C.Structure):
 
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
-           "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count"]
+           "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
+           "pp_photon_count", "pp_debug_plan_launches"]
+
+
+class _LaunchPlan(C.Structure):
+    _fields_ = [("first_source", C.c_uint64), ("n_sources", C.c_uint64), ("g_begin", C.c_uint64),
+                ("g_end", C.c_uint64)]
 
 _lib = None
 
@@ -100,12 +106,62 @@ def load_library(path: str = LIB_PATH):
     L.pp_run_resident.argtypes = [vp, vp, vp, vp, C.c_size_t, vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
     L.pp_version.restype = C.c_char_p
     L.pp_kernel_launch_count.restype = C.c_uint64
+    L.pp_check_inputs.restype = C.c_int
+    L.pp_check_inputs.argtypes = [C.POINTER(_Geometry), C.POINTER(_Ice), C.c_uint32]
+    L.pp_photon_count.restype = C.c_int
+    L.pp_photon_count.argtypes = [C.c_float, C.c_float, C.POINTER(C.c_uint64)]
+    L.pp_debug_plan_launches.restype = C.c_int
+    L.pp_debug_plan_launches.argtypes = [u32p, C.c_size_t, C.c_uint64, C.POINTER(_LaunchPlan), C.c_size_t,
+                                         C.POINTER(C.c_size_t)]
     _lib = L
     return L
 
 
 def kernel_launch_count() -> int:
     return int(load_library().pp_kernel_launch_count())
+
+
+def _marshal_inputs(geometry, ice):
+    fp = C.POINTER(C.c_float)
+    xyz = np.ascontiguousarray(geometry.xyz, dtype=np.float32).reshape(-1, 3)
+    a = np.ascontiguousarray(ice.abs_len, dtype=np.float32)
+    s = np.ascontiguousarray(ice.scat_len, dtype=np.float32)
+    geo = _Geometry(xyz.shape[0], xyz.ctypes.data_as(fp), float(geometry.radius))
+    ic = _Ice(a.shape[0], float(ice.z_top), float(ice.dz), a.ctypes.data_as(fp), s.ctypes.data_as(fp), float(ice.g),
+              float(ice.n_group), float(ice.cos_cherenkov), float(ice.photons_per_GeV))
+    return geo, ic, (xyz, a, s)
+
+
+def check_inputs(geometry, ice, flags: int = 0) -> int:
+    """pp_check_inputs: host-only validation; returns the status code (0 = OK)."""
+    geo, ic, keep = _marshal_inputs(geometry, ice)
+    return int(load_library().pp_check_inputs(C.byref(geo), C.byref(ic), int(flags)))
+
+
+def photon_count(energy_gev: float, photons_per_gev: float = 1.0e4) -> int:
+    n = C.c_uint64(0)
+    rc = load_library().pp_photon_count(float(np.float32(energy_gev)), float(np.float32(photons_per_gev)), C.byref(n))
+    if rc != PP_OK:
+        raise PPError(rc, "pp_photon_count")
+    return int(n.value)
+
+
+def plan_launches(photon_counts, target: int):
+    """pp_debug_plan_launches: list of (first_source, n_sources, g_begin, g_end)."""
+    cnt = np.ascontiguousarray(photon_counts, dtype=np.uint32)
+    L = load_library()
+    n_out = C.c_size_t(0)
+    cap = 64
+    while True:
+        buf = (_LaunchPlan * cap)()
+        rc = L.pp_debug_plan_launches(cnt.ctypes.data_as(C.POINTER(C.c_uint32)), cnt.shape[0], int(target), buf, cap,
+                                      C.byref(n_out))
+        if rc == -2:
+            cap = int(n_out.value)
+            continue
+        if rc != PP_OK:
+            raise PPError(rc, "pp_debug_plan_launches")
+        return [(int(b.first_source), int(b.n_sources), int(b.g_begin), int(b.g_end)) for b in buf[: n_out.value]]
 
 
 def pack_sources(src: np.ndarray) -> np.ndarray:
@@ -147,14 +203,7 @@ class Propagator:
             raise PPError(-3, "no CUDA device: the photon propagator has no CPU fallback")
         self._torch = torch
         self._L = load_library()
-        self._xyz = np.ascontiguousarray(geometry.xyz, dtype=np.float32).reshape(-1, 3)
-        self._abs = np.ascontiguousarray(ice.abs_len, dtype=np.float32)
-        self._scat = np.ascontiguousarray(ice.scat_len, dtype=np.float32)
-        fp = C.POINTER(C.c_float)
-        self._geo = _Geometry(self._xyz.shape[0], self._xyz.ctypes.data_as(fp), float(geometry.radius))
-        self._ice = _Ice(self._abs.shape[0], float(ice.z_top), float(ice.dz), self._abs.ctypes.data_as(fp),
-                         self._scat.ctypes.data_as(fp), float(ice.g), float(ice.n_group), float(ice.cos_cherenkov),
-                         float(ice.photons_per_GeV))
+        self._geo, self._ice, self._inputs_keep = _marshal_inputs(geometry, ice)
         cfg = _Config()
         cfg.seed = int(seed)
         cfg.launch_photons_target = int(launch_photons_target)
@@ -194,6 +243,7 @@ class Propagator:
         if getattr(self, "_h", None):
             self._L.pp_destroy(self._h)
             self._h = None
+            self._keep = []  # give the torch workspace back
 
     def __enter__(self):
         return self

@@ -462,37 +462,42 @@ int drain_slot(pp_handle* h, Slot& s, bool may_block) {
 // a1: the batching server thread
 // ---------------------------------------------------------------------------------------------
 
-// Cut the next launch from the source ring (caller holds h->mu).  Returns false if nothing to launch.
-struct Cut { uint64_t rec_a, rec_b, g_begin, g_end, photons; bool last_partial; };
+// Launch cutting (a1).  `count_at(i)` is the photon count of the i-th queued source, the first of
+// which has `first_offset` photons already launched.  Takes sources until `target` photons are
+// reached, splitting the last source's photon range if needed.  Pure function: also exposed for
+// CPU tests through pp_debug_plan_launches().
+struct Cut {
+  uint64_t n_rec;       // queued sources that take part in this launch (the last may be partial)
+  uint64_t g_begin;     // first photon of the launch, numbered within the launch's own prefix sum
+  uint64_t g_end;       // one past the last photon
+  uint64_t photons;     // g_end - g_begin
+  bool last_partial;    // the last source continues in the next launch ...
+  uint64_t next_offset; // ... from this photon index
+};
 
-bool cut_launch(pp_handle* h, bool force, Cut* c) {
-  if (h->queued_photons == 0) {
-    // nothing but zero-photon sources (or nothing at all): drop them
-    h->ring_launch = h->ring_head; h->launch_offset = 0;
-    return false;
-  }
-  const bool ring_pressure = h->space_waiters > 0;
-  if (h->queued_photons < h->sz.target && !force && !ring_pressure) return false;
-  uint64_t pos = h->ring_launch, acc = 0, cum_all = 0;
-  const uint64_t target = h->sz.target;
-  c->rec_a = pos; c->g_begin = h->launch_offset; c->last_partial = false;
-  while (pos < h->ring_head) {
-    const uint64_t np = h->ring[pos % h->sz.cap_src].n_photons;
-    const uint64_t avail = np - (pos == h->ring_launch ? h->launch_offset : 0);
+template <class CountAt>
+bool plan_cut(CountAt count_at, uint64_t n_avail, uint64_t first_offset, uint64_t target, Cut* c) {
+  uint64_t acc = 0, cum_all = 0;
+  c->g_begin = first_offset; c->last_partial = false; c->next_offset = 0;
+  uint64_t i = 0;
+  while (i < n_avail) {
+    const uint64_t np = count_at(i);
+    const uint64_t skip = (i == 0 ? first_offset : 0);
+    const uint64_t avail = np - skip;
     if (acc + avail > target) {  // split this source across launches
       const uint64_t take = target - acc;
-      acc += take; cum_all += np;
+      c->n_rec = i + 1;
+      c->g_end = cum_all + skip + take;
+      c->photons = acc + take;
       c->last_partial = true;
-      c->rec_b = pos + 1;
-      c->g_end = (cum_all - np) + (pos == h->ring_launch ? h->launch_offset : 0) + take;
-      c->photons = acc;
-      return true;
+      c->next_offset = skip + take;
+      return c->photons > 0;
     }
     acc += avail; cum_all += np;
-    ++pos;
+    ++i;
     if (acc == target) break;
   }
-  c->rec_b = pos; c->g_end = cum_all; c->photons = acc;
+  c->n_rec = i; c->g_end = cum_all; c->photons = acc;
   return acc > 0;
 }
 
@@ -530,28 +535,32 @@ void server_main(pp_handle* h) {
     if (!h->resident_active && h->n_in_flight < 2 && h->sticky.load() == PP_OK) {
       Slot& s = h->slot[next_slot].in_flight ? h->slot[next_slot ^ 1] : h->slot[next_slot];
       Cut c{};
-      const bool force = h->flush_upto > h->ring_launch;
-      if (!s.in_flight && cut_launch(h, force, &c)) {
-        const uint32_t n_src = (uint32_t)(c.rec_b - c.rec_a);
-        // bookkeeping under the lock; the records [rec_a, rec_b) stay valid until ring_tail passes them
-        h->queued_photons -= c.photons;
-        if (c.last_partial) {
-          // the split record stays queued; launch_offset counts its photons already launched
-          uint64_t before = 0;
-          for (uint64_t p = c.rec_a; p + 1 < c.rec_b; ++p) before += h->ring[p % h->sz.cap_src].n_photons;
-          h->ring_launch = c.rec_b - 1;
-          h->launch_offset = c.g_end - before;
-        } else {
-          h->ring_launch = c.rec_b;
-          h->launch_offset = 0;
+      const bool force = h->flush_upto > h->ring_launch || h->space_waiters > 0;
+      bool have = false;
+      if (!s.in_flight) {
+        if (h->queued_photons == 0) {  // nothing but zero-photon sources (or nothing at all): drop them
+          h->ring_launch = h->ring_tail = h->ring_head; h->launch_offset = 0;
+          h->cv_space.notify_all();
+        } else if (h->queued_photons >= h->sz.target || force) {
+          const uint64_t cap = h->sz.cap_src, base = h->ring_launch;
+          have = plan_cut([&](uint64_t i) { return (uint64_t)h->ring[(base + i) % cap].n_photons; },
+                          h->ring_head - base, h->launch_offset, h->sz.target, &c);
         }
+      }
+      if (have) {
+        const uint32_t n_src = (uint32_t)c.n_rec;
+        const uint64_t rec_a = h->ring_launch;
+        // bookkeeping under the lock; the records stay valid until ring_tail passes them
+        h->queued_photons -= c.photons;
+        if (c.last_partial) { h->ring_launch = rec_a + c.n_rec - 1; h->launch_offset = c.next_offset; }
+        else { h->ring_launch = rec_a + c.n_rec; h->launch_offset = 0; }
         s.in_flight = true;  // reserve
         h->n_in_flight++;
         lk.unlock();
         int rc = PP_OK;
         {
           const uint64_t cap = h->sz.cap_src;
-          const uint64_t a = c.rec_a % cap;
+          const uint64_t a = rec_a % cap;
           const uint64_t first = std::min<uint64_t>(n_src, cap - a);
           cudaError_t e = cudaMemcpyAsync(s.d_src, h->ring + a, first * sizeof(SrcRec), cudaMemcpyHostToDevice, s.stream);
           if (e == cudaSuccess && first < n_src)
@@ -599,6 +608,43 @@ bool idle_locked(pp_handle* h) {
 extern "C" {
 
 const char* pp_version(void) { return "pp 0.1 (sm_100a)"; }
+
+int pp_check_inputs(const pp_geometry* geo, const pp_ice* ice, uint32_t flags) {
+  std::string why;
+  int rc = validate_inputs(geo, ice, &why);
+  if (rc != PP_OK) return rc;
+  HostGeometry hg;
+  const bool brute = (flags & PP_FLAG_BRUTE_FORCE_DOMS) != 0;
+  build_geometry(geo, brute, &hg);
+  return (brute || hg.fast_ok) ? PP_OK : PP_E_UNSUPPORTED;
+}
+
+int pp_photon_count(float energy_GeV, float photons_per_GeV, uint64_t* n_out) {
+  if (!n_out || !std::isfinite(energy_GeV) || !std::isfinite(photons_per_GeV) || energy_GeV < 0.0f ||
+      photons_per_GeV < 0.0f)
+    return PP_E_INVAL;
+  const unsigned long long n = host_photon_count(energy_GeV, photons_per_GeV);
+  *n_out = n;
+  return n > 0xFFFFFFFFull ? PP_E_OVERFLOW : PP_OK;
+}
+
+int pp_debug_plan_launches(const uint32_t* photon_counts, size_t n, uint64_t target, pp_launch_plan* out, size_t cap,
+                           size_t* n_out) {
+  if ((!photon_counts && n) || !n_out || (!out && cap) || target == 0) return PP_E_INVAL;
+  size_t k = 0;
+  uint64_t first = 0, offset = 0;
+  while (first < n) {
+    Cut c{};
+    const bool ok = plan_cut([&](uint64_t i) { return (uint64_t)photon_counts[first + i]; }, n - first, offset, target, &c);
+    if (!ok) break;  // only zero-photon sources are left
+    if (k < cap) out[k] = pp_launch_plan{first, c.n_rec, c.g_begin, c.g_end};
+    ++k;
+    if (c.last_partial) { first += c.n_rec - 1; offset = c.next_offset; }
+    else { first += c.n_rec; offset = 0; }
+  }
+  *n_out = k;
+  return k > cap ? PP_E_NOMEM : PP_OK;
+}
 uint64_t pp_kernel_launch_count(void) { return kernel_launch_count(); }
 
 int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, uint64_t* device_bytes,

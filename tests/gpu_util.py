@@ -1,0 +1,66 @@
+"""Helpers shared by the -m gpu tests (which all drive the CUDA path through the C ABI binding)."""
+import numpy as np
+
+from oracle import oracle as O
+from paper_2405_05700_b200 import binding as B
+
+KEY = ["event_id", "source_id", "photon_idx"]
+TOL_NS = 1.0e-3  # BASELINE.json north_star: |dt| <= 1e-3 ns
+
+
+def sort_hits(h):
+    return np.sort(h, order=KEY)
+
+
+def total_photons(src, ice):
+    return int(sum(O.photon_count(e, ice.photons_per_GeV) for e in src.src[:, 7]))
+
+
+def gpu_run_resident(geo, ice, src, seed, want_fates=False, **kw):
+    """pp_run_resident through the binding; returns (sorted hits, fates, stats)."""
+    with B.Propagator(geo, ice, seed=seed, **kw) as p:
+        d = p.upload(src.src, src.event_id, src.source_id)
+        n_ph = total_photons(src, ice) if want_fates else None
+        ph, ms, fates = p.run_resident(*d, want_fates=want_fates, n_photons_hint=n_ph)
+        hits = sort_hits(p.drain())
+        st = p.stats()
+    return hits, fates, st
+
+
+def gpu_run(geo, ice, src, seed, **kw):
+    """pp_submit + pp_flush + pp_collect through the binding; returns (sorted hits, stats)."""
+    with B.Propagator(geo, ice, seed=seed, **kw) as p:
+        hits = sort_hits(p.run(src.src, src.event_id, src.source_id))
+        st = p.stats()
+    return hits, st
+
+
+def key_tuple(h):
+    return (h["event_id"].astype(np.uint64) << np.uint64(40)) ^ (h["source_id"].astype(np.uint64) << np.uint64(32)) ^ \
+        h["photon_idx"].astype(np.uint64)
+
+
+def compare_hits(gpu, ref, n_photons):
+    """Per-photon comparison of two hit lists (BASELINE.json north_star, reading R-13).
+
+    Returns a dict with: frac_all = fraction of ALL compared photons with the same hit DOM sequence and
+    |dt| <= 1e-3 ns (non-hitting photons agree trivially); frac_hit = the same fraction among photons
+    that hit in either implementation; n_union; max_dt over common same-DOM hits."""
+    kg = {(int(a), int(b), int(c)): i for i, (a, b, c) in enumerate(zip(gpu["event_id"], gpu["source_id"], gpu["photon_idx"]))}
+    kr = {(int(a), int(b), int(c)): i for i, (a, b, c) in enumerate(zip(ref["event_id"], ref["source_id"], ref["photon_idx"]))}
+    assert len(kg) == len(gpu) and len(kr) == len(ref), "a photon hit twice"
+    union = set(kg) | set(kr)
+    good = 0
+    dts = []
+    for k in union:
+        if k in kg and k in kr:
+            a, b = gpu[kg[k]], ref[kr[k]]
+            if a["dom_id"] == b["dom_id"]:
+                dt = abs(float(a["time_ns"]) - float(b["time_ns"]))
+                dts.append(dt)
+                if dt <= TOL_NS:
+                    good += 1
+    bad = len(union) - good
+    return {"frac_all": 1.0 - bad / max(1, n_photons), "frac_hit": good / max(1, len(union)), "n_union": len(union),
+            "n_gpu": len(gpu), "n_ref": len(ref), "max_dt": max(dts) if dts else 0.0,
+            "median_dt": float(np.median(dts)) if dts else 0.0}

@@ -1,0 +1,135 @@
+"""-m gpu: statistical comparison with INDEPENDENT random streams (reading R-14/R-15) and closed forms
+checked directly on the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from oracle import oracle as O
+from paper_2405_05700_b200 import binding as B
+from paper_2405_05700_b200 import workloads as W
+
+from gpu_util import gpu_run, gpu_run_resident, total_photons
+
+pytestmark = pytest.mark.gpu
+
+V = W.C_VACUUM / float(np.float32(W.N_GROUP))
+FAR = W.Geometry(xyz=np.array([[1.0e7, 0.0, 0.0]], np.float32), radius=0.1651)
+
+
+def test_gpu_homogeneous_closed_forms():
+    """The pins of tests/test_oracle_propagate.py applied to the CUDA path itself (2e6 photons)."""
+    ice = W.ice_homogeneous(cos_cherenkov=1.0)
+    src = W.pencil_beam([1.0, 2.0, 3.0], [0.3, -0.5, 0.81], 2.0e6, t0=12.5)
+    hits, fates, st = gpu_run_resident(FAR, ice, src, 17, want_fates=True)
+    n = len(fates)
+    assert st.photons_done == n == 2000000 and st.photons_hit == 0 and st.photons_aborted == 0
+    nf = fates["n_flights"].astype(np.int64)
+    assert nf.mean() == pytest.approx(5.0, abs=4 * math.sqrt(20.0 / n))
+    path = fates["path_m"].astype(np.float64)
+    assert path.mean() == pytest.approx(100.0, abs=4 * 100 / math.sqrt(n))
+    assert stats.kstest(path[::10], "expon", args=(0, 100.0)).pvalue > 1e-3
+    assert np.allclose(fates["time_ns"], 12.5 + path / V, atol=2e-3)
+    d0 = src.src[0, 3:6].astype(np.float64)
+    d0 /= np.linalg.norm(d0)
+    along = (np.stack([fates["x"] - 1.0, fates["y"] - 2.0, fates["z"] - 3.0], axis=1).astype(np.float64)) @ d0
+    assert along.mean() == pytest.approx(1 / (0.01 + 0.04 * 0.1), abs=4 * along.std() / math.sqrt(n))
+
+
+@pytest.mark.parametrize("dist", [20.0, 50.0])
+def test_gpu_unscattered_survival_to_a_sphere(dist):
+    R = 0.1651
+    geo = W.Geometry(xyz=np.array([[dist, 0.0, 0.0]], np.float32), radius=R)
+    src = W.pencil_beam([0, 0, 0], [1, 0, 0], 2.0e6)
+    hits, st = gpu_run(geo, W.ice_homogeneous(cos_cherenkov=1.0), src, 5)
+    Rf = float(np.float32(R))
+    expect = math.exp(-(dist - Rf) * (1 / 100.0 + 1 / 25.0))
+    direct = hits[hits["n_scatter"] == 0]
+    n = st.photons_done
+    assert len(direct) / n == pytest.approx(expect, abs=4 * math.sqrt(expect * (1 - expect) / n))
+    assert np.allclose(direct["time_ns"], (dist - Rf) / V, atol=1e-4)
+    hits2, st2 = gpu_run(geo, W.ice_homogeneous(scat_len=1e30, cos_cherenkov=1.0), src, 6)
+    e2 = math.exp(-(dist - Rf) / 100.0)
+    assert len(hits2) / n == pytest.approx(e2, abs=4 * math.sqrt(e2 * (1 - e2) / n))
+    assert np.all(hits2["n_scatter"] == 0)
+
+
+def test_gpu_hg_mean_cosine_via_transport():
+    """<cos theta> = g enters the closed form 1/(a + b(1-g)); vary g and check the GPU follows it."""
+    for g in (0.0, 0.5, 0.95):
+        ice = W.ice_homogeneous(g=g, cos_cherenkov=1.0)
+        src = W.pencil_beam([0, 0, 0], [0, 0, 1], 1.0e6)
+        _, fates, st = gpu_run_resident(FAR, ice, src, 3, want_fates=True)
+        z = fates["z"].astype(np.float64)
+        assert z.mean() == pytest.approx(1 / (0.01 + 0.04 * (1 - g)), abs=4.5 * z.std() / math.sqrt(len(z)))
+
+
+@pytest.mark.slow
+def test_independent_streams_per_dom_chi2_and_mean_times():
+    """BASELINE.json north_star: per-DOM hit counts agree with the oracle at chi^2 p > 0.01 over 10 seeds,
+    per-DOM mean arrival time within 0.5 %.  Reading R-14: independent streams (GPU seeds 0-9, oracle seeds
+    100-109), two-sample chi^2 per DOM with bins of expected count < 10 pooled, summed over the seeds;
+    R-15: mean times compared on DOMs whose standard error of the mean is < 0.1 %, else by z-score.
+    DOM radius 1 m so that the oracle's bounded sample has enough hits per DOM."""
+    geo, ice = W.geometry_full(radius=1.0), W.ice_layered()
+    src = W.sources_c1()
+    src.src[:, 7] = np.minimum(src.src[:, 7], 2.0) * 0.25  # <= 5000 photons per cascade: ~7e5 photons per seed
+    n_ph = total_photons(src, ice)
+    chi2_sum, dof_sum, pvals = 0.0, 0, []
+    tg_all, to_all = {}, {}
+    for k in range(10):
+        hg, _ = gpu_run(geo, ice, src, k)
+        ro = O.propagate(geo, ice, src, seed=100 + k)
+        cg = np.bincount(hg["dom_id"], minlength=geo.n_dom).astype(np.float64)
+        co = np.bincount(ro.hits["dom_id"], minlength=geo.n_dom).astype(np.float64)
+        # pool DOMs with small expectation into one bin
+        exp = 0.5 * (cg + co)
+        big = exp >= 10
+        a = np.concatenate([cg[big], [cg[~big].sum()]])
+        b = np.concatenate([co[big], [co[~big].sum()]])
+        keep = (a + b) > 0
+        chi2 = (((a - b) ** 2) / (a + b))[keep].sum()  # two equal-size samples
+        dof = int(keep.sum())
+        chi2_sum += chi2
+        dof_sum += dof
+        pvals.append(stats.chi2.sf(chi2, dof))
+        for dom, t in zip(hg["dom_id"], hg["time_ns"]):
+            tg_all.setdefault(int(dom), []).append(t)
+        for dom, t in zip(ro.hits["dom_id"], ro.hits["time_ns"]):
+            to_all.setdefault(int(dom), []).append(t)
+    p_tot = stats.chi2.sf(chi2_sum, dof_sum)
+    assert p_tot > 0.01, (p_tot, pvals)
+    assert sum(p < 0.01 for p in pvals) <= 1, pvals
+    # mean arrival times
+    zs = []
+    for dom in tg_all:
+        if dom in to_all and len(tg_all[dom]) >= 100 and len(to_all[dom]) >= 100:
+            a, b = np.array(tg_all[dom]), np.array(to_all[dom])
+            se = math.sqrt(a.var() / len(a) + b.var() / len(b))
+            rel = abs(a.mean() - b.mean()) / b.mean()
+            if se / b.mean() < 1e-3:
+                assert rel < 5e-3, (dom, rel)
+            zs.append((a.mean() - b.mean()) / se)
+    assert len(zs) > 20
+    zs = np.array(zs)
+    assert abs(zs.mean()) < 4 / math.sqrt(len(zs)) and np.abs(zs).max() < 5.0
+
+
+def test_identical_streams_per_dom_mean_time_bias():
+    """R-15 first half: with IDENTICAL streams, per-DOM mean arrival times of DOMs with >= 100 hits agree
+    to far better than 0.5 % (tests arithmetic bias, not statistics)."""
+    geo, ice = W.geometry_full(radius=1.0), W.ice_layered()
+    src = W.sources_c1()
+    src.src[:, 7] = np.minimum(src.src[:, 7], 2.0)  # <= 2e4 photons per cascade
+    hg, _ = gpu_run(geo, ice, src, 0)
+    ro = O.propagate(geo, ice, src, seed=0)
+    cg = np.bincount(hg["dom_id"], minlength=geo.n_dom)
+    co = np.bincount(ro.hits["dom_id"], minlength=geo.n_dom)
+    assert np.abs(cg - co).sum() <= 0.002 * co.sum() + 2
+    tg = np.bincount(hg["dom_id"], weights=hg["time_ns"], minlength=geo.n_dom)
+    to = np.bincount(ro.hits["dom_id"], weights=ro.hits["time_ns"], minlength=geo.n_dom)
+    sel = (co >= 100) & (cg == co)
+    assert sel.sum() > 10
+    rel = np.abs(tg[sel] / cg[sel] - to[sel] / co[sel]) / (to[sel] / co[sel])
+    assert rel.max() < 1e-6
