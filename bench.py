@@ -272,7 +272,8 @@ def run_ours(args):
                            "l2": "flushed between timed steps (256 MB write); inputs are 9.6 KB, the path is issue-bound",
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "hits_per_step": hits / args.steps},
-                "flights_per_s": flights / (dev_ms * 1e-3) * world, "device_busy_frac_resident": busy_ms / dev_ms,
+                "flights_per_s": flights / (dev_ms * 1e-3) * world, "flights_per_step": flights / args.steps,
+                "propagate_launches_per_step": n_prop_launches / args.steps, "device_busy_frac_resident": busy_ms / dev_ms,
                 "wall_s_timed_region": t_wall,
                 "e2e": {"value": e2e_value, "unit": UNIT,
                         "h2d_bytes_per_step": int(len(src) * 48 + 0),

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <condition_variable>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <deque>
 #include <map>
@@ -45,9 +46,10 @@ struct Carver {  // hands out aligned pieces of one workspace
 struct HostGeometry {
   std::vector<StringRec> strings;
   std::vector<float4> dom_xyzw;
-  std::vector<uint16_t> cell_start, cell_items;
-  uint32_t nx = 1, ny = 1;
-  float gx0 = 0, gy0 = 0, inv_cell = 1;
+  std::vector<float4> blk_xy;     // block table, see pp_types.h
+  std::vector<uint32_t> blk_id;
+  uint32_t bx = 1, by = 1, kq = 1;
+  float gx0 = 0, gy0 = 0, inv_cell = 1, cell = 1, xy_cap = 1;
   bool fast_ok = false;
   std::string why;
 };
@@ -189,6 +191,11 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
   const uint32_t n = geo->n_dom;
   out->fast_ok = false;
   if (brute) {
+    // validation mode: every DOM in input order; the block table of the fast path is still built when
+    // the geometry allows it, so that both modes cut sub-flights at the same xy cap (bit-identical results)
+    HostGeometry fast;
+    build_geometry(geo, false, &fast);
+    out->xy_cap = fast.fast_ok ? fast.xy_cap : 100.0f;
     out->dom_xyzw.resize(n);
     for (uint32_t j = 0; j < n; ++j) {
       float4 v;
@@ -196,7 +203,8 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
       std::memcpy(&v.w, &j, 4);
       out->dom_xyzw[j] = v;
     }
-    out->cell_start.assign(2, 0);
+    out->blk_xy.assign(1, make_float4(kEmptyXY, kEmptyXY, kEmptyXY, kEmptyXY));
+    out->blk_id.assign(1, 0xFFFFFFFFu);
     return;
   }
   struct Dom { float z; uint32_t id; };
@@ -236,7 +244,8 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
       out->dom_xyzw.push_back(c);
     }
   }
-  // cell size ~ median nearest-neighbour distance of the lines (100 m for a single line)
+  // cell size c ~ median nearest-neighbour distance of the lines (100 m for a single line), scaled by
+  // PP_CELL_SCALE (tuning knob, default 0.5); halved until no 2c x 2c block lists more than 8 lines
   const size_t ns = xy.size();
   double cell = 100.0;
   if (ns > 1) {
@@ -247,32 +256,53 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
     std::nth_element(nn.begin(), nn.begin() + ns / 2, nn.end());
     cell = std::max(1.0, nn[ns / 2]);
   }
-  const double Rm = (double)geo->radius + 5e-3, pad = Rm + 1e-2;
+  double scale = 0.5;
+  if (const char* e = std::getenv("PP_CELL_SCALE")) { const double v = std::atof(e); if (v > 0.01 && v < 100.0) scale = v; }
+  cell *= scale;
+  const double Rm = (double)geo->radius + 5e-3, slack = 0.05, pad = Rm + slack + 0.05;
   double x0 = 1e30, x1 = -1e30, y0 = 1e30, y1 = -1e30;
   for (auto& p : xy) { x0 = std::min(x0, (double)p.first); x1 = std::max(x1, (double)p.first);
                        y0 = std::min(y0, (double)p.second); y1 = std::max(y1, (double)p.second); }
   x0 -= pad; y0 -= pad; x1 += pad; y1 += pad;
-  uint32_t nx, ny;
   for (;;) {
-    nx = (uint32_t)std::floor((x1 - x0) / cell) + 1; ny = (uint32_t)std::floor((y1 - y0) / cell) + 1;
-    if ((uint64_t)nx * ny <= 4096) break;
-    cell *= 2.0;
+    if (cell - 2.0 * Rm - 2.0 * slack < 0.25 * cell) { out->why = "lines of DOMs too dense for the block table"; return; }
+    const uint32_t nx = (uint32_t)std::floor((x1 - x0) / cell) + 1, ny = (uint32_t)std::floor((y1 - y0) / cell) + 1;
+    const uint32_t bx = nx + 1, by = ny + 1;  // anchors -1 .. n-1
+    if ((uint64_t)bx * by > 16384) { cell *= 2.0; continue; }
+    std::vector<std::vector<uint16_t>> blocks((size_t)bx * by);
+    size_t kmax = 0;
+    for (size_t s = 0; s < ns; ++s) {
+      // block anchored at cell a covers [x0 + a c, x0 + (a + 2) c): the line's disc meets it for
+      // a in [floor((x - r - x0)/c) - 1, floor((x + r - x0)/c)], r = Rm + slack
+      const double r = Rm + slack;
+      const int ax0 = std::max(-1, (int)std::floor(((double)xy[s].first - r - x0) / cell) - 1);
+      const int ax1 = std::min((int)nx - 1, (int)std::floor(((double)xy[s].first + r - x0) / cell));
+      const int ay0 = std::max(-1, (int)std::floor(((double)xy[s].second - r - y0) / cell) - 1);
+      const int ay1 = std::min((int)ny - 1, (int)std::floor(((double)xy[s].second + r - y0) / cell));
+      for (int ay = ay0; ay <= ay1; ++ay)
+        for (int ax = ax0; ax <= ax1; ++ax) {
+          auto& b = blocks[(size_t)(ay + 1) * bx + (size_t)(ax + 1)];
+          b.push_back((uint16_t)s);
+          kmax = std::max(kmax, b.size());
+        }
+    }
+    if (kmax > 8) { cell *= 0.5; continue; }
+    const uint32_t kq = (uint32_t)std::max<size_t>(1, (kmax + 1) / 2);
+    out->blk_xy.assign((size_t)bx * by * kq, make_float4(kEmptyXY, kEmptyXY, kEmptyXY, kEmptyXY));
+    out->blk_id.assign((size_t)bx * by * kq, 0xFFFFFFFFu);
+    for (size_t b = 0; b < blocks.size(); ++b)
+      for (size_t i = 0; i < blocks[b].size(); ++i) {
+        const uint16_t si = blocks[b][i];
+        float4& e = out->blk_xy[b * kq + i / 2];
+        uint32_t& id = out->blk_id[b * kq + i / 2];
+        if (i % 2 == 0) { e.x = xy[si].first; e.y = xy[si].second; id = (id & 0xFFFF0000u) | si; }
+        else { e.z = xy[si].first; e.w = xy[si].second; id = (id & 0x0000FFFFu) | ((uint32_t)si << 16); }
+      }
+    out->bx = bx; out->by = by; out->kq = kq;
+    break;
   }
-  std::vector<std::vector<uint16_t>> cells((size_t)nx * ny);
-  for (size_t s = 0; s < ns; ++s) {
-    const int ix0 = std::max(0, (int)std::floor(((double)xy[s].first - pad - x0) / cell));
-    const int ix1 = std::min((int)nx - 1, (int)std::floor(((double)xy[s].first + pad - x0) / cell));
-    const int iy0 = std::max(0, (int)std::floor(((double)xy[s].second - pad - y0) / cell));
-    const int iy1 = std::min((int)ny - 1, (int)std::floor(((double)xy[s].second + pad - y0) / cell));
-    for (int iy = iy0; iy <= iy1; ++iy)
-      for (int ix = ix0; ix <= ix1; ++ix) cells[(size_t)iy * nx + ix].push_back((uint16_t)s);
-  }
-  out->cell_start.assign((size_t)nx * ny + 1, 0);
-  for (size_t c = 0; c < cells.size(); ++c) {
-    out->cell_start[c + 1] = (uint16_t)(out->cell_start[c] + cells[c].size());
-    for (auto s : cells[c]) out->cell_items.push_back(s);
-  }
-  out->nx = nx; out->ny = ny; out->gx0 = (float)x0; out->gy0 = (float)y0; out->inv_cell = (float)(1.0 / cell);
+  out->gx0 = (float)x0; out->gy0 = (float)y0; out->cell = (float)cell; out->inv_cell = (float)(1.0 / cell);
+  out->xy_cap = (float)(cell - 2.0 * Rm - 2.0 * slack);
   out->fast_ok = true;
 }
 
@@ -293,10 +323,10 @@ uint64_t carve_device(pp_handle* h, void* base) {
   auto* d_ice = c.take<IceLayer>(h->ice.n_layers);
   auto* d_strings = c.take<StringRec>(std::max<size_t>(1, g.strings.size()));
   auto* d_dom = c.take<float4>(g.dom_xyzw.size());
-  auto* d_cs = c.take<uint16_t>(g.cell_start.size());
-  auto* d_ci = c.take<uint16_t>(std::max<size_t>(1, g.cell_items.size()));
-  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.cell_start = d_cs;
-  h->base.cell_items = d_ci;
+  auto* d_bxy = c.take<float4>(g.blk_xy.size());
+  auto* d_bid = c.take<uint32_t>(g.blk_id.size());
+  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.blk_xy = d_bxy;
+  h->base.blk_id = d_bid;
   for (int i = 0; i < 2; ++i) {
     Slot& s = h->slot[i];
     s.d_src = c.take<SrcRec>(h->sz.cap_src);
@@ -743,20 +773,27 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   }
   B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
   B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
-  B.nx = h->hg.nx; B.ny = h->hg.ny; B.gx0 = h->hg.gx0; B.gy0 = h->hg.gy0; B.inv_cell = h->hg.inv_cell;
+  B.bx = h->hg.bx; B.by = h->hg.by; B.kq = h->hg.kq; B.gx0 = h->hg.gx0; B.gy0 = h->hg.gy0; B.inv_cell = h->hg.inv_cell;
   B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
+  B.xy_cap = h->hg.xy_cap;
+  {
+    // vertical sub-flight cap in layers (tuning knob PP_VCAP_LAYERS, default 6)
+    double t = 6.0;
+    if (const char* e = std::getenv("PP_VCAP_LAYERS")) { const double v = std::atof(e); if (v >= 1.0 && v <= 1000.0) t = v; }
+    B.v_cap = (float)(t * (double)ice->dz);
+  }
   auto up = [&](const void* dst, const void* src, size_t bytes) {
     return bytes == 0 || cudaMemcpy(const_cast<void*>(dst), src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
   if (!up(B.ice, layers.data(), layers.size() * sizeof(IceLayer)) ||
       !up(B.strings, h->hg.strings.data(), h->hg.strings.size() * sizeof(StringRec)) ||
       !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)) ||
-      !up(B.cell_start, h->hg.cell_start.data(), h->hg.cell_start.size() * sizeof(uint16_t)) ||
-      !up(B.cell_items, h->hg.cell_items.data(), h->hg.cell_items.size() * sizeof(uint16_t)))
+      !up(B.blk_xy, h->hg.blk_xy.data(), h->hg.blk_xy.size() * sizeof(float4)) ||
+      !up(B.blk_id, h->hg.blk_id.data(), h->hg.blk_id.size() * sizeof(uint32_t)))
     return bail(PP_E_CUDA);
 
   // ---- persistent grid: every SM filled to the kernel's occupancy ----
-  h->smem = propagate_smem_bytes(h->hg.nx * h->hg.ny, (uint32_t)h->hg.cell_items.size());
+  h->smem = propagate_smem_bytes((uint32_t)h->hg.blk_xy.size());
   {
     // make the opt-in dynamic shared memory size known before asking for the occupancy
     int bps = 0;

@@ -6,6 +6,10 @@
 #include "pp_internal.h"
 #include "pp_device.cuh"
 
+#ifndef PP_MIN_BLOCKS
+#define PP_MIN_BLOCKS 4  // resident CTAs of 256 threads per SM the propagation kernel is compiled for
+#endif
+
 namespace pp {
 
 static_assert(sizeof(SrcRec) == 48, "SrcRec layout");
@@ -101,13 +105,32 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   return m;
 }
 
-// Step 7 (slow path, rare): the flight passes within the pre-filter radius of the axis of string `si`;
-// test the DOMs whose z lies in the swept interval with the exact ray-sphere solve, using the
-// compensated position (ph + pl).  Updates (best_t, best_row) keeping the smallest t, ties to the
-// smaller public dom id.
-__device__ __noinline__ void test_string(const LaunchParams& P, const Smem& sm, uint32_t si, float phx, float phy,
+struct Best {  // nearest DOM entry found so far on the current sub-flight
+  float t;
+  uint32_t dom;
+};
+
+__device__ __forceinline__ void sphere_test(const float4 c, float R, float phx, float phy, float phz, float plx,
+                                            float ply, float plz, float dx, float dy, float dz, float s, Best& best) {
+  // Step 7: first point of [0, s] inside the closed ball; compensated position ph + pl (R-5, R-8)
+  const float ox = (phx - c.x) + plx, oy = (phy - c.y) + ply, oz = (phz - c.z) + plz;
+  const float b = fmaf(ox, dx, fmaf(oy, dy, oz * dz));
+  const float qx = fmaf(-b, dx, ox), qy = fmaf(-b, dy, oy), qz = fmaf(-b, dz, oz);  // closest-approach vector
+  const float disc = fmaf(R, R, -fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+  if (disc < 0.0f) return;
+  const float h = sqrtf(disc);
+  const float t_in = -b - h, t_out = -b + h;
+  if (t_out < 0.0f || t_in > s) return;
+  const float t = fmaxf(t_in, 0.0f);
+  const uint32_t dom = __float_as_uint(c.w);
+  if (t < best.t || (t == best.t && dom < best.dom)) { best.t = t; best.dom = dom; }
+}
+
+// Step 7 (slow path, rare): the sub-flight passes within the pre-filter radius of the axis of string
+// `si`; test the DOMs whose z lies in the swept interval with the exact ray-sphere solve.
+__device__ __noinline__ Best test_string(const LaunchParams& P, const Smem& sm, uint32_t si, float phx, float phy,
                                          float phz, float plx, float ply, float plz, float dx, float dy, float dz,
-                                         float s, float& best_t, uint32_t& best_dom) {
+                                         float s, Best best) {
   const float4 sa = sm.str_a[si];
   const uint2 sb = sm.str_b[si];
   const uint32_t n = sb.x, base = sb.y;
@@ -121,13 +144,13 @@ __device__ __noinline__ void test_string(const LaunchParams& P, const Smem& sm, 
     const float tc = fmaf(ax, dx, ay * dy) * inv;
     const float cr = fmaf(ax, dy, -ay * dx);
     const float h2 = fmaf(Rm * Rm, rho2, -cr * cr);
-    if (h2 < 0.0f) return;
+    if (h2 < 0.0f) return best;
     const float h = sqrtf(h2) * inv;
     ta = fmaxf(0.0f, tc - h);
     tb = fminf(s, tc + h);
-    if (ta > tb) return;
+    if (ta > tb) return best;
   } else if (fmaf(ax, ax, ay * ay) > Rm * Rm) {
-    return;
+    return best;
   }
   const float za = fmaf(dz, ta, phz), zb = fmaf(dz, tb, phz);
   const float zhi = fmaxf(za, zb) + Rm, zlo = fminf(za, zb) - Rm;
@@ -135,50 +158,25 @@ __device__ __noinline__ void test_string(const LaunchParams& P, const Smem& sm, 
   int k_hi = (int)floorf((sa.z - zlo) * sa.w);
   k_lo = max(k_lo - 1, 0);  // one extra on each side: the arithmetic lookup is only a candidate filter
   k_hi = min(k_hi + 1, (int)n - 1);
-  const float R = P.radius;
-  for (int k = k_lo; k <= k_hi; ++k) {
-    const float4 c = __ldg(&P.dom_xyzw[base + k]);
-    const float ox = (phx - c.x) + plx, oy = (phy - c.y) + ply, oz = (phz - c.z) + plz;
-    const float b = fmaf(ox, dx, fmaf(oy, dy, oz * dz));
-    const float qx = fmaf(-b, dx, ox), qy = fmaf(-b, dy, oy), qz = fmaf(-b, dz, oz);  // closest-approach vector
-    const float disc = fmaf(R, R, -fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
-    if (disc < 0.0f) continue;
-    const float h = sqrtf(disc);
-    const float t_in = -b - h, t_out = -b + h;
-    if (t_out < 0.0f || t_in > s) continue;
-    const float t = fmaxf(t_in, 0.0f);
-    const uint32_t dom = __float_as_uint(c.w);
-    if (t < best_t || (t == best_t && dom < best_dom)) { best_t = t; best_dom = dom; }
-  }
+  for (int k = k_lo; k <= k_hi; ++k)
+    sphere_test(__ldg(&P.dom_xyzw[base + k]), P.radius, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+  return best;
 }
 
-// Validation variant of step 7: every DOM, every flight.
-__device__ __noinline__ void test_all_doms(const LaunchParams& P, float phx, float phy, float phz, float plx, float ply,
-                                           float plz, float dx, float dy, float dz, float s, float& best_t,
-                                           uint32_t& best_dom) {
-  const float R = P.radius;
-  for (uint32_t j = 0; j < P.n_dom; ++j) {
-    const float4 c = __ldg(&P.dom_xyzw[j]);
-    const float ox = (phx - c.x) + plx, oy = (phy - c.y) + ply, oz = (phz - c.z) + plz;
-    const float b = fmaf(ox, dx, fmaf(oy, dy, oz * dz));
-    const float qx = fmaf(-b, dx, ox), qy = fmaf(-b, dy, oy), qz = fmaf(-b, dz, oz);
-    const float disc = fmaf(R, R, -fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
-    if (disc < 0.0f) continue;
-    const float h = sqrtf(disc);
-    const float t_in = -b - h, t_out = -b + h;
-    if (t_out < 0.0f || t_in > s) continue;
-    const float t = fmaxf(t_in, 0.0f);
-    const uint32_t dom = __float_as_uint(c.w);
-    if (t < best_t || (t == best_t && dom < best_dom)) { best_t = t; best_dom = dom; }
-  }
+// Validation variant of step 7: every DOM, every sub-flight.
+__device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, float phy, float phz, float plx, float ply,
+                                           float plz, float dx, float dy, float dz, float s, Best best) {
+  for (uint32_t j = 0; j < P.n_dom; ++j)
+    sphere_test(__ldg(&P.dom_xyzw[j]), P.radius, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+  return best;
 }
 
 template <bool kBrute, bool kFates>
-__global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __grid_constant__ LaunchParams P) {
+__global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
-  uint16_t* const cell_start = reinterpret_cast<uint16_t*>(smem_raw + sizeof(Smem));
-  uint16_t* const cell_items = cell_start + (P.nx * P.ny + 1);
+  float4* const blk_xy = reinterpret_cast<float4*>(smem_raw + sizeof(Smem));
+  uint32_t* const blk_id = reinterpret_cast<uint32_t*>(blk_xy + (size_t)P.bx * P.by * P.kq);
 
   // ---- stage the medium and the DOM lookup in shared memory (a4, a5) ----
   for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) sm.ice[i] = P.ice[i];
@@ -188,16 +186,15 @@ __global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __gri
       sm.str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
       sm.str_b[i] = make_uint2(r.n, r.base);
     }
-    const uint32_t n_cells = P.nx * P.ny;
-    for (uint32_t i = threadIdx.x; i <= n_cells; i += blockDim.x) cell_start[i] = P.cell_start[i];
-    const uint32_t n_items = P.cell_start[n_cells];
-    for (uint32_t i = threadIdx.x; i < n_items; i += blockDim.x) cell_items[i] = P.cell_items[i];
+    const uint32_t n_ent = P.bx * P.by * P.kq;
+    for (uint32_t i = threadIdx.x; i < n_ent; i += blockDim.x) { blk_xy[i] = P.blk_xy[i]; blk_id[i] = P.blk_id[i]; }
   }
   __syncthreads();
 
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
   Status* const st = P.status;
+  const float inf = __int_as_float(0x7f800000);
 
   // ---- warp-uniform work state ----
   unsigned long long g_next = 0, g_end = 0;  // current work item
@@ -206,14 +203,15 @@ __global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __gri
   bool use_resume = P.n_resume_in > 0;
   bool warp_stop = false;                    // this warp saw the hit ring fill up: no more refills
   unsigned long long w_started = 0, w_flights = 0;
-  uint32_t w_hits = 0, w_aborted = 0;
+  uint32_t w_hits = 0, w_aborted = 0;        // w_aborted is per lane
 
   // ---- per-lane photon state ----
   bool alive = false;
+  bool cont = false;  // the current free flight was cut by a sub-flight cap and continues
   float phx = 0, phy = 0, phz = 0, plx = 0, ply = 0, plz = 0;  // position, two-float (hi + lo)
   float dx = 0, dy = 0, dz = 1;
   float Lh = 0, Ll = 0;  // path length, two-float
-  float tau_a = 0;
+  float tau_a = 0, tau_s = 0;
   uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
 
   for (;;) {
@@ -278,7 +276,7 @@ __global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __gri
           ev = r2.x; sid = r2.y;
           pidx = (uint32_t)(g - __ldg(&P.cum[s]));
           k = 0; s_mine = s;
-          alive = true;
+          alive = true; cont = false;
           need = false;
         }
         s_cur = __reduce_max_sync(0xffffffffu, s_new);
@@ -290,89 +288,94 @@ __global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __gri
     }
     const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
     if (!alive_mask) break;
-    w_flights += __popc(alive_mask);
+    w_flights += __popc(__ballot_sync(0xffffffffu, alive && !cont));
 
     bool hit = false, done = false, aborted = false;
     uint32_t hit_dom = 0xFFFFFFFFu;
     if (alive) {
-      // =========================== a7': Philox block k of this photon ===========================
-      uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
-      philox4x32_10(c0, c1, c2, c3, P.rk);
-      const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
-      const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
-      // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
-      const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
-      const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
-      rotate(dx, dy, dz, m, u_az);
-      // =========================== a3: absorption budget (once per photon) ======================
-      const float tau_new = -__logf(u_abs);
-      tau_a = (k == 0) ? tau_new : tau_a;
-      // =========================== a4: free path + fused layer walk =============================
-      float tau_s = -logf(u_dist);
-      int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
-      li = max(0, min(li, (int)P.n_layers - 1));
-      const bool up = dz > 0.0f;
-      const bool flat = fabsf(dz) < 1e-12f;
-      const float inv_dz = flat ? 0.0f : fast_rcp(dz);
-      const int last = (int)P.n_layers - 1;
-      const float zb = P.z_top - P.dz_layer * (float)(li + (up ? 0 : 1));
-      float l = fmaxf((zb - phz) * inv_dz, 0.0f);
-      const float step = P.dz_layer * fabsf(inv_dz);
-      const float inf = __int_as_float(0x7f800000);
-      if (flat || (up ? li == 0 : li == last)) l = inf;
-      float s = 0.0f;
-      bool absorbed;
-      for (;;) {
-        const IceLayer L = sm.ice[li];
-        const float ss = tau_s * L.lb, sa = tau_a * L.la;
-        const float mm = fminf(ss, sa);
-        if (mm <= l) {
-          s += mm;
-          absorbed = sa <= ss;
-          tau_a = fmaxf(0.0f, fmaf(-L.a, mm, tau_a));
-          break;
-        }
-        s += l;
-        tau_s = fmaxf(0.0f, fmaf(-L.b, l, tau_s));
-        tau_a = fmaxf(0.0f, fmaf(-L.a, l, tau_a));
-        li += up ? -1 : 1;
-        l = (up ? li == 0 : li == last) ? inf : step;
+      if (!cont) {
+        // =========================== a7': Philox block k of this photon =========================
+        uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
+        philox4x32_10(c0, c1, c2, c3, P.rk);
+        const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
+        const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
+        // =========================== a7: emission (k = 0) or scatter (k > 0) ====================
+        const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
+        const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
+        rotate(dx, dy, dz, m, u_az);
+        // =========================== a3: absorption budget (once per photon) ====================
+        const float tau_new = -__logf(u_abs);
+        tau_a = (k == 0) ? tau_new : tau_a;
+        // =========================== a4: optical depth to the next scatter ======================
+        tau_s = -logf(u_dist);
       }
+      // =========================== a4: layer walk in vertical optical depth ======================
+      // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
+      // so the budgets are scaled by w = |d_z| once and the loop works in vertical metres.
+      const float w = fmaxf(fabsf(dz), 1e-9f);
+      const float inv_w = fast_rcp(w);
+      const float rho2 = fmaf(dx, dx, dy * dy);
+      const float inv_rho = fast_rsqrt(fmaxf(rho2, 1e-18f));
+      const bool up = dz > 0.0f;
+      const int last = (int)P.n_layers - 1;
+      int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
+      li = max(0, min(li, last));
+      const float zb = P.z_top - P.dz_layer * (float)(li + (up ? 0 : 1));
+      const float h0 = fmaxf(up ? zb - phz : phz - zb, 0.0f);  // vertical distance to the first boundary
+      // sub-flight cap in vertical metres, and the number of boundaries that fit under it
+      const float v_cap = fminf(P.v_cap, P.xy_cap * w * inv_rho);
+      int nb = up ? li : last - li;  // boundaries ahead before the infinite end layer
+      nb = min(nb, v_cap < h0 ? 0 : 1 + (int)((v_cap - h0) * P.inv_dz_layer));
+      const int dir = up ? -1 : 1;
+      float Ts = tau_s * w, Ta = tau_a * w, V = 0.0f, h = h0;
+      IceLayer L = sm.ice[li];
+      while (nb > 0) {
+        const float t1 = fmaf(-L.b, h, Ts), t2 = fmaf(-L.a, h, Ta);
+        if (t1 <= 0.0f || t2 <= 0.0f) break;  // the flight ends inside this layer
+        Ts = t1; Ta = t2; V += h;
+        h = P.dz_layer;
+        li += dir; --nb;
+        L = sm.ice[li];
+      }
+      const float vs = Ts * L.lb, va = Ta * L.la, vc = fmaxf(v_cap - V, 0.0f);
+      const float v = fminf(fminf(vs, va), vc);
+      const bool absorbed = (va <= vs) && (va <= vc);
+      const bool scattered = !absorbed && (vs <= vc);
+      V += v;
+      const float s = V * inv_w;
+      tau_a = fmaxf(0.0f, fmaf(-L.a, v, Ta)) * inv_w;
+      tau_s = fmaxf(0.0f, fmaf(-L.b, v, Ts)) * inv_w;
       // =========================== a5: DOM intersection on [0, s] ===============================
-      float best_t = inf;
+      Best best{inf, 0xFFFFFFFFu};
       if (kBrute) {
-        test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best_t, hit_dom);
+        best = test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
       } else {
         const float Rm = P.radius_margin;
         const float ex = dx * s, ey = dy * s;
-        const float x_lo = fminf(phx, phx + ex) - Rm, x_hi = fmaxf(phx, phx + ex) + Rm;
-        const float y_lo = fminf(phy, phy + ey) - Rm, y_hi = fmaxf(phy, phy + ey) + Rm;
-        const float fx0 = (x_lo - P.gx0) * P.inv_cell, fx1 = (x_hi - P.gx0) * P.inv_cell;
-        const float fy0 = (y_lo - P.gy0) * P.inv_cell, fy1 = (y_hi - P.gy0) * P.inv_cell;
-        if (fx1 >= 0.0f && fy1 >= 0.0f && fx0 < (float)P.nx && fy0 < (float)P.ny) {
-          const int ix0 = max(0, (int)fx0), ix1 = min((int)P.nx - 1, (int)fx1);
-          const int iy0 = max(0, (int)fy0), iy1 = min((int)P.ny - 1, (int)fy1);
-          const float rho2 = fmaf(dx, dx, dy * dy);
+        const float x_lo = fminf(phx, phx + ex) - Rm, y_lo = fminf(phy, phy + ey) - Rm;
+        const float fx = floorf((x_lo - P.gx0) * P.inv_cell), fy = floorf((y_lo - P.gy0) * P.inv_cell);
+        // anchors -1 .. (bx - 2) are stored at 0 .. (bx - 1); anything else cannot meet a string
+        if (fx >= -1.0f && fy >= -1.0f && fx < (float)(P.bx - 1) && fy < (float)(P.by - 1)) {
+          const uint32_t bidx = (((uint32_t)((int)fy + 1)) * P.bx + (uint32_t)((int)fx + 1)) * P.kq;
           const float thr = fmaf(Rm * Rm, rho2, 1e-12f);
-          for (int iy = iy0; iy <= iy1; ++iy) {
-            for (int ix = ix0; ix <= ix1; ++ix) {
-              const int cidx = iy * (int)P.nx + ix;
-              const uint32_t i0 = cell_start[cidx], i1 = cell_start[cidx + 1];
-              for (uint32_t it = i0; it < i1; ++it) {
-                const uint32_t si = cell_items[it];
-                const float4 sa4 = sm.str_a[si];
-                const float ax = sa4.x - phx, ay = sa4.y - phy;
-                const float cr = fmaf(ax, dy, -ay * dx);
-                if (cr * cr <= thr)
-                  test_string(P, sm, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best_t, hit_dom);
-              }
+          for (uint32_t q = 0; q < P.kq; ++q) {
+            const float4 c = blk_xy[bidx + q];
+            const float ax0 = c.x - phx, ay0 = c.y - phy, ax1 = c.z - phx, ay1 = c.w - phy;
+            const float cr0 = fmaf(ax0, dy, -ay0 * dx), cr1 = fmaf(ax1, dy, -ay1 * dx);
+            const bool p0 = cr0 * cr0 <= thr, p1 = cr1 * cr1 <= thr;
+            if (p0 || p1) {
+              const uint32_t ids = blk_id[bidx + q];
+              const uint32_t i0 = ids & 0xFFFFu, i1 = ids >> 16;
+              if (p0 && i0 != 0xFFFFu) best = test_string(P, sm, i0, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+              if (p1 && i1 != 0xFFFFu) best = test_string(P, sm, i1, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
             }
           }
         }
       }
-      hit = best_t <= s;
+      hit = best.t <= s;
+      hit_dom = best.dom;
       // =========================== a6: advance / terminate ======================================
-      const float adv = hit ? best_t : s;
+      const float adv = hit ? best.t : s;
       {
         // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
         // more fma (exact unless |p| << |d*adv| ulp-wise, where it is negligible anyway)
@@ -381,8 +384,9 @@ __global__ void __launch_bounds__(kBlockThreads, 3) propagate_kernel(const __gri
         const float nz_ = fmaf(dz, adv, phz); plz += fmaf(dz, adv, phz - nz_); phz = nz_;
         const float nl = Lh + adv; Ll += adv - (nl - Lh); Lh = nl;
       }
-      ++k;
-      aborted = !hit && !absorbed && k >= P.max_flights;
+      cont = !hit && !absorbed && !scattered;
+      k += cont ? 0u : 1u;  // k counts the free flights started = index of the next Philox block
+      aborted = !hit && !absorbed && !cont && k >= P.max_flights;
       done = hit || absorbed || aborted;
     }
 
@@ -486,8 +490,8 @@ cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsign
   return cudaGetLastError();
 }
 
-size_t propagate_smem_bytes(uint32_t n_cells, uint32_t n_items) {
-  return sizeof(Smem) + sizeof(uint16_t) * (size_t)(n_cells + 1 + n_items + 8);
+size_t propagate_smem_bytes(uint32_t n_block_entries) {
+  return sizeof(Smem) + (sizeof(float4) + sizeof(uint32_t)) * (size_t)n_block_entries + 16;
 }
 
 template <bool B, bool F>

@@ -47,6 +47,7 @@ struct Status {                 // one per launch slot, device memory, copied ba
 constexpr int kTilePhotons = 1024;  // photons per fresh work tile
 constexpr int kMaxStringsSmem = 512;
 constexpr float kPoleRho2 = 1e-10f;  // R-9
+constexpr float kEmptyXY = 3.0e18f;   // coordinate of an empty block-table slot (its square still fits fp32)
 
 // Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).
 struct LaunchParams {
@@ -75,11 +76,17 @@ struct LaunchParams {
   // geometry
   const StringRec* strings;  // [n_strings]
   const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
-  const uint16_t* cell_start;  // [nx*ny + 1]
-  const uint16_t* cell_items;  // string indices
+  // block table (a5): block (ix, iy) lists every string whose pre-filter disc meets the 2c x 2c square
+  // [gx0 + ix c, gx0 + (ix+2) c) x [gy0 + iy c, ...); a sub-flight is capped to an xy extent < c, so the
+  // block anchored at the cell of its bounding box's low corner holds all its candidates.
+  const float4* blk_xy;     // [bx*by][kq]: (x0, y0, x1, y1) of two strings; empty slots hold kEmptyXY
+  const uint32_t* blk_id;   // [bx*by][kq]: string indices, two 16-bit halves; 0xFFFF = empty
   uint32_t n_strings, n_dom;
-  uint32_t nx, ny;
+  uint32_t bx, by, kq;
   float gx0, gy0, inv_cell, radius, radius_margin;  // radius_margin = R + safety used by the pre-filter
+  // sub-flight caps: one loop iteration covers at most xy_cap metres in the xy-plane and v_cap metres
+  // in z; a longer free flight continues in the next iteration without a new random draw
+  float xy_cap, v_cap;
 };
 
 }  // namespace pp
