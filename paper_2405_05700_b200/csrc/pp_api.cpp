@@ -46,10 +46,9 @@ struct Carver {  // hands out aligned pieces of one workspace
 struct HostGeometry {
   std::vector<StringRec> strings;
   std::vector<float4> dom_xyzw;
-  std::vector<float4> blk_xy;     // block table, see pp_types.h
-  std::vector<uint32_t> blk_id;
-  uint32_t bx = 1, by = 1, kq = 1;
-  float gx0 = 0, gy0 = 0, inv_cell = 1, cell = 1, xy_cap = 1;
+  std::vector<uint16_t> cell_sid;  // cell table, see pp_types.h
+  uint32_t nx = 1, ny = 1;
+  float cell_ox = 0, cell_oy = 0, inv_cell = 1, xy_cap = 1;
   bool fast_ok = false;
   std::string why;
 };
@@ -67,6 +66,7 @@ struct Slot {
   // device
   SrcRec* d_src = nullptr;
   unsigned long long* d_cum = nullptr;
+  uint32_t* d_cum_rel = nullptr;
   uint32_t* d_tile_src = nullptr;
   Status* d_status = nullptr;
   WorkItem* d_resume[2] = {nullptr, nullptr};
@@ -203,8 +203,7 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
       std::memcpy(&v.w, &j, 4);
       out->dom_xyzw[j] = v;
     }
-    out->blk_xy.assign(1, make_float4(kEmptyXY, kEmptyXY, kEmptyXY, kEmptyXY));
-    out->blk_id.assign(1, 0xFFFFFFFFu);
+    out->cell_sid.assign(1, kNoString);
     return;
   }
   struct Dom { float z; uint32_t id; };
@@ -244,65 +243,64 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
       out->dom_xyzw.push_back(c);
     }
   }
-  // cell size c ~ median nearest-neighbour distance of the lines (100 m for a single line), scaled by
-  // PP_CELL_SCALE (tuning knob, default 0.5); halved until no 2c x 2c block lists more than 8 lines
+  // ---- cell table: THE candidate line for a sub-flight whose xy midpoint lies in a cell ----
+  // A sub-flight of xy length <= L that passes within Rm of a line has its midpoint within L/2 + Rm of it.
+  // If every cell is within reach = L/2 + Rm + slack of at most one line, the cell names that line; this
+  // holds when 2 reach + (cell diagonal) < d_min, the smallest distance between two lines.
   const size_t ns = xy.size();
-  double cell = 100.0;
-  if (ns > 1) {
-    std::vector<double> nn(ns, 1e30);
-    for (size_t i = 0; i < ns; ++i)
-      for (size_t j = 0; j < ns; ++j)
-        if (i != j) nn[i] = std::min(nn[i], std::hypot((double)xy[i].first - xy[j].first, (double)xy[i].second - xy[j].second));
-    std::nth_element(nn.begin(), nn.begin() + ns / 2, nn.end());
-    cell = std::max(1.0, nn[ns / 2]);
-  }
-  double scale = 0.5;
-  if (const char* e = std::getenv("PP_CELL_SCALE")) { const double v = std::atof(e); if (v > 0.01 && v < 100.0) scale = v; }
-  cell *= scale;
-  const double Rm = (double)geo->radius + 5e-3, slack = 0.05, pad = Rm + slack + 0.05;
+  double d_min = 1e30;
+  for (size_t i = 0; i < ns; ++i)
+    for (size_t j = i + 1; j < ns; ++j)
+      d_min = std::min(d_min, std::hypot((double)xy[i].first - xy[j].first, (double)xy[i].second - xy[j].second));
+  const double Rm = (double)geo->radius + 5e-3, slack = 0.02;
+  double L_max = 100.0;  // tuning knob PP_XY_CAP (metres)
+  if (const char* e = std::getenv("PP_XY_CAP")) { const double v = std::atof(e); if (v >= 1.0 && v <= 1.0e4) L_max = v; }
+  double cell = ns > 1 ? d_min / 6.0 : 32.0;
+  double L = ns > 1 ? std::min(L_max, d_min - 2.0 * (Rm + slack) - cell * std::sqrt(2.0) - slack) : L_max;
   double x0 = 1e30, x1 = -1e30, y0 = 1e30, y1 = -1e30;
   for (auto& p : xy) { x0 = std::min(x0, (double)p.first); x1 = std::max(x1, (double)p.first);
                        y0 = std::min(y0, (double)p.second); y1 = std::max(y1, (double)p.second); }
-  x0 -= pad; y0 -= pad; x1 += pad; y1 += pad;
-  for (;;) {
-    if (cell - 2.0 * Rm - 2.0 * slack < 0.25 * cell) { out->why = "lines of DOMs too dense for the block table"; return; }
-    const uint32_t nx = (uint32_t)std::floor((x1 - x0) / cell) + 1, ny = (uint32_t)std::floor((y1 - y0) / cell) + 1;
-    const uint32_t bx = nx + 1, by = ny + 1;  // anchors -1 .. n-1
-    if ((uint64_t)bx * by > 16384) { cell *= 2.0; continue; }
-    std::vector<std::vector<uint16_t>> blocks((size_t)bx * by);
-    size_t kmax = 0;
-    for (size_t s = 0; s < ns; ++s) {
-      // block anchored at cell a covers [x0 + a c, x0 + (a + 2) c): the line's disc meets it for
-      // a in [floor((x - r - x0)/c) - 1, floor((x + r - x0)/c)], r = Rm + slack
-      const double r = Rm + slack;
-      const int ax0 = std::max(-1, (int)std::floor(((double)xy[s].first - r - x0) / cell) - 1);
-      const int ax1 = std::min((int)nx - 1, (int)std::floor(((double)xy[s].first + r - x0) / cell));
-      const int ay0 = std::max(-1, (int)std::floor(((double)xy[s].second - r - y0) / cell) - 1);
-      const int ay1 = std::min((int)ny - 1, (int)std::floor(((double)xy[s].second + r - y0) / cell));
-      for (int ay = ay0; ay <= ay1; ++ay)
-        for (int ax = ax0; ax <= ax1; ++ax) {
-          auto& b = blocks[(size_t)(ay + 1) * bx + (size_t)(ax + 1)];
-          b.push_back((uint16_t)s);
-          kmax = std::max(kmax, b.size());
+  for (int attempt = 0;; ++attempt) {
+    if (!(L >= 1.0) || attempt > 60) { out->why = "lines of DOMs too dense for the cell table"; return; }
+    const double reach = 0.5 * L + Rm + slack, pad = reach + 2.0 * cell;  // >= one ring of empty cells all around
+    const double gx0 = x0 - pad, gy0 = y0 - pad;
+    const uint64_t nx = (uint64_t)std::ceil((x1 + pad - gx0) / cell) + 1, ny = (uint64_t)std::ceil((y1 + pad - gy0) / cell) + 1;
+    if (nx * ny > 40000) {  // keep the table in shared memory: coarser cells, shorter sub-flights
+      cell *= 1.25;
+      L = std::min(L, d_min - 2.0 * (Rm + slack) - cell * std::sqrt(2.0) - slack);
+      continue;
+    }
+    out->cell_sid.assign((size_t)(nx * ny), kNoString);
+    bool clash = false;
+    for (size_t s = 0; s < ns && !clash; ++s) {
+      const double sx = xy[s].first, sy = xy[s].second;
+      const int64_t ix0 = std::max<int64_t>(0, (int64_t)std::floor((sx - reach - gx0) / cell) - 1);
+      const int64_t ix1 = std::min<int64_t>((int64_t)nx - 1, (int64_t)std::floor((sx + reach - gx0) / cell) + 1);
+      const int64_t iy0 = std::max<int64_t>(0, (int64_t)std::floor((sy - reach - gy0) / cell) - 1);
+      const int64_t iy1 = std::min<int64_t>((int64_t)ny - 1, (int64_t)std::floor((sy + reach - gy0) / cell) + 1);
+      for (int64_t iy = iy0; iy <= iy1 && !clash; ++iy)
+        for (int64_t ix = ix0; ix <= ix1; ++ix) {
+          // distance from the line's axis to the cell rectangle
+          const double cx0 = gx0 + ix * cell, cy0 = gy0 + iy * cell;
+          const double ddx = std::max({cx0 - sx, 0.0, sx - (cx0 + cell)}), ddy = std::max({cy0 - sy, 0.0, sy - (cy0 + cell)});
+          if (ddx * ddx + ddy * ddy > reach * reach) continue;
+          uint16_t& c = out->cell_sid[(size_t)iy * nx + (size_t)ix];
+          if (c != kNoString) { clash = true; break; }
+          c = (uint16_t)s;
         }
     }
-    if (kmax > 8) { cell *= 0.5; continue; }
-    const uint32_t kq = (uint32_t)std::max<size_t>(1, (kmax + 1) / 2);
-    out->blk_xy.assign((size_t)bx * by * kq, make_float4(kEmptyXY, kEmptyXY, kEmptyXY, kEmptyXY));
-    out->blk_id.assign((size_t)bx * by * kq, 0xFFFFFFFFu);
-    for (size_t b = 0; b < blocks.size(); ++b)
-      for (size_t i = 0; i < blocks[b].size(); ++i) {
-        const uint16_t si = blocks[b][i];
-        float4& e = out->blk_xy[b * kq + i / 2];
-        uint32_t& id = out->blk_id[b * kq + i / 2];
-        if (i % 2 == 0) { e.x = xy[si].first; e.y = xy[si].second; id = (id & 0xFFFF0000u) | si; }
-        else { e.z = xy[si].first; e.w = xy[si].second; id = (id & 0x0000FFFFu) | ((uint32_t)si << 16); }
-      }
-    out->bx = bx; out->by = by; out->kq = kq;
+    if (clash) { L *= 0.9; continue; }
+    // the clamp in the kernel relies on an empty outer ring
+    for (uint64_t ix = 0; ix < nx; ++ix)
+      if (out->cell_sid[ix] != kNoString || out->cell_sid[(ny - 1) * nx + ix] != kNoString) { out->why = "internal: cell ring"; return; }
+    for (uint64_t iy = 0; iy < ny; ++iy)
+      if (out->cell_sid[iy * nx] != kNoString || out->cell_sid[iy * nx + nx - 1] != kNoString) { out->why = "internal: cell ring"; return; }
+    out->nx = (uint32_t)nx; out->ny = (uint32_t)ny;
+    out->inv_cell = (float)(1.0 / cell);
+    out->cell_ox = (float)(-gx0 / cell); out->cell_oy = (float)(-gy0 / cell);
+    out->xy_cap = (float)L;
     break;
   }
-  out->gx0 = (float)x0; out->gy0 = (float)y0; out->cell = (float)cell; out->inv_cell = (float)(1.0 / cell);
-  out->xy_cap = (float)(cell - 2.0 * Rm - 2.0 * slack);
   out->fast_ok = true;
 }
 
@@ -323,14 +321,13 @@ uint64_t carve_device(pp_handle* h, void* base) {
   auto* d_ice = c.take<IceLayer>(h->ice.n_layers);
   auto* d_strings = c.take<StringRec>(std::max<size_t>(1, g.strings.size()));
   auto* d_dom = c.take<float4>(g.dom_xyzw.size());
-  auto* d_bxy = c.take<float4>(g.blk_xy.size());
-  auto* d_bid = c.take<uint32_t>(g.blk_id.size());
-  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.blk_xy = d_bxy;
-  h->base.blk_id = d_bid;
+  auto* d_cell = c.take<uint16_t>(g.cell_sid.size());
+  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.cell_sid = d_cell;
   for (int i = 0; i < 2; ++i) {
     Slot& s = h->slot[i];
     s.d_src = c.take<SrcRec>(h->sz.cap_src);
     s.d_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
+    s.d_cum_rel = c.take<uint32_t>(h->sz.cap_src + 1);
     s.d_tile_src = c.take<uint32_t>(h->sz.max_tiles);
     s.d_status = c.take<Status>(1);
     s.d_resume[0] = c.take<WorkItem>(h->sz.resume_cap);
@@ -369,9 +366,9 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long
   const uint64_t n_ph = g_end - g_begin;
   const uint32_t n_tiles = (uint32_t)((n_ph + kTilePhotons - 1) / kTilePhotons);
   if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");
-  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, s.d_tile_src, s.stream));
+  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, s.d_tile_src, s.d_cum_rel, s.stream));
   LaunchParams P = h->base;
-  P.src = src; P.cum = cum; P.tile_src = s.d_tile_src;
+  P.src = src; P.cum = cum; P.cum_rel = s.d_cum_rel; P.tile_src = s.d_tile_src;
   P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles;
   s.resume_sel = 0;
   P.resume_in = s.d_resume[1]; P.resume_out = s.d_resume[0];
@@ -773,7 +770,8 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   }
   B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
   B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
-  B.bx = h->hg.bx; B.by = h->hg.by; B.kq = h->hg.kq; B.gx0 = h->hg.gx0; B.gy0 = h->hg.gy0; B.inv_cell = h->hg.inv_cell;
+  B.nx = h->hg.nx; B.ny = h->hg.ny; B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
+  B.cell_xmax = (float)(h->hg.nx - 1); B.cell_ymax = (float)(h->hg.ny - 1);
   B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
   B.xy_cap = h->hg.xy_cap;
   {
@@ -788,12 +786,11 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   if (!up(B.ice, layers.data(), layers.size() * sizeof(IceLayer)) ||
       !up(B.strings, h->hg.strings.data(), h->hg.strings.size() * sizeof(StringRec)) ||
       !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)) ||
-      !up(B.blk_xy, h->hg.blk_xy.data(), h->hg.blk_xy.size() * sizeof(float4)) ||
-      !up(B.blk_id, h->hg.blk_id.data(), h->hg.blk_id.size() * sizeof(uint32_t)))
+      !up(B.cell_sid, h->hg.cell_sid.data(), h->hg.cell_sid.size() * sizeof(uint16_t)))
     return bail(PP_E_CUDA);
 
   // ---- persistent grid: every SM filled to the kernel's occupancy ----
-  h->smem = propagate_smem_bytes((uint32_t)h->hg.blk_xy.size());
+  h->smem = propagate_smem_bytes(ice->n_layers, (uint32_t)h->hg.strings.size(), (uint32_t)h->hg.cell_sid.size());
   {
     // make the opt-in dynamic shared memory size known before asking for the occupancy
     int bps = 0;
@@ -804,7 +801,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.status = h->slot[0].d_status; P.n_tiles = 0; P.g_begin = P.g_end = 0; P.n_resume_in = 0;
     P.resume_out = h->slot[0].d_resume[0]; P.resume_in = h->slot[0].d_resume[1]; P.resume_cap = (uint32_t)h->sz.resume_cap;
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
-    P.tile_src = h->slot[0].d_tile_src;
+    P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
     for (int f = 0; f < 2; ++f)
       if (launch_propagate(P, h->brute, f == 1, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);

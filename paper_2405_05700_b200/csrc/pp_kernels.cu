@@ -74,10 +74,15 @@ __global__ void __launch_bounds__(1024) scan_kernel(const SrcRec* __restrict__ s
 }
 
 // tile_src[j] = index of the source that holds batch-global photon g_begin + j * kTilePhotons,
-// i.e. the last s with cum[s] <= g (sources with zero photons are skipped by construction).
+// i.e. the last s with cum[s] <= g (sources with zero photons are skipped by construction); and
+// cum_rel[s] = cum[s] - g_begin in 32 bits for the refill (see LaunchParams::cum_rel).
 __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_t n_src, unsigned long long g_begin,
-                             uint32_t n_tiles, uint32_t* __restrict__ tile_src) {
+                             uint32_t n_tiles, uint32_t* __restrict__ tile_src, uint32_t* __restrict__ cum_rel) {
   const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j <= n_src) {
+    const unsigned long long c = cum[j];
+    cum_rel[j] = c < g_begin ? (uint32_t)(c - g_begin) : (uint32_t)min(c - g_begin, 0xFFFFFFFFull);
+  }
   if (j >= n_tiles) return;
   const unsigned long long g = g_begin + (unsigned long long)j * kTilePhotons;
   uint32_t lo = 0, hi = n_src;  // invariant: cum[lo] <= g < cum[hi]
@@ -93,10 +98,12 @@ __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_
 // =============================================================================================
 constexpr int kBlockThreads = 256;
 
-struct Smem {
-  IceLayer ice[PP_MAX_LAYERS];
-  float4 str_a[kMaxStringsSmem];  // x, y, z0, 1/pitch
-  uint2 str_b[kMaxStringsSmem];   // n, base
+// Shared-memory tables, staged once per launch: [IceLayer x n_layers][float4 x n_str][uint2 x n_str][u16 x cells]
+struct Tables {
+  const IceLayer* ice;
+  const float4* str_a;   // x, y, z0, 1/pitch
+  const uint2* str_b;    // n, base
+  const uint16_t* cell;  // candidate line per cell
 };
 
 __device__ __forceinline__ unsigned lanemask_lt() {
@@ -126,13 +133,13 @@ __device__ __forceinline__ void sphere_test(const float4 c, float R, float phx, 
   if (t < best.t || (t == best.t && dom < best.dom)) { best.t = t; best.dom = dom; }
 }
 
-// Step 7 (slow path, rare): the sub-flight passes within the pre-filter radius of the axis of string
+// Step 7 (slow path, rare): the sub-flight passes within the pre-filter radius of the axis of line
 // `si`; test the DOMs whose z lies in the swept interval with the exact ray-sphere solve.
-__device__ __noinline__ Best test_string(const LaunchParams& P, const Smem& sm, uint32_t si, float phx, float phy,
+__device__ __noinline__ Best test_string(const LaunchParams& P, const Tables& T, uint32_t si, float phx, float phy,
                                          float phz, float plx, float ply, float plz, float dx, float dy, float dz,
                                          float s, Best best) {
-  const float4 sa = sm.str_a[si];
-  const uint2 sb = sm.str_b[si];
+  const float4 sa = T.str_a[si];
+  const uint2 sb = T.str_b[si];
   const uint32_t n = sb.x, base = sb.y;
   // interval of the flight inside the infinite cylinder of radius Rm about the axis
   const float Rm = P.radius_margin;
@@ -174,36 +181,37 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
 template <bool kBrute, bool kFates>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
-  float4* const blk_xy = reinterpret_cast<float4*>(smem_raw + sizeof(Smem));
-  uint32_t* const blk_id = reinterpret_cast<uint32_t*>(blk_xy + (size_t)P.bx * P.by * P.kq);
+  const uint32_t n_str_alloc = max(P.n_strings, 1u);
+  IceLayer* const s_ice = reinterpret_cast<IceLayer*>(smem_raw);
+  float4* const s_str_a = reinterpret_cast<float4*>(s_ice + P.n_layers);
+  uint2* const s_str_b = reinterpret_cast<uint2*>(s_str_a + n_str_alloc);
+  uint16_t* const s_cell = reinterpret_cast<uint16_t*>(s_str_b + n_str_alloc);
 
   // ---- stage the medium and the DOM lookup in shared memory (a4, a5) ----
-  for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) sm.ice[i] = P.ice[i];
+  for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) s_ice[i] = P.ice[i];
   if (!kBrute) {
     for (uint32_t i = threadIdx.x; i < P.n_strings; i += blockDim.x) {
       const StringRec r = P.strings[i];
-      sm.str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
-      sm.str_b[i] = make_uint2(r.n, r.base);
+      s_str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
+      s_str_b[i] = make_uint2(r.n, r.base);
     }
-    const uint32_t n_ent = P.bx * P.by * P.kq;
-    for (uint32_t i = threadIdx.x; i < n_ent; i += blockDim.x) { blk_xy[i] = P.blk_xy[i]; blk_id[i] = P.blk_id[i]; }
+    const uint32_t n_cell = P.nx * P.ny;
+    for (uint32_t i = threadIdx.x; i < n_cell; i += blockDim.x) s_cell[i] = P.cell_sid[i];
   }
   __syncthreads();
+  const Tables T{s_ice, s_str_a, s_str_b, s_cell};
+  const float2* const lay = reinterpret_cast<const float2*>(s_ice);  // [2 li] = (a, b), [2 li + 1] = (1/a, 1/b)
 
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
   Status* const st = P.status;
   const float inf = __int_as_float(0x7f800000);
 
-  // ---- warp-uniform work state ----
-  unsigned long long g_next = 0, g_end = 0;  // current work item
-  uint32_t s_cur = 0;
-  bool more_work = true;                     // global queues may still hold work
+  // ---- warp-uniform work state: photons [t_next, t_end) of the launch (numbered from g_begin) ----
+  uint32_t t_next = 0, t_end = 0, s_cur = 0;
+  bool refill_ok = true;   // false once the queues are empty or the hit ring filled up
   bool use_resume = P.n_resume_in > 0;
-  bool warp_stop = false;                    // this warp saw the hit ring fill up: no more refills
-  unsigned long long w_started = 0, w_flights = 0;
-  uint32_t w_hits = 0, w_aborted = 0;        // w_aborted is per lane
+  uint32_t w_started = 0, w_hits = 0;
 
   // ---- per-lane photon state ----
   bool alive = false;
@@ -213,82 +221,76 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   float Lh = 0, Ll = 0;  // path length, two-float
   float tau_a = 0, tau_s = 0;
   uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
+  uint32_t n_flights = 0, n_aborted = 0;  // per-lane totals over finished photons
 
   for (;;) {
     // =========================== refill dead lanes (a2 -> a3) ===========================
-    unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
-    if (need_mask && more_work && !warp_stop) {
-      bool need = !alive;
-      for (;;) {
-        if (g_next == g_end) {
-          // fetch the next work item: resume list first, then fresh tiles
-          unsigned long long a = 0, b = 0;
-          uint32_t sh = 0, res_left = use_resume ? 1u : 0u;
-          if (lane == 0 && *(volatile unsigned int*)&st->stop == 0u) {
-            if (use_resume) {
-              const unsigned r = atomicAdd(&st->resume_counter, 1u);
-              if (r < P.n_resume_in) {
-                const WorkItem w = P.resume_in[r];
-                a = w.g0; b = w.g1; sh = w.src;
-              } else {
-                res_left = 0u;
-              }
+    const unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
+    if (need_mask != 0u && refill_ok) {
+      if (t_next == t_end) {
+        // fetch the next work item: resume list first, then fresh tiles
+        unsigned long long a = 0, b = 0;
+        uint32_t sh = 0, res_left = use_resume ? 1u : 0u;
+        if (lane == 0 && *(volatile unsigned int*)&st->stop == 0u) {
+          if (use_resume) {
+            const unsigned r = atomicAdd(&st->resume_counter, 1u);
+            if (r < P.n_resume_in) {
+              const WorkItem w = P.resume_in[r];
+              a = w.g0; b = w.g1; sh = w.src;
+            } else {
+              res_left = 0u;
             }
-            if (a == b) {
-              const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
-              if (j < P.n_tiles) {
-                a = P.g_begin + j * kTilePhotons;
-                b = min(a + (unsigned long long)kTilePhotons, P.g_end);
-                sh = __ldg(&P.tile_src[j]);
-                if (*(volatile unsigned int*)&st->stop != 0u) {
-                  // the ring filled up while we were fetching: hand the whole tile to the next launch
-                  const unsigned o = atomicAdd(&st->n_resume_out, 1u);
-                  if (o < P.resume_cap) P.resume_out[o] = WorkItem{a, b, sh, 0u}; else atomicExch(&st->error, 1u);
-                  a = b = 0;
-                }
+          }
+          if (a == b) {
+            const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
+            if (j < P.n_tiles) {
+              a = P.g_begin + j * kTilePhotons;
+              b = min(a + (unsigned long long)kTilePhotons, P.g_end);
+              sh = __ldg(&P.tile_src[j]);
+              if (*(volatile unsigned int*)&st->stop != 0u) {
+                // the ring filled up while we were fetching: hand the whole tile to the next launch
+                const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+                if (o < P.resume_cap) P.resume_out[o] = WorkItem{a, b, sh, 0u}; else atomicExch(&st->error, 1u);
+                a = b = 0;
               }
             }
           }
-          a = __shfl_sync(0xffffffffu, a, 0);
-          b = __shfl_sync(0xffffffffu, b, 0);
-          sh = __shfl_sync(0xffffffffu, sh, 0);
-          use_resume = __shfl_sync(0xffffffffu, res_left, 0) != 0u;
-          if (a == b) { more_work = false; break; }
-          g_next = a; g_end = b; s_cur = sh;
         }
-        const unsigned long long avail = g_end - g_next;
-        const unsigned n_need = __popc(need_mask);
-        const unsigned take = (unsigned)min((unsigned long long)n_need, avail);
-        const unsigned rank = __popc(need_mask & lt);
+        t_next = __shfl_sync(0xffffffffu, (uint32_t)(a - P.g_begin), 0);
+        t_end = __shfl_sync(0xffffffffu, (uint32_t)(b - P.g_begin), 0);
+        s_cur = __shfl_sync(0xffffffffu, sh, 0);
+        use_resume = __shfl_sync(0xffffffffu, res_left, 0) != 0u;
+        if (t_next == t_end) refill_ok = false;
+      }
+      if (t_next != t_end) {
+        // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
+        const uint32_t r = t_next + __popc(need_mask & lt);
         uint32_t s_new = s_cur;
-        if (need && rank < take) {
-          // ---- a2/a3: initial state of batch-global photon g (fused expansion) ----
-          const unsigned long long g = g_next + rank;
+        if (!alive && r < t_end) {
           uint32_t s = s_cur;
-          while (g >= __ldg(&P.cum[s + 1])) ++s;
+          while (r >= __ldg(&P.cum_rel[s + 1])) ++s;
           s_new = s;
           const float4* rp = reinterpret_cast<const float4*>(P.src + s);
           const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
-          const uint4 r2 = __ldg(reinterpret_cast<const uint4*>(rp + 2));
+          const uint2 r2 = __ldg(reinterpret_cast<const uint2*>(rp + 2));
           phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
           dx = r0.w; dy = r1.x; dz = r1.y;
           Lh = 0.0f; Ll = 0.0f;
           ev = r2.x; sid = r2.y;
-          pidx = (uint32_t)(g - __ldg(&P.cum[s]));
+          pidx = r - __ldg(&P.cum_rel[s]);  // mod 2^32: right for the launch's first (split) source too
           k = 0; s_mine = s;
           alive = true; cont = false;
-          need = false;
         }
         s_cur = __reduce_max_sync(0xffffffffu, s_new);
-        g_next += take;
+        const uint32_t take = min((uint32_t)__popc(need_mask), t_end - t_next);
+        t_next += take;
         w_started += take;
-        need_mask = __ballot_sync(0xffffffffu, need);
-        if (!need_mask) break;
       }
     }
-    const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
-    if (!alive_mask) break;
-    w_flights += __popc(__ballot_sync(0xffffffffu, alive && !cont));
+    if (__ballot_sync(0xffffffffu, alive) == 0u) {
+      if (!refill_ok) break;
+      continue;  // the tile ran out exactly here: fetch the next one
+    }
 
     bool hit = false, done = false, aborted = false;
     uint32_t hit_dom = 0xFFFFFFFFu;
@@ -307,7 +309,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         const float tau_new = -__logf(u_abs);
         tau_a = (k == 0) ? tau_new : tau_a;
         // =========================== a4: optical depth to the next scatter ======================
-        tau_s = -logf(u_dist);
+        tau_s = neg_log_uniform(u_dist);
       }
       // =========================== a4: layer walk in vertical optical depth ======================
       // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
@@ -326,50 +328,44 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       const float v_cap = fminf(P.v_cap, P.xy_cap * w * inv_rho);
       int nb = up ? li : last - li;  // boundaries ahead before the infinite end layer
       nb = min(nb, v_cap < h0 ? 0 : 1 + (int)((v_cap - h0) * P.inv_dz_layer));
-      const int dir = up ? -1 : 1;
+      const int dstep = up ? -2 : 2;
+      int idx = 2 * li;
       float Ts = tau_s * w, Ta = tau_a * w, V = 0.0f, h = h0;
-      IceLayer L = sm.ice[li];
+      float2 ab = lay[idx];
       while (nb > 0) {
-        const float t1 = fmaf(-L.b, h, Ts), t2 = fmaf(-L.a, h, Ta);
-        if (t1 <= 0.0f || t2 <= 0.0f) break;  // the flight ends inside this layer
+        const float t1 = fmaf(-ab.y, h, Ts), t2 = fmaf(-ab.x, h, Ta);
+        if (fminf(t1, t2) <= 0.0f) break;  // the flight ends inside this layer
         Ts = t1; Ta = t2; V += h;
         h = P.dz_layer;
-        li += dir; --nb;
-        L = sm.ice[li];
+        idx += dstep; --nb;
+        ab = lay[idx];
       }
-      const float vs = Ts * L.lb, va = Ta * L.la, vc = fmaxf(v_cap - V, 0.0f);
+      const float2 ll = lay[idx + 1];
+      const float vs = Ts * ll.y, va = Ta * ll.x, vc = fmaxf(v_cap - V, 0.0f);
       const float v = fminf(fminf(vs, va), vc);
       const bool absorbed = (va <= vs) && (va <= vc);
       const bool scattered = !absorbed && (vs <= vc);
       V += v;
       const float s = V * inv_w;
-      tau_a = fmaxf(0.0f, fmaf(-L.a, v, Ta)) * inv_w;
-      tau_s = fmaxf(0.0f, fmaf(-L.b, v, Ts)) * inv_w;
+      tau_a = fmaxf(0.0f, fmaf(-ab.x, v, Ta)) * inv_w;
+      tau_s = fmaxf(0.0f, fmaf(-ab.y, v, Ts)) * inv_w;
       // =========================== a5: DOM intersection on [0, s] ===============================
       Best best{inf, 0xFFFFFFFFu};
       if (kBrute) {
         best = test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
       } else {
-        const float Rm = P.radius_margin;
-        const float ex = dx * s, ey = dy * s;
-        const float x_lo = fminf(phx, phx + ex) - Rm, y_lo = fminf(phy, phy + ey) - Rm;
-        const float fx = floorf((x_lo - P.gx0) * P.inv_cell), fy = floorf((y_lo - P.gy0) * P.inv_cell);
-        // anchors -1 .. (bx - 2) are stored at 0 .. (bx - 1); anything else cannot meet a string
-        if (fx >= -1.0f && fy >= -1.0f && fx < (float)(P.bx - 1) && fy < (float)(P.by - 1)) {
-          const uint32_t bidx = (((uint32_t)((int)fy + 1)) * P.bx + (uint32_t)((int)fx + 1)) * P.kq;
-          const float thr = fmaf(Rm * Rm, rho2, 1e-12f);
-          for (uint32_t q = 0; q < P.kq; ++q) {
-            const float4 c = blk_xy[bidx + q];
-            const float ax0 = c.x - phx, ay0 = c.y - phy, ax1 = c.z - phx, ay1 = c.w - phy;
-            const float cr0 = fmaf(ax0, dy, -ay0 * dx), cr1 = fmaf(ax1, dy, -ay1 * dx);
-            const bool p0 = cr0 * cr0 <= thr, p1 = cr1 * cr1 <= thr;
-            if (p0 || p1) {
-              const uint32_t ids = blk_id[bidx + q];
-              const uint32_t i0 = ids & 0xFFFFu, i1 = ids >> 16;
-              if (p0 && i0 != 0xFFFFu) best = test_string(P, sm, i0, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
-              if (p1 && i1 != 0xFFFFu) best = test_string(P, sm, i1, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
-            }
-          }
+        // the one line of DOMs this sub-flight can meet is named by the cell of its xy midpoint
+        const float hs = 0.5f * s;
+        const float cxf = fminf(fmaxf(fmaf(fmaf(hs, dx, phx), P.inv_cell, P.cell_ox), 0.0f), P.cell_xmax);
+        const float cyf = fminf(fmaxf(fmaf(fmaf(hs, dy, phy), P.inv_cell, P.cell_oy), 0.0f), P.cell_ymax);
+        const uint32_t si = s_cell[(uint32_t)(int)cyf * P.nx + (uint32_t)(int)cxf];
+        if (si != kNoString) {
+          const float4 sa = s_str_a[si];
+          const float ax = sa.x - phx, ay = sa.y - phy;
+          const float cr = fmaf(ax, dy, -ay * dx);
+          const float Rm = P.radius_margin;
+          if (cr * cr <= fmaf(Rm * Rm, rho2, 1e-12f))
+            best = test_string(P, T, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
         }
       }
       hit = best.t <= s;
@@ -424,12 +420,10 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       w_hits += n_hit - __popc(def_mask);
       if (def_mask) {
         // the replay will count these photons (and their flights) again: take them out here
-        warp_stop = true;
+        refill_ok = false;
         w_started -= __popc(def_mask);
-        w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
       }
     }
-    if (aborted) ++w_aborted;
 
     if (kFates) {
       if (alive && done && !deferred) {
@@ -445,21 +439,26 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         reinterpret_cast<pp_fate*>(P.fates)[g] = f;
       }
     }
-    if (done) alive = false;
+    if (done) {
+      alive = false;
+      if (!deferred) { n_flights += k; n_aborted += aborted ? 1u : 0u; }
+    }
   }
 
   // ---- leftovers of a stopped warp go to the next launch; fold the counters ----
+  const unsigned long long fl = __reduce_add_sync(0xffffffffu, n_flights);  // < 2^32 per warp for any launch < 2^32 photons / warps
+  const unsigned ab = __reduce_add_sync(0xffffffffu, n_aborted);
   if (lane == 0) {
-    if (g_next < g_end) {
+    if (t_next < t_end) {
       const unsigned o = atomicAdd(&st->n_resume_out, 1u);
-      if (o < P.resume_cap) P.resume_out[o] = WorkItem{g_next, g_end, s_cur, 0u}; else atomicExch(&st->error, 1u);
+      if (o < P.resume_cap) P.resume_out[o] = WorkItem{P.g_begin + t_next, P.g_begin + t_end, s_cur, 0u};
+      else atomicExch(&st->error, 1u);
     }
-    atomicAdd(&st->photons_started, w_started);
-    atomicAdd(&st->flights, w_flights);
+    atomicAdd(&st->photons_started, (unsigned long long)w_started);
+    atomicAdd(&st->flights, fl);
     if (w_hits) atomicAdd(&st->photons_hit, (unsigned long long)w_hits);
+    if (ab) atomicAdd(&st->photons_aborted, (unsigned long long)ab);
   }
-  const unsigned ab = __reduce_add_sync(0xffffffffu, w_aborted);
-  if (lane == 0 && ab) atomicAdd(&st->photons_aborted, (unsigned long long)ab);
 }
 
 // =============================================================================================
@@ -483,15 +482,17 @@ cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_c
 }
 
 cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
-                         uint32_t* d_tile_src, cudaStream_t st) {
+                         uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st) {
   if (n_tiles == 0) return cudaSuccess;
-  tiles_kernel<<<(n_tiles + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, d_tile_src);
+  const uint32_t n_thr = max(n_tiles, n_src + 1);
+  tiles_kernel<<<(n_thr + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, d_tile_src, d_cum_rel);
   g_launches++;
   return cudaGetLastError();
 }
 
-size_t propagate_smem_bytes(uint32_t n_block_entries) {
-  return sizeof(Smem) + (sizeof(float4) + sizeof(uint32_t)) * (size_t)n_block_entries + 16;
+size_t propagate_smem_bytes(uint32_t n_layers, uint32_t n_strings, uint32_t n_cells) {
+  const size_t n_str = n_strings ? n_strings : 1;
+  return sizeof(IceLayer) * n_layers + (sizeof(float4) + sizeof(uint2)) * n_str + sizeof(uint16_t) * (size_t)n_cells + 16;
 }
 
 template <bool B, bool F>

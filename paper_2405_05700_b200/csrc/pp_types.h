@@ -47,13 +47,15 @@ struct Status {                 // one per launch slot, device memory, copied ba
 constexpr int kTilePhotons = 1024;  // photons per fresh work tile
 constexpr int kMaxStringsSmem = 512;
 constexpr float kPoleRho2 = 1e-10f;  // R-9
-constexpr float kEmptyXY = 3.0e18f;   // coordinate of an empty block-table slot (its square still fits fp32)
+constexpr uint16_t kNoString = 0xFFFFu;  // cell-table entry: no line of DOMs within reach of this cell
 
 // Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).
 struct LaunchParams {
   // work
   const SrcRec* src;
-  const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons
+  const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons (batch-global photon numbers)
+  const uint32_t* cum_rel;        // [n_src + 1] cum[s] - g_begin as 32 bits: wraps below 0 (only the launch's first
+                                  // source can be there, and it is never compared), saturates at 2^32 - 1 above
   const uint32_t* tile_src;       // [n_tiles] source holding the first photon of each tile
   unsigned long long g_begin, g_end;
   uint32_t n_src, n_tiles;
@@ -76,14 +78,16 @@ struct LaunchParams {
   // geometry
   const StringRec* strings;  // [n_strings]
   const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
-  // block table (a5): block (ix, iy) lists every string whose pre-filter disc meets the 2c x 2c square
-  // [gx0 + ix c, gx0 + (ix+2) c) x [gy0 + iy c, ...); a sub-flight is capped to an xy extent < c, so the
-  // block anchored at the cell of its bounding box's low corner holds all its candidates.
-  const float4* blk_xy;     // [bx*by][kq]: (x0, y0, x1, y1) of two strings; empty slots hold kEmptyXY
-  const uint32_t* blk_id;   // [bx*by][kq]: string indices, two 16-bit halves; 0xFFFF = empty
+  // cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter
+  // disc can be met by a sub-flight whose xy midpoint lies in that cell (kNoString if none).  Unique because a
+  // sub-flight is capped to an xy length xy_cap < (smallest distance between two lines) - 2 radius_margin - cell
+  // diagonal; the outermost ring of cells is empty, so the cell index may simply be clamped into the grid.
+  const uint16_t* cell_sid;  // [nx*ny]
   uint32_t n_strings, n_dom;
-  uint32_t bx, by, kq;
-  float gx0, gy0, inv_cell, radius, radius_margin;  // radius_margin = R + safety used by the pre-filter
+  uint32_t nx, ny;
+  float cell_ox, cell_oy, inv_cell;  // cell coordinate = x * inv_cell + cell_ox
+  float cell_xmax, cell_ymax;        // nx - 1, ny - 1 as floats (clamp bounds)
+  float radius, radius_margin;       // radius_margin = R + safety used by the pre-filter
   // sub-flight caps: one loop iteration covers at most xy_cap metres in the xy-plane and v_cap metres
   // in z; a longer free flight continues in the next iteration without a new random draw
   float xy_cap, v_cap;
