@@ -319,6 +319,9 @@ uint64_t carve_device(pp_handle* h, void* base) {
   Carver c(base);
   const HostGeometry& g = h->hg;
   auto* d_ice = c.take<IceLayer>(h->ice.n_layers);
+  h->base.walk = c.take<float4>(h->ice.n_layers + 1);
+  h->base.inv_b = c.take<uint16_t>(kMaxWalkInv);
+  h->base.inv_a = c.take<uint16_t>(kMaxWalkInv);
   auto* d_strings = c.take<StringRec>(std::max<size_t>(1, g.strings.size()));
   auto* d_dom = c.take<float4>(g.dom_xyzw.size());
   auto* d_cell = c.take<uint16_t>(g.cell_sid.size());
@@ -773,24 +776,58 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   B.nx = h->hg.nx; B.ny = h->hg.ny; B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
   B.cell_xmax = (float)(h->hg.nx - 1); B.cell_ymax = (float)(h->hg.ny - 1);
   B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
-  B.xy_cap = h->hg.xy_cap;
+  B.xy_cap2 = h->hg.xy_cap * h->hg.xy_cap; B.inv_xy_cap = 1.0f / h->hg.xy_cap;
+  // ---- a4: tables of the direct layer walk (pp_types.h) ----
+  const uint32_t nl = ice->n_layers;
+  std::vector<float4> walk(nl + 1);
+  std::vector<uint16_t> inv_tab[2];
   {
-    // vertical sub-flight cap in layers (tuning knob PP_VCAP_LAYERS, default 6)
-    double t = 6.0;
-    if (const char* e = std::getenv("PP_VCAP_LAYERS")) { const double v = std::atof(e); if (v >= 1.0 && v <= 1000.0) t = v; }
-    B.v_cap = (float)(t * (double)ice->dz);
+    std::vector<double> cum[2] = {std::vector<double>(nl + 1, 0.0), std::vector<double>(nl + 1, 0.0)};  // B, A
+    for (uint32_t i = 0; i < nl; ++i) {
+      cum[0][i + 1] = cum[0][i] + (double)ice->dz / (double)ice->scat_len[i];
+      cum[1][i + 1] = cum[1][i] + (double)ice->dz / (double)ice->abs_len[i];
+    }
+    for (uint32_t i = 0; i <= nl; ++i) {
+      const float bh = (float)cum[0][i], ah = (float)cum[1][i];
+      walk[i] = make_float4(bh, ah, (float)(cum[0][i] - (double)bh), (float)(cum[1][i] - (double)ah));
+    }
+    walk[nl].x = walk[nl].y = INFINITY; walk[nl].z = walk[nl].w = 0.0f;
+    B.walk_loop = 0;
+    for (int t = 0; t < 2; ++t) {
+      // bin width: just under the thinnest layer, so that a bin holds at most one boundary; coarser (and the
+      // kernel then loops) if that would need more than kMaxWalkInv bins
+      double thin = 1e300;
+      for (uint32_t i = 0; i < nl; ++i) thin = std::min(thin, cum[t][i + 1] - cum[t][i]);
+      const double top = nl > 1 ? cum[t][nl - 1] : 0.0;  // cumulative depth at the upper edge of the last layer
+      double step = 0.99 * thin;
+      if (top / step + 3.0 > (double)kMaxWalkInv) { step = top / ((double)kMaxWalkInv - 3.0); B.walk_loop = 1; }
+      const uint32_t m = (uint32_t)std::ceil(top / step) + 1;  // bins 0..m
+      inv_tab[t].resize(m + 1);
+      uint32_t j = 0;
+      for (uint32_t b = 0; b <= m; ++b) {
+        // a lower bound of the layer for every depth that can land in bin b (index rounding slack 4e-3 bins)
+        const double x = ((double)b - 4e-3) * step;
+        while (j + 1 < nl && (double)walk[j + 1].x * (t == 0) + (double)walk[j + 1].y * (t == 1) <= x) ++j;
+        inv_tab[t][b] = (uint16_t)j;
+      }
+      (t == 0 ? B.m_b : B.m_a) = m;
+      (t == 0 ? B.k_b : B.k_a) = (float)(1.0 / step);
+    }
   }
   auto up = [&](const void* dst, const void* src, size_t bytes) {
     return bytes == 0 || cudaMemcpy(const_cast<void*>(dst), src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
   if (!up(B.ice, layers.data(), layers.size() * sizeof(IceLayer)) ||
+      !up(B.walk, walk.data(), walk.size() * sizeof(float4)) ||
+      !up(B.inv_b, inv_tab[0].data(), inv_tab[0].size() * sizeof(uint16_t)) ||
+      !up(B.inv_a, inv_tab[1].data(), inv_tab[1].size() * sizeof(uint16_t)) ||
       !up(B.strings, h->hg.strings.data(), h->hg.strings.size() * sizeof(StringRec)) ||
       !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)) ||
       !up(B.cell_sid, h->hg.cell_sid.data(), h->hg.cell_sid.size() * sizeof(uint16_t)))
     return bail(PP_E_CUDA);
 
   // ---- persistent grid: every SM filled to the kernel's occupancy ----
-  h->smem = propagate_smem_bytes(ice->n_layers, (uint32_t)h->hg.strings.size(), (uint32_t)h->hg.cell_sid.size());
+  h->smem = propagate_smem_layout(&B);
   {
     // make the opt-in dynamic shared memory size known before asking for the occupancy
     int bps = 0;

@@ -98,13 +98,8 @@ __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_
 // =============================================================================================
 constexpr int kBlockThreads = 256;
 
-// Shared-memory tables, staged once per launch: [IceLayer x n_layers][float4 x n_str][uint2 x n_str][u16 x cells]
-struct Tables {
-  const IceLayer* ice;
-  const float4* str_a;   // x, y, z0, 1/pitch
-  const uint2* str_b;    // n, base
-  const uint16_t* cell;  // candidate line per cell
-};
+// Shared-memory tables, staged once per launch (offsets in LaunchParams::off_*):
+// [IceLayer x n_layers][float4 walk x (n_layers + 1)][float4 x n_str][uint2 x n_str][u16 inv_b][u16 inv_a][u16 x cells]
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -135,11 +130,11 @@ __device__ __forceinline__ void sphere_test(const float4 c, float R, float phx, 
 
 // Step 7 (slow path, rare): the sub-flight passes within the pre-filter radius of the axis of line
 // `si`; test the DOMs whose z lies in the swept interval with the exact ray-sphere solve.
-__device__ __noinline__ Best test_string(const LaunchParams& P, const Tables& T, uint32_t si, float phx, float phy,
-                                         float phz, float plx, float ply, float plz, float dx, float dy, float dz,
-                                         float s, Best best) {
-  const float4 sa = T.str_a[si];
-  const uint2 sb = T.str_b[si];
+__device__ __noinline__ Best test_string(const LaunchParams& P, uint32_t si, float phx, float phy, float phz, float plx,
+                                         float ply, float plz, float dx, float dy, float dz, float s, Best best) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const float4 sa = reinterpret_cast<const float4*>(smem_raw + P.off_str_a)[si];
+  const uint2 sb = reinterpret_cast<const uint2*>(smem_raw + P.off_str_b)[si];
   const uint32_t n = sb.x, base = sb.y;
   // interval of the flight inside the infinite cylinder of radius Rm about the axis
   const float Rm = P.radius_margin;
@@ -181,14 +176,20 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
 template <bool kBrute, bool kFates>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const uint32_t n_str_alloc = max(P.n_strings, 1u);
+  // table offsets come from the constant bank (LaunchParams), not from registers
   IceLayer* const s_ice = reinterpret_cast<IceLayer*>(smem_raw);
-  float4* const s_str_a = reinterpret_cast<float4*>(s_ice + P.n_layers);
-  uint2* const s_str_b = reinterpret_cast<uint2*>(s_str_a + n_str_alloc);
-  uint16_t* const s_cell = reinterpret_cast<uint16_t*>(s_str_b + n_str_alloc);
+  float4* const s_walk = reinterpret_cast<float4*>(smem_raw + P.off_walk);
+  float4* const s_str_a = reinterpret_cast<float4*>(smem_raw + P.off_str_a);
+  uint2* const s_str_b = reinterpret_cast<uint2*>(smem_raw + P.off_str_b);
+  uint16_t* const s_inv_b = reinterpret_cast<uint16_t*>(smem_raw + P.off_inv_b);
+  uint16_t* const s_inv_a = reinterpret_cast<uint16_t*>(smem_raw + P.off_inv_a);
+  uint16_t* const s_cell = reinterpret_cast<uint16_t*>(smem_raw + P.off_cell);
 
   // ---- stage the medium and the DOM lookup in shared memory (a4, a5) ----
   for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) s_ice[i] = P.ice[i];
+  for (uint32_t i = threadIdx.x; i <= P.n_layers; i += blockDim.x) s_walk[i] = P.walk[i];
+  for (uint32_t i = threadIdx.x; i <= P.m_b; i += blockDim.x) s_inv_b[i] = P.inv_b[i];
+  for (uint32_t i = threadIdx.x; i <= P.m_a; i += blockDim.x) s_inv_a[i] = P.inv_a[i];
   if (!kBrute) {
     for (uint32_t i = threadIdx.x; i < P.n_strings; i += blockDim.x) {
       const StringRec r = P.strings[i];
@@ -199,8 +200,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     for (uint32_t i = threadIdx.x; i < n_cell; i += blockDim.x) s_cell[i] = P.cell_sid[i];
   }
   __syncthreads();
-  const Tables T{s_ice, s_str_a, s_str_b, s_cell};
-  const float2* const lay = reinterpret_cast<const float2*>(s_ice);  // [2 li] = (a, b), [2 li + 1] = (1/a, 1/b)
+  const float4* const lay = reinterpret_cast<const float4*>(s_ice);  // (a, b, 1/a, 1/b) per layer
 
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
@@ -211,17 +211,15 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   uint32_t t_next = 0, t_end = 0, s_cur = 0;
   bool refill_ok = true;   // false once the queues are empty or the hit ring filled up
   bool use_resume = P.n_resume_in > 0;
-  uint32_t w_started = 0, w_hits = 0;
+  uint32_t w_started = 0, w_hits = 0, w_flights = 0;
 
   // ---- per-lane photon state ----
   bool alive = false;
-  bool cont = false;  // the current free flight was cut by a sub-flight cap and continues
   float phx = 0, phy = 0, phz = 0, plx = 0, ply = 0, plz = 0;  // position, two-float (hi + lo)
   float dx = 0, dy = 0, dz = 1;
   float Lh = 0, Ll = 0;  // path length, two-float
-  float tau_a = 0, tau_s = 0;
+  float tau_a = 0;
   uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
-  uint32_t n_flights = 0, n_aborted = 0;  // per-lane totals over finished photons
 
   for (;;) {
     // =========================== refill dead lanes (a2 -> a3) ===========================
@@ -279,7 +277,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           ev = r2.x; sid = r2.y;
           pidx = r - __ldg(&P.cum_rel[s]);  // mod 2^32: right for the launch's first (split) source too
           k = 0; s_mine = s;
-          alive = true; cont = false;
+          alive = true;
         }
         s_cur = __reduce_max_sync(0xffffffffu, s_new);
         const uint32_t take = min((uint32_t)__popc(need_mask), t_end - t_next);
@@ -287,85 +285,112 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         w_started += take;
       }
     }
-    if (__ballot_sync(0xffffffffu, alive) == 0u) {
+    const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
+    if (alive_mask == 0u) {
       if (!refill_ok) break;
       continue;  // the tile ran out exactly here: fetch the next one
     }
+    w_flights += __popc(alive_mask);  // every live lane flies once per iteration
 
     bool hit = false, done = false, aborted = false;
     uint32_t hit_dom = 0xFFFFFFFFu;
     if (alive) {
-      if (!cont) {
-        // =========================== a7': Philox block k of this photon =========================
-        uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
-        philox4x32_10(c0, c1, c2, c3, P.rk);
-        const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
-        const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
-        // =========================== a7: emission (k = 0) or scatter (k > 0) ====================
-        const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
-        const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
-        rotate(dx, dy, dz, m, u_az);
-        // =========================== a3: absorption budget (once per photon) ====================
-        const float tau_new = -__logf(u_abs);
-        tau_a = (k == 0) ? tau_new : tau_a;
-        // =========================== a4: optical depth to the next scatter ======================
-        tau_s = neg_log_uniform(u_dist);
-      }
+      // =========================== a7': Philox block k of this photon ===========================
+      uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
+      philox4x32_10(c0, c1, c2, c3, P.rk);
+      const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
+      const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
+      // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
+      const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
+      const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
+      rotate(dx, dy, dz, m, u_az);
+      // =========================== a3: absorption budget (once per photon) ======================
+      const float tau_new = -__logf(u_abs);
+      tau_a = (k == 0) ? tau_new : tau_a;
+      // =========================== a4: optical depth to the next scatter ========================
+      const float tau_s = neg_log_uniform(u_dist);
       // =========================== a4: layer walk in vertical optical depth ======================
       // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
-      // so the budgets are scaled by w = |d_z| once and the loop works in vertical metres.
+      // so the budgets are scaled by w = |d_z| once and the walk works in vertical metres.
       const float w = fmaxf(fabsf(dz), 1e-9f);
       const float inv_w = fast_rcp(w);
-      const float rho2 = fmaf(dx, dx, dy * dy);
-      const float inv_rho = fast_rsqrt(fmaxf(rho2, 1e-18f));
       const bool up = dz > 0.0f;
       const int last = (int)P.n_layers - 1;
       int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
       li = max(0, min(li, last));
       const float zb = P.z_top - P.dz_layer * (float)(li + (up ? 0 : 1));
-      const float h0 = fmaxf(up ? zb - phz : phz - zb, 0.0f);  // vertical distance to the first boundary
-      // sub-flight cap in vertical metres, and the number of boundaries that fit under it
-      const float v_cap = fminf(P.v_cap, P.xy_cap * w * inv_rho);
-      int nb = up ? li : last - li;  // boundaries ahead before the infinite end layer
-      nb = min(nb, v_cap < h0 ? 0 : 1 + (int)((v_cap - h0) * P.inv_dz_layer));
-      const int dstep = up ? -2 : 2;
-      int idx = 2 * li;
-      float Ts = tau_s * w, Ta = tau_a * w, V = 0.0f, h = h0;
-      float2 ab = lay[idx];
-      while (nb > 0) {
-        const float t1 = fmaf(-ab.y, h, Ts), t2 = fmaf(-ab.x, h, Ta);
-        if (fminf(t1, t2) <= 0.0f) break;  // the flight ends inside this layer
-        Ts = t1; Ta = t2; V += h;
-        h = P.dz_layer;
-        idx += dstep; --nb;
-        ab = lay[idx];
+      const bool open = up ? (li == 0) : (li == last);  // no boundary ahead: the end layers are infinite (R-6)
+      const float h0 = open ? inf : fabsf(zb - phz);    // vertical distance to the first boundary
+      float Ts = tau_s * w, Ta = tau_a * w, Vb = 0.0f;
+      float4 L4 = lay[li];
+      {
+        const float t1 = fmaf(-L4.y, h0, Ts), t2 = fmaf(-L4.x, h0, Ta);
+        if (fminf(t1, t2) > 0.0f) {
+          // The flight leaves layer li through boundary i1 with budgets t1, t2 left.  Direct walk: the cumulative
+          // depths X at which the budgets run out name the layers js, ja (inverse table + one step); the nearer
+          // one is where the flight ends, and the budgets left at its entry boundary jb come from the two-float
+          // cumulative sums, so their error is relative to the budget, not to the cumulative depth.
+          const int i1 = li + (up ? 0 : 1);
+          const float4 W1 = s_walk[i1];
+          const float Xs = up ? W1.x - t1 : W1.x + t1, Xa = up ? W1.y - t2 : W1.y + t2;
+          int js = s_inv_b[min((uint32_t)max((int)fmaf(Xs, P.k_b, -1e-3f), 0), P.m_b)];
+          int ja = s_inv_a[min((uint32_t)max((int)fmaf(Xa, P.k_a, -1e-3f), 0), P.m_a)];
+          js += (s_walk[js + 1].x <= Xs) ? 1 : 0;
+          ja += (s_walk[ja + 1].y <= Xa) ? 1 : 0;
+          if (P.walk_loop) {
+            while (s_walk[js + 1].x <= Xs) ++js;
+            while (s_walk[ja + 1].y <= Xa) ++ja;
+          }
+          const int lj = up ? min(max(js, ja), li - 1) : max(min(js, ja), li + 1);
+          const int jb = lj + (up ? 1 : 0);
+          const float4 Wb = s_walk[jb];
+          Ts = t1 - fabsf((Wb.x - W1.x) + (Wb.z - W1.z));
+          Ta = t2 - fabsf((Wb.y - W1.y) + (Wb.w - W1.w));
+          Vb = fmaf(P.dz_layer, (float)abs(jb - i1), h0);
+          L4 = lay[lj];
+        }
       }
-      const float2 ll = lay[idx + 1];
-      const float vs = Ts * ll.y, va = Ta * ll.x, vc = fmaxf(v_cap - V, 0.0f);
-      const float v = fminf(fminf(vs, va), vc);
-      const bool absorbed = (va <= vs) && (va <= vc);
-      const bool scattered = !absorbed && (vs <= vc);
-      V += v;
-      const float s = V * inv_w;
-      tau_a = fmaxf(0.0f, fmaf(-ab.x, v, Ta)) * inv_w;
-      tau_s = fmaxf(0.0f, fmaf(-ab.y, v, Ts)) * inv_w;
+      const float vs = Ts * L4.w, va = Ta * L4.z;  // vertical distance left in the final layer
+      const bool absorbed = va <= vs;
+      const float v_in = fminf(vs, va);
+      const float s = (Vb + v_in) * inv_w;
+      tau_a = fmaxf(0.0f, fmaf(-L4.x, v_in, Ta)) * inv_w;
       // =========================== a5: DOM intersection on [0, s] ===============================
       Best best{inf, 0xFFFFFFFFu};
       if (kBrute) {
         best = test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
       } else {
-        // the one line of DOMs this sub-flight can meet is named by the cell of its xy midpoint
-        const float hs = 0.5f * s;
-        const float cxf = fminf(fmaxf(fmaf(fmaf(hs, dx, phx), P.inv_cell, P.cell_ox), 0.0f), P.cell_xmax);
-        const float cyf = fminf(fmaxf(fmaf(fmaf(hs, dy, phy), P.inv_cell, P.cell_oy), 0.0f), P.cell_ymax);
-        const uint32_t si = s_cell[(uint32_t)(int)cyf * P.nx + (uint32_t)(int)cxf];
-        if (si != kNoString) {
-          const float4 sa = s_str_a[si];
-          const float ax = sa.x - phx, ay = sa.y - phy;
-          const float cr = fmaf(ax, dy, -ay * dx);
-          const float Rm = P.radius_margin;
-          if (cr * cr <= fmaf(Rm * Rm, rho2, 1e-12f))
-            best = test_string(P, T, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+        // the one line of DOMs a piece of flight no longer than xy_cap in the xy-plane can meet is named by the
+        // cell of the piece's xy midpoint; a longer flight is looked up piece by piece
+        const float rho2 = fmaf(dx, dx, dy * dy);
+        const float sxy2 = s * s * rho2;
+        float ds = s;
+        int n_ch = 1;
+        if (sxy2 > P.xy_cap2) {
+          const float f = floorf(fast_sqrt(sxy2) * P.inv_xy_cap) + 1.0f;
+          n_ch = f > 64.0f ? 1 : (int)f;
+          ds = s * fast_rcp(f);
+        }
+        const float rm2 = fmaf(P.radius_margin * P.radius_margin, rho2, 1e-12f);
+        float tm = 0.5f * ds;
+#pragma unroll 1
+        for (;;) {
+          const float cxf = fminf(fmaxf(fmaf(fmaf(tm, dx, phx), P.inv_cell, P.cell_ox), 0.0f), P.cell_xmax);
+          const float cyf = fminf(fmaxf(fmaf(fmaf(tm, dy, phy), P.inv_cell, P.cell_oy), 0.0f), P.cell_ymax);
+          const uint32_t si = s_cell[(uint32_t)(int)cyf * P.nx + (uint32_t)(int)cxf];
+          if (si != kNoString) {
+            const float4 sa = s_str_a[si];
+            const float cr = fmaf(sa.x - phx, dy, -(sa.y - phy) * dx);
+            if (cr * cr <= rm2)
+              best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+          }
+          if (--n_ch <= 0) break;
+          tm += ds;
+        }
+        if (sxy2 > P.xy_cap2 * 4096.0f) {
+          // a flight of more than 64 pieces (far longer than the detector is wide): every line
+          for (uint32_t si = 0; si < P.n_strings; ++si)
+            best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
         }
       }
       hit = best.t <= s;
@@ -380,9 +405,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         const float nz_ = fmaf(dz, adv, phz); plz += fmaf(dz, adv, phz - nz_); phz = nz_;
         const float nl = Lh + adv; Ll += adv - (nl - Lh); Lh = nl;
       }
-      cont = !hit && !absorbed && !scattered;
-      k += cont ? 0u : 1u;  // k counts the free flights started = index of the next Philox block
-      aborted = !hit && !absorbed && !cont && k >= P.max_flights;
+      k += 1u;  // k counts the free flights started = index of the next Philox block
+      aborted = !hit && !absorbed && k >= P.max_flights;
       done = hit || absorbed || aborted;
     }
 
@@ -422,6 +446,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         // the replay will count these photons (and their flights) again: take them out here
         refill_ok = false;
         w_started -= __popc(def_mask);
+        w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
       }
     }
 
@@ -441,13 +466,11 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     }
     if (done) {
       alive = false;
-      if (!deferred) { n_flights += k; n_aborted += aborted ? 1u : 0u; }
+      if (aborted) atomicAdd(&st->photons_aborted, 1ull);  // never in practice (R-10)
     }
   }
 
   // ---- leftovers of a stopped warp go to the next launch; fold the counters ----
-  const unsigned long long fl = __reduce_add_sync(0xffffffffu, n_flights);  // < 2^32 per warp for any launch < 2^32 photons / warps
-  const unsigned ab = __reduce_add_sync(0xffffffffu, n_aborted);
   if (lane == 0) {
     if (t_next < t_end) {
       const unsigned o = atomicAdd(&st->n_resume_out, 1u);
@@ -455,9 +478,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       else atomicExch(&st->error, 1u);
     }
     atomicAdd(&st->photons_started, (unsigned long long)w_started);
-    atomicAdd(&st->flights, fl);
+    atomicAdd(&st->flights, (unsigned long long)w_flights);  // < 2^32 per warp for any launch of < 2^32 photons
     if (w_hits) atomicAdd(&st->photons_hit, (unsigned long long)w_hits);
-    if (ab) atomicAdd(&st->photons_aborted, (unsigned long long)ab);
   }
 }
 
@@ -490,9 +512,17 @@ cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsign
   return cudaGetLastError();
 }
 
-size_t propagate_smem_bytes(uint32_t n_layers, uint32_t n_strings, uint32_t n_cells) {
-  const size_t n_str = n_strings ? n_strings : 1;
-  return sizeof(IceLayer) * n_layers + (sizeof(float4) + sizeof(uint2)) * n_str + sizeof(uint16_t) * (size_t)n_cells + 16;
+size_t propagate_smem_layout(LaunchParams* P) {
+  auto up16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
+  const size_t n_str = P->n_strings ? P->n_strings : 1;
+  size_t o = up16(sizeof(IceLayer) * P->n_layers);
+  P->off_walk = (uint32_t)o; o = up16(o + sizeof(float4) * (P->n_layers + 1));
+  P->off_str_a = (uint32_t)o; o = up16(o + sizeof(float4) * n_str);
+  P->off_str_b = (uint32_t)o; o = up16(o + sizeof(uint2) * n_str);
+  P->off_inv_b = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (P->m_b + 1));
+  P->off_inv_a = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (P->m_a + 1));
+  P->off_cell = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (size_t)P->nx * P->ny);
+  return o;
 }
 
 template <bool B, bool F>

@@ -47,6 +47,7 @@ struct Status {                 // one per launch slot, device memory, copied ba
 constexpr int kTilePhotons = 1024;  // photons per fresh work tile
 constexpr int kMaxStringsSmem = 512;
 constexpr float kPoleRho2 = 1e-10f;  // R-9
+constexpr uint32_t kMaxWalkInv = 4096;  // entries per inverse walk table (device and shared memory)
 constexpr uint16_t kNoString = 0xFFFFu;  // cell-table entry: no line of DOMs within reach of this cell
 
 // Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).
@@ -69,6 +70,18 @@ struct LaunchParams {
   void* fates;        // pp_fate[g_end] or nullptr
   // medium
   const IceLayer* ice;  // [n_layers]
+  // Direct layer walk (a4): cumulative vertical optical depth at the layer boundaries, boundary i = upper edge of
+  // layer i, as two-float sums {B_hi, A_hi, B_lo, A_lo} (B scattering, A absorption); entry n_layers holds +inf in
+  // the hi parts (only ever compared against).  inv_b / inv_a map a quantised cumulative depth to a layer j0 such
+  // that the layer holding that depth is j0 or j0 + 1 (or beyond, when walk_loop is set for a coarse table).
+  const float4* walk;     // [n_layers + 1]
+  const uint16_t* inv_b;  // [m_b + 1]
+  const uint16_t* inv_a;  // [m_a + 1]
+  uint32_t m_b, m_a;      // largest table index
+  float k_b, k_a;         // table index = cumulative depth * k
+  uint32_t walk_loop;
+  // byte offsets of the tables in dynamic shared memory (ice table at 0)
+  uint32_t off_walk, off_str_a, off_str_b, off_inv_b, off_inv_a, off_cell;
   uint32_t n_layers;
   float z_top, dz_layer, inv_dz_layer;
   float hg_one_minus_g, hg_two_g, hg_one_minus_g2;  // 1-g, 2g, 1-g^2
@@ -88,9 +101,8 @@ struct LaunchParams {
   float cell_ox, cell_oy, inv_cell;  // cell coordinate = x * inv_cell + cell_ox
   float cell_xmax, cell_ymax;        // nx - 1, ny - 1 as floats (clamp bounds)
   float radius, radius_margin;       // radius_margin = R + safety used by the pre-filter
-  // sub-flight caps: one loop iteration covers at most xy_cap metres in the xy-plane and v_cap metres
-  // in z; a longer free flight continues in the next iteration without a new random draw
-  float xy_cap, v_cap;
+  // a flight longer than xy_cap metres in the xy-plane is looked up in the cell table in chunks of at most xy_cap
+  float xy_cap2, inv_xy_cap;  // xy_cap^2, 1/xy_cap
 };
 
 }  // namespace pp
