@@ -255,7 +255,9 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
   const double Rm = (double)geo->radius + 5e-3, slack = 0.02;
   double L_max = 100.0;  // tuning knob PP_XY_CAP (metres)
   if (const char* e = std::getenv("PP_XY_CAP")) { const double v = std::atof(e); if (v >= 1.0 && v <= 1.0e4) L_max = v; }
-  double cell = ns > 1 ? d_min / 6.0 : 32.0;
+  double cell_div = 6.0;  // tuning knob PP_CELL_DIV: cells per smallest line distance
+  if (const char* e = std::getenv("PP_CELL_DIV")) { const double v = std::atof(e); if (v >= 2.0 && v <= 64.0) cell_div = v; }
+  double cell = ns > 1 ? d_min / cell_div : 32.0;
   double L = ns > 1 ? std::min(L_max, d_min - 2.0 * (Rm + slack) - cell * std::sqrt(2.0) - slack) : L_max;
   double x0 = 1e30, x1 = -1e30, y0 = 1e30, y1 = -1e30;
   for (auto& p : xy) { x0 = std::min(x0, (double)p.first); x1 = std::max(x1, (double)p.first);
@@ -774,7 +776,6 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
   B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
   B.nx = h->hg.nx; B.ny = h->hg.ny; B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
-  B.cell_xmax = (float)(h->hg.nx - 1); B.cell_ymax = (float)(h->hg.ny - 1);
   B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
   B.xy_cap2 = h->hg.xy_cap * h->hg.xy_cap; B.inv_xy_cap = 1.0f / h->hg.xy_cap;
   // ---- a4: tables of the direct layer walk (pp_types.h) ----

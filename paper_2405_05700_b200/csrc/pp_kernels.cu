@@ -96,7 +96,10 @@ __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_
 // =============================================================================================
 // a3-a8  Persistent propagation kernel
 // =============================================================================================
-constexpr int kBlockThreads = 256;
+#ifndef PP_BLOCK_THREADS
+#define PP_BLOCK_THREADS 256
+#endif
+constexpr int kBlockThreads = PP_BLOCK_THREADS;
 
 // Shared-memory tables, staged once per launch (offsets in LaunchParams::off_*):
 // [IceLayer x n_layers][float4 walk x (n_layers + 1)][float4 x n_str][uint2 x n_str][u16 inv_b][u16 inv_a][u16 x cells]
@@ -333,8 +336,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           const int i1 = li + (up ? 0 : 1);
           const float4 W1 = s_walk[i1];
           const float Xs = up ? W1.x - t1 : W1.x + t1, Xa = up ? W1.y - t2 : W1.y + t2;
-          int js = s_inv_b[min((uint32_t)max((int)fmaf(Xs, P.k_b, -1e-3f), 0), P.m_b)];
-          int ja = s_inv_a[min((uint32_t)max((int)fmaf(Xa, P.k_a, -1e-3f), 0), P.m_a)];
+          int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
+          int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
           js += (s_walk[js + 1].x <= Xs) ? 1 : 0;
           ja += (s_walk[ja + 1].y <= Xa) ? 1 : 0;
           if (P.walk_loop) {
@@ -375,9 +378,10 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         float tm = 0.5f * ds;
 #pragma unroll 1
         for (;;) {
-          const float cxf = fminf(fmaxf(fmaf(fmaf(tm, dx, phx), P.inv_cell, P.cell_ox), 0.0f), P.cell_xmax);
-          const float cyf = fminf(fmaxf(fmaf(fmaf(tm, dy, phy), P.inv_cell, P.cell_oy), 0.0f), P.cell_ymax);
-          const uint32_t si = s_cell[(uint32_t)(int)cyf * P.nx + (uint32_t)(int)cxf];
+          // cell of the piece's midpoint; the saturating conversion sends negative coordinates to cell 0
+          const uint32_t cx = min(__float2uint_rz(fmaf(fmaf(tm, dx, phx), P.inv_cell, P.cell_ox)), P.nx - 1u);
+          const uint32_t cy = min(__float2uint_rz(fmaf(fmaf(tm, dy, phy), P.inv_cell, P.cell_oy)), P.ny - 1u);
+          const uint32_t si = s_cell[cy * P.nx + cx];
           if (si != kNoString) {
             const float4 sa = s_str_a[si];
             const float cr = fmaf(sa.x - phx, dy, -(sa.y - phy) * dx);

@@ -99,7 +99,6 @@ struct LaunchParams {
   uint32_t n_strings, n_dom;
   uint32_t nx, ny;
   float cell_ox, cell_oy, inv_cell;  // cell coordinate = x * inv_cell + cell_ox
-  float cell_xmax, cell_ymax;        // nx - 1, ny - 1 as floats (clamp bounds)
   float radius, radius_margin;       // radius_margin = R + safety used by the pre-filter
   // a flight longer than xy_cap metres in the xy-plane is looked up in the cell table in chunks of at most xy_cap
   float xy_cap2, inv_xy_cap;  // xy_cap^2, 1/xy_cap
