@@ -36,10 +36,13 @@ WORKLOAD = "C1: BASELINE.json configs[1], 200 cascades E^-1 1 GeV-10 TeV on a 1 
 INSTR_PER_FLIGHT_FILE = os.path.join(ROOT, "profiles", "instr_per_flight.json")
 
 
-def load_instr_per_flight():
+def load_instr_per_flight(library_version):
+    """The per-unit figure of the roofline; only valid for the library version it was measured on."""
     try:
         with open(INSTR_PER_FLIGHT_FILE) as f:
             d = json.load(f)
+        if d.get("library") != library_version:
+            return None, None, f"stale: measured on {d.get('library')!r}, library is {library_version!r}"
         return float(d["thread_instructions_per_flight"]), d.get("dram_bytes_per_launch"), d.get("source", "")
     except Exception:
         return None, None, ""
@@ -240,7 +243,7 @@ def run_ours(args):
     if rank == 0:
         peaks = measured_peaks()
         clocks = clk.summary()
-        ipf, dram_bytes, ipf_src = load_instr_per_flight()
+        ipf, dram_bytes, ipf_src = load_instr_per_flight(B.version())
         sm_max = peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         roofline = None

@@ -121,6 +121,10 @@ def kernel_launch_count() -> int:
     return int(load_library().pp_kernel_launch_count())
 
 
+def version() -> str:
+    return load_library().pp_version().decode()
+
+
 def _marshal_inputs(geometry, ice):
     fp = C.POINTER(C.c_float)
     xyz = np.ascontiguousarray(geometry.xyz, dtype=np.float32).reshape(-1, 3)
