@@ -290,6 +290,128 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------
+# C3: launch-size sweep; C2: streaming from worker threads (report modes, one JSON line per point)
+# ------------------------------------------------------------------------------------------------
+def run_sweep(args):
+    """BASELINE.json configs[3]: photons per launch 1e5..1e9 on C1's geometry and ice; one pp_submit + pp_flush +
+    drain per launch with launch_photons_target = N.  Reports photons/s (wall clock, host buffers in and out) and the
+    device-busy fraction (kernel time / wall time) per launch size."""
+    import torch
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import workloads as W
+    torch.cuda.set_device(0)
+    geo, ice = W.geometry_full(), W.ice_layered()
+    sizes = [10 ** k for k in range(5, 10)] if not args.sweep_sizes else [int(float(x)) for x in args.sweep_sizes.split(",")]
+    for n in sizes:
+        src = W.sources_c3(float(n), seed=3)
+        reps = int(max(3, min(50, 2e9 // n)))
+        with B.Propagator(geo, ice, seed=0, launch_photons_target=n) as prop:
+            for _ in range(2):
+                prop.run(src.src, src.event_id, src.source_id)
+            st0 = prop.stats()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            hits = 0
+            for _ in range(reps):
+                hits += len(prop.run(src.src, src.event_id, src.source_id))
+            wall = time.perf_counter() - t0
+            st1 = prop.stats()
+        ph = st1.photons_done - st0.photons_done
+        busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+        print(json.dumps({"mode": "sweep", "workload": "C3: cascades uniform in the instrumented volume, 1-100 TeV, cut at N photons",
+                          "photons_per_launch": n, "sources": len(src), "launches": st1.launches - st0.launches, "reps": reps,
+                          "photons_per_s": ph / wall, "kernel_photons_per_s": ph / busy, "device_busy_frac": busy / wall,
+                          "ms_per_launch_wall": 1e3 * wall / reps, "ms_per_launch_kernel": 1e3 * busy / reps,
+                          "hits_per_launch": hits / reps, "flights_per_photon": (st1.flights - st0.flights) / ph}), flush=True)
+    return 0
+
+
+def run_stream(args):
+    """BASELINE.json configs[2] through the batching server.  `--threads` producer threads play the paper's
+    propagation clients: each owns a share of the events of `--replicas` re-numbered replicas of
+    C2, queues their light sources and ships a block to the server whenever `--block-sources` sources have piled up
+    ("when the step queue is sufficiently full, a block of steps is sent"); one consumer thread collects hits
+    meanwhile; the server cuts launches at 1e8 photons.  The blocks are packed before the clock starts (producing the
+    sources is the CPU stages' work, not this path's).  Reports photons/s and the device-busy fraction between the
+    first submit and the drain."""
+    import torch
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import workloads as W
+    torch.cuda.set_device(0)
+    geo, ice = W.geometry_full(), W.ice_layered()
+    src = W.sources_c2()
+    order = np.argsort(src.event_id, kind="stable")
+    rec = B.pack_sources(src.src[order])
+    ev, sid = src.event_id[order], src.source_id[order]
+    n_events = int(ev.max()) + 1
+    first = np.searchsorted(ev, np.arange(n_events + 1))  # sources of event g: [first[g], first[g+1])
+    replicas, n_thr = args.replicas, max(1, args.threads)
+    # client t owns events g with g % n_thr == t of every replica; its blocks end on event boundaries
+    blocks = [[] for _ in range(n_thr)]
+    for t in range(n_thr):
+        cur, cur_n = [], 0
+        for r in range(replicas):
+            for g in range(t, n_events, n_thr):
+                a, b = int(first[g]), int(first[g + 1])
+                if b > a:
+                    cur.append((r, a, b))
+                    cur_n += b - a
+                if cur_n >= args.block_sources:
+                    blocks[t].append(cur)
+                    cur, cur_n = [], 0
+        if cur:
+            blocks[t].append(cur)
+    packed = [[(np.concatenate([rec[a:b] for _, a, b in blk]),
+                np.concatenate([ev[a:b] + np.uint32(r * n_events) for r, a, b in blk]),
+                np.concatenate([sid[a:b] for _, a, b in blk])) for blk in bl] for bl in blocks]
+    with B.Propagator(geo, ice, seed=0, launch_photons_target=10 ** 8) as prop:
+        prop.run(src.src, src.event_id, src.source_id)  # warm-up
+        st0 = prop.stats()
+
+        def producer(t):
+            for r_, e_, s_ in packed[t]:
+                prop.submit(r_, e_, s_)
+
+        n_hits = [0]
+        done = threading.Event()
+
+        def consumer():
+            while True:
+                h = prop.collect(1 << 20, block=True)
+                if len(h) == 0:
+                    if done.is_set():
+                        return
+                    time.sleep(0.0005)
+                    continue
+                n_hits[0] += len(h)
+
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        cons = threading.Thread(target=consumer)
+        cons.start()
+        th = [threading.Thread(target=producer, args=(t,)) for t in range(n_thr)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        prop.flush()
+        done.set()
+        cons.join()
+        n_hits[0] += len(prop.collect_all())
+        wall = time.perf_counter() - t0
+        st1 = prop.stats()
+    ph = st1.photons_done - st0.photons_done
+    busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+    print(json.dumps({"mode": "stream", "workload": f"C2 x {replicas} replicas of {n_events} events, shipped in blocks of >= "
+                      f"{args.block_sources} sources by {n_thr} client threads", "threads": n_thr,
+                      "blocks": sum(len(b) for b in blocks), "sources": int(len(src) * replicas), "photons": int(ph),
+                      "launches": st1.launches - st0.launches, "photons_per_s": ph / wall, "device_busy_frac": busy / wall,
+                      "wall_s": wall, "kernel_s": busy, "hits": n_hits[0],
+                      "source_ring_high_water": st1.source_ring_high_water}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -297,9 +419,19 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="C3 launch-size sweep (report mode)")
+    ap.add_argument("--sweep-sizes", default="", help="comma-separated photons per launch (default 1e5..1e9)")
+    ap.add_argument("--stream", action="store_true", help="C2 replicas through the batching server from worker threads")
+    ap.add_argument("--threads", type=int, default=8)
+    ap.add_argument("--replicas", type=int, default=10)
+    ap.add_argument("--block-sources", type=int, default=8192, help="sources a client queues before it ships a block")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    if args.stream:
+        return run_stream(args)
     return run_ours(args)
 
 

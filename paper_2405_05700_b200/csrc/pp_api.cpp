@@ -310,7 +310,8 @@ void fill_sizes(const pp_config& cfg, int n_sm, Sizes* s) {
   s->target = cfg.launch_photons_target ? cfg.launch_photons_target : 100000000ull;
   const uint64_t src_bytes = cfg.source_ring_bytes ? cfg.source_ring_bytes : (64ull << 20);
   s->cap_src = std::max<uint64_t>(64, src_bytes / sizeof(SrcRec));
-  s->max_tiles = (s->target + kTilePhotons - 1) / kTilePhotons + 2;
+  // large launches: target / kTilePhotons tiles; small ones use smaller tiles but never more than 8 per warp
+  s->max_tiles = std::max<uint64_t>((s->target + kTilePhotons - 1) / kTilePhotons, (uint64_t)n_sm * 64ull * 8ull) + 2;
   s->resume_cap = (uint64_t)n_sm * 2048ull * 2ull + 4096ull;
   const uint64_t hit_bytes = cfg.hit_ring_bytes ? cfg.hit_ring_bytes : (256ull << 20);
   s->ring_cap = std::max<uint64_t>(32, std::min<uint64_t>(hit_bytes / 2 / sizeof(pp_hit), 0xFFFFFF00ull));
@@ -369,12 +370,17 @@ uint64_t carve_pinned(pp_handle* h, void* base) {
 int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long long* cum, uint32_t n_src,
                    uint64_t g_begin, uint64_t g_end, pp_fate* fates) {
   const uint64_t n_ph = g_end - g_begin;
-  const uint32_t n_tiles = (uint32_t)((n_ph + kTilePhotons - 1) / kTilePhotons);
+  // tile size: 1024 photons for large launches; a small launch is cut finer so that every resident warp gets work
+  // (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3)
+  uint32_t tile = kTilePhotons;
+  const uint64_t want_tiles = (uint64_t)h->grid * 8ull * 4ull;  // 8 warps per CTA
+  while (tile > (uint32_t)kMinTilePhotons && n_ph / tile < want_tiles) tile >>= 1;
+  const uint32_t n_tiles = (uint32_t)((n_ph + tile - 1) / tile);
   if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");
-  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, s.d_tile_src, s.d_cum_rel, s.stream));
+  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, tile, s.d_tile_src, s.d_cum_rel, s.stream));
   LaunchParams P = h->base;
   P.src = src; P.cum = cum; P.cum_rel = s.d_cum_rel; P.tile_src = s.d_tile_src;
-  P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles;
+  P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles; P.tile_photons = tile;
   s.resume_sel = 0;
   P.resume_in = s.d_resume[1]; P.resume_out = s.d_resume[0];
   P.n_resume_in = 0; P.resume_cap = (uint32_t)h->sz.resume_cap;
@@ -774,6 +780,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
   }
   B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
+  B.tile_photons = kTilePhotons;
   B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
   B.nx = h->hg.nx; B.ny = h->hg.ny; B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
   B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;

@@ -73,18 +73,19 @@ __global__ void __launch_bounds__(1024) scan_kernel(const SrcRec* __restrict__ s
   if (t == 1023) cum[n] = part[1023];
 }
 
-// tile_src[j] = index of the source that holds batch-global photon g_begin + j * kTilePhotons,
+// tile_src[j] = index of the source that holds batch-global photon g_begin + j * tile_photons,
 // i.e. the last s with cum[s] <= g (sources with zero photons are skipped by construction); and
 // cum_rel[s] = cum[s] - g_begin in 32 bits for the refill (see LaunchParams::cum_rel).
 __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_t n_src, unsigned long long g_begin,
-                             uint32_t n_tiles, uint32_t* __restrict__ tile_src, uint32_t* __restrict__ cum_rel) {
+                             uint32_t n_tiles, uint32_t tile_photons, uint32_t* __restrict__ tile_src,
+                             uint32_t* __restrict__ cum_rel) {
   const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j <= n_src) {
     const unsigned long long c = cum[j];
     cum_rel[j] = c < g_begin ? (uint32_t)(c - g_begin) : (uint32_t)min(c - g_begin, 0xFFFFFFFFull);
   }
   if (j >= n_tiles) return;
-  const unsigned long long g = g_begin + (unsigned long long)j * kTilePhotons;
+  const unsigned long long g = g_begin + (unsigned long long)j * tile_photons;
   uint32_t lo = 0, hi = n_src;  // invariant: cum[lo] <= g < cum[hi]
   while (hi - lo > 1) {
     const uint32_t mid = (lo + hi) >> 1;
@@ -245,8 +246,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           if (a == b) {
             const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
             if (j < P.n_tiles) {
-              a = P.g_begin + j * kTilePhotons;
-              b = min(a + (unsigned long long)kTilePhotons, P.g_end);
+              a = P.g_begin + j * P.tile_photons;
+              b = min(a + (unsigned long long)P.tile_photons, P.g_end);
               sh = __ldg(&P.tile_src[j]);
               if (*(volatile unsigned int*)&st->stop != 0u) {
                 // the ring filled up while we were fetching: hand the whole tile to the next launch
@@ -508,10 +509,10 @@ cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_c
 }
 
 cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
-                         uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st) {
+                         uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st) {
   if (n_tiles == 0) return cudaSuccess;
   const uint32_t n_thr = max(n_tiles, n_src + 1);
-  tiles_kernel<<<(n_thr + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, d_tile_src, d_cum_rel);
+  tiles_kernel<<<(n_thr + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, tile_photons, d_tile_src, d_cum_rel);
   g_launches++;
   return cudaGetLastError();
 }

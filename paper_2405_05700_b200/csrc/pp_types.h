@@ -44,7 +44,8 @@ struct Status {                 // one per launch slot, device memory, copied ba
   unsigned int pad[3];
 };
 
-constexpr int kTilePhotons = 1024;  // photons per fresh work tile
+constexpr int kTilePhotons = 1024;  // photons per fresh work tile of a large launch (small launches use smaller tiles)
+constexpr int kMinTilePhotons = 32;
 constexpr int kMaxStringsSmem = 512;
 constexpr float kPoleRho2 = 1e-10f;  // R-9
 constexpr uint32_t kMaxWalkInv = 4096;  // entries per inverse walk table (device and shared memory)
@@ -60,6 +61,7 @@ struct LaunchParams {
   const uint32_t* tile_src;       // [n_tiles] source holding the first photon of each tile
   unsigned long long g_begin, g_end;
   uint32_t n_src, n_tiles;
+  uint32_t tile_photons;          // photons per fresh tile of this launch: kMinTilePhotons..kTilePhotons, a power of two
   const WorkItem* resume_in;
   WorkItem* resume_out;
   uint32_t n_resume_in, resume_cap;
