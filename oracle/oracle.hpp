@@ -25,6 +25,10 @@
 //   propagate            homogeneous-ice closed forms (segments ~ Geom, path ~ Exp(lambda_a),
 //                        <displacement> = 1/(a+b(1-g))), unscattered survival exp(-(d-R)(a+b)),
 //                        arrival time (d-R)/v, causality, conservation
+//   acceptance / propagate with acceptance (NEXT-1, R-17)
+//                        polynomial values by hand; photons started inside a DOM: accepted fraction = p(cos theta_c)
+//                        and every weight = p(cos theta_c); pencil beam: hit fraction = survival x p(d_z);
+//                        weighted and probabilistic modes agree in expectation; mode 0 unchanged
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -263,9 +267,35 @@ inline int intersect_lines(const Geometry& geo, const StringIndex& idx, const Re
 // ------------------------------------------------------------------------------------------
 // One photon, steps 2-10.
 // ------------------------------------------------------------------------------------------
-enum Fate : int { kAbsorbed = 0, kHit = 1, kAborted = 2 };
+enum Fate : int { kAbsorbed = 0, kHit = 1, kAborted = 2, kRejected = 3 };
+
+// ------------------------------------------------------------------------------------------
+// DOM acceptance (NEXT-1; "When a photon intersects a detector, it creates a photoelectron
+// with a probability calculated from its position, direction, time, and wavelength"; the
+// hit record carries a weight).  Reading R-17: the probability depends on the arrival
+// direction only, p(eta) = clamp(sum_k c_k eta^k, 0, 1) with eta = d_z, the cosine between the photon's
+// travel direction at the intersection and +z (the PMT looks down, so an upgoing photon meets its face).
+//   mode 0: every intersection is a hit of weight 1 (acceptance off).
+//   mode 1 (probabilistic): one more uniform, word 0 of Philox block (photon, source, event, 2^31 | k) for an
+//           intersection on flight k; hit of weight 1 iff u < p(eta), otherwise the photon ends in the DOM
+//           without a photoelectron (kRejected).
+//   mode 2 (weighted): no draw; hit of weight p(eta) iff p(eta) > 0, otherwise kRejected.
+// Either way the photon stops at the DOM (R-8).
+// ------------------------------------------------------------------------------------------
+struct Acceptance {
+  int mode;
+  int n_coef;
+  double coef[8];
+};
+
+inline double acceptance(const Acceptance& acc, double eta) {
+  double p = 0, x = 1;
+  for (int k = 0; k < acc.n_coef; ++k) { p += acc.coef[k] * x; x *= eta; }
+  return std::min(1.0, std::max(0.0, p));
+}
 
 struct PhotonResult {
+  double weight;      // hit weight (1 unless the acceptance is in weighted mode)
   int fate;
   int dom;            // hit DOM or -1
   uint32_t n_flights;  // number of flights (segments) started
@@ -279,7 +309,7 @@ constexpr uint32_t kMaxFlights = 100000;  // R-10
 template <class Real>
 inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx, const Ice& ice, uint64_t seed,
                                      const float src[8], uint32_t event_id, uint32_t source_id,
-                                     uint32_t photon_idx) {
+                                     uint32_t photon_idx, const Acceptance* acc = nullptr) {
   const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
   const Real v = Real(kC / ice.n_group);  // group velocity, m/ns
   const Real two_pi = Real(6.283185307179586476925286766559);
@@ -320,7 +350,19 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
       for (int a = 0; a < 3; ++a) p[a] += d[a] * t_hit;
       path += double(t_hit);
       t += double(t_hit) / double(v);
-      r.fate = kHit; r.dom = dom;
+      r.fate = kHit; r.dom = dom; r.weight = 1.0;
+      if (acc && acc->mode != 0) {  // R-17
+        const double pa = acceptance(*acc, double(d[2]));
+        if (acc->mode == 1) {
+          const uint32_t actr[4] = {photon_idx, source_id, event_id, 0x80000000u | k};
+          uint32_t aw[4];
+          philox4x32_10(actr, key, aw);
+          if (!(uniform_from_word(aw[0]) < pa)) r.fate = kRejected;
+        } else {
+          r.weight = pa;
+          if (!(pa > 0.0)) r.fate = kRejected;
+        }
+      }
       break;
     }
     // step 8: advance

@@ -47,15 +47,15 @@ class _Geo(C.Structure):
 
 
 HIT_DTYPE = np.dtype([("event_id", "<u4"), ("source_id", "<u4"), ("photon_idx", "<u4"), ("dom_id", "<u4"),
-                      ("time_ns", "<f8")])
+                      ("time_ns", "<f8"), ("weight", "<f8")])
 FATE_DTYPE = np.dtype([("fate", "<i4"), ("dom", "<i4"), ("n_flights", "<u4"), ("pad", "<u4"),
                        ("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("time_ns", "<f8"), ("path_m", "<f8")])
-FATE_ABSORBED, FATE_HIT, FATE_ABORTED = 0, 1, 2
+FATE_ABSORBED, FATE_HIT, FATE_ABORTED, FATE_REJECTED = 0, 1, 2, 3
 
 
 class _Stats(C.Structure):
     _fields_ = [("photons", C.c_uint64), ("absorbed", C.c_uint64), ("hit", C.c_uint64), ("aborted", C.c_uint64),
-                ("flights", C.c_uint64)]
+                ("flights", C.c_uint64), ("rejected", C.c_uint64)]
 
 
 class _Job(C.Structure):
@@ -64,7 +64,8 @@ class _Job(C.Structure):
                 ("source_id", C.POINTER(C.c_uint32)), ("first", C.POINTER(C.c_uint64)),
                 ("count", C.POINTER(C.c_uint64)), ("stride", C.c_uint64), ("offset", C.c_uint64),
                 ("brute_force", C.c_int32), ("real_type", C.c_int32), ("n_threads", C.c_int32), ("pad", C.c_int32),
-                ("hits", C.c_void_p), ("hit_cap", C.c_uint64), ("fates", C.c_void_p), ("fate_cap", C.c_uint64)]
+                ("hits", C.c_void_p), ("hit_cap", C.c_uint64), ("fates", C.c_void_p), ("fate_cap", C.c_uint64),
+                ("acc_mode", C.c_int32), ("acc_n_coef", C.c_int32), ("acc_coef", C.c_double * 8)]
 
 
 _lib = None
@@ -81,6 +82,8 @@ def lib():
         L.orc_photon_count.argtypes = [C.c_float, C.c_float]
         L.orc_hg_cos.restype = C.c_double
         L.orc_hg_cos.argtypes = [C.c_double, C.c_double]
+        L.orc_acceptance.restype = C.c_double
+        L.orc_acceptance.argtypes = [C.POINTER(C.c_double), C.c_int32, C.c_double]
         L.orc_rotate.restype = None
         L.orc_rotate.argtypes = [C.POINTER(C.c_double), C.c_double, C.c_double, C.POINTER(C.c_double)]
         L.orc_philox4x32_10.restype = None
@@ -139,6 +142,15 @@ def hg_cos(g: float, u: float) -> float:
     return lib().orc_hg_cos(float(g), float(u))
 
 
+def acceptance(coef, eta: float) -> float:
+    """p(eta) of DESIGN.md R-17: the clamped polynomial in the arrival direction cosine."""
+    c = (C.c_double * len(coef))(*[float(np.float32(x)) for x in coef])
+    return lib().orc_acceptance(c, len(coef), float(eta))
+
+
+ACCEPTANCE_MODES = {"off": 0, "probabilistic": 1, "weighted": 2}
+
+
 def rotate(d, cos_t: float, phi: float) -> np.ndarray:
     a = (C.c_double * 3)(*[float(x) for x in d])
     o = (C.c_double * 3)()
@@ -179,11 +191,12 @@ class Result:
     hit: int
     aborted: int
     flights: int
+    rejected: int = 0
 
 
 def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int = 0, first=None, count=None,
               brute_force: bool = False, real_type: str = "f64", n_threads: int = 0, want_fates: bool = False,
-              hit_cap: int | None = None) -> Result:
+              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=()) -> Result:
     """Run the selected photons (``first <= i < first+count`` and ``i % stride == offset``) of
     every source through the oracle.  Hits come back sorted by (event, source, photon)."""
     L = lib()
@@ -221,6 +234,10 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     job.hit_cap = hit_cap
     job.fates = fates.ctypes.data if want_fates and n_sel else None
     job.fate_cap = n_sel if want_fates else 0
+    job.acc_mode = ACCEPTANCE_MODES[acceptance_mode]
+    job.acc_n_coef = len(acceptance_coef)
+    for k, c in enumerate(acceptance_coef):
+        job.acc_coef[k] = float(np.float32(c))  # the same fp32 coefficients the CUDA library receives
     st = _Stats()
     nh = L.orc_propagate(C.byref(job), C.byref(st))
     if nh < 0:
@@ -228,7 +245,7 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     if nh > hit_cap:
         raise RuntimeError(f"oracle: {nh} hits exceed hit_cap {hit_cap}")
     return Result(hits[:nh].copy(), fates if want_fates else None, int(st.photons), int(st.absorbed), int(st.hit),
-                  int(st.aborted), int(st.flights))
+                  int(st.aborted), int(st.flights), int(st.rejected))
 
 
 if __name__ == "__main__":

@@ -27,6 +27,7 @@ struct orc_geometry {
 struct orc_hit {
   uint32_t event_id, source_id, photon_idx, dom_id;
   double time_ns;
+  double weight;
 };
 
 struct orc_fate {
@@ -36,7 +37,7 @@ struct orc_fate {
 };
 
 struct orc_stats {
-  uint64_t photons, absorbed, hit, aborted, flights;
+  uint64_t photons, absorbed, hit, aborted, flights, rejected;
 };
 
 struct orc_job {
@@ -58,12 +59,20 @@ struct orc_job {
   uint64_t hit_cap;
   orc_fate* fates;             // nullable out, capacity fate_cap, in (source, photon) order
   uint64_t fate_cap;
+  int32_t acc_mode;            // DOM acceptance (oracle.hpp, R-17): 0 off, 1 probabilistic, 2 weighted
+  int32_t acc_n_coef;
+  double acc_coef[8];
 };
 
 void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
 double orc_uniform(uint32_t w) { return uniform_from_word(w); }
 uint64_t orc_photon_count(float e, float y) { return photon_count(e, y); }
 double orc_hg_cos(double g, double u) { return hg_cos<double>(g, u); }
+double orc_acceptance(const double* coef, int32_t n_coef, double eta) {
+  Acceptance a{1, n_coef, {0}};
+  for (int k = 0; k < n_coef && k < 8; ++k) a.coef[k] = coef[k];
+  return acceptance(a, eta);
+}
 void orc_rotate(const double* d, double cos_t, double phi, double* out) {
   double v[3] = {d[0], d[1], d[2]};
   rotate<double>(v, cos_t, phi);
@@ -102,6 +111,9 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
   const Ice ice = to_ice(&job->ice);
   StringIndex idx(geo);
   const StringIndex* pidx = job->brute_force ? nullptr : &idx;
+  if (job->acc_n_coef < 0 || job->acc_n_coef > 8 || job->acc_mode < 0 || job->acc_mode > 2) return -1;
+  Acceptance acc{job->acc_mode, job->acc_n_coef, {0}};
+  for (int k = 0; k < job->acc_n_coef; ++k) acc.coef[k] = job->acc_coef[k];
 
   // flatten the selection into work units of (source, [lo, hi)) so threads can share big sources
   struct Unit { uint64_t s, lo, hi, fate_base; };
@@ -137,12 +149,13 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
         const float* src = job->src + 8 * un.s;
         const uint32_t ev = job->event_id[un.s], sid = job->source_id[un.s];
         PhotonResult r = job->real_type == 1
-                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i))
-                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i));
+                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc)
+                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc);
         st[tid].photons++;
         st[tid].flights += r.n_flights;
         if (r.fate == kAbsorbed) st[tid].absorbed++;
-        else if (r.fate == kHit) { st[tid].hit++; hits[tid].push_back(orc_hit{ev, sid, uint32_t(i), uint32_t(r.dom), r.time_ns}); }
+        else if (r.fate == kHit) { st[tid].hit++; hits[tid].push_back(orc_hit{ev, sid, uint32_t(i), uint32_t(r.dom), r.time_ns, r.weight}); }
+        else if (r.fate == kRejected) st[tid].rejected++;
         else st[tid].aborted++;
         if (job->fates && fi < job->fate_cap) {
           orc_fate& f = job->fates[fi];
@@ -163,7 +176,7 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
   for (int t = 0; t < nt; ++t) {
     all.insert(all.end(), hits[t].begin(), hits[t].end());
     tot.photons += st[t].photons; tot.absorbed += st[t].absorbed; tot.hit += st[t].hit;
-    tot.aborted += st[t].aborted; tot.flights += st[t].flights;
+    tot.aborted += st[t].aborted; tot.flights += st[t].flights; tot.rejected += st[t].rejected;
   }
   std::sort(all.begin(), all.end(), [](const orc_hit& a, const orc_hit& b) {
     if (a.event_id != b.event_id) return a.event_id < b.event_id;

@@ -31,6 +31,10 @@ DEPTH_ORIGIN = 1950.0  # m
 STRING_PITCH = 125.0  # m, BASELINE.json configs[1]
 DOM_PITCH = 17.0  # m
 DOMS_PER_STRING = 60
+# Stand-in angular acceptance (R-17; the real DOM acceptance curves are not available): coefficients of
+# p(eta) = 0.35 + 0.5 eta + 0.15 eta^2, eta = cosine between the photon's travel direction and +z; p(-1) = 0 (photon
+# arriving on the back of the down-looking PMT), p(+1) = 1, monotone in between.
+ACCEPTANCE_COEF = (0.35, 0.5, 0.15)
 
 
 @dataclass
