@@ -136,6 +136,7 @@ typedef struct pp_stats_t {
   double wall_ms;           /* first pp_submit .. last drain */
   uint64_t source_ring_high_water; /* bytes */
   uint64_t hit_ring_high_water;    /* bytes */
+  uint64_t photons_rejected;       /* met a DOM but made no photoelectron (pp_set_acceptance); done = absorbed + hit + aborted + rejected */
 } pp_stats_t;
 
 typedef struct pp_handle pp_handle;
@@ -162,6 +163,26 @@ int pp_flush(pp_handle* h);
  * propagated and handed out.  *n_out == 0 with PP_OK then means "drained".  One collector at a time. */
 int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block);
 
+/* DOM acceptance ("When a photon intersects a detector, it creates a photoelectron with a probability
+ * calculated from its position, direction, time, and wavelength"; the hit record carries a weight).
+ * Reading R-17 of DESIGN.md: the probability depends on the arrival direction only,
+ *   p(eta) = clamp(coef[0] + coef[1] eta + ... + coef[n_coef-1] eta^(n_coef-1), 0, 1),
+ * eta = d_z of the photon at the intersection (cosine between its travel direction and +z).
+ *   PP_ACCEPT_OFF            every intersection is a hit of weight 1 (the default after pp_create);
+ *   PP_ACCEPT_PROBABILISTIC  one more uniform, word 0 of Philox block (photon, source, event, 2^31 | k) for an
+ *                            intersection on flight k: hit of weight 1 iff u < p(eta), else the photon is counted in
+ *                            photons_rejected;
+ *   PP_ACCEPT_WEIGHTED       no draw: hit of weight p(eta) iff p(eta) > 0, else rejected.
+ * The photon stops at the DOM in every mode (R-8).  coef is a HOST array of n_coef <= PP_MAX_ACCEPT_COEF floats,
+ * copied before returning (ignored for PP_ACCEPT_OFF).  Applies to launches cut after the call; the server must be
+ * idle (nothing queued or in flight), otherwise PP_E_STATE.  PP_E_INVAL for a bad mode, n_coef or a non-finite
+ * coefficient. */
+#define PP_ACCEPT_OFF 0u
+#define PP_ACCEPT_PROBABILISTIC 1u
+#define PP_ACCEPT_WEIGHTED 2u
+#define PP_MAX_ACCEPT_COEF 8u
+int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n_coef);
+
 int pp_stats(pp_handle* h, pp_stats_t* out);
 const char* pp_last_error(pp_handle* h);
 void pp_destroy(pp_handle* h);
@@ -181,7 +202,7 @@ typedef struct pp_fate {
   double time_ns;      /* end time */
   uint32_t n_flights;
   int32_t dom;         /* hit DOM or -1 */
-  uint32_t fate;       /* 0 absorbed, 1 hit, 2 aborted */
+  uint32_t fate;       /* 0 absorbed, 1 hit, 2 aborted, 3 rejected by the DOM acceptance */
   uint32_t photon_idx;
 } pp_fate;
 

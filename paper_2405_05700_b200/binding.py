@@ -21,6 +21,7 @@ ERRORS = {-1: "PP_E_INVAL", -2: "PP_E_NOMEM", -3: "PP_E_CUDA", -4: "PP_E_OVERFLO
           -6: "PP_E_UNSUPPORTED", -7: "PP_E_STATE"}
 FLAG_BRUTE_FORCE_DOMS = 1
 FLAG_NONBLOCKING_SUBMIT = 2
+ACCEPTANCE_MODES = {"off": 0, "probabilistic": 1, "weighted": 2}
 
 SOURCE_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("dx", "<f4"), ("dy", "<f4"), ("dz", "<f4"),
                          ("t_ns", "<f4"), ("energy_GeV", "<f4")])
@@ -60,12 +61,13 @@ class _Stats(C.Structure):
                 ("photons_absorbed", C.c_uint64), ("photons_hit", C.c_uint64), ("photons_aborted", C.c_uint64),
                 ("flights", C.c_uint64), ("launches", C.c_uint64), ("relaunches", C.c_uint64),
                 ("hits_collected", C.c_uint64), ("kernel_busy_ms", C.c_double), ("wall_ms", C.c_double),
-                ("source_ring_high_water", C.c_uint64), ("hit_ring_high_water", C.c_uint64)]
+                ("source_ring_high_water", C.c_uint64), ("hit_ring_high_water", C.c_uint64),
+                ("photons_rejected", C.c_uint64)]
 
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
-           "pp_photon_count", "pp_debug_plan_launches"]
+           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance"]
 
 
 class _LaunchPlan(C.Structure):
@@ -96,6 +98,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_flush.argtypes = [vp]
     L.pp_collect.restype = C.c_int
     L.pp_collect.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_int]
+    L.pp_set_acceptance.restype = C.c_int
+    L.pp_set_acceptance.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.c_uint32]
     L.pp_stats.restype = C.c_int
     L.pp_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.pp_last_error.restype = C.c_char_p
@@ -190,6 +194,7 @@ class Stats:
     wall_ms: float
     source_ring_high_water: int
     hit_ring_high_water: int
+    photons_rejected: int = 0
 
 
 class Propagator:
@@ -270,6 +275,13 @@ class Propagator:
         assert ev.shape[0] == rec.shape[0] and (sid is None or sid.shape[0] == rec.shape[0])
         rc = self._L.pp_submit(self._h, rec.ctypes.data, ev.ctypes.data, None if sid is None else sid.ctypes.data,
                                rec.shape[0])
+        self._check(rc, self._h)
+
+    def set_acceptance(self, mode: str = "off", coef=()):
+        """pp_set_acceptance: ``mode`` in ACCEPTANCE_MODES; ``coef`` = polynomial coefficients in d_z."""
+        c = np.ascontiguousarray(coef, dtype=np.float32)
+        rc = self._L.pp_set_acceptance(self._h, ACCEPTANCE_MODES[mode], c.ctypes.data_as(C.POINTER(C.c_float)),
+                                       c.shape[0])
         self._check(rc, self._h)
 
     def flush(self):

@@ -454,7 +454,8 @@ int finish_slot(pp_handle* h, Slot& s, bool may_block) {
     h->st.photons_done += hs.photons_started;
     h->st.photons_hit += hs.photons_hit;
     h->st.photons_aborted += hs.photons_aborted;
-    h->st.photons_absorbed += hs.photons_started - hs.photons_hit - hs.photons_aborted;
+    h->st.photons_rejected += hs.photons_rejected;
+    h->st.photons_absorbed += hs.photons_started - hs.photons_hit - hs.photons_aborted - hs.photons_rejected;
     h->st.flights += hs.flights;
     h->st.launches += 1;
     if (t0 > h->busy_end_ms) h->st.kernel_busy_ms += (double)t1 - t0;
@@ -463,15 +464,26 @@ int finish_slot(pp_handle* h, Slot& s, bool may_block) {
   }
   int rc = push_hits(h, std::move(hits), may_block);
   if (rc != PP_OK) return rc;
-  if (hs.n_resume_out > 0) {
+  // items of this launch's resume list that no warp fetched before the ring filled up again
+  const uint32_t res_consumed = std::min<uint32_t>(hs.resume_counter, s.P.n_resume_in);
+  const uint32_t res_rest = s.P.n_resume_in - res_consumed;
+  if (hs.n_resume_out > 0 || res_rest > 0) {
     // ---- ring filled up: relaunch for the deferred photons, the unfinished tiles and the fresh tiles ----
     Status ns{};
     ns.tile_counter = hs.tile_counter;
     *s.h_status_in = ns;
     PP_CUDA(h, cudaMemcpyAsync(s.d_status, s.h_status_in, sizeof(Status), cudaMemcpyHostToDevice, s.stream));
     LaunchParams& P = s.P;
+    uint32_t n_next = std::min<uint32_t>(hs.n_resume_out, P.resume_cap);
+    if (res_rest > 0) {
+      // carry the unfetched items over: append them to the list the launch wrote
+      if ((uint64_t)n_next + res_rest > P.resume_cap) return fail(h, PP_E_CUDA, "internal: resume list overflow");
+      PP_CUDA(h, cudaMemcpyAsync(s.d_resume[s.resume_sel] + n_next, P.resume_in + res_consumed,
+                                 (size_t)res_rest * sizeof(WorkItem), cudaMemcpyDeviceToDevice, s.stream));
+      n_next += res_rest;
+    }
     P.resume_in = s.d_resume[s.resume_sel];
-    P.n_resume_in = std::min<uint32_t>(hs.n_resume_out, P.resume_cap);
+    P.n_resume_in = n_next;
     s.resume_sel ^= 1;
     P.resume_out = s.d_resume[s.resume_sel];
     PP_CUDA(h, cudaEventRecord(s.ev_k0, s.stream));
@@ -960,6 +972,22 @@ int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block) 
     if (idle_locked(h) && h->ring_launch == h->ring_head) return PP_OK;  // drained
     h->cv_hits.wait_for(lk, std::chrono::milliseconds(5));
   }
+}
+
+int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n_coef) {
+  if (!h) return PP_E_INVAL;
+  if (mode > PP_ACCEPT_WEIGHTED) return fail(h, PP_E_INVAL, "pp_set_acceptance: unknown mode");
+  if (mode != PP_ACCEPT_OFF) {
+    if (!coef || n_coef == 0 || n_coef > PP_MAX_ACCEPT_COEF) return fail(h, PP_E_INVAL, "pp_set_acceptance: n_coef out of range");
+    for (uint32_t k = 0; k < n_coef; ++k)
+      if (!finite_f(coef[k])) return fail(h, PP_E_INVAL, "pp_set_acceptance: non-finite coefficient");
+  }
+  std::lock_guard<std::mutex> g(h->mu);
+  if (!idle_locked(h)) return PP_E_STATE;
+  h->base.acc_mode = mode;
+  h->base.acc_n = mode == PP_ACCEPT_OFF ? 0u : n_coef;
+  for (uint32_t k = 0; k < PP_MAX_ACCEPT_COEF; ++k) h->base.acc_coef[k] = (mode != PP_ACCEPT_OFF && k < n_coef) ? coef[k] : 0.0f;
+  return PP_OK;
 }
 
 int pp_stats(pp_handle* h, pp_stats_t* out) {

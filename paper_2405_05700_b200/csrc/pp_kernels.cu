@@ -416,8 +416,29 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     }
 
     // =========================== a8: hit write (warp-aggregated) ================================
-    bool deferred = false;
-    const unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
+    bool deferred = false, rejected = false;
+    unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
+    float weight = 1.0f;
+    if (hit_mask && P.acc_mode != 0u) {
+      // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z; rare path ----
+      if (hit) {
+        float pa = 0.0f;
+        for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
+        pa = fminf(fmaxf(pa, 0.0f), 1.0f);
+        if (P.acc_mode == 1u) {
+          uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | (k - 1u);  // k was advanced: the hit flight is k - 1
+          philox4x32_10(a0, a1, a2, a3, P.rk);
+          rejected = !(uniform_from_word(a0) < pa);
+        } else {
+          weight = pa;
+          rejected = !(pa > 0.0f);
+        }
+        hit = !rejected;
+      }
+      const unsigned rej_mask = __ballot_sync(0xffffffffu, rejected);
+      if (rej_mask && (int)lane == __ffs(rej_mask) - 1) atomicAdd(&st->photons_rejected, (unsigned long long)__popc(rej_mask));
+      hit_mask &= ~rej_mask;
+    }
     if (hit_mask) {
       const unsigned n_hit = __popc(hit_mask);
       unsigned base = 0;
@@ -431,7 +452,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           pp_hit h;
           h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
           h.time_ns = t0 + ((double)Lh + (double)Ll) * P.inv_v;
-          h.weight = 1.0f; h.n_scatter = k - 1;
+          h.weight = weight; h.n_scatter = k - 1;
           uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
           const uint4* srcv = reinterpret_cast<const uint4*>(&h);
           dst[0] = srcv[0];
@@ -463,8 +484,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         f.path_m = Lh + Ll;
         f.time_ns = (double)__ldg(&P.src[s_mine].t) + ((double)Lh + (double)Ll) * P.inv_v;
         f.n_flights = k;
-        f.dom = hit ? (int32_t)hit_dom : -1;
-        f.fate = hit ? 1u : (aborted ? 2u : 0u);
+        f.dom = (hit || rejected) ? (int32_t)hit_dom : -1;
+        f.fate = hit ? 1u : (rejected ? 3u : (aborted ? 2u : 0u));
         f.photon_idx = pidx;
         reinterpret_cast<pp_fate*>(P.fates)[g] = f;
       }

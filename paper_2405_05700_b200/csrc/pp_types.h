@@ -36,6 +36,7 @@ struct Status {                 // one per launch slot, device memory, copied ba
   unsigned long long photons_hit;
   unsigned long long photons_aborted;
   unsigned long long flights;
+  unsigned long long photons_rejected;  // met a DOM, no photoelectron (acceptance)
   unsigned int hit_count;       // hits reserved in the ring this launch (may exceed ring_cap)
   unsigned int resume_counter;  // next resume_in item
   unsigned int n_resume_out;    // items written to resume_out
@@ -90,6 +91,9 @@ struct LaunchParams {
   float one_minus_cos_c;                             // 1 - cos(theta_c)
   double inv_v;                                      // n_group / c  [ns/m]
   uint32_t rk[10][2];                                // Philox round keys
+  // DOM acceptance (pp_set_acceptance, R-17): mode 0 off, 1 probabilistic, 2 weighted
+  uint32_t acc_mode, acc_n;
+  float acc_coef[8];
   // geometry
   const StringRec* strings;  // [n_strings]
   const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id

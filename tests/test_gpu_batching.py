@@ -82,6 +82,21 @@ def test_hit_ring_overflow_replay_protocol(case, reference_hits, ring_bytes):
     assert st.photons_hit == len(hits)
 
 
+def test_ring_overflow_with_unfetched_resume_items():
+    """Hits so frequent (5 m DOMs) that a 32-hit ring fills up again before the warps have fetched the whole resume
+    list of a relaunch: the unfetched items must be carried over to the next relaunch, not dropped."""
+    geo, ice = W.geometry_full(radius=5.0), W.ice_layered()
+    src = W.sources_c1().subset(slice(0, 8))
+    src.src[:, 7] = 2.0  # 2e4 photons per cascade
+    n = total_photons(src, ice)
+    ref, st0 = gpu_run(geo, ice, src, 4)
+    assert st0.relaunches == 0 and len(ref) > 5000
+    hits, st = gpu_run(geo, ice, src, 4, launch_photons_target=10 ** 6, hit_ring_bytes=2 * 32 * 32)
+    assert st.relaunches > 100
+    assert st.photons_done == n == st.photons_absorbed + st.photons_hit and st.flights == st0.flights
+    assert np.array_equal(hits, ref)
+
+
 def test_streaming_collect_while_producing(case, reference_hits):
     """Hits of one event may arrive across several pp_collect calls; a consumer thread drains while
     producers are still submitting."""
