@@ -657,7 +657,7 @@ bool idle_locked(pp_handle* h) {
 // =============================================================================================
 extern "C" {
 
-const char* pp_version(void) { return "pp 0.2 (sm_100a)"; }
+const char* pp_version(void) { return "pp 0.3 (sm_100a)"; }
 
 int pp_check_inputs(const pp_geometry* geo, const pp_ice* ice, uint32_t flags) {
   std::string why;
@@ -859,8 +859,10 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.resume_out = h->slot[0].d_resume[0]; P.resume_in = h->slot[0].d_resume[1]; P.resume_cap = (uint32_t)h->sz.resume_cap;
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
     P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
-    for (int f = 0; f < 2; ++f)
-      if (launch_propagate(P, h->brute, f == 1, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
+    for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x acceptance
+      P.acc_mode = (f & 2) ? 1u : 0u;
+      if (launch_propagate(P, h->brute, (f & 1) != 0, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
+    }
     if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     if (propagate_occupancy(h->brute, false, h->smem, &bps) != cudaSuccess || bps < 1) return bail(PP_E_CUDA);
     h->grid = h->n_sm * bps;

@@ -177,7 +177,7 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
   return best;
 }
 
-template <bool kBrute, bool kFates>
+template <bool kBrute, bool kFates, bool kAcc>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // table offsets come from the constant bank (LaunchParams), not from registers
@@ -419,7 +419,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     bool deferred = false, rejected = false;
     unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
     float weight = 1.0f;
-    if (hit_mask && P.acc_mode != 0u) {
+    if (kAcc && hit_mask) {
       // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z; rare path ----
       if (hit) {
         float pa = 0.0f;
@@ -551,30 +551,45 @@ size_t propagate_smem_layout(LaunchParams* P) {
   return o;
 }
 
-template <bool B, bool F>
+template <bool B, bool F, bool A>
 static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
   static std::atomic<size_t> attr_smem{0};  // opt-in dynamic shared memory size set so far
   if (smem > attr_smem.load()) {
-    cudaError_t e = cudaFuncSetAttribute(propagate_kernel<B, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(propagate_kernel<B, F, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_smem.store(smem);
   }
-  propagate_kernel<B, F><<<grid, kBlockThreads, smem, st>>>(P);
+  propagate_kernel<B, F, A><<<grid, kBlockThreads, smem, st>>>(P);
   g_launches++;
   return cudaGetLastError();
 }
 
+// the kernel variant is picked by (brute-force DOM test, fate dump, DOM acceptance on)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  if (brute) return fates ? launch_prop_t<true, true>(P, grid, smem, st) : launch_prop_t<true, false>(P, grid, smem, st);
-  return fates ? launch_prop_t<false, true>(P, grid, smem, st) : launch_prop_t<false, false>(P, grid, smem, st);
+  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | (P.acc_mode != 0u ? 1 : 0);
+  switch (v) {
+    case 0: return launch_prop_t<false, false, false>(P, grid, smem, st);
+    case 1: return launch_prop_t<false, false, true>(P, grid, smem, st);
+    case 2: return launch_prop_t<false, true, false>(P, grid, smem, st);
+    case 3: return launch_prop_t<false, true, true>(P, grid, smem, st);
+    case 4: return launch_prop_t<true, false, false>(P, grid, smem, st);
+    case 5: return launch_prop_t<true, false, true>(P, grid, smem, st);
+    case 6: return launch_prop_t<true, true, false>(P, grid, smem, st);
+    default: return launch_prop_t<true, true, true>(P, grid, smem, st);
+  }
 }
 
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
-  if (brute)
-    return fates ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<true, true>, kBlockThreads, smem)
-                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<true, false>, kBlockThreads, smem);
-  return fates ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<false, true>, kBlockThreads, smem)
-               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, propagate_kernel<false, false>, kBlockThreads, smem);
+  // all variants are compiled for the same launch bounds; the leanest and the fullest bracket the rest
+  int a = 0, b = 0;
+  cudaError_t e = brute ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, propagate_kernel<true, true, true>, kBlockThreads, smem)
+                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, propagate_kernel<false, true, true>, kBlockThreads, smem);
+  if (e != cudaSuccess) return e;
+  e = brute ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, propagate_kernel<true, false, false>, kBlockThreads, smem)
+            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, propagate_kernel<false, false, false>, kBlockThreads, smem);
+  (void)fates;
+  *blocks_per_sm = a < b ? a : b;
+  return e;
 }
 
 }  // namespace pp
