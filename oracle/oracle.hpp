@@ -29,6 +29,10 @@
 //                        polynomial values by hand; photons started inside a DOM: accepted fraction = p(cos theta_c)
 //                        and every weight = p(cos theta_c); pencil beam: hit fraction = survival x p(d_z);
 //                        weighted and probabilistic modes agree in expectation; mode 0 unchanged
+//   propagate with a source length (NEXT-2, R-18)
+//                        beam along the axis at a DOM ahead: hit fraction (lambda/L) e^{-(D-R)/lambda} (e^{L/lambda} - 1),
+//                        arrival times l/c + (D-R-l)/v and the mean emission offset of the hits; mean end-point
+//                        displacement L/2 + 1/(a+b(1-g)); L = 0 is the point source bit for bit
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -309,7 +313,7 @@ constexpr uint32_t kMaxFlights = 100000;  // R-10
 template <class Real>
 inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx, const Ice& ice, uint64_t seed,
                                      const float src[8], uint32_t event_id, uint32_t source_id,
-                                     uint32_t photon_idx, const Acceptance* acc = nullptr) {
+                                     uint32_t photon_idx, const Acceptance* acc = nullptr, float length = 0.0f) {
   const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
   const Real v = Real(kC / ice.n_group);  // group velocity, m/ns
   const Real two_pi = Real(6.283185307179586476925286766559);
@@ -330,6 +334,14 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
     const Real u_dist = Real(uniform_from_word(w[2])), u_abs = Real(uniform_from_word(w[3]));
     Real cos_t;
     if (k == 0) {
+      // R-18 (NEXT-2, track segments: PAPER.md:29 continuous losses, "photon emitting steps"): a source of
+      // length L > 0 emits from a point uniform on [0, L] along its axis, at the time the muon (speed c, R-11b) is
+      // there; the offset uses the word of block 0 that flight 0 leaves unused (u_hg).  L = 0: point cascade (R-4).
+      if (length > 0.0f) {
+        const Real ell = u_hg * Real(length);
+        for (int a = 0; a < 3; ++a) p[a] += d[a] * ell;  // d is still the source axis here
+        t += double(ell) / kC;
+      }
       cos_t = Real(ice.cos_cherenkov);  // step 2: emission on the Cherenkov cone about the source axis (R-4)
       tau_a = -std::log(u_abs);         // step 3: absorption budget, drawn once per photon
     } else {

@@ -65,7 +65,8 @@ class _Job(C.Structure):
                 ("count", C.POINTER(C.c_uint64)), ("stride", C.c_uint64), ("offset", C.c_uint64),
                 ("brute_force", C.c_int32), ("real_type", C.c_int32), ("n_threads", C.c_int32), ("pad", C.c_int32),
                 ("hits", C.c_void_p), ("hit_cap", C.c_uint64), ("fates", C.c_void_p), ("fate_cap", C.c_uint64),
-                ("acc_mode", C.c_int32), ("acc_n_coef", C.c_int32), ("acc_coef", C.c_double * 8)]
+                ("acc_mode", C.c_int32), ("acc_n_coef", C.c_int32), ("acc_coef", C.c_double * 8),
+                ("length", C.POINTER(C.c_float))]
 
 
 _lib = None
@@ -196,7 +197,7 @@ class Result:
 
 def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int = 0, first=None, count=None,
               brute_force: bool = False, real_type: str = "f64", n_threads: int = 0, want_fates: bool = False,
-              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=()) -> Result:
+              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None) -> Result:
     """Run the selected photons (``first <= i < first+count`` and ``i % stride == offset``) of
     every source through the oracle.  Hits come back sorted by (event, source, photon)."""
     L = lib()
@@ -234,6 +235,11 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     job.hit_cap = hit_cap
     job.fates = fates.ctypes.data if want_fates and n_sel else None
     job.fate_cap = n_sel if want_fates else 0
+    if lengths is None:
+        lengths = getattr(sources, "length", None)
+    len_arr = None if lengths is None else np.ascontiguousarray(lengths, dtype=np.float32)
+    assert len_arr is None or len_arr.shape[0] == n
+    job.length = None if len_arr is None else _fp(len_arr)
     job.acc_mode = ACCEPTANCE_MODES[acceptance_mode]
     job.acc_n_coef = len(acceptance_coef)
     for k, c in enumerate(acceptance_coef):

@@ -62,6 +62,7 @@ struct orc_job {
   int32_t acc_mode;            // DOM acceptance (oracle.hpp, R-17): 0 off, 1 probabilistic, 2 weighted
   int32_t acc_n_coef;
   double acc_coef[8];
+  const float* length;         // nullable: source lengths in metres (oracle.hpp, R-18); default 0 = point sources
 };
 
 void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
@@ -148,9 +149,10 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
       for (uint64_t i = un.lo; i < un.hi; i += job->stride, ++fi) {
         const float* src = job->src + 8 * un.s;
         const uint32_t ev = job->event_id[un.s], sid = job->source_id[un.s];
+        const float len = job->length ? job->length[un.s] : 0.0f;
         PhotonResult r = job->real_type == 1
-                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc)
-                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc);
+                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len)
+                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len);
         st[tid].photons++;
         st[tid].flights += r.n_flights;
         if (r.fate == kAbsorbed) st[tid].absorbed++;

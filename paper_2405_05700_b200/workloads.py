@@ -76,13 +76,15 @@ class Sources:
     event_id: np.ndarray  # uint32 [n]
     source_id: np.ndarray  # uint32 [n]  (index of the source within its event)
     meta: dict = field(default_factory=dict)
+    length: np.ndarray | None = None  # float32 [n] metres: track segments (R-18); None = point sources
 
     def __len__(self) -> int:
         return int(self.src.shape[0])
 
     def subset(self, sel) -> "Sources":
         return Sources(np.ascontiguousarray(self.src[sel]), np.ascontiguousarray(self.event_id[sel]),
-                       np.ascontiguousarray(self.source_id[sel]), dict(self.meta))
+                       np.ascontiguousarray(self.source_id[sel]), dict(self.meta),
+                       None if self.length is None else np.ascontiguousarray(self.length[sel]))
 
 
 # --------------------------------------------------------------------------------------
@@ -224,6 +226,28 @@ def sources_c1(seed: int = 1, n_casc: int = 200) -> Sources:
     e = np.exp(rng.uniform(math.log(1.0), math.log(1.0e4), size=n_casc))
     dirs = np.repeat(d[None, :], n_casc, axis=0)
     return _pack(pos, dirs, t, e, np.zeros(n_casc), np.arange(n_casc), {"config": "C1", "gen_seed": seed})
+
+
+def sources_track(seed: int = 5, n_seg: int = 100, seg_len: float = 10.0, gev_per_m: float = 0.03,
+                  n_casc: int = 20) -> Sources:
+    """NEXT-2 stand-in (R-18): a muon through the array centre (zenith 30 deg, seeded azimuth) whose own
+    Cherenkov light comes from ``n_seg`` contiguous track segments of ``seg_len`` metres (light-equivalent energy
+    ``gev_per_m`` per metre), plus ``n_casc`` point cascades (length 0) with dN/dE ~ 1/E on [1, 100] GeV."""
+    rng = np.random.default_rng(seed)
+    azimuth = 2.0 * math.pi * rng.uniform()
+    d = travel_direction(math.radians(30.0), azimuth)
+    half = 0.5 * n_seg * seg_len
+    start = -half + seg_len * np.arange(n_seg)
+    pos = start[:, None] * d[None, :]
+    t = (start + half) / C_VACUUM
+    e = np.full(n_seg, gev_per_m * seg_len)
+    cpos, ct = _track_cascades(rng, np.zeros(3), d, n_casc, half_len=half)
+    ce = np.exp(rng.uniform(math.log(1.0), math.log(100.0), size=n_casc))
+    n = n_seg + n_casc
+    out = _pack(np.concatenate([pos, cpos]), np.repeat(d[None, :], n, axis=0), np.concatenate([t, ct]),
+                np.concatenate([e, ce]), np.zeros(n), np.arange(n), {"config": "track", "gen_seed": seed})
+    out.length = np.concatenate([np.full(n_seg, seg_len), np.zeros(n_casc)]).astype(np.float32)
+    return out
 
 
 def _power_law(rng, gamma, e0, e1, size=None):
