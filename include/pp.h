@@ -155,6 +155,16 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
 int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids, const uint32_t* source_ids,
               size_t n);
 
+/* pp_submit for extended sources (NEXT-2, reading R-18 of DESIGN.md; a muon's energy loss is split into
+ * continuous and stochastic losses; "photon emitting steps").  lengths_m[n] (HOST, nullable = all 0):
+ * a source with length L > 0 is a straight track segment from its position along its direction; each of its
+ * photons starts at a point uniform on the segment, offset l = u L with u = word 1 of the photon's Philox block 0
+ * (the word flight 0 leaves unused), at time t_ns + l / c (the muon moves at c), on the Cherenkov cone about the
+ * direction as for a point source.  L = 0 is the point cascade of pp_submit.  PP_E_INVAL for a negative or
+ * non-finite length.  Everything else as pp_submit. */
+int pp_submit_segments(pp_handle* h, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
+                       const uint32_t* source_ids, size_t n);
+
 /* Asks the server to launch whatever is queued even if it is less than launch_photons_target. */
 int pp_flush(pp_handle* h);
 

@@ -67,7 +67,7 @@ class _Stats(C.Structure):
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
-           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance"]
+           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments"]
 
 
 class _LaunchPlan(C.Structure):
@@ -94,6 +94,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Ice), C.POINTER(_Config), C.POINTER(vp)]
     L.pp_submit.restype = C.c_int
     L.pp_submit.argtypes = [vp, vp, vp, vp, C.c_size_t]
+    L.pp_submit_segments.restype = C.c_int
+    L.pp_submit_segments.argtypes = [vp, vp, vp, vp, vp, C.c_size_t]
     L.pp_flush.restype = C.c_int
     L.pp_flush.argtypes = [vp]
     L.pp_collect.restype = C.c_int
@@ -267,14 +269,21 @@ class Propagator:
             pass
 
     # ---- the paper's calls ----
-    def submit(self, sources, event_ids, source_ids=None):
-        """pp_submit: ``sources`` float32 [n, 8] (or SOURCE_DTYPE [n]); host buffers; thread-safe."""
+    def submit(self, sources, event_ids, source_ids=None, lengths=None):
+        """pp_submit (pp_submit_segments when ``lengths`` [n] metres is given): ``sources`` float32 [n, 8] (or
+        SOURCE_DTYPE [n]); host buffers; thread-safe."""
         rec = pack_sources(sources) if sources.dtype != SOURCE_DTYPE else np.ascontiguousarray(sources)
         ev = np.ascontiguousarray(event_ids, dtype=np.uint32)
         sid = None if source_ids is None else np.ascontiguousarray(source_ids, dtype=np.uint32)
         assert ev.shape[0] == rec.shape[0] and (sid is None or sid.shape[0] == rec.shape[0])
-        rc = self._L.pp_submit(self._h, rec.ctypes.data, ev.ctypes.data, None if sid is None else sid.ctypes.data,
-                               rec.shape[0])
+        if lengths is None:
+            rc = self._L.pp_submit(self._h, rec.ctypes.data, ev.ctypes.data, None if sid is None else sid.ctypes.data,
+                                   rec.shape[0])
+        else:
+            ln = np.ascontiguousarray(lengths, dtype=np.float32)
+            assert ln.shape[0] == rec.shape[0]
+            rc = self._L.pp_submit_segments(self._h, rec.ctypes.data, ln.ctypes.data, ev.ctypes.data,
+                                            None if sid is None else sid.ctypes.data, rec.shape[0])
         self._check(rc, self._h)
 
     def set_acceptance(self, mode: str = "off", coef=()):
@@ -305,9 +314,9 @@ class Propagator:
             parts.append(h.copy())
         return np.concatenate(parts) if parts else np.empty(0, dtype=HIT_DTYPE)
 
-    def run(self, sources, event_ids, source_ids=None) -> np.ndarray:
+    def run(self, sources, event_ids, source_ids=None, lengths=None) -> np.ndarray:
         """End-to-end convenience: submit + flush + collect everything (host buffers in and out)."""
-        self.submit(sources, event_ids, source_ids)
+        self.submit(sources, event_ids, source_ids, lengths)
         return self.collect_all()
 
     def stats(self) -> Stats:

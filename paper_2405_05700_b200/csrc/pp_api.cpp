@@ -368,7 +368,7 @@ uint64_t carve_pinned(pp_handle* h, void* base) {
 // Enqueue tiles + propagate (+ status read-back) for photons [g_begin, g_end) of the batch
 // (src, cum, n_src), which must already be (or be enqueued to become) resident on slot.stream.
 int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long long* cum, uint32_t n_src,
-                   uint64_t g_begin, uint64_t g_end, pp_fate* fates) {
+                   uint64_t g_begin, uint64_t g_end, pp_fate* fates, bool has_segments) {
   const uint64_t n_ph = g_end - g_begin;
   // tile size: 1024 photons for large launches; a small launch is cut finer so that every resident warp gets work
   // (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3)
@@ -381,6 +381,7 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long
   LaunchParams P = h->base;
   P.src = src; P.cum = cum; P.cum_rel = s.d_cum_rel; P.tile_src = s.d_tile_src;
   P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles; P.tile_photons = tile;
+  P.has_segments = has_segments ? 1u : 0u;
   s.resume_sel = 0;
   P.resume_in = s.d_resume[1]; P.resume_out = s.d_resume[0];
   P.n_resume_in = 0; P.resume_cap = (uint32_t)h->sz.resume_cap;
@@ -618,7 +619,9 @@ void server_main(pp_handle* h) {
           if (e == cudaSuccess) e = cudaEventRecord(s.ev_h2d, s.stream);
           if (e == cudaSuccess) e = launch_scan(s.d_src, n_src, s.d_cum, s.stream);
           if (e != cudaSuccess) rc = fail(h, PP_E_CUDA, std::string("upload: ") + cudaGetErrorString(e));
-          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr);
+          bool seg = false;  // any track segment among the records of this launch?
+          for (uint32_t q = 0; q < n_src && !seg; ++q) seg = h->ring[(rec_a + q) % cap].length > 0.0f;
+          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg);
           if (rc == PP_OK && cudaEventSynchronize(s.ev_h2d) != cudaSuccess) rc = fail(h, PP_E_CUDA, "upload sync failed");
         }
         lk.lock();
@@ -787,6 +790,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   B.hg_one_minus_g = (float)(1.0 - g); B.hg_two_g = (float)(2.0 * g); B.hg_one_minus_g2 = (float)(1.0 - g * g);
   B.one_minus_cos_c = (float)(1.0 - (double)ice->cos_cherenkov);
   B.inv_v = (double)ice->n_group / kC;
+  B.inv_c = (float)(1.0 / kC);
   {
     uint32_t k0 = (uint32_t)cfg->seed, k1 = (uint32_t)(cfg->seed >> 32);
     for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
@@ -859,7 +863,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.resume_out = h->slot[0].d_resume[0]; P.resume_in = h->slot[0].d_resume[1]; P.resume_cap = (uint32_t)h->sz.resume_cap;
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
     P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
-    for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x acceptance
+    for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x optional physics
       P.acc_mode = (f & 2) ? 1u : 0u;
       if (launch_propagate(P, h->brute, (f & 1) != 0, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     }
@@ -875,6 +879,11 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
 }
 
 int pp_submit(pp_handle* h, const pp_source* src, const uint32_t* event_ids, const uint32_t* source_ids, size_t n) {
+  return pp_submit_segments(h, src, nullptr, event_ids, source_ids, n);
+}
+
+int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths, const uint32_t* event_ids,
+                       const uint32_t* source_ids, size_t n) {
   if (!h) return PP_E_INVAL;
   if (h->sticky.load() != PP_OK) return h->sticky.load();
   if (n == 0) return PP_OK;
@@ -889,6 +898,7 @@ int pp_submit(pp_handle* h, const pp_source* src, const uint32_t* event_ids, con
     const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
     if (std::fabs(n2 - 1.0) > 1e-4) return fail(h, PP_E_INVAL, "source direction is not a unit vector");
     if (a.energy_GeV < 0.0f) return fail(h, PP_E_INVAL, "negative source energy");
+    if (lengths && !(std::isfinite(lengths[i]) && lengths[i] >= 0.0f)) return fail(h, PP_E_INVAL, "bad source length");
     if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
       return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
   }
@@ -922,7 +932,7 @@ int pp_submit(pp_handle* h, const pp_source* src, const uint32_t* event_ids, con
       r.event_id = event_ids[i];
       r.source_id = source_ids ? source_ids[i] : (uint32_t)i;
       r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
-      r.pad = 0;
+      r.length = lengths ? lengths[i] : 0.0f;
       ph += r.n_photons;
     }
     h->ring_head += m;
@@ -1085,7 +1095,7 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
     rc = drain_slot(h, s, false);
     if (rc != PP_OK) break;
     const uint64_t g1 = std::min(total, g0 + h->sz.target);
-    rc = enqueue_launch(h, s, h->d_res_src, h->d_res_cum, (uint32_t)n, g0, g1, d_fates);
+    rc = enqueue_launch(h, s, h->d_res_src, h->d_res_cum, (uint32_t)n, g0, g1, d_fates, false);
     which ^= 1;
   }
   // retire in launch order

@@ -41,7 +41,7 @@ __global__ void ingest_kernel(const pp_source* __restrict__ s, const uint32_t* _
   if (cnt > 0xFFFFFFFFull) { atomicExch(overflow, 1u); cnt = 0; }
   SrcRec r;
   r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
-  r.event_id = ev[i]; r.source_id = sid ? sid[i] : i; r.n_photons = (uint32_t)cnt; r.pad = 0;
+  r.event_id = ev[i]; r.source_id = sid ? sid[i] : i; r.n_photons = (uint32_t)cnt; r.length = 0.0f;
   out[i] = r;
 }
 
@@ -177,7 +177,8 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
   return best;
 }
 
-template <bool kBrute, bool kFates, bool kAcc>
+// kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18) is compiled in
+template <bool kBrute, bool kFates, bool kExt>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // table offsets come from the constant bank (LaunchParams), not from registers
@@ -307,6 +308,13 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
       const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
       const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
+      if (kExt && P.has_segments != 0u && k == 0) {
+        // R-18: a source with a length emits from a point uniform along it; u_hg is free on flight 0
+        const float ell = u_hg * __ldg(&P.src[s_mine].length);
+        const float nx_ = fmaf(dx, ell, phx); plx += fmaf(dx, ell, phx - nx_); phx = nx_;
+        const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
+        const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
+      }
       rotate(dx, dy, dz, m, u_az);
       // =========================== a3: absorption budget (once per photon) ======================
       const float tau_new = -__logf(u_abs);
@@ -419,7 +427,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     bool deferred = false, rejected = false;
     unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
     float weight = 1.0f;
-    if (kAcc && hit_mask) {
+    if (kExt && P.acc_mode != 0u && hit_mask) {
       // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z; rare path ----
       if (hit) {
         float pa = 0.0f;
@@ -448,7 +456,13 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       if (hit) {
         const unsigned slot = base + __popc(hit_mask & lt);
         if (slot < P.ring_cap) {
-          const double t0 = (double)__ldg(&P.src[s_mine].t);
+          double t0 = (double)__ldg(&P.src[s_mine].t);
+          if (kExt && P.has_segments != 0u) {
+            // R-18: emitted l / c after the source time; l is recomputed from block 0 instead of being carried
+            uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0u;
+            philox4x32_10(e0, e1, e2, e3, P.rk);
+            t0 += (double)(uniform_from_word(e1) * __ldg(&P.src[s_mine].length)) * (double)P.inv_c;
+          }
           pp_hit h;
           h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
           h.time_ns = t0 + ((double)Lh + (double)Ll) * P.inv_v;
@@ -564,9 +578,9 @@ static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, c
   return cudaGetLastError();
 }
 
-// the kernel variant is picked by (brute-force DOM test, fate dump, DOM acceptance on)
+// the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | (P.acc_mode != 0u ? 1 : 0);
+  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u) ? 1 : 0);
   switch (v) {
     case 0: return launch_prop_t<false, false, false>(P, grid, smem, st);
     case 1: return launch_prop_t<false, false, true>(P, grid, smem, st);

@@ -12,7 +12,8 @@ namespace pp {
 struct __align__(16) SrcRec {  // 48 B: one light source as the kernels see it
   float x, y, z, dx;
   float dy, dz, t, energy;
-  uint32_t event_id, source_id, n_photons, pad;
+  uint32_t event_id, source_id, n_photons;
+  float length;  // metres; 0 = point source (R-18)
 };
 
 struct __align__(16) IceLayer {  // per-layer coefficients (1/m) and lengths (m)
@@ -93,6 +94,8 @@ struct LaunchParams {
   uint32_t rk[10][2];                                // Philox round keys
   // DOM acceptance (pp_set_acceptance, R-17): mode 0 off, 1 probabilistic, 2 weighted
   uint32_t acc_mode, acc_n;
+  uint32_t has_segments;  // some source of this launch has length > 0 (R-18)
+  float inv_c;            // 1 / c  [ns/m]
   float acc_coef[8];
   // geometry
   const StringRec* strings;  // [n_strings]

@@ -1,0 +1,89 @@
+"""GPU parity of the extended (track-segment) sources (NEXT-2, R-18) against the oracle, through the C ABI."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2405_05700_b200 import binding as B
+from paper_2405_05700_b200 import workloads as W
+
+from gpu_util import compare_hits, sort_hits, total_photons
+
+pytestmark = pytest.mark.gpu
+C = W.C_VACUUM
+V = C / float(np.float32(W.N_GROUP))
+
+
+def run(geo, ice, src, seed, lengths, acceptance=None, **kw):
+    with B.Propagator(geo, ice, seed=seed, **kw) as p:
+        if acceptance:
+            p.set_acceptance(acceptance, W.ACCEPTANCE_COEF)
+        hits = sort_hits(p.run(src.src, src.event_id, src.source_id, lengths))
+        st = p.stats()
+    return hits, st
+
+
+def test_track_with_cascades_per_photon():
+    """A muon as 100 track segments of 10 m plus 20 point cascades, full detector with oversized DOMs, layered ice."""
+    geo, ice = W.geometry_full(radius=1.0), W.ice_layered()
+    src = W.sources_track()
+    src.src[:, 7] = np.minimum(src.src[:, 7], 2.0) + 1.0
+    n = total_photons(src, ice)
+    assert n > 1.0e6
+    hits, st = run(geo, ice, src, 6, src.length, launch_photons_target=400000)
+    ref = O.propagate(geo, ice, src, seed=6)
+    assert st.photons_done == n == ref.photons and st.launches >= 3
+    assert st.flights == ref.flights
+    assert ref.hit > 1000 and abs(st.photons_hit - ref.hit) <= 2
+    c = compare_hits(hits, ref.hits, n)
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.97, c
+    # the lengths matter: the same list as point sources gives a different hit list
+    pts, _ = run(geo, ice, src, 6, None, launch_photons_target=400000)
+    assert not np.array_equal(pts, hits)
+    # ... and lengths of zero are the point sources bit for bit
+    zer, _ = run(geo, ice, src, 6, np.zeros(len(src), np.float32), launch_photons_target=400000)
+    assert np.array_equal(pts, zer)
+    # batching invariance with segments on (a launch of point sources only next to launches with segments)
+    one, st1 = run(geo, ice, src, 6, src.length, launch_photons_target=10 ** 8)
+    assert st1.launches == 1 and np.array_equal(one, hits)
+
+
+def test_closed_form_on_the_gpu():
+    """The oracle's pin: beam along the axis from a 20 m segment at a DOM 30 m ahead, scattering off."""
+    lam, L, D, n = 100.0, 20.0, 30.0, 400000
+    R = float(np.float32(W.DOM_RADIUS))
+    geo = W.Geometry(xyz=np.array([[0.0, 0.0, D]], np.float32), radius=W.DOM_RADIUS)
+    ice = W.ice_homogeneous(scat_len=1.0e30, cos_cherenkov=1.0)
+    src = W.pencil_beam([0, 0, 0], [0, 0, 1], float(n), t0=7.0)
+    hits, st = run(geo, ice, src, 21, [L], flags=B.FLAG_BRUTE_FORCE_DOMS)
+    frac = lam / L * math.exp(-(D - R) / lam) * (math.exp(L / lam) - 1.0)
+    assert st.photons_hit / n == pytest.approx(frac, abs=4 * math.sqrt(frac * (1 - frac) / n))
+    t = hits["time_ns"] - 7.0
+    t_hi = (D - R) / V
+    t_lo = t_hi - L * (1.0 / V - 1.0 / C)
+    assert t.min() >= t_lo - 1e-4 and t.max() <= t_hi + 1e-4
+    ell = (t_hi - t) / (1.0 / V - 1.0 / C)
+    mean_ell = L * math.exp(L / lam) / (math.exp(L / lam) - 1.0) - lam
+    assert ell.mean() == pytest.approx(mean_ell, abs=4 * L / math.sqrt(12 * len(ell)))
+    ref = O.propagate(geo, ice, src, seed=21, brute_force=True, lengths=[L])
+    c = compare_hits(hits, ref.hits, n)
+    assert c["frac_all"] >= 0.9999 and c["max_dt"] <= 1e-3, c
+
+
+def test_segments_with_acceptance_and_bad_lengths():
+    geo, ice = W.geometry_full(radius=1.0), W.ice_layered()
+    src = W.sources_track(n_seg=40, n_casc=10)
+    src.src[:, 7] = 2.0
+    n = total_photons(src, ice)
+    hits, st = run(geo, ice, src, 8, src.length, acceptance="weighted")
+    ref = O.propagate(geo, ice, src, seed=8, acceptance_mode="weighted", acceptance_coef=W.ACCEPTANCE_COEF)
+    assert st.photons_done == n and st.flights == ref.flights and abs(st.photons_hit - ref.hit) <= 2
+    c = compare_hits(hits, ref.hits, n)
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.97, c
+    with B.Propagator(geo, ice, seed=0) as p:
+        for bad in (-1.0, float("nan"), float("inf")):
+            with pytest.raises(B.PPError) as e:
+                p.submit(src.src[:1], src.event_id[:1], src.source_id[:1], [bad])
+            assert e.value.code == -1
+        assert len(p.collect_all()) == 0
