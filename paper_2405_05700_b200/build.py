@@ -12,8 +12,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpp.so")
-SOURCES = ["pp_kernels.cu", "pp_api.cpp"]
-DEPS = SOURCES + ["pp_device.cuh", "pp_types.h", "pp_internal.h", os.path.join("..", "..", "include", "pp.h")]
+SOURCES = ["pp_kernels.cu", "pp_api.cpp", "pp_ipc.cpp"]
+DEPS = SOURCES + ["pp_device.cuh", "pp_types.h", "pp_internal.h", os.path.join("..", "..", "include", "pp.h"),
+                  os.path.join("..", "..", "include", "pp_ipc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -31,7 +32,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     extra = os.environ.get("PP_NVCC_EXTRA", "").split()  # e.g. -DPP_MIN_BLOCKS=4 (tuning experiments)
     cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
-        [os.path.join(CSRC, s) for s in SOURCES]
+        [os.path.join(CSRC, s) for s in SOURCES] + ["-lrt", "-lpthread"]
     subprocess.check_call(cmd)
     return LIB
 

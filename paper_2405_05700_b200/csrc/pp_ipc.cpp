@@ -1,0 +1,419 @@
+// Multi-process front end (include/pp_ipc.h): one server process owns the
+// pp_handle, client processes ship blocks of light sources through a POSIX shared-memory segment and get their
+// events' hits back.  Host-only code: no CUDA call in this file.  Product code: shares nothing with oracle/.
+#include "../../include/pp_ipc.h"
+
+#include <fcntl.h>
+#include <sys/mman.h>
+#include <sys/stat.h>
+#include <unistd.h>
+
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <thread>
+#include <unordered_map>
+#include <vector>
+
+namespace {
+
+constexpr uint64_t kMagic = 0x70705f6970633031ull;  // "pp_ipc01"
+constexpr size_t kHeaderBytes = 4096;
+constexpr size_t kCtlBytes = 256;
+constexpr size_t kIngestChunk = 16384;  // sources per back-end submit
+
+struct SrcSlot {  // 48 B
+  pp_source s;
+  float length;
+  uint32_t event_id, source_id, pad;
+};
+static_assert(sizeof(SrcSlot) == 48, "SrcSlot layout");
+
+struct ShmHeader {
+  uint64_t magic;
+  uint32_t max_clients, pad;
+  uint64_t src_cap, hit_cap;  // records per client ring
+  uint64_t client_stride, total_bytes;
+  std::atomic<uint32_t> server_alive;
+  std::atomic<uint32_t> next_slot;
+};
+static_assert(sizeof(ShmHeader) <= kHeaderBytes, "header");
+
+enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2 };
+
+struct ClientCtl {
+  std::atomic<uint32_t> state;
+  std::atomic<uint64_t> src_head;  // written by the client
+  std::atomic<uint64_t> src_tail;  // written by the server: sources before it have been handed to the back end
+  std::atomic<uint64_t> hit_head;  // written by the server
+  std::atomic<uint64_t> hit_tail;  // written by the client
+  std::atomic<uint64_t> flush_seq;      // client: src_head at its last flush request
+  std::atomic<uint64_t> flushed_seq;    // server: flush requests honoured up to here
+  std::atomic<uint64_t> completed_seq;  // server: sources before it are propagated and their hits are in the hit ring
+};
+static_assert(sizeof(ClientCtl) <= kCtlBytes, "ctl");
+static_assert(std::atomic<uint64_t>::is_always_lock_free, "address-free atomics needed in shared memory");
+
+struct Segment {
+  void* base = nullptr;
+  size_t bytes = 0;
+  ShmHeader* hdr() const { return reinterpret_cast<ShmHeader*>(base); }
+  unsigned char* client_base(uint32_t c) const {
+    return reinterpret_cast<unsigned char*>(base) + kHeaderBytes + (size_t)c * hdr()->client_stride;
+  }
+  ClientCtl* ctl(uint32_t c) const { return reinterpret_cast<ClientCtl*>(client_base(c)); }
+  SrcSlot* src_ring(uint32_t c) const { return reinterpret_cast<SrcSlot*>(client_base(c) + kCtlBytes); }
+  pp_hit* hit_ring(uint32_t c) const {
+    return reinterpret_cast<pp_hit*>(client_base(c) + kCtlBytes + hdr()->src_cap * sizeof(SrcSlot));
+  }
+};
+
+inline void nap(int us) { std::this_thread::sleep_for(std::chrono::microseconds(us)); }
+
+// ---- back end bound to a pp_handle ----
+int h_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
+  return pp_submit_segments(static_cast<pp_handle*>(ctx), s, len, ev, sid, n);
+}
+int h_flush(void* ctx) { return pp_flush(static_cast<pp_handle*>(ctx)); }
+int h_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
+  pp_handle* h = static_cast<pp_handle*>(ctx);
+  int rc = pp_collect(h, out, cap, n_out, 0);
+  *drained = 0;
+  if (rc != PP_OK || *n_out != 0) return rc;
+  // nothing to hand out right now: drained iff every submitted photon is done and every hit found was collected
+  // (pp_stats: photons_hit is raised before the hits are queued, hits_collected when they are handed out)
+  pp_stats_t st;
+  rc = pp_stats(h, &st);
+  if (rc == PP_OK && st.photons_done == st.photons_submitted && st.hits_collected == st.photons_hit) *drained = 1;
+  return rc;
+}
+
+// ---- host-only echo back end (tests without a GPU) ----
+struct Echo {
+  std::mutex mu;
+  std::vector<pp_hit> pending, ready;
+};
+int e_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
+  Echo* e = static_cast<Echo*>(ctx);
+  std::lock_guard<std::mutex> g(e->mu);
+  for (size_t i = 0; i < n; ++i) {
+    pp_hit h{};
+    uint64_t cnt = 0;
+    pp_photon_count(s[i].energy_GeV, 1.0e4f, &cnt);
+    h.event_id = ev[i]; h.source_id = sid ? sid[i] : (uint32_t)i; h.photon_idx = (uint32_t)cnt; h.dom_id = 0;
+    h.time_ns = (double)s[i].t_ns + (len ? (double)len[i] : 0.0); h.weight = s[i].energy_GeV; h.n_scatter = 0;
+    e->pending.push_back(h);
+  }
+  return PP_OK;
+}
+int e_flush(void* ctx) {
+  Echo* e = static_cast<Echo*>(ctx);
+  std::lock_guard<std::mutex> g(e->mu);
+  e->ready.insert(e->ready.end(), e->pending.begin(), e->pending.end());
+  e->pending.clear();
+  return PP_OK;
+}
+int e_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
+  Echo* e = static_cast<Echo*>(ctx);
+  std::lock_guard<std::mutex> g(e->mu);
+  const size_t n = std::min(cap, e->ready.size());
+  std::memcpy(out, e->ready.data(), n * sizeof(pp_hit));
+  e->ready.erase(e->ready.begin(), e->ready.begin() + (long)n);
+  *n_out = n;
+  *drained = (n == 0 && e->pending.empty() && e->ready.empty()) ? 1 : 0;
+  return PP_OK;
+}
+
+}  // namespace
+
+struct pp_ipc_server {
+  Segment seg;
+  std::string name;
+  pp_ipc_backend be{};
+  std::thread ingest, dispatch;
+  std::atomic<bool> stop{false};
+  std::mutex map_mu;
+  std::unordered_map<uint32_t, uint32_t> owner;  // event id -> client slot
+  std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0};
+  std::atomic<int> error{PP_OK};
+};
+
+struct pp_ipc_client {
+  Segment seg;
+  uint32_t slot = 0;
+};
+
+namespace {
+
+void ingest_main(pp_ipc_server* s) {
+  ShmHeader* H = s->seg.hdr();
+  std::vector<pp_source> src(kIngestChunk);
+  std::vector<float> len(kIngestChunk);
+  std::vector<uint32_t> ev(kIngestChunk), sid(kIngestChunk);
+  while (!s->stop.load()) {
+    bool progressed = false;
+    const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
+    for (uint32_t c = 0; c < n_slots; ++c) {
+      ClientCtl* ctl = s->seg.ctl(c);
+      const uint64_t head = ctl->src_head.load(std::memory_order_acquire);
+      uint64_t tail = ctl->src_tail.load(std::memory_order_relaxed);
+      if (head != tail) {
+        const size_t n = (size_t)std::min<uint64_t>(head - tail, kIngestChunk);
+        const SrcSlot* ring = s->seg.src_ring(c);
+        bool any_len = false;
+        for (size_t i = 0; i < n; ++i) {
+          const SrcSlot& r = ring[(tail + i) % H->src_cap];
+          src[i] = r.s; len[i] = r.length; ev[i] = r.event_id; sid[i] = r.source_id;
+          any_len |= r.length != 0.0f;
+        }
+        {
+          std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
+          uint32_t last = ~ev[0];
+          for (size_t i = 0; i < n; ++i)
+            if (ev[i] != last) { s->owner.emplace(ev[i], c); last = ev[i]; }
+        }
+        const int rc = s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
+        if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
+        s->blocks++; s->sources += n;
+        tail += n;
+        ctl->src_tail.store(tail, std::memory_order_release);
+        progressed = true;
+      }
+      const uint64_t fs = ctl->flush_seq.load(std::memory_order_acquire);
+      if (fs > ctl->flushed_seq.load(std::memory_order_relaxed) && tail >= fs) {
+        const int rc = s->be.flush(s->be.ctx);
+        if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
+        ctl->flushed_seq.store(fs, std::memory_order_release);
+        progressed = true;
+      }
+    }
+    if (!progressed) nap(50);
+  }
+}
+
+void dispatch_main(pp_ipc_server* s) {
+  ShmHeader* H = s->seg.hdr();
+  const size_t cap = 1 << 16;
+  std::vector<pp_hit> buf(cap);
+  std::vector<uint64_t> snap(H->max_clients);
+  while (!s->stop.load()) {
+    const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
+    for (uint32_t c = 0; c < n_slots; ++c) snap[c] = s->seg.ctl(c)->src_tail.load(std::memory_order_acquire);
+    size_t n = 0;
+    int drained = 0;
+    const int rc = s->be.collect(s->be.ctx, buf.data(), cap, &n, &drained);
+    if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
+    size_t i = 0;
+    while (i < n && !s->stop.load()) {
+      // route a run of hits of one event in one go
+      uint32_t c = ~0u;
+      {
+        std::lock_guard<std::mutex> g(s->map_mu);
+        auto it = s->owner.find(buf[i].event_id);
+        if (it != s->owner.end()) c = it->second;
+      }
+      size_t j = i + 1;
+      while (j < n && buf[j].event_id == buf[i].event_id) ++j;
+      if (c == ~0u) { s->unrouted += j - i; i = j; continue; }
+      ClientCtl* ctl = s->seg.ctl(c);
+      pp_hit* ring = s->seg.hit_ring(c);
+      while (i < j && !s->stop.load()) {
+        if (ctl->state.load(std::memory_order_acquire) == kClosed) { i = j; break; }  // nobody will read them
+        const uint64_t head = ctl->hit_head.load(std::memory_order_relaxed);
+        const uint64_t space = H->hit_cap - (head - ctl->hit_tail.load(std::memory_order_acquire));
+        if (space == 0) { nap(50); continue; }  // back-pressure: the client is behind
+        const size_t m = (size_t)std::min<uint64_t>(space, j - i);
+        for (size_t q = 0; q < m; ++q) ring[(head + q) % H->hit_cap] = buf[i + q];
+        ctl->hit_head.store(head + m, std::memory_order_release);
+        s->routed += m;
+        i += m;
+      }
+    }
+    if (n == 0) {
+      if (drained)
+        for (uint32_t c = 0; c < n_slots; ++c) {
+          ClientCtl* ctl = s->seg.ctl(c);
+          if (snap[c] > ctl->completed_seq.load(std::memory_order_relaxed))
+            ctl->completed_seq.store(snap[c], std::memory_order_release);
+        }
+      nap(100);
+    }
+  }
+}
+
+int map_segment(const char* name, bool create, size_t bytes, Segment* seg) {
+  const int fd = create ? shm_open(name, O_CREAT | O_EXCL | O_RDWR, 0600) : shm_open(name, O_RDWR, 0600);
+  if (fd < 0) return PP_E_STATE;
+  if (create && ftruncate(fd, (off_t)bytes) != 0) { close(fd); shm_unlink(name); return PP_E_NOMEM; }
+  if (!create) {
+    struct stat st;
+    if (fstat(fd, &st) != 0 || (size_t)st.st_size < kHeaderBytes) { close(fd); return PP_E_STATE; }
+    bytes = (size_t)st.st_size;
+  }
+  void* p = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_SHARED, fd, 0);
+  close(fd);
+  if (p == MAP_FAILED) { if (create) shm_unlink(name); return PP_E_NOMEM; }
+  seg->base = p; seg->bytes = bytes;
+  return PP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const pp_ipc_backend* pp_ipc_echo_backend(void) {
+  auto* be = new pp_ipc_backend{new Echo(), e_submit, e_flush, e_collect};  // lives as long as the process
+  return be;
+}
+
+int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name, const pp_ipc_config* cfg,
+                                 pp_ipc_server** out) {
+  if (!be || !be->submit || !be->flush || !be->collect || !shm_name || shm_name[0] != '/' || !out) return PP_E_INVAL;
+  *out = nullptr;
+  const uint32_t max_clients = cfg && cfg->max_clients ? cfg->max_clients : 16u;
+  const uint64_t src_bytes = cfg && cfg->source_ring_bytes ? cfg->source_ring_bytes : (4ull << 20);
+  const uint64_t hit_bytes = cfg && cfg->hit_ring_bytes ? cfg->hit_ring_bytes : (4ull << 20);
+  if (max_clients > 1024) return PP_E_INVAL;
+  const uint64_t src_cap = std::max<uint64_t>(1, src_bytes / sizeof(SrcSlot));
+  const uint64_t hit_cap = std::max<uint64_t>(1, hit_bytes / sizeof(pp_hit));
+  const uint64_t stride = (kCtlBytes + src_cap * sizeof(SrcSlot) + hit_cap * sizeof(pp_hit) + 255) / 256 * 256;
+  const size_t total = kHeaderBytes + (size_t)stride * max_clients;
+  auto* s = new pp_ipc_server();
+  s->name = shm_name;
+  s->be = *be;
+  const int rc = map_segment(shm_name, true, total, &s->seg);
+  if (rc != PP_OK) { delete s; return rc; }
+  std::memset(s->seg.base, 0, kHeaderBytes);
+  ShmHeader* H = new (s->seg.base) ShmHeader();
+  H->max_clients = max_clients; H->src_cap = src_cap; H->hit_cap = hit_cap;
+  H->client_stride = stride; H->total_bytes = total;
+  for (uint32_t c = 0; c < max_clients; ++c) new (s->seg.ctl(c)) ClientCtl();  // ftruncate zero-filled the rings
+  H->next_slot.store(0);
+  H->magic = kMagic;
+  H->server_alive.store(1, std::memory_order_release);
+  s->ingest = std::thread(ingest_main, s);
+  s->dispatch = std::thread(dispatch_main, s);
+  *out = s;
+  return PP_OK;
+}
+
+int pp_ipc_server_create(pp_handle* h, const char* shm_name, const pp_ipc_config* cfg, pp_ipc_server** out) {
+  if (!h) return PP_E_INVAL;
+  const pp_ipc_backend be{h, h_submit, h_flush, h_collect};
+  return pp_ipc_server_create_backend(&be, shm_name, cfg, out);
+}
+
+void pp_ipc_server_destroy(pp_ipc_server* s) {
+  if (!s) return;
+  s->stop.store(true);
+  if (s->ingest.joinable()) s->ingest.join();
+  if (s->dispatch.joinable()) s->dispatch.join();
+  s->seg.hdr()->server_alive.store(0, std::memory_order_release);
+  munmap(s->seg.base, s->seg.bytes);
+  shm_unlink(s->name.c_str());
+  delete s;
+}
+
+int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out) {
+  if (!s || !out) return PP_E_INVAL;
+  out->clients_attached = std::min(s->seg.hdr()->next_slot.load(), s->seg.hdr()->max_clients);
+  out->blocks_ingested = s->blocks.load(); out->sources_ingested = s->sources.load();
+  out->hits_routed = s->routed.load(); out->hits_unrouted = s->unrouted.load();
+  return s->error.load();
+}
+
+int pp_ipc_client_open(const char* shm_name, pp_ipc_client** out) {
+  if (!shm_name || !out) return PP_E_INVAL;
+  *out = nullptr;
+  auto* c = new pp_ipc_client();
+  const int rc = map_segment(shm_name, false, 0, &c->seg);
+  if (rc != PP_OK) { delete c; return rc; }
+  ShmHeader* H = c->seg.hdr();
+  if (H->magic != kMagic || H->total_bytes != c->seg.bytes || !H->server_alive.load(std::memory_order_acquire)) {
+    munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_STATE;
+  }
+  const uint32_t slot = H->next_slot.fetch_add(1);
+  if (slot >= H->max_clients) { munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_NOMEM; }
+  c->slot = slot;
+  c->seg.ctl(slot)->state.store(kAttached, std::memory_order_release);
+  *out = c;
+  return PP_OK;
+}
+
+int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengths, const uint32_t* event_ids,
+                  const uint32_t* source_ids, size_t n) {
+  if (!c) return PP_E_INVAL;
+  if (n == 0) return PP_OK;
+  if (!sources || !event_ids) return PP_E_INVAL;
+  for (size_t i = 0; i < n; ++i) {  // the cheap checks here, so that a bad block never reaches the shared ring
+    const pp_source& a = sources[i];
+    const float v[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
+    for (float f : v) if (!std::isfinite(f)) return PP_E_INVAL;
+    if (a.energy_GeV < 0.0f || (lengths && !(std::isfinite(lengths[i]) && lengths[i] >= 0.0f))) return PP_E_INVAL;
+    const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
+    if (std::fabs(n2 - 1.0) > 1e-4) return PP_E_INVAL;
+  }
+  ShmHeader* H = c->seg.hdr();
+  ClientCtl* ctl = c->seg.ctl(c->slot);
+  SrcSlot* ring = c->seg.src_ring(c->slot);
+  size_t i = 0;
+  while (i < n) {
+    if (!H->server_alive.load(std::memory_order_acquire)) return PP_E_STATE;
+    const uint64_t head = ctl->src_head.load(std::memory_order_relaxed);
+    const uint64_t space = H->src_cap - (head - ctl->src_tail.load(std::memory_order_acquire));
+    if (space == 0) { nap(50); continue; }  // bounded ring: the client waits for the GPU
+    const size_t m = (size_t)std::min<uint64_t>(space, n - i);
+    for (size_t q = 0; q < m; ++q, ++i) {
+      SrcSlot& r = ring[(head + q) % H->src_cap];
+      r.s = sources[i]; r.length = lengths ? lengths[i] : 0.0f; r.event_id = event_ids[i];
+      r.source_id = source_ids ? source_ids[i] : (uint32_t)i; r.pad = 0;
+    }
+    ctl->src_head.store(head + m, std::memory_order_release);
+  }
+  return PP_OK;
+}
+
+int pp_ipc_flush(pp_ipc_client* c) {
+  if (!c) return PP_E_INVAL;
+  ClientCtl* ctl = c->seg.ctl(c->slot);
+  ctl->flush_seq.store(ctl->src_head.load(std::memory_order_relaxed), std::memory_order_release);
+  return c->seg.hdr()->server_alive.load(std::memory_order_acquire) ? PP_OK : PP_E_STATE;
+}
+
+int pp_ipc_collect(pp_ipc_client* c, pp_hit* out, size_t cap, size_t* n_out, int block) {
+  if (!c || !n_out || (!out && cap)) return PP_E_INVAL;
+  *n_out = 0;
+  ShmHeader* H = c->seg.hdr();
+  ClientCtl* ctl = c->seg.ctl(c->slot);
+  const pp_hit* ring = c->seg.hit_ring(c->slot);
+  for (;;) {
+    // read "complete" before the ring: hits are published before completed_seq moves
+    const bool complete = ctl->completed_seq.load(std::memory_order_acquire) >= ctl->src_head.load(std::memory_order_relaxed);
+    const uint64_t tail = ctl->hit_tail.load(std::memory_order_relaxed);
+    const uint64_t avail = ctl->hit_head.load(std::memory_order_acquire) - tail;
+    if (avail > 0) {
+      const size_t m = (size_t)std::min<uint64_t>(avail, cap);
+      for (size_t q = 0; q < m; ++q) out[q] = ring[(tail + q) % H->hit_cap];
+      ctl->hit_tail.store(tail + m, std::memory_order_release);
+      *n_out = m;
+      return PP_OK;
+    }
+    if (complete || !block) return PP_OK;  // drained, or nothing yet
+    if (!H->server_alive.load(std::memory_order_acquire)) return PP_E_STATE;
+    nap(100);
+  }
+}
+
+void pp_ipc_client_close(pp_ipc_client* c) {
+  if (!c) return;
+  c->seg.ctl(c->slot)->state.store(kClosed, std::memory_order_release);
+  munmap(c->seg.base, c->seg.bytes);
+  delete c;
+}
+
+}  // extern "C"

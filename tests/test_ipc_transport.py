@@ -1,0 +1,118 @@
+"""The multi-process front end (include/pp_ipc.h, NEXT-3) without a GPU: client processes
+ship blocks through shared memory to a server bound to the host-only echo back end (one hit per source)."""
+import multiprocessing as mp
+import os
+
+import numpy as np
+import pytest
+
+from paper_2405_05700_b200 import binding as B
+from paper_2405_05700_b200 import ipc
+from paper_2405_05700_b200 import workloads as W
+
+
+def _sources(client: int, n_events: int, per_event: int):
+    """Deterministic sources of one client: event ids client*1000 + e."""
+    rng = np.random.default_rng(100 + client)
+    n = n_events * per_event
+    d = rng.normal(size=(n, 3))
+    d /= np.linalg.norm(d, axis=1)[:, None]
+    src = np.zeros((n, 8), np.float32)
+    src[:, 0:3] = rng.uniform(-100, 100, size=(n, 3))
+    src[:, 3:6] = d
+    src[:, 6] = rng.uniform(0, 1000, size=n)
+    src[:, 7] = rng.uniform(0.1, 10.0, size=n)
+    ev = (client * 1000 + np.repeat(np.arange(n_events), per_event)).astype(np.uint32)
+    sid = np.tile(np.arange(per_event), n_events).astype(np.uint32)
+    ln = rng.uniform(0, 5, size=n).astype(np.float32)
+    return src, ev, sid, ln
+
+
+def _expected(src, ev, sid, ln):
+    out = np.zeros(len(ev), dtype=B.HIT_DTYPE)
+    out["event_id"], out["source_id"] = ev, sid
+    out["photon_idx"] = [B.photon_count(e) for e in src[:, 7]]
+    out["time_ns"] = src[:, 6].astype(np.float64) + ln.astype(np.float64)
+    out["weight"] = src[:, 7]
+    return np.sort(out, order=["event_id", "source_id"])
+
+
+def _client_main(name, client, n_events, per_event, block, q):
+    try:
+        src, ev, sid, ln = _sources(client, n_events, per_event)
+        got = []
+        with ipc.IpcClient(name) as c:
+            for a in range(0, len(ev), block):  # ship block by block, collecting in between (streaming)
+                c.submit(src[a:a + block], ev[a:a + block], sid[a:a + block], ln[a:a + block])
+                h = c.collect(block=False)
+                if len(h):
+                    got.append(h.copy())
+            got.append(c.collect_all())
+        hits = np.sort(np.concatenate(got), order=["event_id", "source_id"])
+        q.put((client, hits.tobytes()))
+    except Exception as e:  # pragma: no cover
+        q.put((client, repr(e)))
+
+
+@pytest.mark.parametrize("n_clients,ring_kib", [(1, 4096), (4, 4096), (8, 8)])
+def test_clients_get_exactly_their_events_back(n_clients, ring_kib):
+    """n client processes, one server; tiny rings (8 KiB = 170 sources / 256 hits) force back-pressure both ways."""
+    name = f"/pp_ipc_test_{os.getpid()}_{n_clients}_{ring_kib}"
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    n_events, per_event, block = 20, 37, 111
+    with ipc.IpcServer(None, name, max_clients=n_clients, source_ring_bytes=ring_kib * 1024,
+                       hit_ring_bytes=ring_kib * 1024, echo=True) as srv:
+        procs = [ctx.Process(target=_client_main, args=(name, c, n_events, per_event, block, q)) for c in range(n_clients)]
+        for p in procs:
+            p.start()
+        res = dict(q.get(timeout=120) for _ in procs)
+        for p in procs:
+            p.join(timeout=60)
+        st = srv.stats()
+    assert st["error"] == 0 and st["hits_unrouted"] == 0
+    assert st["clients_attached"] == n_clients and st["sources_ingested"] == n_clients * n_events * per_event
+    assert st["hits_routed"] == st["sources_ingested"]
+    for c in range(n_clients):
+        assert isinstance(res[c], bytes), res[c]
+        hits = np.frombuffer(res[c], dtype=B.HIT_DTYPE)
+        assert np.array_equal(hits, _expected(*_sources(c, n_events, per_event)))
+
+
+def test_open_errors_and_slot_limit():
+    with pytest.raises(B.PPError) as e:
+        ipc.IpcClient(f"/pp_ipc_nobody_{os.getpid()}")
+    assert e.value.code == -7  # PP_E_STATE: no server
+    name = f"/pp_ipc_test_{os.getpid()}_lim"
+    with ipc.IpcServer(None, name, max_clients=2, echo=True):
+        with pytest.raises(B.PPError):
+            ipc.IpcServer(None, name, echo=True)  # the segment exists already
+        a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+        with pytest.raises(B.PPError) as e:
+            ipc.IpcClient(name)
+        assert e.value.code == -2  # PP_E_NOMEM: no free slot
+        src, ev, sid, ln = _sources(0, 2, 3)
+        bad = src.copy()
+        bad[0, 3:6] = 0.0
+        with pytest.raises(B.PPError):
+            a.submit(bad, ev, sid, ln)
+        with pytest.raises(B.PPError):
+            a.submit(src, ev, sid, -ln - 1.0)
+        assert len(a.collect_all()) == 0  # nothing was shipped: drained at once
+        b.submit(src, ev, sid, ln)
+        assert np.array_equal(np.sort(b.collect_all(), order=["event_id", "source_id"]), _expected(src, ev, sid, ln))
+        a.close(), b.close()
+    with pytest.raises(B.PPError):
+        ipc.IpcClient(name)  # unlinked with the server
+
+
+def test_ipc_symbols_are_exported():
+    """Every function include/pp_ipc.h declares is exported by the library and bound in ipc.py."""
+    import re
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(root, "include", "pp_ipc.h")).read(), flags=re.S)
+    declared = set(re.findall(r"\b(pp_ipc_[a-z_]+)\s*\(", hdr))
+    lib = B.load_library()
+    for s in declared:
+        assert hasattr(lib, s), s
+    assert declared == set(ipc.EXPORTS)
