@@ -412,6 +412,83 @@ def run_stream(args):
     return 0
 
 
+def _ipc_client_main(name, client, n_clients, replicas, block_sources, barrier, q):
+    """One propagation client process of `--stream --ipc-clients` (no CUDA, no torch in here)."""
+    try:
+        from paper_2405_05700_b200 import binding as B
+        from paper_2405_05700_b200 import ipc
+        from paper_2405_05700_b200 import workloads as W
+        src = W.sources_c2()
+        order = np.argsort(src.event_id, kind="stable")
+        rec, ev, sid = B.pack_sources(src.src[order]), src.event_id[order], src.source_id[order]
+        n_events = int(ev.max()) + 1
+        mine = (ev % n_clients) == client
+        rec, ev, sid = rec[mine], ev[mine], sid[mine]
+        blocks = []
+        for r in range(replicas):
+            e_r = ev + np.uint32(r * n_events)
+            for a in range(0, len(ev), block_sources):
+                blocks.append((rec[a:a + block_sources], e_r[a:a + block_sources], sid[a:a + block_sources]))
+        n_hits = 0
+        with ipc.IpcClient(name) as c:
+            barrier.wait()
+            for r_, e_, s_ in blocks:
+                c.submit(r_, e_, s_)
+                n_hits += len(c.collect(block=False))
+            n_hits += len(c.collect_all())
+        q.put((client, n_hits, len(blocks)))
+    except Exception as e:  # pragma: no cover
+        q.put((client, repr(e), 0))
+
+
+def run_stream_ipc(args):
+    """`--stream --ipc-clients N`: the paper's instance-count scan (1, 2, 4, 8, 16 client instances share
+    ONE photon server).  N client PROCESSES ship blocks of C2's light sources through shared memory (include/pp_ipc.h)
+    to this process, which owns the propagator; photons/s and device-busy between the start signal and the last
+    client's drain."""
+    import multiprocessing as mp
+    import torch
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import ipc
+    from paper_2405_05700_b200 import workloads as W
+    torch.cuda.set_device(0)
+    geo, ice = W.geometry_full(), W.ice_layered()
+    src = W.sources_c2()
+    n = args.ipc_clients
+    name = f"/pp_bench_{os.getpid()}"
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    barrier = ctx.Barrier(n + 1)
+    with B.Propagator(geo, ice, seed=0, launch_photons_target=10 ** 8) as prop:
+        prop.run(src.src, src.event_id, src.source_id)  # warm-up
+        with ipc.IpcServer(prop, name, max_clients=n) as srv:
+            procs = [ctx.Process(target=_ipc_client_main, args=(name, c, n, args.replicas, args.block_sources, barrier, q))
+                     for c in range(n)]
+            for p in procs:
+                p.start()
+            barrier.wait()  # every client has packed its blocks and attached
+            st0 = prop.stats()
+            t0 = time.perf_counter()
+            res = [q.get(timeout=600) for _ in procs]
+            wall = time.perf_counter() - t0
+            st1 = prop.stats()
+            for p in procs:
+                p.join(timeout=60)
+            ist = srv.stats()
+    bad = [r for r in res if not isinstance(r[1], int)]
+    if bad:
+        raise SystemExit(f"ipc client failed: {bad}")
+    ph = st1.photons_done - st0.photons_done
+    busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+    print(json.dumps({"mode": "stream-ipc", "workload": f"C2 x {args.replicas} replicas shipped in blocks of {args.block_sources} "
+                      f"sources by {n} client processes over shared memory", "client_processes": n,
+                      "blocks": int(sum(r[2] for r in res)), "photons": int(ph), "launches": st1.launches - st0.launches,
+                      "photons_per_s": ph / wall, "device_busy_frac": busy / wall, "wall_s": wall, "kernel_s": busy,
+                      "hits": int(sum(r[1] for r in res)), "hits_unrouted": ist["hits_unrouted"],
+                      "server_blocks_ingested": ist["blocks_ingested"]}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -424,6 +501,7 @@ def main():
     ap.add_argument("--stream", action="store_true", help="C2 replicas through the batching server from worker threads")
     ap.add_argument("--threads", type=int, default=8)
     ap.add_argument("--replicas", type=int, default=10)
+    ap.add_argument("--ipc-clients", type=int, default=0, help="with --stream: N client processes over include/pp_ipc.h")
     ap.add_argument("--block-sources", type=int, default=8192, help="sources a client queues before it ships a block")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -431,7 +509,7 @@ def main():
     if args.sweep:
         return run_sweep(args)
     if args.stream:
-        return run_stream(args)
+        return run_stream_ipc(args) if args.ipc_clients > 0 else run_stream(args)
     return run_ours(args)
 
 
