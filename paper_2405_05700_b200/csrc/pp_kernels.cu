@@ -378,9 +378,11 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         const float sxy2 = s * s * rho2;
         float ds = s;
         int n_ch = 1;
+        bool all_lines = false;  // a flight of more than 64 pieces (far longer than the detector is wide)
         if (sxy2 > P.xy_cap2) {
           const float f = floorf(fast_sqrt(sxy2) * P.inv_xy_cap) + 1.0f;
-          n_ch = f > 64.0f ? 1 : (int)f;
+          all_lines = f > 64.0f;
+          n_ch = all_lines ? 1 : (int)f;
           ds = s * fast_rcp(f);
         }
         const float rm2 = fmaf(P.radius_margin * P.radius_margin, rho2, 1e-12f);
@@ -400,8 +402,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           if (--n_ch <= 0) break;
           tm += ds;
         }
-        if (sxy2 > P.xy_cap2 * 4096.0f) {
-          // a flight of more than 64 pieces (far longer than the detector is wide): every line
+        if (all_lines) {
           for (uint32_t si = 0; si < P.n_strings; ++si)
             best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
         }
