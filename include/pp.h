@@ -99,6 +99,9 @@ typedef struct pp_ice {
 /* pp_config.flags */
 #define PP_FLAG_BRUTE_FORCE_DOMS 1u /* test every DOM on every flight (validation; any geometry) */
 #define PP_FLAG_NONBLOCKING_SUBMIT 2u /* pp_submit enqueues all n sources or none: PP_E_WOULDBLOCK if the ring lacks space */
+#define PP_FLAG_EFFECTIVE_SCATTERING 4u /* pp_ice.scat_len holds effective scattering lengths lambda_e = lambda_s/(1-g)
+                                           (the convention of measured ice tables); the mean free path between
+                                           scatters is then lambda_e (1-g) (reading R-20; needs g < 1) */
 
 /* Sizes and resources.  Zero means "default".  device_workspace / pinned_workspace / streams may be
  * NULL: the library then allocates them itself (cudaMalloc / cudaHostAlloc / cudaStreamCreate) and

@@ -33,6 +33,8 @@
 //                        beam along the axis at a DOM ahead: hit fraction (lambda/L) e^{-(D-R)/lambda} (e^{L/lambda} - 1),
 //                        arrival times l/c + (D-R-l)/v and the mean emission offset of the hits; mean end-point
 //                        displacement L/2 + 1/(a+b(1-g)); L = 0 is the point source bit for bit
+//   effective scattering lengths (NEXT-2, R-20): table 200 m at g = 0.875 == table 25 m geometric, bit for bit;
+//                        mean displacement 1/(a + 1/lambda_e)
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -89,6 +91,9 @@ struct Ice {
   const float* abs_len;   // [n_layers] metres
   const float* scat_len;  // [n_layers] metres, geometric mean free path (R-7)
   double g, n_group, cos_cherenkov, photons_per_gev;
+  // NEXT-2 option (R-20): scat_len holds EFFECTIVE scattering lengths lambda_e = lambda_s / (1 - g), the
+  // convention of measured ice tables; the geometric mean free path of R-7 is then lambda_e (1 - g).
+  int effective_scattering = 0;
 };
 
 struct Geometry {
@@ -350,7 +355,9 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
     rotate(d, cos_t, two_pi * u_az);
     r.n_flights = k + 1;
     // step 5/6: distance to the next scatter and to the absorption point
-    const Real tau_s = -std::log(u_dist);
+    // R-20: with effective scattering lengths b = 1/(lambda_e (1-g)), so the optical depth along the lambda_e table
+    // that corresponds to tau_s is tau_s (1 - g)
+    const Real tau_s = -std::log(u_dist) * (ice.effective_scattering ? Real(1.0 - ice.g) : Real(1));
     const Real s_scat = walk(ice, ice.scat_len, p[2], d[2], tau_s);
     const Real s_abs = walk(ice, ice.abs_len, p[2], d[2], tau_a);
     const bool absorbed = (s_abs <= s_scat);

@@ -39,7 +39,7 @@ class _Ice(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("z_top", C.c_double), ("dz", C.c_double),
                 ("abs_len", C.POINTER(C.c_float)), ("scat_len", C.POINTER(C.c_float)),
                 ("g", C.c_double), ("n_group", C.c_double), ("cos_cherenkov", C.c_double),
-                ("photons_per_gev", C.c_double)]
+                ("photons_per_gev", C.c_double), ("effective_scattering", C.c_int32), ("pad", C.c_int32)]
 
 
 class _Geo(C.Structure):
@@ -113,7 +113,7 @@ def _mk_ice(ice):
     s = np.ascontiguousarray(ice.scat_len, dtype=np.float32)
     st = _Ice(int(a.shape[0]), float(ice.z_top), float(ice.dz), _fp(a), _fp(s), float(np.float32(ice.g)),
               float(np.float32(ice.n_group)), float(np.float32(ice.cos_cherenkov)),
-              float(np.float32(ice.photons_per_GeV)))
+              float(np.float32(ice.photons_per_GeV)), 1 if getattr(ice, "effective_scattering", False) else 0, 0)
     return st, (a, s)
 
 

@@ -16,6 +16,7 @@ struct orc_ice {
   const float* abs_len;
   const float* scat_len;
   double g, n_group, cos_cherenkov, photons_per_gev;
+  int32_t effective_scattering, pad;
 };
 
 struct orc_geometry {
@@ -82,7 +83,7 @@ void orc_rotate(const double* d, double cos_t, double phi, double* out) {
 
 static Ice to_ice(const orc_ice* i) {
   return Ice{i->n_layers, i->z_top, i->dz, i->abs_len, i->scat_len, i->g, i->n_group, i->cos_cherenkov,
-             i->photons_per_gev};
+             i->photons_per_gev, i->effective_scattering};
 }
 static Geometry to_geo(const orc_geometry* g) { return Geometry{g->n_dom, g->xyz, g->radius}; }
 

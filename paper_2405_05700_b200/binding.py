@@ -21,6 +21,7 @@ ERRORS = {-1: "PP_E_INVAL", -2: "PP_E_NOMEM", -3: "PP_E_CUDA", -4: "PP_E_OVERFLO
           -6: "PP_E_UNSUPPORTED", -7: "PP_E_STATE"}
 FLAG_BRUTE_FORCE_DOMS = 1
 FLAG_NONBLOCKING_SUBMIT = 2
+FLAG_EFFECTIVE_SCATTERING = 4
 ACCEPTANCE_MODES = {"off": 0, "probabilistic": 1, "weighted": 2}
 
 SOURCE_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("dx", "<f4"), ("dy", "<f4"), ("dz", "<f4"),
@@ -220,7 +221,7 @@ class Propagator:
         cfg.launch_photons_target = int(launch_photons_target)
         cfg.hit_ring_bytes = int(hit_ring_bytes)
         cfg.source_ring_bytes = int(source_ring_bytes)
-        cfg.flags = int(flags)
+        cfg.flags = int(flags) | (FLAG_EFFECTIVE_SCATTERING if getattr(ice, "effective_scattering", False) else 0)
         cfg.max_flights = int(max_flights)
         cfg.device = int(device)
         self.device = torch.device("cuda", device if device else torch.cuda.current_device())

@@ -780,10 +780,14 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
 
   // ---- medium and geometry constants ----
   LaunchParams& B = h->base;
+  const double scat_scale = (cfg->flags & PP_FLAG_EFFECTIVE_SCATTERING) ? 1.0 - (double)ice->g : 1.0;
+  if (!(scat_scale > 0.0)) return bail(PP_E_INVAL);
   std::vector<IceLayer> layers(ice->n_layers);
   for (uint32_t i = 0; i < ice->n_layers; ++i) {
-    layers[i].la = ice->abs_len[i]; layers[i].lb = ice->scat_len[i];
-    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / (double)ice->scat_len[i]);
+    // R-20: an effective scattering length is turned into the geometric mean free path here, once
+    const double ls = (double)ice->scat_len[i] * scat_scale;
+    layers[i].la = ice->abs_len[i]; layers[i].lb = (float)ls;
+    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / ls);
   }
   B.n_layers = ice->n_layers; B.z_top = ice->z_top; B.dz_layer = ice->dz; B.inv_dz_layer = (float)(1.0 / (double)ice->dz);
   const double g = ice->g;
@@ -808,7 +812,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   {
     std::vector<double> cum[2] = {std::vector<double>(nl + 1, 0.0), std::vector<double>(nl + 1, 0.0)};  // B, A
     for (uint32_t i = 0; i < nl; ++i) {
-      cum[0][i + 1] = cum[0][i] + (double)ice->dz / (double)ice->scat_len[i];
+      cum[0][i + 1] = cum[0][i] + (double)ice->dz / ((double)ice->scat_len[i] * scat_scale);
       cum[1][i + 1] = cum[1][i] + (double)ice->dz / (double)ice->abs_len[i];
     }
     for (uint32_t i = 0; i <= nl; ++i) {

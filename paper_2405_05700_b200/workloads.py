@@ -62,6 +62,7 @@ class Ice:
     n_group: float = N_GROUP
     cos_cherenkov: float = float(np.float32(math.cos(math.radians(CHERENKOV_DEG))))
     photons_per_GeV: float = PHOTONS_PER_GEV
+    effective_scattering: bool = False  # scat_len holds lambda_e = lambda_s / (1 - g) (R-20)
 
     @property
     def n_layers(self) -> int:

@@ -87,3 +87,24 @@ def test_segments_with_acceptance_and_bad_lengths():
                 p.submit(src.src[:1], src.event_id[:1], src.source_id[:1], [bad])
             assert e.value.code == -1
         assert len(p.collect_all()) == 0
+
+
+def test_effective_scattering_lengths():
+    """NEXT-2, R-20: the scattering table given as lambda_e = lambda_s/(1-g) (PP_FLAG_EFFECTIVE_SCATTERING)."""
+    geo = W.geometry_full(radius=1.0)
+    ice = W.ice_layered()
+    eff = W.ice_layered()
+    eff.scat_len = (ice.scat_len.astype(np.float64) / (1.0 - float(np.float32(ice.g)))).astype(np.float32)
+    eff.effective_scattering = True
+    src = W.sources_c1().subset(slice(0, 30))
+    src.src[:, 7] = 3.0
+    n = total_photons(src, ice)
+    hits, st = run(geo, eff, src, 10, None)
+    ref = O.propagate(geo, eff, src, seed=10)
+    assert st.photons_done == n == ref.photons and ref.hit > 500
+    assert abs(st.flights - ref.flights) <= 2 and abs(st.photons_hit - ref.hit) <= 2
+    c = compare_hits(hits, ref.hits, n)
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.97, c
+    # the same physics as the geometric table (lambda_e (1-g) rounds to lambda_s within an ulp): same statistics
+    base, st_b = run(geo, ice, src, 10, None)
+    assert abs(st.flights - st_b.flights) <= 1e-3 * st_b.flights and abs(len(base) - len(hits)) <= 6 * math.sqrt(len(base))
