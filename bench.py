@@ -489,6 +489,40 @@ def run_stream_ipc(args):
     return 0
 
 
+def run_c4(args):
+    """BASELINE.json configs[4]: one 1e8 GeV bundle (500 muons, ~5e9 photons) with the hit ring capped at 2 GB, and
+    the same event with a 256 KiB ring (stop/replay relaunches all the time): time, device memory, hits."""
+    import torch
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import workloads as W
+    torch.cuda.set_device(0)
+    geo, ice, src = W.geometry_full(), W.ice_layered(), W.sources_c4()
+    for ring in (2 << 30, 256 << 10):
+        torch.cuda.synchronize()
+        torch.cuda.reset_peak_memory_stats()
+        mem0 = torch.cuda.memory_allocated()
+        with B.Propagator(geo, ice, seed=0, launch_photons_target=5 * 10 ** 8, hit_ring_bytes=ring,
+                          source_ring_bytes=16 << 20) as prop:
+            prop.run(src.src[:64], src.event_id[:64], src.source_id[:64])  # warm-up
+            st0 = prop.stats()
+            t0 = time.perf_counter()
+            hits = prop.run(src.src, src.event_id, src.source_id)
+            wall = time.perf_counter() - t0
+            st1 = prop.stats()
+            peak = torch.cuda.max_memory_allocated() - mem0
+            ws, pin = prop.device_workspace_bytes, prop.pinned_workspace_bytes
+        ph = st1.photons_done - st0.photons_done
+        busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+        print(json.dumps({"mode": "c4", "workload": "C4: one 1e8 GeV bundle, 500 muons", "sources": len(src), "photons": int(ph),
+                          "hit_ring_bytes": ring, "device_workspace_bytes": int(ws), "pinned_workspace_bytes": int(pin),
+                          "peak_device_bytes_over_baseline": int(peak), "hits": int(len(hits)),
+                          "hit_bytes": int(len(hits) * 32), "launches": st1.launches - st0.launches,
+                          "relaunches": st1.relaunches - st0.relaunches, "photons_per_s": ph / wall,
+                          "device_busy_frac": busy / wall, "wall_s": wall,
+                          "hit_ring_high_water_bytes": int(st1.hit_ring_high_water)}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -496,6 +530,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--c4", action="store_true", help="C4 memory-bounded extreme event (report mode)")
     ap.add_argument("--sweep", action="store_true", help="C3 launch-size sweep (report mode)")
     ap.add_argument("--sweep-sizes", default="", help="comma-separated photons per launch (default 1e5..1e9)")
     ap.add_argument("--stream", action="store_true", help="C2 replicas through the batching server from worker threads")
@@ -506,6 +541,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.c4:
+        return run_c4(args)
     if args.sweep:
         return run_sweep(args)
     if args.stream:
