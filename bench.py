@@ -42,10 +42,11 @@ def load_instr_per_flight(library_version):
         with open(INSTR_PER_FLIGHT_FILE) as f:
             d = json.load(f)
         if d.get("library") != library_version:
-            return None, None, f"stale: measured on {d.get('library')!r}, library is {library_version!r}"
-        return float(d["thread_instructions_per_flight"]), d.get("dram_bytes_per_launch"), d.get("source", "")
+            return None, None, f"stale: measured on {d.get('library')!r}, library is {library_version!r}", None
+        return float(d["thread_instructions_per_flight"]), d.get("dram_bytes_per_launch"), d.get("source", ""), \
+            d.get("fp32_flops_per_flight")
     except Exception:
-        return None, None, ""
+        return None, None, "", None
 
 
 def measured_peaks():
@@ -243,7 +244,7 @@ def run_ours(args):
     if rank == 0:
         peaks = measured_peaks()
         clocks = clk.summary()
-        ipf, dram_bytes, ipf_src = load_instr_per_flight(B.version())
+        ipf, dram_bytes, ipf_src, fpf = load_instr_per_flight(B.version())
         sm_max = peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         roofline = None
@@ -262,6 +263,13 @@ def run_ours(args):
                                        "MEASURED_PEAKS.json sm_max_mhz)",
                         "frac_at_observed_clock": (achieved / (n_sm * 4 * 32 * clocks["sm_mhz"] * 1e-3)
                                                    if clocks.get("sm_mhz") else None)}
+            if fpf:
+                # the metric's "% of SM FP32 roofline": FP32 flops (FFMA = 2, FMUL/FADD = 1) per flight from the same
+                # ncu capture, against SMs x 128 lanes x 2 x f; capped near 30 % by the integer/control share of the mix
+                fp32_peak = n_sm * 128 * 2 * sm_max * 1e6 / 1e12
+                fp32 = flights * float(fpf) / (busy_ms * 1e-3) / 1e12
+                roofline["fp32"] = {"achieved_tflops": fp32, "peak_tflops": fp32_peak, "frac": fp32 / fp32_peak,
+                                    "fp32_flops_per_flight": float(fpf)}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             o = oracle_rate(geo, ice, src, 0, 15.0)

@@ -660,7 +660,7 @@ bool idle_locked(pp_handle* h) {
 // =============================================================================================
 extern "C" {
 
-const char* pp_version(void) { return "pp 0.3 (sm_100a)"; }
+const char* pp_version(void) { return "pp 0.4 (sm_100a)"; }
 
 int pp_check_inputs(const pp_geometry* geo, const pp_ice* ice, uint32_t flags) {
   std::string why;
