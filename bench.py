@@ -255,7 +255,7 @@ def run_ours(args):
             achieved = flights * ipf / (busy_ms * 1e-3) / 1e9
             roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-level)",
                         "frac": achieved / peak, "traffic": dram_bytes,
-                        "kernel": "pp::propagate_kernel<false,false>",
+                        "kernel": "pp::propagate_kernel<false,false,false>",
                         "kernel_ms_per_launch": busy_ms / max(1, n_prop_launches),
                         "units_per_launch": {"flights": flights / max(1, n_prop_launches)},
                         "thread_instructions_per_flight": ipf, "per_unit_source": ipf_src,
