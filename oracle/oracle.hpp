@@ -35,6 +35,9 @@
 //                        displacement L/2 + 1/(a+b(1-g)); L = 0 is the point source bit for bit
 //   effective scattering lengths (NEXT-2, R-20): table 200 m at g = 0.875 == table 25 m geometric, bit for bit;
 //                        mean displacement 1/(a + 1/lambda_e)
+//   wavelength bins (NEXT-2, R-21): one bin with unit scales == monochromatic bit for bit; two bins: bin frequencies,
+//                        mean path sum_j w_j lambda_a / abs_scale_j, flights per photon per bin, two arrival times
+//                        (d-R) n_j / c at a DOM with frequencies ~ w_j exp(-(d-R) a_j)
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -303,6 +306,29 @@ inline double acceptance(const Acceptance& acc, double eta) {
   return std::min(1.0, std::max(0.0, p));
 }
 
+// ------------------------------------------------------------------------------------------
+// Wavelength bins (NEXT-2; the photoelectron probability depends on "position, direction, time, and
+// wavelength"; the optical properties vary).  Reading R-21: a photon belongs to one of
+// n <= 32 wavelength bins for its whole life, bin j = the first with cdf[j] > u, u = word 0 of Philox block
+// (photon, source, event, 2^30); in bin j the absorption and scattering coefficients of every layer are multiplied by
+// abs_scale[j] and scat_scale[j], the group index is n_group[j], and the acceptance probability becomes
+// min(1, p(eta) acc_scale[j]).  n = 0: monochromatic (R-4b).
+// ------------------------------------------------------------------------------------------
+struct Spectrum {
+  int n;
+  const float* cdf;         // [n] cumulative bin probabilities, non-decreasing, cdf[n-1] >= 1
+  const float* abs_scale;   // [n] > 0
+  const float* scat_scale;  // [n] > 0
+  const float* n_group;     // [n] >= 1
+  const float* acc_scale;   // [n] >= 0
+};
+
+inline int spectrum_bin(const Spectrum& sp, double u) {
+  int j = 0;
+  while (j + 1 < sp.n && !(double(sp.cdf[j]) > u)) ++j;
+  return j;
+}
+
 struct PhotonResult {
   double weight;      // hit weight (1 unless the acceptance is in weighted mode)
   int fate;
@@ -318,9 +344,21 @@ constexpr uint32_t kMaxFlights = 100000;  // R-10
 template <class Real>
 inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx, const Ice& ice, uint64_t seed,
                                      const float src[8], uint32_t event_id, uint32_t source_id,
-                                     uint32_t photon_idx, const Acceptance* acc = nullptr, float length = 0.0f) {
+                                     uint32_t photon_idx, const Acceptance* acc = nullptr, float length = 0.0f,
+                                     const Spectrum* spec = nullptr) {
   const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
-  const Real v = Real(kC / ice.n_group);  // group velocity, m/ns
+  // R-21: the photon's wavelength bin fixes its coefficient scales and its group index
+  Real sc_a = 1, sc_b = 1, sc_acc = 1;
+  double n_group = ice.n_group;
+  if (spec && spec->n > 0) {
+    const uint32_t sctr[4] = {photon_idx, source_id, event_id, 0x40000000u};
+    uint32_t sw[4];
+    philox4x32_10(sctr, key, sw);
+    const int j = spectrum_bin(*spec, uniform_from_word(sw[0]));
+    sc_a = Real(spec->abs_scale[j]); sc_b = Real(spec->scat_scale[j]); sc_acc = Real(spec->acc_scale[j]);
+    n_group = double(spec->n_group[j]);
+  }
+  const Real v = Real(kC / n_group);  // group velocity, m/ns
   const Real two_pi = Real(6.283185307179586476925286766559);
   Real p[3] = {Real(src[0]), Real(src[1]), Real(src[2])};
   Real d[3] = {Real(src[3]), Real(src[4]), Real(src[5])};  // source axis; rotated below (step 2)
@@ -358,8 +396,9 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
     // R-20: with effective scattering lengths b = 1/(lambda_e (1-g)), so the optical depth along the lambda_e table
     // that corresponds to tau_s is tau_s (1 - g)
     const Real tau_s = -std::log(u_dist) * (ice.effective_scattering ? Real(1.0 - ice.g) : Real(1));
-    const Real s_scat = walk(ice, ice.scat_len, p[2], d[2], tau_s);
-    const Real s_abs = walk(ice, ice.abs_len, p[2], d[2], tau_a);
+    // R-21: coefficients scaled by sc <=> optical depth along the unscaled table divided by sc
+    const Real s_scat = walk(ice, ice.scat_len, p[2], d[2], tau_s / sc_b);
+    const Real s_abs = walk(ice, ice.abs_len, p[2], d[2], tau_a / sc_a);
     const bool absorbed = (s_abs <= s_scat);
     const Real s = absorbed ? s_abs : s_scat;
     // step 7: first DOM met on [0, s]
@@ -371,7 +410,7 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
       t += double(t_hit) / double(v);
       r.fate = kHit; r.dom = dom; r.weight = 1.0;
       if (acc && acc->mode != 0) {  // R-17
-        const double pa = acceptance(*acc, double(d[2]));
+        const double pa = std::min(1.0, acceptance(*acc, double(d[2])) * double(sc_acc));
         if (acc->mode == 1) {
           const uint32_t actr[4] = {photon_idx, source_id, event_id, 0x80000000u | k};
           uint32_t aw[4];
@@ -385,7 +424,7 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
       break;
     }
     // step 8: advance
-    tau_a -= depth(ice, ice.abs_len, p[2], d[2], s);
+    tau_a -= depth(ice, ice.abs_len, p[2], d[2], s) * sc_a;
     for (int a = 0; a < 3; ++a) p[a] += d[a] * s;
     path += double(s);
     t += double(s) / double(v);

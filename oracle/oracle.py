@@ -66,7 +66,10 @@ class _Job(C.Structure):
                 ("brute_force", C.c_int32), ("real_type", C.c_int32), ("n_threads", C.c_int32), ("pad", C.c_int32),
                 ("hits", C.c_void_p), ("hit_cap", C.c_uint64), ("fates", C.c_void_p), ("fate_cap", C.c_uint64),
                 ("acc_mode", C.c_int32), ("acc_n_coef", C.c_int32), ("acc_coef", C.c_double * 8),
-                ("length", C.POINTER(C.c_float))]
+                ("length", C.POINTER(C.c_float)), ("spec_n", C.c_int32), ("pad2", C.c_int32),
+                ("spec_cdf", C.POINTER(C.c_float)), ("spec_abs_scale", C.POINTER(C.c_float)),
+                ("spec_scat_scale", C.POINTER(C.c_float)), ("spec_n_group", C.POINTER(C.c_float)),
+                ("spec_acc_scale", C.POINTER(C.c_float))]
 
 
 _lib = None
@@ -197,7 +200,7 @@ class Result:
 
 def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int = 0, first=None, count=None,
               brute_force: bool = False, real_type: str = "f64", n_threads: int = 0, want_fates: bool = False,
-              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None) -> Result:
+              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None, spectrum=None) -> Result:
     """Run the selected photons (``first <= i < first+count`` and ``i % stride == offset``) of
     every source through the oracle.  Hits come back sorted by (event, source, photon)."""
     L = lib()
@@ -240,6 +243,15 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     len_arr = None if lengths is None else np.ascontiguousarray(lengths, dtype=np.float32)
     assert len_arr is None or len_arr.shape[0] == n
     job.length = None if len_arr is None else _fp(len_arr)
+    spec_keep = []
+    job.spec_n = 0
+    if spectrum is not None:  # anything with cdf, abs_scale, scat_scale, n_group, acc_scale (workloads.Spectrum)
+        for name in ("cdf", "abs_scale", "scat_scale", "n_group", "acc_scale"):
+            a = np.ascontiguousarray(getattr(spectrum, name), dtype=np.float32)
+            spec_keep.append(a)
+            setattr(job, "spec_" + name, _fp(a))
+        job.spec_n = int(spec_keep[0].shape[0])
+        assert all(a.shape[0] == job.spec_n for a in spec_keep)
     job.acc_mode = ACCEPTANCE_MODES[acceptance_mode]
     job.acc_n_coef = len(acceptance_coef)
     for k, c in enumerate(acceptance_coef):

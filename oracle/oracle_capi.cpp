@@ -64,6 +64,12 @@ struct orc_job {
   int32_t acc_n_coef;
   double acc_coef[8];
   const float* length;         // nullable: source lengths in metres (oracle.hpp, R-18); default 0 = point sources
+  int32_t spec_n, pad2;        // wavelength bins (oracle.hpp, R-21); 0 = monochromatic
+  const float* spec_cdf;
+  const float* spec_abs_scale;
+  const float* spec_scat_scale;
+  const float* spec_n_group;
+  const float* spec_acc_scale;
 };
 
 void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
@@ -116,6 +122,9 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
   if (job->acc_n_coef < 0 || job->acc_n_coef > 8 || job->acc_mode < 0 || job->acc_mode > 2) return -1;
   Acceptance acc{job->acc_mode, job->acc_n_coef, {0}};
   for (int k = 0; k < job->acc_n_coef; ++k) acc.coef[k] = job->acc_coef[k];
+  if (job->spec_n < 0 || job->spec_n > 32) return -1;
+  const Spectrum spec{job->spec_n, job->spec_cdf, job->spec_abs_scale, job->spec_scat_scale, job->spec_n_group,
+                      job->spec_acc_scale};
 
   // flatten the selection into work units of (source, [lo, hi)) so threads can share big sources
   struct Unit { uint64_t s, lo, hi, fate_base; };
@@ -152,8 +161,8 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
         const uint32_t ev = job->event_id[un.s], sid = job->source_id[un.s];
         const float len = job->length ? job->length[un.s] : 0.0f;
         PhotonResult r = job->real_type == 1
-                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len)
-                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len);
+                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec)
+                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec);
         st[tid].photons++;
         st[tid].flights += r.n_flights;
         if (r.fate == kAbsorbed) st[tid].absorbed++;

@@ -70,6 +70,30 @@ class Ice:
 
 
 @dataclass
+class Spectrum:
+    """Wavelength bins (R-21): per bin the cumulative probability, the factors on the absorption and
+    scattering coefficients, the group index and the factor on the acceptance.  A stand-in: the real Cherenkov
+    spectrum, ice dispersion and DOM efficiency curves are not available."""
+
+    cdf: np.ndarray  # float32 [n], non-decreasing, last = 1
+    abs_scale: np.ndarray
+    scat_scale: np.ndarray
+    n_group: np.ndarray
+    acc_scale: np.ndarray
+
+
+def spectrum_standin(n_bins: int = 8) -> Spectrum:
+    """8 bins from blue to red: bluer light is drawn more often (1/lambda^2-like weights), scatters more and is
+    absorbed less in the blue-green, travels a little slower; the acceptance falls off towards both ends."""
+    x = (np.arange(n_bins) + 0.5) / n_bins  # 0 = blue end, 1 = red end
+    w = 1.0 / (1.0 + x) ** 2
+    cdf = np.cumsum(w) / w.sum()
+    cdf[-1] = 1.0
+    return Spectrum(cdf.astype(np.float32), (0.6 + 1.6 * x ** 2).astype(np.float32), (1.25 - 0.5 * x).astype(np.float32),
+                    (1.38 - 0.05 * x).astype(np.float32), (1.0 - 1.6 * (x - 0.4) ** 2).astype(np.float32))
+
+
+@dataclass
 class Sources:
     """A list of light sources.  ``src`` rows are (x, y, z, dx, dy, dz, t_ns, E_GeV)."""
 
