@@ -196,6 +196,19 @@ int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block);
 #define PP_MAX_ACCEPT_COEF 8u
 int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n_coef);
 
+/* Wavelength bins (NEXT-2, reading R-21 of DESIGN.md; PAPER.md:33 names the wavelength among the things the
+ * photoelectron probability depends on, PAPER.md:9 the varying optical properties).  A photon belongs to one of
+ * n_bins <= PP_MAX_SPECTRUM_BINS bins for its whole life: bin j = the first with cdf[j] > u, u = word 0 of Philox block
+ * (photon, source, event, 2^30).  In bin j the absorption and scattering coefficients of every ice layer are
+ * multiplied by abs_scale[j] and scat_scale[j], the photon travels at c / n_group[j], and the acceptance
+ * probability of pp_set_acceptance becomes min(1, p(eta) acc_scale[j]).  All arrays are HOST arrays of n_bins
+ * floats, copied before returning: cdf non-decreasing in (0, 1] (the last bin takes whatever is left), scales > 0,
+ * n_group >= 1, acc_scale >= 0 (PP_E_INVAL otherwise).  n_bins = 0 switches back to monochromatic photons
+ * (pp_ice.n_group, scales 1).  Applies to launches cut after the call; idle server required (PP_E_STATE). */
+#define PP_MAX_SPECTRUM_BINS 32u
+int pp_set_spectrum(pp_handle* h, uint32_t n_bins, const float* cdf, const float* abs_scale, const float* scat_scale,
+                    const float* n_group, const float* acc_scale);
+
 int pp_stats(pp_handle* h, pp_stats_t* out);
 const char* pp_last_error(pp_handle* h);
 void pp_destroy(pp_handle* h);

@@ -68,7 +68,7 @@ class _Stats(C.Structure):
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
-           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments"]
+           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum"]
 
 
 class _LaunchPlan(C.Structure):
@@ -103,6 +103,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_collect.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_int]
     L.pp_set_acceptance.restype = C.c_int
     L.pp_set_acceptance.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.c_uint32]
+    L.pp_set_spectrum.restype = C.c_int
+    L.pp_set_spectrum.argtypes = [vp, C.c_uint32] + [C.POINTER(C.c_float)] * 5
     L.pp_stats.restype = C.c_int
     L.pp_stats.argtypes = [vp, C.POINTER(_Stats)]
     L.pp_last_error.restype = C.c_char_p
@@ -292,6 +294,18 @@ class Propagator:
         c = np.ascontiguousarray(coef, dtype=np.float32)
         rc = self._L.pp_set_acceptance(self._h, ACCEPTANCE_MODES[mode], c.ctypes.data_as(C.POINTER(C.c_float)),
                                        c.shape[0])
+        self._check(rc, self._h)
+
+    def set_spectrum(self, spectrum=None):
+        """pp_set_spectrum: ``spectrum`` has cdf, abs_scale, scat_scale, n_group, acc_scale arrays (None: off)."""
+        fp = C.POINTER(C.c_float)
+        if spectrum is None:
+            rc = self._L.pp_set_spectrum(self._h, 0, None, None, None, None, None)
+        else:
+            arrs = [np.ascontiguousarray(getattr(spectrum, k), dtype=np.float32)
+                    for k in ("cdf", "abs_scale", "scat_scale", "n_group", "acc_scale")]
+            assert all(a.shape == arrs[0].shape for a in arrs)
+            rc = self._L.pp_set_spectrum(self._h, arrs[0].shape[0], *[a.ctypes.data_as(fp) for a in arrs])
         self._check(rc, self._h)
 
     def flush(self):

@@ -868,7 +868,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
     P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
     for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x optional physics
-      P.acc_mode = (f & 2) ? 1u : 0u;
+      P.acc_mode = (f & 2) ? 1u : 0u;  // (any of the optional-physics switches selects the same variant)
       if (launch_propagate(P, h->brute, (f & 1) != 0, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     }
     if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
@@ -1003,6 +1003,32 @@ int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n
   h->base.acc_mode = mode;
   h->base.acc_n = mode == PP_ACCEPT_OFF ? 0u : n_coef;
   for (uint32_t k = 0; k < PP_MAX_ACCEPT_COEF; ++k) h->base.acc_coef[k] = (mode != PP_ACCEPT_OFF && k < n_coef) ? coef[k] : 0.0f;
+  return PP_OK;
+}
+
+int pp_set_spectrum(pp_handle* h, uint32_t n_bins, const float* cdf, const float* abs_scale, const float* scat_scale,
+                    const float* n_group, const float* acc_scale) {
+  if (!h) return PP_E_INVAL;
+  if (n_bins > PP_MAX_SPECTRUM_BINS) return fail(h, PP_E_INVAL, "pp_set_spectrum: too many bins");
+  if (n_bins && (!cdf || !abs_scale || !scat_scale || !n_group || !acc_scale)) return fail(h, PP_E_INVAL, "pp_set_spectrum: null array");
+  for (uint32_t j = 0; j < n_bins; ++j) {
+    const bool ok = finite_f(cdf[j]) && cdf[j] > 0.0f && cdf[j] <= 1.0f && (j == 0 || cdf[j] >= cdf[j - 1]) &&
+                    finite_f(abs_scale[j]) && abs_scale[j] > 0.0f && finite_f(scat_scale[j]) && scat_scale[j] > 0.0f &&
+                    finite_f(n_group[j]) && n_group[j] >= 1.0f && finite_f(acc_scale[j]) && acc_scale[j] >= 0.0f;
+    if (!ok) return fail(h, PP_E_INVAL, "pp_set_spectrum: bad value in bin " + std::to_string(j));
+  }
+  std::lock_guard<std::mutex> g(h->mu);
+  if (!idle_locked(h)) return PP_E_STATE;
+  LaunchParams& B = h->base;
+  B.spec_n = n_bins;
+  for (uint32_t j = 0; j < PP_MAX_SPECTRUM_BINS; ++j) {
+    const bool in = j < n_bins;
+    B.spec_cdf[j] = in ? cdf[j] : 2.0f;
+    B.spec_inv_a[j] = in ? (float)(1.0 / (double)abs_scale[j]) : 1.0f;
+    B.spec_inv_b[j] = in ? (float)(1.0 / (double)scat_scale[j]) : 1.0f;
+    B.spec_acc[j] = in ? acc_scale[j] : 1.0f;
+    B.spec_inv_v[j] = in ? (double)n_group[j] / kC : B.inv_v;
+  }
   return PP_OK;
 }
 

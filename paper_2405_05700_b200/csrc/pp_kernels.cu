@@ -177,6 +177,17 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
   return best;
 }
 
+// R-21: bin j = the first with cdf[j] > u, u = word 0 of Philox block (photon, source, event, 2^30); entries past
+// spec_n hold 2, so the search needs no bound.  Recomputed where needed instead of carried in a register.
+__device__ __noinline__ uint32_t spectrum_bin(const LaunchParams& P, uint32_t pidx, uint32_t sid, uint32_t ev) {
+  uint32_t b0 = pidx, b1 = sid, b2 = ev, b3 = 0x40000000u;
+  philox4x32_10(b0, b1, b2, b3, P.rk);
+  const float u = uniform_from_word(b0);
+  uint32_t j = 0;
+  while (j + 1u < P.spec_n && !(P.spec_cdf[j] > u)) ++j;
+  return j;
+}
+
 // kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18) is compiled in
 template <bool kBrute, bool kFates, bool kExt>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
@@ -224,6 +235,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   float dx = 0, dy = 0, dz = 1;
   float Lh = 0, Ll = 0;  // path length, two-float
   float tau_a = 0;
+  float sc_b = 1.0f;  // kExt only: 1 / scat_scale of the photon's wavelength bin (R-21)
   uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
 
   for (;;) {
@@ -317,10 +329,17 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       }
       rotate(dx, dy, dz, m, u_az);
       // =========================== a3: absorption budget (once per photon) ======================
-      const float tau_new = -__logf(u_abs);
+      float tau_new = -__logf(u_abs);
+      if (kExt && P.spec_n != 0u && k == 0) {
+        // R-21: the photon's wavelength bin; both budgets are kept in units of the unscaled ice table
+        const uint32_t j = spectrum_bin(P, pidx, sid, ev);
+        tau_new *= P.spec_inv_a[j];
+        sc_b = P.spec_inv_b[j];
+      }
       tau_a = (k == 0) ? tau_new : tau_a;
       // =========================== a4: optical depth to the next scatter ========================
-      const float tau_s = neg_log_uniform(u_dist);
+      float tau_s = neg_log_uniform(u_dist);
+      if (kExt && P.spec_n != 0u) tau_s *= sc_b;
       // =========================== a4: layer walk in vertical optical depth ======================
       // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
       // so the budgets are scaled by w = |d_z| once and the walk works in vertical metres.
@@ -434,6 +453,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         float pa = 0.0f;
         for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
         pa = fminf(fmaxf(pa, 0.0f), 1.0f);
+        if (P.spec_n != 0u) pa = fminf(1.0f, pa * P.spec_acc[spectrum_bin(P, pidx, sid, ev)]);  // R-21
         if (P.acc_mode == 1u) {
           uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | (k - 1u);  // k was advanced: the hit flight is k - 1
           philox4x32_10(a0, a1, a2, a3, P.rk);
@@ -466,7 +486,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           }
           pp_hit h;
           h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
-          h.time_ns = t0 + ((double)Lh + (double)Ll) * P.inv_v;
+          double inv_v = P.inv_v;
+          if (kExt && P.spec_n != 0u) inv_v = P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)];  // R-21
+          h.time_ns = t0 + ((double)Lh + (double)Ll) * inv_v;
           h.weight = weight; h.n_scatter = k - 1;
           uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
           const uint4* srcv = reinterpret_cast<const uint4*>(&h);
@@ -497,7 +519,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         pp_fate f;
         f.x = phx + plx; f.y = phy + ply; f.z = phz + plz;
         f.path_m = Lh + Ll;
-        f.time_ns = (double)__ldg(&P.src[s_mine].t) + ((double)Lh + (double)Ll) * P.inv_v;
+        f.time_ns = (double)__ldg(&P.src[s_mine].t) + ((double)Lh + (double)Ll) *
+                    ((kExt && P.spec_n != 0u) ? P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)] : P.inv_v);
         f.n_flights = k;
         f.dom = (hit || rejected) ? (int32_t)hit_dom : -1;
         f.fate = hit ? 1u : (rejected ? 3u : (aborted ? 2u : 0u));
@@ -581,7 +604,7 @@ static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, c
 
 // the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u) ? 1 : 0);
+  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u) ? 1 : 0);
   switch (v) {
     case 0: return launch_prop_t<false, false, false>(P, grid, smem, st);
     case 1: return launch_prop_t<false, false, true>(P, grid, smem, st);

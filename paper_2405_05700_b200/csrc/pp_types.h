@@ -94,6 +94,10 @@ struct LaunchParams {
   uint32_t rk[10][2];                                // Philox round keys
   // DOM acceptance (pp_set_acceptance, R-17): mode 0 off, 1 probabilistic, 2 weighted
   uint32_t acc_mode, acc_n;
+  // wavelength bins (pp_set_spectrum, R-21): 0 = monochromatic
+  uint32_t spec_n;
+  float spec_cdf[32], spec_inv_a[32], spec_inv_b[32], spec_acc[32];  // cumulative probability, 1/abs_scale, 1/scat_scale
+  double spec_inv_v[32];                                             // n_group[j] / c  [ns/m]
   uint32_t has_segments;  // some source of this launch has length > 0 (R-18)
   float inv_c;            // 1 / c  [ns/m]
   float acc_coef[8];
