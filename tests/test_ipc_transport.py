@@ -106,6 +106,33 @@ def test_open_errors_and_slot_limit():
         ipc.IpcClient(name)  # unlinked with the server
 
 
+def test_server_gone_and_client_gone():
+    """A client that outlives the server gets PP_E_STATE instead of hanging; a client that leaves without reading its
+    hits does not wedge the server (its hits are dropped), and the other client still drains."""
+    name = f"/pp_ipc_test_{os.getpid()}_gone"
+    src, ev, sid, ln = _sources(0, 4, 50)
+    srv = ipc.IpcServer(None, name, max_clients=2, hit_ring_bytes=32 * 8, echo=True)  # hit ring of 8 hits
+    a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+    a.submit(src, ev, sid, ln)          # 200 hits will come back into a ring of 8 ...
+    a.flush()
+    assert len(a.collect(cap=4, block=True)) > 0
+    a.close()                           # ... but the client leaves after reading a few
+    s2, e2, i2, l2 = _sources(1, 3, 20)
+    b.submit(s2, e2, i2, l2)
+    got = np.sort(b.collect_all(), order=["event_id", "source_id"])
+    assert np.array_equal(got, _expected(s2, e2, i2, l2))
+    st = srv.stats()
+    assert st["error"] == 0 and st["sources_ingested"] == 260
+    b.submit(s2[:5], e2[:5] + 500, i2[:5], l2[:5])  # shipped but never flushed: not drained ...
+    srv.close()                                       # ... when the server goes away
+    with pytest.raises(B.PPError) as e:
+        b.collect(block=True)
+    assert e.value.code == -7
+    with pytest.raises(B.PPError):
+        b.submit(s2[:1], e2[:1], i2[:1], l2[:1])
+    b.close()
+
+
 def test_ipc_symbols_are_exported():
     """Every function include/pp_ipc.h declares is exported by the library and bound in ipc.py."""
     import re
