@@ -531,6 +531,39 @@ def run_c4(args):
     return 0
 
 
+def run_ext(args):
+    """C1 with the optional physics on (report mode): the stand-in wavelength bins (R-21), weighted DOM acceptance
+    (R-17) and C1's cascades given a 5 m length (R-18), through the device-resident path, next to the plain run."""
+    import torch
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import workloads as W
+    torch.cuda.set_device(0)
+    geo, ice, src = workload()
+    for name in ("plain", "acceptance", "spectrum", "acceptance+spectrum+segments"):
+        with B.Propagator(geo, ice, seed=0, launch_photons_target=10 ** 8) as prop:
+            if "acceptance" in name:
+                prop.set_acceptance("weighted", W.ACCEPTANCE_COEF)
+            if "spectrum" in name:
+                prop.set_spectrum(W.spectrum_standin())
+            ln = np.full(len(src), 5.0, np.float32) if "segments" in name else None
+            for _ in range(2):
+                prop.run(src.src, src.event_id, src.source_id, ln)
+            st0 = prop.stats()
+            t0 = time.perf_counter()
+            hits = 0
+            for _ in range(args.steps):
+                hits += len(prop.run(src.src, src.event_id, src.source_id, ln))
+            wall = time.perf_counter() - t0
+            st1 = prop.stats()
+        ph = st1.photons_done - st0.photons_done
+        busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+        print(json.dumps({"mode": "ext", "physics": name, "photons_per_step": ph / args.steps, "photons_per_s": ph / wall,
+                          "kernel_photons_per_s": ph / busy, "flights_per_photon": (st1.flights - st0.flights) / ph,
+                          "hits_per_step": hits / args.steps,
+                          "rejected_per_step": (st1.photons_rejected - st0.photons_rejected) / args.steps}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -538,6 +571,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ext", action="store_true", help="C1 with the optional physics on (report mode)")
     ap.add_argument("--c4", action="store_true", help="C4 memory-bounded extreme event (report mode)")
     ap.add_argument("--sweep", action="store_true", help="C3 launch-size sweep (report mode)")
     ap.add_argument("--sweep-sizes", default="", help="comma-separated photons per launch (default 1e5..1e9)")
@@ -549,6 +583,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.ext:
+        return run_ext(args)
     if args.c4:
         return run_c4(args)
     if args.sweep:

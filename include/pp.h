@@ -198,8 +198,9 @@ int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n
 
 /* Wavelength bins (NEXT-2, reading R-21 of DESIGN.md; PAPER.md:33 names the wavelength among the things the
  * photoelectron probability depends on, PAPER.md:9 the varying optical properties).  A photon belongs to one of
- * n_bins <= PP_MAX_SPECTRUM_BINS bins for its whole life: bin j = the first with cdf[j] > u, u = word 0 of Philox block
- * (photon, source, event, 2^30).  In bin j the absorption and scattering coefficients of every ice layer are
+ * n_bins <= PP_MAX_SPECTRUM_BINS bins for its whole life: bin j = the first with cdf[j] > u, u = the uniform of the word
+ * made of the low 9 bits of words 0, 1, 2 of the photon's Philox block 0 (bits the other uniforms do not use, so no
+ * extra block is drawn).  In bin j the absorption and scattering coefficients of every ice layer are
  * multiplied by abs_scale[j] and scat_scale[j], the photon travels at c / n_group[j], and the acceptance
  * probability of pp_set_acceptance becomes min(1, p(eta) acc_scale[j]).  All arrays are HOST arrays of n_bins
  * floats, copied before returning: cdf non-decreasing in (0, 1] (the last bin takes whatever is left), scales > 0,

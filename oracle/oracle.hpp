@@ -309,8 +309,8 @@ inline double acceptance(const Acceptance& acc, double eta) {
 // ------------------------------------------------------------------------------------------
 // Wavelength bins (NEXT-2; the photoelectron probability depends on "position, direction, time, and
 // wavelength"; the optical properties vary).  Reading R-21: a photon belongs to one of
-// n <= 32 wavelength bins for its whole life, bin j = the first with cdf[j] > u, u = word 0 of Philox block
-// (photon, source, event, 2^30); in bin j the absorption and scattering coefficients of every layer are multiplied by
+// n <= 32 wavelength bins for its whole life, bin j = the first with cdf[j] > u, u = the uniform of the word made of
+// the low 9 bits of words 0, 1, 2 of the photon's Philox block 0 (spectrum_word); in bin j the absorption and scattering coefficients of every layer are multiplied by
 // abs_scale[j] and scat_scale[j], the group index is n_group[j], and the acceptance probability becomes
 // min(1, p(eta) acc_scale[j]).  n = 0: monochromatic (R-4b).
 // ------------------------------------------------------------------------------------------
@@ -322,6 +322,12 @@ struct Spectrum {
   const float* n_group;     // [n] >= 1
   const float* acc_scale;   // [n] >= 0
 };
+
+// The wavelength draw costs no extra Philox block: a uniform takes the top 23 bits of its word (R-3), so the low 9
+// bits of the words of block 0 are unused; the low 9 bits of words 0, 1, 2 make the word of the wavelength uniform.
+inline uint32_t spectrum_word(const uint32_t w[4]) {
+  return ((w[0] & 0x1FFu) << 23) | ((w[1] & 0x1FFu) << 14) | ((w[2] & 0x1FFu) << 5);
+}
 
 inline int spectrum_bin(const Spectrum& sp, double u) {
   int j = 0;
@@ -351,10 +357,10 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
   Real sc_a = 1, sc_b = 1, sc_acc = 1;
   double n_group = ice.n_group;
   if (spec && spec->n > 0) {
-    const uint32_t sctr[4] = {photon_idx, source_id, event_id, 0x40000000u};
+    const uint32_t sctr[4] = {photon_idx, source_id, event_id, 0u};
     uint32_t sw[4];
     philox4x32_10(sctr, key, sw);
-    const int j = spectrum_bin(*spec, uniform_from_word(sw[0]));
+    const int j = spectrum_bin(*spec, uniform_from_word(spectrum_word(sw)));
     sc_a = Real(spec->abs_scale[j]); sc_b = Real(spec->scat_scale[j]); sc_acc = Real(spec->acc_scale[j]);
     n_group = double(spec->n_group[j]);
   }

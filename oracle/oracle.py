@@ -86,6 +86,8 @@ def lib():
         L.orc_photon_count.argtypes = [C.c_float, C.c_float]
         L.orc_hg_cos.restype = C.c_double
         L.orc_hg_cos.argtypes = [C.c_double, C.c_double]
+        L.orc_spectrum_word.restype = C.c_uint32
+        L.orc_spectrum_word.argtypes = [C.POINTER(C.c_uint32)]
         L.orc_acceptance.restype = C.c_double
         L.orc_acceptance.argtypes = [C.POINTER(C.c_double), C.c_int32, C.c_double]
         L.orc_rotate.restype = None
@@ -144,6 +146,12 @@ def photon_count(energy_gev, photons_per_gev=1.0e4) -> int:
 
 def hg_cos(g: float, u: float) -> float:
     return lib().orc_hg_cos(float(g), float(u))
+
+
+def spectrum_word(words) -> int:
+    """The word of the wavelength uniform, from the four words of a photon's Philox block 0 (R-21)."""
+    w = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in words])
+    return int(lib().orc_spectrum_word(w))
 
 
 def acceptance(coef, eta: float) -> float:

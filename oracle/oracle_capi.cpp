@@ -76,6 +76,7 @@ void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) 
 double orc_uniform(uint32_t w) { return uniform_from_word(w); }
 uint64_t orc_photon_count(float e, float y) { return photon_count(e, y); }
 double orc_hg_cos(double g, double u) { return hg_cos<double>(g, u); }
+uint32_t orc_spectrum_word(const uint32_t* w) { return spectrum_word(w); }
 double orc_acceptance(const double* coef, int32_t n_coef, double eta) {
   Acceptance a{1, n_coef, {0}};
   for (int k = 0; k < n_coef && k < 8; ++k) a.coef[k] = coef[k];

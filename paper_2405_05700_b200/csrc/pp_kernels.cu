@@ -177,15 +177,20 @@ __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, flo
   return best;
 }
 
-// R-21: bin j = the first with cdf[j] > u, u = word 0 of Philox block (photon, source, event, 2^30); entries past
-// spec_n hold 2, so the search needs no bound.  Recomputed where needed instead of carried in a register.
-__device__ __noinline__ uint32_t spectrum_bin(const LaunchParams& P, uint32_t pidx, uint32_t sid, uint32_t ev) {
-  uint32_t b0 = pidx, b1 = sid, b2 = ev, b3 = 0x40000000u;
-  philox4x32_10(b0, b1, b2, b3, P.rk);
-  const float u = uniform_from_word(b0);
+// R-21: the wavelength uniform is made of the low 9 bits of words 0, 1, 2 of the photon's Philox block 0 (the
+// uniforms of R-3 use the top 23 bits of a word); bin j = the first with cdf[j] > u.  Entries past spec_n hold 2, and
+// the count below runs over the warp-uniform bound spec_n, so the constant-bank loads are uniform.
+__device__ __forceinline__ uint32_t spectrum_bin_from_words(const LaunchParams& P, uint32_t w0, uint32_t w1, uint32_t w2) {
+  const float u = uniform_from_word(((w0 & 0x1FFu) << 23) | ((w1 & 0x1FFu) << 14) | ((w2 & 0x1FFu) << 5));
   uint32_t j = 0;
-  while (j + 1u < P.spec_n && !(P.spec_cdf[j] > u)) ++j;
+  for (uint32_t i = 0; i + 1u < P.spec_n; ++i) j += (P.spec_cdf[i] > u) ? 0u : 1u;
   return j;
+}
+// the same, recomputed from scratch where a hit's time or acceptance is formed (rare)
+__device__ __noinline__ uint32_t spectrum_bin(const LaunchParams& P, uint32_t pidx, uint32_t sid, uint32_t ev) {
+  uint32_t b0 = pidx, b1 = sid, b2 = ev, b3 = 0u;
+  philox4x32_10(b0, b1, b2, b3, P.rk);
+  return spectrum_bin_from_words(P, b0, b1, b2);
 }
 
 // kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18) is compiled in
@@ -331,8 +336,10 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       // =========================== a3: absorption budget (once per photon) ======================
       float tau_new = -__logf(u_abs);
       if (kExt && P.spec_n != 0u && k == 0) {
-        // R-21: the photon's wavelength bin; both budgets are kept in units of the unscaled ice table
-        const uint32_t j = spectrum_bin(P, pidx, sid, ev);
+        // R-21: the photon's wavelength bin from the spare bits of block 0.  Both optical-depth budgets are kept in
+        // units of the unscaled ice table: tau_a is divided by abs_scale once, sc_b = 1 / scat_scale multiplies
+        // every tau_s.
+        const uint32_t j = spectrum_bin_from_words(P, c0, c1, c2);
         tau_new *= P.spec_inv_a[j];
         sc_b = P.spec_inv_b[j];
       }

@@ -43,10 +43,17 @@ def test_absorption_and_bin_frequencies():
     assert np.all(is0 | is1)
     assert is0.mean() == pytest.approx(0.25, abs=4 * math.sqrt(0.25 * 0.75 / n))
     assert path[is0].mean() == pytest.approx(50.0, rel=0.01) and path[is1].mean() == pytest.approx(200.0, rel=0.01)
-    # the bin is word 0 of block (photon, source, event, 2^30) against the cdf
+    # the bin is the uniform made of the low 9 bits of words 0, 1, 2 of block 0, against the cdf
+    assert O.spectrum_word((0x1FF, 0, 0, 0)) == 0xFF800000 and O.spectrum_word((0xFFFFFE00, 0x101, 0xFFFFFFFF, 7)) == \
+        (0x101 << 14) | (0x1FF << 5)
     for i in range(200):
-        u = O.uniform(O.philox4x32_10((i, 0, 0, 0x40000000), (13, 0))[0])
-        assert bool(is0[i]) == (u < 0.25)
+        w = O.philox4x32_10((i, 0, 0, 0), (13, 0))
+        x = ((w[0] & 0x1FF) << 23) | ((w[1] & 0x1FF) << 14) | ((w[2] & 0x1FF) << 5)
+        assert x == O.spectrum_word(w)
+        assert bool(is0[i]) == (O.uniform(x) < 0.25)
+    # ... and is independent of the uniforms that share the block (they use the top 23 bits of each word)
+    az = np.array([O.uniform(O.philox4x32_10((i, 0, 0, 0), (13, 0))[0]) for i in range(4000)])
+    assert abs(np.corrcoef(az, is0[:4000].astype(float))[0, 1]) < 0.06
 
 
 def test_scattering_scale_and_arrival_times():
