@@ -636,8 +636,23 @@ void server_main(pp_handle* h) {
     if (progressed) continue;
     if (h->shutdown && h->n_in_flight == 0 && h->queued_photons == 0) return;
     if (h->n_in_flight > 0 && !h->resident_active) {
-      // nothing launchable: sleep briefly (new sources may arrive) -- the GPU is busy meanwhile
-      h->cv_work.wait_for(lk, std::chrono::microseconds(100));
+      // nothing launchable and the GPU is busy.  A short launch (C3's 1e5-1e6 photons take 0.1-0.2 ms) would lose
+      // half a sleep period of latency, so first poll the oldest launch's completion event for up to 150 us
+      // (bounded spinning, only while a launch is in flight), then sleep briefly (new sources may arrive).
+      Slot* oldest = nullptr;
+      for (auto& s : h->slot)
+        if (s.in_flight && (!oldest || s.seq < oldest->seq)) oldest = &s;
+      bool ready = false;
+      if (oldest) {
+        lk.unlock();
+        const auto t_end = Clock::now() + std::chrono::microseconds(150);
+        do {
+          ready = cudaEventQuery(oldest->ev_done) != cudaErrorNotReady;
+          if (!ready) std::this_thread::yield();
+        } while (!ready && Clock::now() < t_end);
+        lk.lock();
+      }
+      if (!ready) h->cv_work.wait_for(lk, std::chrono::microseconds(100));
     } else {
       h->cv_work.wait_for(lk, std::chrono::milliseconds(20));
     }
