@@ -14,7 +14,8 @@
  * submitted the hit's event.
  *
  * Contract: event ids are global -- an event belongs to the client that first submits a source of it, until the
- * server is closed; two clients submitting the same event id is a caller error (its hits all go to the first).  The
+ * server next runs dry (nothing queued, in flight or uncollected anywhere: the owner table is emptied then); two
+ * clients submitting the same event id at the same time is a caller error (its hits all go to the first).  The
  * hits a client receives are exactly the hits of its events, and, as everywhere in pp.h, they do not depend on how
  * many clients there are, on block sizes or on timing.
  *

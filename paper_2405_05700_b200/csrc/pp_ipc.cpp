@@ -140,6 +140,8 @@ struct pp_ipc_server {
   std::mutex map_mu;
   std::unordered_map<uint32_t, uint32_t> owner;  // event id -> client slot
   std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0};
+  std::atomic<uint32_t> ingest_busy{0};  // a block is between "events announced" and "handed to the back end"
+
   std::atomic<int> error{PP_OK};
 };
 
@@ -171,6 +173,7 @@ void ingest_main(pp_ipc_server* s) {
           src[i] = r.s; len[i] = r.length; ev[i] = r.event_id; sid[i] = r.source_id;
           any_len |= r.length != 0.0f;
         }
+        s->ingest_busy.store(1);
         {
           std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
           uint32_t last = ~ev[0];
@@ -182,6 +185,7 @@ void ingest_main(pp_ipc_server* s) {
         s->blocks++; s->sources += n;
         tail += n;
         ctl->src_tail.store(tail, std::memory_order_release);
+        s->ingest_busy.store(0);
         progressed = true;
       }
       const uint64_t fs = ctl->flush_seq.load(std::memory_order_acquire);
@@ -204,6 +208,7 @@ void dispatch_main(pp_ipc_server* s) {
   while (!s->stop.load()) {
     const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
     for (uint32_t c = 0; c < n_slots; ++c) snap[c] = s->seg.ctl(c)->src_tail.load(std::memory_order_acquire);
+    const uint64_t sources_before = s->sources.load();
     size_t n = 0;
     int drained = 0;
     const int rc = s->be.collect(s->be.ctx, buf.data(), cap, &n, &drained);
@@ -235,12 +240,18 @@ void dispatch_main(pp_ipc_server* s) {
       }
     }
     if (n == 0) {
-      if (drained)
+      if (drained) {
         for (uint32_t c = 0; c < n_slots; ++c) {
           ClientCtl* ctl = s->seg.ctl(c);
           if (snap[c] > ctl->completed_seq.load(std::memory_order_relaxed))
             ctl->completed_seq.store(snap[c], std::memory_order_release);
         }
+        // Forget the event owners once nothing can still produce a hit: the back end was drained at the collect
+        // above, and no block has been announced or ingested since the snapshot taken before it (the ingest thread
+        // needs map_mu to announce, so it cannot slip in while the map is cleared).
+        std::lock_guard<std::mutex> g(s->map_mu);
+        if (!s->owner.empty() && s->ingest_busy.load() == 0 && s->sources.load() == sources_before) s->owner.clear();
+      }
       nap(100);
     }
   }
