@@ -586,7 +586,10 @@ void server_main(pp_handle* h) {
     if (!h->resident_active && h->n_in_flight < 2 && h->sticky.load() == PP_OK) {
       Slot& s = h->slot[next_slot].in_flight ? h->slot[next_slot ^ 1] : h->slot[next_slot];
       Cut c{};
-      const bool force = h->flush_upto > h->ring_launch || h->space_waiters > 0;
+      // an idle GPU is fed early: with nothing in flight a launch is cut as soon as an eighth of the target is queued
+      // ("to keep the GPU as busy as possible"); with a launch in flight the queue fills to the target
+      const bool idle_feed = h->n_in_flight == 0 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8);
+      const bool force = h->flush_upto > h->ring_launch || h->space_waiters > 0 || idle_feed;
       bool have = false;
       if (!s.in_flight) {
         if (h->queued_photons == 0) {  // nothing but zero-photon sources (or nothing at all): drop them
@@ -960,7 +963,9 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
     h->st.photons_submitted += ph;
     h->st.source_ring_high_water =
         std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_head - h->ring_tail) * sizeof(SrcRec));
-    if (h->queued_photons >= h->sz.target) h->cv_work.notify_all();
+    if (h->queued_photons >= h->sz.target ||
+        (h->n_in_flight == 0 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
+      h->cv_work.notify_all();
   }
   return PP_OK;
 }
