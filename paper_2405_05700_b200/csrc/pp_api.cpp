@@ -191,8 +191,8 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
   const uint32_t n = geo->n_dom;
   out->fast_ok = false;
   if (brute) {
-    // validation mode: every DOM in input order; the block table of the fast path is still built when
-    // the geometry allows it, so that both modes cut sub-flights at the same xy cap (bit-identical results)
+    // validation mode: every DOM in input order (the cell table of the fast path is still built when the
+    // geometry allows it, only to report the same xy cap)
     HostGeometry fast;
     build_geometry(geo, false, &fast);
     out->xy_cap = fast.fast_ok ? fast.xy_cap : 100.0f;
@@ -243,8 +243,8 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
       out->dom_xyzw.push_back(c);
     }
   }
-  // ---- cell table: THE candidate line for a sub-flight whose xy midpoint lies in a cell ----
-  // A sub-flight of xy length <= L that passes within Rm of a line has its midpoint within L/2 + Rm of it.
+  // ---- cell table: THE candidate line for a piece of flight whose xy midpoint lies in a cell ----
+  // A piece of xy length <= L that passes within Rm of a line has its midpoint within L/2 + Rm of it.
   // If every cell is within reach = L/2 + Rm + slack of at most one line, the cell names that line; this
   // holds when 2 reach + (cell diagonal) < d_min, the smallest distance between two lines.
   const size_t ns = xy.size();
@@ -267,7 +267,7 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
     const double reach = 0.5 * L + Rm + slack, pad = reach + 2.0 * cell;  // >= one ring of empty cells all around
     const double gx0 = x0 - pad, gy0 = y0 - pad;
     const uint64_t nx = (uint64_t)std::ceil((x1 + pad - gx0) / cell) + 1, ny = (uint64_t)std::ceil((y1 + pad - gy0) / cell) + 1;
-    if (nx * ny > 40000) {  // keep the table in shared memory: coarser cells, shorter sub-flights
+    if (nx * ny > 40000) {  // keep the table in shared memory: coarser cells, shorter pieces
       cell *= 1.25;
       L = std::min(L, d_min - 2.0 * (Rm + slack) - cell * std::sqrt(2.0) - slack);
       continue;

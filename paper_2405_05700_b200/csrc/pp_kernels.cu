@@ -111,7 +111,7 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   return m;
 }
 
-struct Best {  // nearest DOM entry found so far on the current sub-flight
+struct Best {  // nearest DOM entry found so far on the current flight
   float t;
   uint32_t dom;
 };
@@ -132,7 +132,7 @@ __device__ __forceinline__ void sphere_test(const float4 c, float R, float phx, 
   if (t < best.t || (t == best.t && dom < best.dom)) { best.t = t; best.dom = dom; }
 }
 
-// Step 7 (slow path, rare): the sub-flight passes within the pre-filter radius of the axis of line
+// Step 7 (slow path, rare): the flight passes within the pre-filter radius of the axis of line
 // `si`; test the DOMs whose z lies in the swept interval with the exact ray-sphere solve.
 __device__ __noinline__ Best test_string(const LaunchParams& P, uint32_t si, float phx, float phy, float phz, float plx,
                                          float ply, float plz, float dx, float dy, float dz, float s, Best best) {
@@ -169,7 +169,7 @@ __device__ __noinline__ Best test_string(const LaunchParams& P, uint32_t si, flo
   return best;
 }
 
-// Validation variant of step 7: every DOM, every sub-flight.
+// Validation variant of step 7: every DOM, every flight.
 __device__ __noinline__ Best test_all_doms(const LaunchParams& P, float phx, float phy, float phz, float plx, float ply,
                                            float plz, float dx, float dy, float dz, float s, Best best) {
   for (uint32_t j = 0; j < P.n_dom; ++j)

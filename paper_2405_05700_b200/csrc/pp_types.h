@@ -105,9 +105,10 @@ struct LaunchParams {
   const StringRec* strings;  // [n_strings]
   const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
   // cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter
-  // disc can be met by a sub-flight whose xy midpoint lies in that cell (kNoString if none).  Unique because a
-  // sub-flight is capped to an xy length xy_cap < (smallest distance between two lines) - 2 radius_margin - cell
-  // diagonal; the outermost ring of cells is empty, so the cell index may simply be clamped into the grid.
+  // disc can be met by a piece of flight whose xy midpoint lies in that cell (kNoString if none).  Unique because
+  // a piece is at most xy_cap long in xy (longer flights are looked up piece by piece), and xy_cap < (smallest
+  // distance between two lines) - 2 radius_margin - cell diagonal; the outermost ring of cells is empty, so the
+  // cell index may simply be clamped into the grid.
   const uint16_t* cell_sid;  // [nx*ny]
   uint32_t n_strings, n_dom;
   uint32_t nx, ny;
