@@ -140,6 +140,9 @@ typedef struct pp_stats_t {
   uint64_t source_ring_high_water; /* bytes */
   uint64_t hit_ring_high_water;    /* bytes */
   uint64_t photons_rejected;       /* met a DOM but made no photoelectron (pp_set_acceptance); done = absorbed + hit + aborted + rejected */
+  uint64_t sources_completed;      /* the first sources_completed sources, in pp_submit order, are fully propagated and all
+                                      their hits are available to pp_collect (== sources_submitted once drained); lets a
+                                      producer finish its events while others keep the server busy */
 } pp_stats_t;
 
 typedef struct pp_handle pp_handle;

@@ -42,8 +42,8 @@ typedef struct pp_ipc_config {
 } pp_ipc_config;
 
 /* The server's back end: where blocks go and hits come from.  pp_ipc_server_create() binds it to a pp_handle
- * (submit = pp_submit_segments, flush = pp_flush, collect = pp_collect with block = 0, busy = something queued or
- * in flight); tests on a machine without a GPU bind it to pp_ipc_echo_backend(). */
+ * (submit = pp_submit_segments, flush = pp_flush, collect = pp_collect with block = 0, completed =
+ * pp_stats.sources_completed); tests on a machine without a GPU bind it to pp_ipc_echo_backend(). */
 typedef struct pp_ipc_backend {
   void* ctx;
   int (*submit)(void* ctx, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
@@ -51,11 +51,13 @@ typedef struct pp_ipc_backend {
   int (*flush)(void* ctx);
   int (*collect)(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained); /* non-blocking; *drained != 0:
                                             everything submitted before this call has been propagated and handed out */
+  int (*completed)(void* ctx, uint64_t* n_sources); /* the first n_sources sources, in submit order, are fully
+                                            propagated and their hits can be collected (pp_stats.sources_completed) */
 } pp_ipc_backend;
 
 /* Creates (O_CREAT | O_EXCL) the shared-memory segment `shm_name` ("/name"), and starts the ingest and dispatch
- * threads.  cfg may be NULL (defaults).  The handle must outlive the server and must not be used for pp_submit /
- * pp_collect by anybody else meanwhile. */
+ * threads.  cfg may be NULL (defaults).  The handle must be drained now, must outlive the server and must not be
+ * used for pp_submit / pp_collect by anybody else meanwhile. */
 int pp_ipc_server_create(pp_handle* h, const char* shm_name, const pp_ipc_config* cfg, pp_ipc_server** out);
 int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name, const pp_ipc_config* cfg,
                                  pp_ipc_server** out);
@@ -86,7 +88,9 @@ int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengt
 /* Asks the server to launch whatever is queued (pp_flush) once it has ingested everything this client shipped. */
 int pp_ipc_flush(pp_ipc_client* c);
 /* Copies up to cap hits of this client's events into out.  block != 0: waits until at least one hit is there or
- * everything this client shipped has been propagated and handed out (*n_out == 0 then means "drained"). */
+ * everything this client shipped has been propagated and handed out (*n_out == 0 then means "drained").  A client
+ * drains on its own: it does not wait for other clients' work (the server tracks completion block by block, in the
+ * order it handed the blocks to the GPU server). */
 int pp_ipc_collect(pp_ipc_client* c, pp_hit* out, size_t cap, size_t* n_out, int block);
 /* Detaches; the slot is not reused.  Hits not yet collected are dropped. */
 void pp_ipc_client_close(pp_ipc_client* c);

@@ -63,7 +63,7 @@ class _Stats(C.Structure):
                 ("flights", C.c_uint64), ("launches", C.c_uint64), ("relaunches", C.c_uint64),
                 ("hits_collected", C.c_uint64), ("kernel_busy_ms", C.c_double), ("wall_ms", C.c_double),
                 ("source_ring_high_water", C.c_uint64), ("hit_ring_high_water", C.c_uint64),
-                ("photons_rejected", C.c_uint64)]
+                ("photons_rejected", C.c_uint64), ("sources_completed", C.c_uint64)]
 
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
@@ -200,6 +200,7 @@ class Stats:
     source_ring_high_water: int
     hit_ring_high_water: int
     photons_rejected: int = 0
+    sources_completed: int = 0
 
 
 class Propagator:

@@ -78,6 +78,7 @@ struct Slot {
   cudaEvent_t ev_h2d = nullptr, ev_k0 = nullptr, ev_k1 = nullptr, ev_done = nullptr, ev_stage[2] = {nullptr, nullptr};
   // state of the launch in flight
   bool in_flight = false;
+  uint64_t sources_end = 0;  // sources [0, sources_end) of the submit order are complete once this launch has retired
   int resume_sel = 0;  // which of d_resume[] is the OUT list of the launch in flight
   LaunchParams P;
   uint64_t seq = 0;
@@ -579,7 +580,12 @@ void server_main(pp_handle* h) {
       const int rc = finish_slot(h, *oldest, true);
       lk.lock();
       if (rc != PP_OK) { oldest->in_flight = false; }
-      if (!oldest->in_flight) { h->n_in_flight--; h->wall_t1 = Clock::now(); h->cv_hits.notify_all(); }
+      if (!oldest->in_flight) {
+        h->n_in_flight--; h->wall_t1 = Clock::now();
+        // launches retire oldest first and their hits are queued by now: everything before sources_end is complete
+        h->st.sources_completed = std::max<uint64_t>(h->st.sources_completed, oldest->sources_end);
+        h->cv_hits.notify_all();
+      }
       progressed = true;
     }
     // 2. launch if a slot is free and enough work is queued
@@ -594,6 +600,7 @@ void server_main(pp_handle* h) {
       if (!s.in_flight) {
         if (h->queued_photons == 0) {  // nothing but zero-photon sources (or nothing at all): drop them
           h->ring_launch = h->ring_tail = h->ring_head; h->launch_offset = 0;
+          if (h->n_in_flight == 0) h->st.sources_completed = std::max<uint64_t>(h->st.sources_completed, h->ring_head);
           h->cv_space.notify_all();
         } else if (h->queued_photons >= h->sz.target || force) {
           const uint64_t cap = h->sz.cap_src, base = h->ring_launch;
@@ -609,6 +616,7 @@ void server_main(pp_handle* h) {
         if (c.last_partial) { h->ring_launch = rec_a + c.n_rec - 1; h->launch_offset = c.next_offset; }
         else { h->ring_launch = rec_a + c.n_rec; h->launch_offset = 0; }
         s.in_flight = true;  // reserve
+        s.sources_end = h->ring_launch;  // a source split across launches completes with the launch that ends it
         h->n_in_flight++;
         lk.unlock();
         int rc = PP_OK;

@@ -13,6 +13,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstring>
+#include <deque>
 #include <mutex>
 #include <new>
 #include <string>
@@ -93,10 +94,18 @@ int h_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
   return rc;
 }
 
+int h_completed(void* ctx, uint64_t* n_sources) {
+  pp_stats_t st;
+  const int rc = pp_stats(static_cast<pp_handle*>(ctx), &st);
+  *n_sources = rc == PP_OK ? st.sources_completed : 0;
+  return rc;
+}
+
 // ---- host-only echo back end (tests without a GPU) ----
 struct Echo {
   std::mutex mu;
   std::vector<pp_hit> pending, ready;
+  uint64_t flushed = 0;  // sources whose hit has been made available
 };
 int e_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
   Echo* e = static_cast<Echo*>(ctx);
@@ -115,7 +124,14 @@ int e_flush(void* ctx) {
   Echo* e = static_cast<Echo*>(ctx);
   std::lock_guard<std::mutex> g(e->mu);
   e->ready.insert(e->ready.end(), e->pending.begin(), e->pending.end());
+  e->flushed += e->pending.size();
   e->pending.clear();
+  return PP_OK;
+}
+int e_completed(void* ctx, uint64_t* n_sources) {
+  Echo* e = static_cast<Echo*>(ctx);
+  std::lock_guard<std::mutex> g(e->mu);
+  *n_sources = e->flushed;
   return PP_OK;
 }
 int e_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
@@ -141,6 +157,10 @@ struct pp_ipc_server {
   std::unordered_map<uint32_t, uint32_t> owner;  // event id -> client slot
   std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0};
   std::atomic<uint32_t> ingest_busy{0};  // a block is between "events announced" and "handed to the back end"
+  struct Block { uint32_t client; uint64_t tail_after, global_end; };
+  std::mutex fifo_mu;
+  std::deque<Block> fifo;       // blocks handed to the back end, in order, not yet known to be complete
+  uint64_t base_completed = 0;  // the back end's completed count when the server started
 
   std::atomic<int> error{PP_OK};
 };
@@ -184,6 +204,10 @@ void ingest_main(pp_ipc_server* s) {
         if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
         s->blocks++; s->sources += n;
         tail += n;
+        {
+          std::lock_guard<std::mutex> g(s->fifo_mu);
+          s->fifo.push_back({c, tail, s->sources.load()});
+        }
         ctl->src_tail.store(tail, std::memory_order_release);
         s->ingest_busy.store(0);
         progressed = true;
@@ -209,6 +233,15 @@ void dispatch_main(pp_ipc_server* s) {
     const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
     for (uint32_t c = 0; c < n_slots; ++c) snap[c] = s->seg.ctl(c)->src_tail.load(std::memory_order_acquire);
     const uint64_t sources_before = s->sources.load();
+    // how many sources (in hand-over order) were complete BEFORE the collect below: their hits are already queued,
+    // so once that collect comes back empty they have all been routed
+    uint64_t n_complete = 0;
+    if (s->be.completed) {
+      uint64_t v = 0;
+      const int rc0 = s->be.completed(s->be.ctx, &v);
+      if (rc0 != PP_OK) { s->error.store(rc0); s->stop.store(true); break; }
+      n_complete = v > s->base_completed ? v - s->base_completed : 0;
+    }
     size_t n = 0;
     int drained = 0;
     const int rc = s->be.collect(s->be.ctx, buf.data(), cap, &n, &drained);
@@ -240,6 +273,17 @@ void dispatch_main(pp_ipc_server* s) {
       }
     }
     if (n == 0) {
+      {
+        // per-client completion, block by block: a client drains without waiting for the others
+        std::lock_guard<std::mutex> g(s->fifo_mu);
+        while (!s->fifo.empty() && s->fifo.front().global_end <= n_complete) {
+          const pp_ipc_server::Block b = s->fifo.front();
+          s->fifo.pop_front();
+          ClientCtl* ctl = s->seg.ctl(b.client);
+          if (b.tail_after > ctl->completed_seq.load(std::memory_order_relaxed))
+            ctl->completed_seq.store(b.tail_after, std::memory_order_release);
+        }
+      }
       if (drained) {
         for (uint32_t c = 0; c < n_slots; ++c) {
           ClientCtl* ctl = s->seg.ctl(c);
@@ -278,7 +322,7 @@ int map_segment(const char* name, bool create, size_t bytes, Segment* seg) {
 extern "C" {
 
 const pp_ipc_backend* pp_ipc_echo_backend(void) {
-  auto* be = new pp_ipc_backend{new Echo(), e_submit, e_flush, e_collect};  // lives as long as the process
+  auto* be = new pp_ipc_backend{new Echo(), e_submit, e_flush, e_collect, e_completed};  // lives as long as the process
   return be;
 }
 
@@ -307,6 +351,7 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
   H->next_slot.store(0);
   H->magic = kMagic;
   H->server_alive.store(1, std::memory_order_release);
+  if (s->be.completed) s->be.completed(s->be.ctx, &s->base_completed);  // the back end must be drained at this point
   s->ingest = std::thread(ingest_main, s);
   s->dispatch = std::thread(dispatch_main, s);
   *out = s;
@@ -315,7 +360,7 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
 
 int pp_ipc_server_create(pp_handle* h, const char* shm_name, const pp_ipc_config* cfg, pp_ipc_server** out) {
   if (!h) return PP_E_INVAL;
-  const pp_ipc_backend be{h, h_submit, h_flush, h_collect};
+  const pp_ipc_backend be{h, h_submit, h_flush, h_collect, h_completed};
   return pp_ipc_server_create_backend(&be, shm_name, cfg, out);
 }
 

@@ -74,3 +74,40 @@ def test_clients_share_one_gpu_server(n_clients, ring_kib):
     allh = np.sort(np.concatenate(parts), order=KEY)
     assert st["hits_routed"] == len(allh) == len(ref)
     assert np.array_equal(allh, ref)
+
+
+def test_completion_is_tracked_source_by_source():
+    """pp_stats.sources_completed: monotone, in submit order, equal to sources_submitted once drained; and through
+    the front end a client drains while another client's block sits unlaunched in the server (steady state)."""
+    import time
+    geo, ice = W.geometry_full(radius=0.6), W.ice_layered()
+    s, ev, sid = _case()
+    with B.Propagator(geo, ice, seed=12, launch_photons_target=10 ** 9) as p:   # target never reached: flush decides
+        assert p.stats().sources_completed == 0
+        p.submit(s[:1000], ev[:1000], sid[:1000])
+        p.flush()
+        h1 = p.collect_all()
+        st = p.stats()
+        assert st.sources_completed == st.sources_submitted == 1000
+        p.submit(s[1000:1200], ev[1000:1200], sid[1000:1200])       # queued, not flushed: below target / 8
+        time.sleep(0.1)
+        st = p.stats()
+        assert st.sources_submitted == 1200 and st.sources_completed == 1000 and st.photons_done < st.photons_submitted
+        name = f"/pp_ipc_gpu_{os.getpid()}_own"
+        p.collect_all()
+        assert p.stats().sources_completed == 1200
+        with ipc.IpcServer(p, name, max_clients=2) as srv:
+            a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+            ma, mb = (ev % 2) == 0, (ev % 2) == 1
+            a.submit(s[ma][:3000], ev[ma][:3000], sid[ma][:3000])
+            ha = a.collect_all()                                     # A's flush launches A's block
+            assert len(ha) > 0 and np.all(ha["event_id"] % 2 == 0)
+            b.submit(s[mb][:300], ev[mb][:300], sid[mb][:300])       # B's block stays queued in the server
+            time.sleep(0.1)
+            assert len(a.collect(block=True)) == 0                   # A is drained although the server is not
+            pst = p.stats()
+            assert pst.photons_done < pst.photons_submitted
+            hb = b.collect_all()
+            assert len(hb) > 0 and np.all(hb["event_id"] % 2 == 1)
+            assert srv.stats()["hits_unrouted"] == 0
+            a.close(), b.close()

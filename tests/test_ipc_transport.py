@@ -106,6 +106,34 @@ def test_open_errors_and_slot_limit():
         ipc.IpcClient(name)  # unlinked with the server
 
 
+def test_a_client_drains_without_waiting_for_the_others():
+    """Steady state (clients keep queueing steps): client A must see its own work drained while client B
+    still has a block in the server that nobody flushed."""
+    name = f"/pp_ipc_test_{os.getpid()}_own"
+    with ipc.IpcServer(None, name, max_clients=2, echo=True) as srv:
+        a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+        sa, ea, ia, la = _sources(0, 5, 11)
+        sb, eb, ib, lb = _sources(1, 3, 7)
+        a.submit(sa, ea, ia, la)
+        got_a = np.sort(a.collect_all(), order=["event_id", "source_id"])   # flushes A's block
+        assert np.array_equal(got_a, _expected(sa, ea, ia, la))
+        b.submit(sb, eb, ib, lb)                                            # shipped, never flushed
+        import time
+        time.sleep(0.05)
+        sa2, ea2, ia2, la2 = _sources(2, 2, 5)
+        a.submit(sa2, ea2, ia2, la2)
+        got_a2 = a.collect_all()             # A's flush makes the server launch B's block too ...
+        assert len(got_a2) == len(ea2)
+        got_b = np.sort(b.collect_all(), order=["event_id", "source_id"])   # ... and B finds its hits
+        assert np.array_equal(got_b, _expected(sb, eb, ib, lb))
+        # now B ships a block that stays unflushed while A runs a whole cycle: A must not hang
+        b.submit(sb, eb + 500, ib, lb)
+        time.sleep(0.05)
+        assert len(a.collect(block=True)) == 0      # nothing outstanding for A: drained at once
+        assert srv.stats()["error"] == 0
+        a.close(), b.close()
+
+
 def test_server_gone_and_client_gone():
     """A client that outlives the server gets PP_E_STATE instead of hanging; a client that leaves without reading its
     hits does not wedge the server (its hits are dropped), and the other client still drains."""
