@@ -17,7 +17,7 @@
  *     weight";
  *   - many producers, one server: "multiple instances of IceTray ... sharing a single photon propagator
  *     server".
- * Everything the paper leaves open is fixed by the readings R-1..R-14 in DESIGN.md section 3.
+ * Everything the paper leaves open is fixed by the readings R-1..R-21 in DESIGN.md section 3.
  *
  * Conventions: metres, nanoseconds, GeV; z up.  All pointers are HOST pointers unless the parameter
  * name starts with d_ (DEVICE pointer).  The caller owns every pointer it passes; the library copies
@@ -65,8 +65,8 @@ typedef struct pp_hit {
   uint32_t source_id;
   uint32_t photon_idx; /* index of the photon within its source, 0 <= photon_idx < N */
   uint32_t dom_id;     /* row index into pp_geometry.xyz */
-  double time_ns;      /* source time + path / group velocity */
-  float weight;        /* 1.0 (acceptance == 1, R-4b) */
+  double time_ns;      /* source time (+ emission delay along a segment, R-18) + path / group velocity */
+  float weight;        /* 1.0 unless pp_set_acceptance is in weighted mode (R-4b, R-17) */
   uint32_t n_scatter;  /* number of scatters before the hit (diagnostic; 0 = direct light) */
 } pp_hit;
 
@@ -81,7 +81,7 @@ typedef struct pp_geometry {
 
 /* Layered ice.  Layer i spans z in (z_top-(i+1)*dz, z_top-i*dz]; layer 0 extends to
  * +infinity and layer n_layers-1 to -infinity (R-6).  Lengths in metres; scat_len is the geometric
- * mean free path between scatters (R-7). */
+ * mean free path between scatters (R-7) unless PP_FLAG_EFFECTIVE_SCATTERING is set (R-20). */
 typedef struct pp_ice {
   uint32_t n_layers;     /* 1..PP_MAX_LAYERS */
   float z_top;
