@@ -38,6 +38,9 @@
 //   wavelength bins (NEXT-2, R-21): one bin with unit scales == monochromatic bit for bit; two bins: bin frequencies,
 //                        mean path sum_j w_j lambda_a / abs_scale_j, flights per photon per bin, two arrival times
 //                        (d-R) n_j / c at a DOM with frequencies ~ w_j exp(-(d-R) a_j)
+//   angular smearing (NEXT-2, R-22): <cos> and <P2> of the emission angle about the source axis are
+//                        g cos(theta_c) and g^2 P2(cos theta_c) (Legendre moments multiply); azimuthal symmetry;
+//                        g_axis = 1 == exact cone bit for bit
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -351,7 +354,7 @@ template <class Real>
 inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx, const Ice& ice, uint64_t seed,
                                      const float src[8], uint32_t event_id, uint32_t source_id,
                                      uint32_t photon_idx, const Acceptance* acc = nullptr, float length = 0.0f,
-                                     const Spectrum* spec = nullptr) {
+                                     const Spectrum* spec = nullptr, double g_axis = 1.0) {
   const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
   // R-21: the photon's wavelength bin fixes its coefficient scales and its group index
   Real sc_a = 1, sc_b = 1, sc_acc = 1;
@@ -390,6 +393,16 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
         const Real ell = u_hg * Real(length);
         for (int a = 0; a < 3; ++a) p[a] += d[a] * ell;  // d is still the source axis here
         t += double(ell) / kC;
+      }
+      // R-22 (NEXT-2, angular smearing; the light of a cascade comes from its secondaries, "parameterized
+      // light yields"): with g_axis < 1 the axis the photon is emitted about is the source axis deflected by a polar
+      // angle drawn from the Henyey-Greenstein law of parameter g_axis and a uniform azimuth -- words 0 and 1 of Philox
+      // block (photon, source, event, 2^29).  g_axis = 1: the exact cone of R-4.
+      if (g_axis < 1.0) {
+        const uint32_t ectr[4] = {photon_idx, source_id, event_id, 0x20000000u};
+        uint32_t ew[4];
+        philox4x32_10(ectr, key, ew);
+        rotate(d, hg_cos(Real(g_axis), Real(uniform_from_word(ew[0]))), two_pi * Real(uniform_from_word(ew[1])));
       }
       cos_t = Real(ice.cos_cherenkov);  // step 2: emission on the Cherenkov cone about the source axis (R-4)
       tau_a = -std::log(u_abs);         // step 3: absorption budget, drawn once per photon

@@ -69,7 +69,7 @@ class _Job(C.Structure):
                 ("length", C.POINTER(C.c_float)), ("spec_n", C.c_int32), ("pad2", C.c_int32),
                 ("spec_cdf", C.POINTER(C.c_float)), ("spec_abs_scale", C.POINTER(C.c_float)),
                 ("spec_scat_scale", C.POINTER(C.c_float)), ("spec_n_group", C.POINTER(C.c_float)),
-                ("spec_acc_scale", C.POINTER(C.c_float))]
+                ("spec_acc_scale", C.POINTER(C.c_float)), ("g_axis", C.c_double)]
 
 
 _lib = None
@@ -208,7 +208,7 @@ class Result:
 
 def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int = 0, first=None, count=None,
               brute_force: bool = False, real_type: str = "f64", n_threads: int = 0, want_fates: bool = False,
-              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None, spectrum=None) -> Result:
+              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None, spectrum=None, g_axis: float = 1.0) -> Result:
     """Run the selected photons (``first <= i < first+count`` and ``i % stride == offset``) of
     every source through the oracle.  Hits come back sorted by (event, source, photon)."""
     L = lib()
@@ -251,6 +251,7 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     len_arr = None if lengths is None else np.ascontiguousarray(lengths, dtype=np.float32)
     assert len_arr is None or len_arr.shape[0] == n
     job.length = None if len_arr is None else _fp(len_arr)
+    job.g_axis = float(np.float32(g_axis))
     spec_keep = []
     job.spec_n = 0
     if spectrum is not None:  # anything with cdf, abs_scale, scat_scale, n_group, acc_scale (workloads.Spectrum)

@@ -70,6 +70,7 @@ struct orc_job {
   const float* spec_scat_scale;
   const float* spec_n_group;
   const float* spec_acc_scale;
+  double g_axis;               // angular smearing of the emission axis (oracle.hpp, R-22); 1 = off
 };
 
 void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
@@ -162,8 +163,8 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
         const uint32_t ev = job->event_id[un.s], sid = job->source_id[un.s];
         const float len = job->length ? job->length[un.s] : 0.0f;
         PhotonResult r = job->real_type == 1
-                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec)
-                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec);
+                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis)
+                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis);
         st[tid].photons++;
         st[tid].flights += r.n_flights;
         if (r.fate == kAbsorbed) st[tid].absorbed++;
