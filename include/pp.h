@@ -17,7 +17,7 @@
  *     weight";
  *   - many producers, one server: "multiple instances of IceTray ... sharing a single photon propagator
  *     server".
- * Everything the paper leaves open is fixed by the readings R-1..R-21 in DESIGN.md section 3.
+ * Everything the paper leaves open is fixed by the readings R-1..R-22 in DESIGN.md section 3.
  *
  * Conventions: metres, nanoseconds, GeV; z up.  All pointers are HOST pointers unless the parameter
  * name starts with d_ (DEVICE pointer).  The caller owns every pointer it passes; the library copies
@@ -212,6 +212,14 @@ int pp_set_acceptance(pp_handle* h, uint32_t mode, const float* coef, uint32_t n
 #define PP_MAX_SPECTRUM_BINS 32u
 int pp_set_spectrum(pp_handle* h, uint32_t n_bins, const float* cdf, const float* abs_scale, const float* scat_scale,
                     const float* n_group, const float* acc_scale);
+
+/* Angular smearing of the emission (NEXT-2, reading R-22 of DESIGN.md; a cascade's light comes from
+ * its secondaries).  With g_axis < 1 the axis a photon is emitted about is the source direction deflected by a polar
+ * angle drawn from the Henyey-Greenstein law of parameter g_axis and a uniform azimuth (words 0 and 1 of Philox block
+ * (photon, source, event, 2^29)); the photon then leaves on the Cherenkov cone about that axis.  g_axis = 1 (the
+ * default) is the exact cone of R-4.  -1 < g_axis <= 1, g_axis != 0 (PP_E_INVAL otherwise).  Applies to launches cut
+ * after the call; idle server required (PP_E_STATE). */
+int pp_set_emission_smearing(pp_handle* h, float g_axis);
 
 int pp_stats(pp_handle* h, pp_stats_t* out);
 const char* pp_last_error(pp_handle* h);

@@ -68,7 +68,8 @@ class _Stats(C.Structure):
 
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
-           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum"]
+           "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum",
+           "pp_set_emission_smearing"]
 
 
 class _LaunchPlan(C.Structure):
@@ -103,6 +104,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_collect.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_int]
     L.pp_set_acceptance.restype = C.c_int
     L.pp_set_acceptance.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.c_uint32]
+    L.pp_set_emission_smearing.restype = C.c_int
+    L.pp_set_emission_smearing.argtypes = [vp, C.c_float]
     L.pp_set_spectrum.restype = C.c_int
     L.pp_set_spectrum.argtypes = [vp, C.c_uint32] + [C.POINTER(C.c_float)] * 5
     L.pp_stats.restype = C.c_int
@@ -296,6 +299,10 @@ class Propagator:
         rc = self._L.pp_set_acceptance(self._h, ACCEPTANCE_MODES[mode], c.ctypes.data_as(C.POINTER(C.c_float)),
                                        c.shape[0])
         self._check(rc, self._h)
+
+    def set_emission_smearing(self, g_axis: float = 1.0):
+        """pp_set_emission_smearing: HG parameter of the emission-axis deflection (1 = exact cone)."""
+        self._check(self._L.pp_set_emission_smearing(self._h, float(g_axis)), self._h)
 
     def set_spectrum(self, spectrum=None):
         """pp_set_spectrum: ``spectrum`` has cdf, abs_scale, scat_scale, n_group, acc_scale arrays (None: off)."""

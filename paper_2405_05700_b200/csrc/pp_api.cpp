@@ -1060,6 +1060,19 @@ int pp_set_spectrum(pp_handle* h, uint32_t n_bins, const float* cdf, const float
   return PP_OK;
 }
 
+int pp_set_emission_smearing(pp_handle* h, float g_axis) {
+  if (!h) return PP_E_INVAL;
+  if (!finite_f(g_axis) || !(g_axis > -1.0f && g_axis <= 1.0f) || g_axis == 0.0f)
+    return fail(h, PP_E_INVAL, "pp_set_emission_smearing: g_axis must be in (-1, 1] and not 0");
+  std::lock_guard<std::mutex> g(h->mu);
+  if (!idle_locked(h)) return PP_E_STATE;
+  const double ga = g_axis;
+  h->base.emit_on = g_axis < 1.0f ? 1u : 0u;
+  h->base.emit_one_minus_g = (float)(1.0 - ga); h->base.emit_two_g = (float)(2.0 * ga);
+  h->base.emit_one_minus_g2 = (float)(1.0 - ga * ga);
+  return PP_OK;
+}
+
 int pp_stats(pp_handle* h, pp_stats_t* out) {
   if (!h || !out) return PP_E_INVAL;
   std::lock_guard<std::mutex> g(h->mu);

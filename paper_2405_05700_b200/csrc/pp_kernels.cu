@@ -332,6 +332,13 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
         const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
       }
+      if (kExt && P.emit_on != 0u && k == 0) {
+        // R-22: the axis the photon is emitted about = the source axis deflected by an HG(g_axis) polar angle
+        uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0x20000000u;
+        philox4x32_10(e0, e1, e2, e3, P.rk);
+        rotate(dx, dy, dz, hg_one_minus_cos(uniform_from_word(e0), P.emit_one_minus_g, P.emit_two_g, P.emit_one_minus_g2),
+               uniform_from_word(e1));
+      }
       rotate(dx, dy, dz, m, u_az);
       // =========================== a3: absorption budget (once per photon) ======================
       float tau_new = -__logf(u_abs);
@@ -611,7 +618,7 @@ static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, c
 
 // the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u) ? 1 : 0);
+  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u) ? 1 : 0);
   switch (v) {
     case 0: return launch_prop_t<false, false, false>(P, grid, smem, st);
     case 1: return launch_prop_t<false, false, true>(P, grid, smem, st);

@@ -98,6 +98,9 @@ struct LaunchParams {
   uint32_t spec_n;
   float spec_cdf[32], spec_inv_a[32], spec_inv_b[32], spec_acc[32];  // cumulative probability, 1/abs_scale, 1/scat_scale
   double spec_inv_v[32];                                             // n_group[j] / c  [ns/m]
+  // angular smearing of the emission axis (pp_set_emission_smearing, R-22): HG constants 1-g, 2g, 1-g^2; off = 0
+  uint32_t emit_on;
+  float emit_one_minus_g, emit_two_g, emit_one_minus_g2;
   uint32_t has_segments;  // some source of this launch has length > 0 (R-18)
   float inv_c;            // 1 / c  [ns/m]
   float acc_coef[8];
