@@ -41,6 +41,8 @@
 //   angular smearing (NEXT-2, R-22): <cos> and <P2> of the emission angle about the source axis are
 //                        g cos(theta_c) and g^2 P2(cos theta_c) (Legendre moments multiply); azimuthal symmetry;
 //                        g_axis = 1 == exact cone bit for bit
+//   longitudinal profile (NEXT-2, R-23): table values by hand; mean and variance of the emission offset for a
+//                        triangular-density table; identity table == no table to rounding
 //   full layered C1-C4 hit lists: PARITY UNPINNED by anything external (no published values);
 //                        pinned only through the invariants above.
 #pragma once
@@ -338,6 +340,26 @@ inline int spectrum_bin(const Spectrum& sp, double u) {
   return j;
 }
 
+// ------------------------------------------------------------------------------------------
+// Longitudinal profile of an extended source (NEXT-2, R-23): where along its length a source of length L emits.
+// The offset is L F(u), u the uniform of R-18, F piecewise linear through n knots f[0..n-1] at u = i/(n-1)
+// (an inverse cumulative distribution given as a table: no rejection sampling, one uniform).  No table: F(u) = u,
+// the uniform segment of R-18.
+// ------------------------------------------------------------------------------------------
+struct SegmentProfile {
+  int n;           // knots, 0 or 2..33
+  const float* f;  // [n] non-decreasing, in [0, 1]
+};
+
+inline double segment_fraction(const SegmentProfile* p, double u) {
+  if (!p || p->n < 2) return u;
+  const double x = u * double(p->n - 1);
+  int i = int(x);
+  if (i > p->n - 2) i = p->n - 2;
+  const double t = x - double(i);
+  return double(p->f[i]) + t * (double(p->f[i + 1]) - double(p->f[i]));
+}
+
 struct PhotonResult {
   double weight;      // hit weight (1 unless the acceptance is in weighted mode)
   int fate;
@@ -354,7 +376,8 @@ template <class Real>
 inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx, const Ice& ice, uint64_t seed,
                                      const float src[8], uint32_t event_id, uint32_t source_id,
                                      uint32_t photon_idx, const Acceptance* acc = nullptr, float length = 0.0f,
-                                     const Spectrum* spec = nullptr, double g_axis = 1.0) {
+                                     const Spectrum* spec = nullptr, double g_axis = 1.0,
+                                     const SegmentProfile* prof = nullptr) {
   const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
   // R-21: the photon's wavelength bin fixes its coefficient scales and its group index
   Real sc_a = 1, sc_b = 1, sc_acc = 1;
@@ -390,7 +413,7 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
       // length L > 0 emits from a point uniform on [0, L] along its axis, at the time the muon (speed c, R-11b) is
       // there; the offset uses the word of block 0 that flight 0 leaves unused (u_hg).  L = 0: point cascade (R-4).
       if (length > 0.0f) {
-        const Real ell = u_hg * Real(length);
+        const Real ell = Real(segment_fraction(prof, double(u_hg))) * Real(length);
         for (int a = 0; a < 3; ++a) p[a] += d[a] * ell;  // d is still the source axis here
         t += double(ell) / kC;
       }

@@ -69,7 +69,8 @@ class _Job(C.Structure):
                 ("length", C.POINTER(C.c_float)), ("spec_n", C.c_int32), ("pad2", C.c_int32),
                 ("spec_cdf", C.POINTER(C.c_float)), ("spec_abs_scale", C.POINTER(C.c_float)),
                 ("spec_scat_scale", C.POINTER(C.c_float)), ("spec_n_group", C.POINTER(C.c_float)),
-                ("spec_acc_scale", C.POINTER(C.c_float)), ("g_axis", C.c_double)]
+                ("spec_acc_scale", C.POINTER(C.c_float)), ("g_axis", C.c_double),
+                ("prof_n", C.c_int32), ("pad3", C.c_int32), ("prof_f", C.POINTER(C.c_float))]
 
 
 _lib = None
@@ -86,6 +87,8 @@ def lib():
         L.orc_photon_count.argtypes = [C.c_float, C.c_float]
         L.orc_hg_cos.restype = C.c_double
         L.orc_hg_cos.argtypes = [C.c_double, C.c_double]
+        L.orc_segment_fraction.restype = C.c_double
+        L.orc_segment_fraction.argtypes = [C.POINTER(C.c_float), C.c_int32, C.c_double]
         L.orc_spectrum_word.restype = C.c_uint32
         L.orc_spectrum_word.argtypes = [C.POINTER(C.c_uint32)]
         L.orc_acceptance.restype = C.c_double
@@ -148,6 +151,12 @@ def hg_cos(g: float, u: float) -> float:
     return lib().orc_hg_cos(float(g), float(u))
 
 
+def segment_fraction(table, u: float) -> float:
+    """F(u) of DESIGN.md R-23: the piecewise-linear inverse cumulative distribution of the emission offset."""
+    t = np.ascontiguousarray(table, dtype=np.float32)
+    return lib().orc_segment_fraction(_fp(t), int(t.shape[0]), float(u))
+
+
 def spectrum_word(words) -> int:
     """The word of the wavelength uniform, from the four words of a photon's Philox block 0 (R-21)."""
     w = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in words])
@@ -208,7 +217,7 @@ class Result:
 
 def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int = 0, first=None, count=None,
               brute_force: bool = False, real_type: str = "f64", n_threads: int = 0, want_fates: bool = False,
-              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None, spectrum=None, g_axis: float = 1.0) -> Result:
+              hit_cap: int | None = None, acceptance_mode: str = "off", acceptance_coef=(), lengths=None, spectrum=None, g_axis: float = 1.0, segment_profile=None) -> Result:
     """Run the selected photons (``first <= i < first+count`` and ``i % stride == offset``) of
     every source through the oracle.  Hits come back sorted by (event, source, photon)."""
     L = lib()
@@ -252,6 +261,9 @@ def propagate(geo, ice, sources, seed: int = 0, *, stride: int = 1, offset: int 
     assert len_arr is None or len_arr.shape[0] == n
     job.length = None if len_arr is None else _fp(len_arr)
     job.g_axis = float(np.float32(g_axis))
+    prof_arr = None if segment_profile is None else np.ascontiguousarray(segment_profile, dtype=np.float32)
+    job.prof_n = 0 if prof_arr is None else int(prof_arr.shape[0])
+    job.prof_f = None if prof_arr is None else _fp(prof_arr)
     spec_keep = []
     job.spec_n = 0
     if spectrum is not None:  # anything with cdf, abs_scale, scat_scale, n_group, acc_scale (workloads.Spectrum)

@@ -71,12 +71,18 @@ struct orc_job {
   const float* spec_n_group;
   const float* spec_acc_scale;
   double g_axis;               // angular smearing of the emission axis (oracle.hpp, R-22); 1 = off
+  int32_t prof_n, pad3;        // longitudinal profile of extended sources (oracle.hpp, R-23); 0 = uniform
+  const float* prof_f;
 };
 
 void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
 double orc_uniform(uint32_t w) { return uniform_from_word(w); }
 uint64_t orc_photon_count(float e, float y) { return photon_count(e, y); }
 double orc_hg_cos(double g, double u) { return hg_cos<double>(g, u); }
+double orc_segment_fraction(const float* f, int32_t n, double u) {
+  const SegmentProfile p{n, f};
+  return segment_fraction(&p, u);
+}
 uint32_t orc_spectrum_word(const uint32_t* w) { return spectrum_word(w); }
 double orc_acceptance(const double* coef, int32_t n_coef, double eta) {
   Acceptance a{1, n_coef, {0}};
@@ -124,7 +130,8 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
   if (job->acc_n_coef < 0 || job->acc_n_coef > 8 || job->acc_mode < 0 || job->acc_mode > 2) return -1;
   Acceptance acc{job->acc_mode, job->acc_n_coef, {0}};
   for (int k = 0; k < job->acc_n_coef; ++k) acc.coef[k] = job->acc_coef[k];
-  if (job->spec_n < 0 || job->spec_n > 32) return -1;
+  if (job->spec_n < 0 || job->spec_n > 32 || job->prof_n < 0 || job->prof_n == 1 || job->prof_n > 33) return -1;
+  const SegmentProfile prof{job->prof_n, job->prof_f};
   const Spectrum spec{job->spec_n, job->spec_cdf, job->spec_abs_scale, job->spec_scat_scale, job->spec_n_group,
                       job->spec_acc_scale};
 
@@ -163,8 +170,8 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
         const uint32_t ev = job->event_id[un.s], sid = job->source_id[un.s];
         const float len = job->length ? job->length[un.s] : 0.0f;
         PhotonResult r = job->real_type == 1
-                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis)
-                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis);
+                             ? propagate_photon<float>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis, &prof)
+                             : propagate_photon<double>(geo, pidx, ice, job->seed, src, ev, sid, uint32_t(i), &acc, len, &spec, job->g_axis, &prof);
         st[tid].photons++;
         st[tid].flights += r.n_flights;
         if (r.fate == kAbsorbed) st[tid].absorbed++;

@@ -88,3 +88,33 @@ def test_zero_length_is_the_point_source_bit_for_bit_and_mixed_lists():
     hd = d.hits[[int(s) in sid_pt for s in d.hits["source_id"]]]
     hc = c.hits[[int(s) in sid_pt for s in c.hits["source_id"]]]
     assert np.array_equal(hd, hc)
+
+
+def test_longitudinal_profile_table():
+    """NEXT-2, R-23: the emission offset is L F(u), F piecewise linear through a caller-supplied table."""
+    tab = [0.0, 0.5, 0.7, 1.0]
+    assert O.segment_fraction(tab, 0.0) == 0.0 and O.segment_fraction(tab, 1.0) == pytest.approx(1.0, abs=1e-7)
+    assert O.segment_fraction(tab, 1 / 3) == pytest.approx(0.5, abs=1e-6)
+    assert O.segment_fraction(tab, 0.5) == pytest.approx(0.6, abs=1e-6)       # halfway between knots 1 and 2
+    assert O.segment_fraction(tab, 0.9) == pytest.approx(0.7 + 0.7 * 0.3, abs=1e-6)
+    # F(u) = sqrt(u) sampled finely = density 2 l / L^2 (light piles up towards the end): mean 2L/3, variance L^2/18
+    knots = np.sqrt(np.linspace(0.0, 1.0, 33)).astype(np.float32)
+    L, n = 30.0, 200000
+    geo = W.Geometry(xyz=np.array([[1.0e6, 0.0, 0.0]], np.float32), radius=W.DOM_RADIUS)
+    ice = W.ice_homogeneous(scat_len=1.0e30, cos_cherenkov=1.0)
+    src = W.pencil_beam([0, 0, 0], [0, 0, 1], float(n))
+    r = O.propagate(geo, ice, src, seed=4, brute_force=True, want_fates=True, lengths=[L], segment_profile=knots)
+    ell = (r.fates["time_ns"] - r.fates["path_m"] / V) * C          # emission delay x c
+    # the table is the chord approximation of sqrt: its exact moments follow from the knots
+    k = knots.astype(np.float64)
+    m1 = L * np.mean((k[:-1] + k[1:]) / 2)
+    m2 = L * L * np.mean((k[:-1] ** 2 + k[:-1] * k[1:] + k[1:] ** 2) / 3)
+    assert m1 == pytest.approx(2 * L / 3, rel=5e-3)
+    assert ell.mean() == pytest.approx(m1, abs=4 * ell.std() / math.sqrt(n))
+    assert np.var(ell) == pytest.approx(m2 - m1 * m1, rel=0.02)
+    assert ell.min() >= -1e-9 and ell.max() <= L + 1e-9
+    # the identity table is the uniform segment of R-18 (to rounding)
+    ident = np.linspace(0.0, 1.0, 9).astype(np.float32)
+    a = O.propagate(geo, ice, src, seed=4, brute_force=True, want_fates=True, lengths=[L])
+    b = O.propagate(geo, ice, src, seed=4, brute_force=True, want_fates=True, lengths=[L], segment_profile=ident)
+    assert np.allclose(a.fates["z"], b.fates["z"], atol=1e-5) and np.allclose(a.fates["time_ns"], b.fates["time_ns"], atol=1e-5)
