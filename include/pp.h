@@ -17,7 +17,7 @@
  *     weight";
  *   - many producers, one server: "multiple instances of IceTray ... sharing a single photon propagator
  *     server".
- * Everything the paper leaves open is fixed by the readings R-1..R-22 in DESIGN.md section 3.
+ * Everything the paper leaves open is fixed by the readings R-1..R-23 in DESIGN.md section 3.
  *
  * Conventions: metres, nanoseconds, GeV; z up.  All pointers are HOST pointers unless the parameter
  * name starts with d_ (DEVICE pointer).  The caller owns every pointer it passes; the library copies
@@ -170,6 +170,15 @@ int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids,
  * non-finite length.  Everything else as pp_submit. */
 int pp_submit_segments(pp_handle* h, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
                        const uint32_t* source_ids, size_t n);
+
+/* Longitudinal profile of extended sources (NEXT-2, reading R-23): where along its length a source of
+ * pp_submit_segments emits.  The offset of a photon becomes l = L F(u) with the same u as above and F piecewise
+ * linear through the n_knots values cum_fraction[i] at u = i / (n_knots - 1): an inverse cumulative distribution given
+ * as a table (one uniform, no rejection).  cum_fraction is a HOST array, non-decreasing, in [0, 1], copied before
+ * returning; 2 <= n_knots <= PP_MAX_PROFILE_KNOTS, or n_knots = 0 for the uniform segment F(u) = u (the default).
+ * PP_E_INVAL otherwise; idle server required (PP_E_STATE). */
+#define PP_MAX_PROFILE_KNOTS 33u
+int pp_set_segment_profile(pp_handle* h, uint32_t n_knots, const float* cum_fraction);
 
 /* Asks the server to launch whatever is queued even if it is less than launch_photons_target. */
 int pp_flush(pp_handle* h);

@@ -69,7 +69,7 @@ class _Stats(C.Structure):
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
            "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum",
-           "pp_set_emission_smearing"]
+           "pp_set_emission_smearing", "pp_set_segment_profile"]
 
 
 class _LaunchPlan(C.Structure):
@@ -106,6 +106,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_set_acceptance.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float), C.c_uint32]
     L.pp_set_emission_smearing.restype = C.c_int
     L.pp_set_emission_smearing.argtypes = [vp, C.c_float]
+    L.pp_set_segment_profile.restype = C.c_int
+    L.pp_set_segment_profile.argtypes = [vp, C.c_uint32, C.POINTER(C.c_float)]
     L.pp_set_spectrum.restype = C.c_int
     L.pp_set_spectrum.argtypes = [vp, C.c_uint32] + [C.POINTER(C.c_float)] * 5
     L.pp_stats.restype = C.c_int
@@ -303,6 +305,15 @@ class Propagator:
     def set_emission_smearing(self, g_axis: float = 1.0):
         """pp_set_emission_smearing: HG parameter of the emission-axis deflection (1 = exact cone)."""
         self._check(self._L.pp_set_emission_smearing(self._h, float(g_axis)), self._h)
+
+    def set_segment_profile(self, cum_fraction=None):
+        """pp_set_segment_profile: knots of the inverse CDF of the emission offset (None: uniform)."""
+        if cum_fraction is None:
+            rc = self._L.pp_set_segment_profile(self._h, 0, None)
+        else:
+            t = np.ascontiguousarray(cum_fraction, dtype=np.float32)
+            rc = self._L.pp_set_segment_profile(self._h, t.shape[0], t.ctypes.data_as(C.POINTER(C.c_float)))
+        self._check(rc, self._h)
 
     def set_spectrum(self, spectrum=None):
         """pp_set_spectrum: ``spectrum`` has cdf, abs_scale, scat_scale, n_group, acc_scale arrays (None: off)."""

@@ -1073,6 +1073,21 @@ int pp_set_emission_smearing(pp_handle* h, float g_axis) {
   return PP_OK;
 }
 
+int pp_set_segment_profile(pp_handle* h, uint32_t n_knots, const float* cum_fraction) {
+  if (!h) return PP_E_INVAL;
+  if (n_knots == 1 || n_knots > PP_MAX_PROFILE_KNOTS || (n_knots && !cum_fraction))
+    return fail(h, PP_E_INVAL, "pp_set_segment_profile: n_knots must be 0 or 2..33");
+  for (uint32_t i = 0; i < n_knots; ++i)
+    if (!finite_f(cum_fraction[i]) || cum_fraction[i] < 0.0f || cum_fraction[i] > 1.0f ||
+        (i > 0 && cum_fraction[i] < cum_fraction[i - 1]))
+      return fail(h, PP_E_INVAL, "pp_set_segment_profile: table must be non-decreasing in [0, 1]");
+  std::lock_guard<std::mutex> g(h->mu);
+  if (!idle_locked(h)) return PP_E_STATE;
+  h->base.seg_n = n_knots;
+  for (uint32_t i = 0; i < PP_MAX_PROFILE_KNOTS; ++i) h->base.seg_tab[i] = i < n_knots ? cum_fraction[i] : 1.0f;
+  return PP_OK;
+}
+
 int pp_stats(pp_handle* h, pp_stats_t* out) {
   if (!h || !out) return PP_E_INVAL;
   std::lock_guard<std::mutex> g(h->mu);

@@ -193,6 +193,15 @@ __device__ __noinline__ uint32_t spectrum_bin(const LaunchParams& P, uint32_t pi
   return spectrum_bin_from_words(P, b0, b1, b2);
 }
 
+// R-23: fraction of a source's length at which a photon is emitted, F(u) piecewise linear through the knots
+__device__ __forceinline__ float segment_fraction(const LaunchParams& P, float u) {
+  if (P.seg_n < 2u) return u;
+  const float x = u * (float)(P.seg_n - 1u);
+  const uint32_t i = min(__float2uint_rz(x), P.seg_n - 2u);
+  const float f0 = P.seg_tab[i], f1 = P.seg_tab[i + 1u];
+  return fmaf(x - (float)i, f1 - f0, f0);
+}
+
 // kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18) is compiled in
 template <bool kBrute, bool kFates, bool kExt>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
@@ -327,7 +336,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
       if (kExt && P.has_segments != 0u && k == 0) {
         // R-18: a source with a length emits from a point uniform along it; u_hg is free on flight 0
-        const float ell = u_hg * __ldg(&P.src[s_mine].length);
+        const float ell = segment_fraction(P, u_hg) * __ldg(&P.src[s_mine].length);
         const float nx_ = fmaf(dx, ell, phx); plx += fmaf(dx, ell, phx - nx_); phx = nx_;
         const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
         const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
@@ -496,7 +505,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
             // R-18: emitted l / c after the source time; l is recomputed from block 0 instead of being carried
             uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0u;
             philox4x32_10(e0, e1, e2, e3, P.rk);
-            t0 += (double)(uniform_from_word(e1) * __ldg(&P.src[s_mine].length)) * (double)P.inv_c;
+            t0 += (double)(segment_fraction(P, uniform_from_word(e1)) * __ldg(&P.src[s_mine].length)) * (double)P.inv_c;
           }
           pp_hit h;
           h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;

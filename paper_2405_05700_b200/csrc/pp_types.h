@@ -101,6 +101,9 @@ struct LaunchParams {
   // angular smearing of the emission axis (pp_set_emission_smearing, R-22): HG constants 1-g, 2g, 1-g^2; off = 0
   uint32_t emit_on;
   float emit_one_minus_g, emit_two_g, emit_one_minus_g2;
+  // longitudinal profile of extended sources (pp_set_segment_profile, R-23): knots of the inverse CDF; 0 = uniform
+  uint32_t seg_n;
+  float seg_tab[33];
   uint32_t has_segments;  // some source of this launch has length > 0 (R-18)
   float inv_c;            // 1 / c  [ns/m]
   float acc_coef[8];

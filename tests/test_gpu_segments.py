@@ -108,3 +108,49 @@ def test_effective_scattering_lengths():
     # the same physics as the geometric table (lambda_e (1-g) rounds to lambda_s within an ulp): same statistics
     base, st_b = run(geo, ice, src, 10, None)
     assert abs(st.flights - st_b.flights) <= 1e-3 * st_b.flights and abs(len(base) - len(hits)) <= 6 * math.sqrt(len(base))
+
+
+def test_longitudinal_profile():
+    """NEXT-2, R-23: emission offsets drawn through a caller-supplied inverse-CDF table."""
+    knots = np.sqrt(np.linspace(0.0, 1.0, 33)).astype(np.float32)
+    geo, ice = W.geometry_full(radius=1.0), W.ice_layered()
+    src = W.sources_track(n_seg=40, n_casc=10)
+    src.src[:, 7] = 3.0
+    n = total_photons(src, ice)
+
+    def go(table, lengths):
+        with B.Propagator(geo, ice, seed=29) as p:
+            p.set_segment_profile(table)
+            hits = sort_hits(p.run(src.src, src.event_id, src.source_id, lengths))
+            return hits, p.stats()
+
+    hits, st = go(knots, src.length)
+    ref = O.propagate(geo, ice, src, seed=29, segment_profile=knots)
+    assert st.photons_done == n == ref.photons and ref.hit > 800
+    assert abs(st.flights - ref.flights) <= 3 and abs(st.photons_hit - ref.hit) <= 2
+    c = compare_hits(hits, ref.hits, n)
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.97, c
+    uni, _ = go(None, src.length)
+    assert not np.array_equal(uni, hits)
+    # closed form on the GPU: beam from a 30 m segment at a DOM 40 m ahead, scattering off, density 2 l / L^2
+    lam, L, D, m = 100.0, 30.0, 40.0, 400000
+    R = float(np.float32(W.DOM_RADIUS))
+    geo2 = W.Geometry(xyz=np.array([[0.0, 0.0, D]], np.float32), radius=W.DOM_RADIUS)
+    ice2 = W.ice_homogeneous(scat_len=1.0e30, cos_cherenkov=1.0)
+    beam = W.pencil_beam([0, 0, 0], [0, 0, 1], float(m))
+    with B.Propagator(geo2, ice2, seed=5, flags=B.FLAG_BRUTE_FORCE_DOMS) as p:
+        p.set_segment_profile(knots)
+        h2 = p.run(beam.src, beam.event_id, beam.source_id, [L])
+    k = knots.astype(np.float64)
+    # hit fraction = E[exp(-(D - R - l)/lam)] over the table's piecewise-uniform offsets
+    a, b = L * k[:-1], L * k[1:]
+    seg = np.where(b > a, lam * (np.exp(b / lam) - np.exp(a / lam)) / np.maximum(b - a, 1e-12), np.exp(a / lam))
+    frac = math.exp(-(D - R) / lam) * seg.mean()
+    assert len(h2) / m == pytest.approx(frac, abs=4 * math.sqrt(frac * (1 - frac) / m))
+    ref2 = O.propagate(geo2, ice2, beam, seed=5, brute_force=True, lengths=[L], segment_profile=knots)
+    c2 = compare_hits(sort_hits(h2), ref2.hits, m)
+    assert c2["frac_all"] >= 0.9999 and c2["max_dt"] <= 1e-3, c2
+    with B.Propagator(geo, ice, seed=0) as p:
+        for bad in ([0.5], [0.0, 0.6, 0.5], [0.0, 1.2], list(np.linspace(0, 1, 34))):
+            with pytest.raises(B.PPError):
+                p.set_segment_profile(bad)
