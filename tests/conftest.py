@@ -11,6 +11,13 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: longer statistical test")
+    # a fresh checkout has no binaries: build the CUDA library (nvcc cross-compiles without a GPU) and the oracle
+    # once if they are missing; an existing build is left alone (rebuild with __graft_entry__.build())
+    from paper_2405_05700_b200 import build as pp_build
+    if not os.path.exists(pp_build.LIB):
+        pp_build.build(force=True)
+    from oracle import oracle as O
+    O.build()
 
 
 def pytest_collection_modifyitems(config, items):
