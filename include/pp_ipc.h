@@ -65,7 +65,7 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
 void pp_ipc_server_destroy(pp_ipc_server* s);
 
 typedef struct pp_ipc_server_stats {
-  uint64_t clients_attached; /* slots ever claimed */
+  uint64_t clients_attached; /* distinct slots ever claimed */
   uint64_t blocks_ingested;  /* calls of the back end's submit */
   uint64_t sources_ingested;
   uint64_t hits_routed;
@@ -79,7 +79,8 @@ int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out);
 const pp_ipc_backend* pp_ipc_echo_backend(void);
 
 /* ---- client side (any process; no CUDA call inside) ---- */
-/* Attaches to the segment and claims a free client slot (PP_E_NOMEM if none, PP_E_STATE if there is no server). */
+/* Attaches to the segment and claims a client slot -- one a former client has left, else a fresh one (PP_E_NOMEM if
+ * none, PP_E_STATE if there is no server). */
 int pp_ipc_client_open(const char* shm_name, pp_ipc_client** out);
 /* Ships a block of n sources.  lengths_m and source_ids may be NULL as in pp_submit_segments.
  * Blocks while the client's source ring is full; a block larger than the ring is shipped in pieces. */
@@ -92,7 +93,7 @@ int pp_ipc_flush(pp_ipc_client* c);
  * drains on its own: it does not wait for other clients' work (the server tracks completion block by block, in the
  * order it handed the blocks to the GPU server). */
 int pp_ipc_collect(pp_ipc_client* c, pp_hit* out, size_t cap, size_t* n_out, int block);
-/* Detaches; the slot is not reused.  Hits not yet collected are dropped. */
+/* Detaches.  Hits not yet collected are dropped; the slot is handed out again once the server has next run dry. */
 void pp_ipc_client_close(pp_ipc_client* c);
 
 #ifdef __cplusplus

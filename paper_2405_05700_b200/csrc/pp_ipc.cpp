@@ -45,7 +45,7 @@ struct ShmHeader {
 };
 static_assert(sizeof(ShmHeader) <= kHeaderBytes, "header");
 
-enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2 };
+enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3 };  // kRecycled: closed, emptied, claimable again
 
 struct ClientCtl {
   std::atomic<uint32_t> state;
@@ -294,7 +294,20 @@ void dispatch_main(pp_ipc_server* s) {
         // above, and no block has been announced or ingested since the snapshot taken before it (the ingest thread
         // needs map_mu to announce, so it cannot slip in while the map is cleared).
         std::lock_guard<std::mutex> g(s->map_mu);
-        if (!s->owner.empty() && s->ingest_busy.load() == 0 && s->sources.load() == sources_before) s->owner.clear();
+        if (s->ingest_busy.load() == 0 && s->sources.load() == sources_before) {
+          s->owner.clear();
+          // the server is dry: slots of clients that have left can be handed out again.  The ring counters are
+          // absolute and simply carry on; hits the old client never read are skipped.
+          std::lock_guard<std::mutex> gf(s->fifo_mu);
+          if (s->fifo.empty())
+            for (uint32_t c = 0; c < n_slots; ++c) {
+              ClientCtl* ctl = s->seg.ctl(c);
+              if (ctl->state.load(std::memory_order_acquire) != kClosed) continue;
+              if (ctl->src_head.load(std::memory_order_acquire) != ctl->src_tail.load(std::memory_order_acquire)) continue;
+              ctl->hit_tail.store(ctl->hit_head.load(std::memory_order_relaxed), std::memory_order_release);
+              ctl->state.store(kRecycled, std::memory_order_release);
+            }
+        }
       }
       nap(100);
     }
@@ -393,10 +406,20 @@ int pp_ipc_client_open(const char* shm_name, pp_ipc_client** out) {
   if (H->magic != kMagic || H->total_bytes != c->seg.bytes || !H->server_alive.load(std::memory_order_acquire)) {
     munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_STATE;
   }
-  const uint32_t slot = H->next_slot.fetch_add(1);
-  if (slot >= H->max_clients) { munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_NOMEM; }
+  // a slot a former client has left (and the server has emptied) first, else a fresh one
+  uint32_t slot = ~0u;
+  const uint32_t used = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
+  for (uint32_t i = 0; i < used && slot == ~0u; ++i) {
+    uint32_t expect = kRecycled;
+    if (c->seg.ctl(i)->state.compare_exchange_strong(expect, kAttached, std::memory_order_acq_rel)) slot = i;
+  }
+  if (slot == ~0u) {
+    if (H->next_slot.load(std::memory_order_acquire) >= H->max_clients) { munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_NOMEM; }
+    slot = H->next_slot.fetch_add(1);
+    if (slot >= H->max_clients) { munmap(c->seg.base, c->seg.bytes); delete c; return PP_E_NOMEM; }
+    c->seg.ctl(slot)->state.store(kAttached, std::memory_order_release);
+  }
   c->slot = slot;
-  c->seg.ctl(slot)->state.store(kAttached, std::memory_order_release);
   *out = c;
   return PP_OK;
 }
