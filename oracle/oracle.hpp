@@ -25,6 +25,9 @@
 //   propagate            homogeneous-ice closed forms (segments ~ Geom, path ~ Exp(lambda_a),
 //                        <displacement> = 1/(a+b(1-g))), unscattered survival exp(-(d-R)(a+b)),
 //                        arrival time (d-R)/v, causality, conservation
+//   propagate, step 8 in LAYERED ice with scattering on (absorption budget carried across flights and layers)
+//                        g -> 1 vertical beam: total path over many flights ~ 1 - exp(-sum a_i dz_i) from the table only;
+//                        abs_len = 4 scat_len in every layer: flights per photon geometric with mean exactly 5
 //   acceptance / propagate with acceptance (NEXT-1, R-17)
 //                        polynomial values by hand; photons started inside a DOM: accepted fraction = p(cos theta_c)
 //                        and every weight = p(cos theta_c); pencil beam: hit fraction = survival x p(d_z);

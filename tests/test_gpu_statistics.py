@@ -65,6 +65,45 @@ def test_gpu_hg_mean_cosine_via_transport():
         assert z.mean() == pytest.approx(1 / (0.01 + 0.04 * (1 - g)), abs=4.5 * z.std() / math.sqrt(len(z)))
 
 
+def test_gpu_layered_absorption_budget_across_many_flights():
+    """The two layered-ice pins of tests/test_oracle_propagate.py (absorption budget carried over many flights
+    and across layer boundaries; PAPER.md:31 + :33) applied to the CUDA path itself."""
+    # (A) g = 0.999999, vertical beam down from z = 495: total path ~ 1 - exp(-sum a_i dz_i), from the table only
+    ice = W.ice_layered(cos_cherenkov=1.0, g=0.999999)
+    z0 = 495.0
+    _, f, st = gpu_run_resident(FAR, ice, W.pencil_beam([0, 0, z0], [0, 0, -1], 1.0e6), 11, want_fates=True)
+    assert st.photons_done == len(f) == 1000000 and st.photons_aborted == 0
+    a = 1.0 / ice.abs_len.astype(np.float64)
+    edges = np.concatenate([[0.0], 5.0 + 10.0 * np.arange(100)])
+    tau_edges = np.concatenate([[0.0], np.cumsum(a[:100] * np.diff(np.concatenate([edges, [1e9]]))[:100])])
+
+    def cdf(s):
+        s = np.asarray(s, dtype=np.float64)
+        i = np.clip(np.searchsorted(edges, s, side="right") - 1, 0, 99)
+        return 1.0 - np.exp(-(tau_edges[i] + a[i] * (s - edges[i])))
+
+    path = f["path_m"].astype(np.float64)
+    assert f["n_flights"].mean() > 3.0
+    assert np.quantile(np.abs(path - (z0 - f["z"].astype(np.float64))), 0.999) < 2e-3
+    assert stats.kstest(path[::5], cdf).pvalue > 1e-3
+    # (B) abs_len = 4 scat_len in every layer: flights per photon geometric with mean exactly 5
+    ice = W.ice_layered()
+    ice.abs_len = (4.0 * ice.scat_len.astype(np.float64)).astype(np.float32)
+    src = W.sources_c1().subset(slice(0, 40))
+    src.src[:, 7] = 2.5  # 25 000 photons per cascade
+    _, f, st = gpu_run_resident(FAR, ice, src, 13, want_fates=True)
+    n = f["n_flights"].astype(np.int64)
+    assert len(n) == 1000000 and st.photons_aborted == 0 and st.photons_hit == 0
+    assert n.mean() == pytest.approx(5.0, abs=4 * math.sqrt(20.0 / len(n)))
+    kmax = 40
+    obs = np.bincount(np.minimum(n, kmax), minlength=kmax + 1)[1:]
+    p = 0.2 * 0.8 ** np.arange(kmax)
+    p[-1] = 0.8 ** (kmax - 1)
+    chi2 = ((obs - len(n) * p) ** 2 / (len(n) * p)).sum()
+    assert stats.chi2.sf(chi2, kmax - 1) > 1e-3
+    assert st.flights == int(n.sum())
+
+
 @pytest.mark.slow
 def test_independent_streams_per_dom_chi2_and_mean_times():
     """BASELINE.json north_star: per-DOM hit counts agree with the oracle at chi^2 p > 0.01 over 10 seeds,

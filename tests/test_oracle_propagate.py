@@ -171,6 +171,61 @@ def test_layered_vertical_beam_absorption_depth_cdf():
     assert stats.kstest(r.fates["path_m"] * abs(dz), lambda x: cdf(x, abs(dz))).pvalue > 1e-3
 
 
+def _vertical_tau_cdf(ice, z0):
+    """CDF of the vertical drop at which a downward beam from z0 = 495 is absorbed, from the table only."""
+    a = 1.0 / ice.abs_len.astype(np.float64)
+    edges = np.concatenate([[0.0], 5.0 + 10.0 * np.arange(100)])
+    tau_edges = np.concatenate([[0.0], np.cumsum(a[:100] * np.diff(np.concatenate([edges, [1e9]]))[:100])])
+
+    def cdf(s):
+        s = np.asarray(s, dtype=np.float64)
+        i = np.clip(np.searchsorted(edges, s, side="right") - 1, 0, 99)
+        return 1.0 - np.exp(-(tau_edges[i] + a[i] * (s - edges[i])))
+
+    return cdf
+
+
+def test_layered_absorption_budget_across_many_flights_forward_peaked():
+    # Step 8's bookkeeping (tau_a -= optical depth of the stretch just flown) in LAYERED ice with scattering ON
+    # (PAPER.md:31 layers with their own coefficients + PAPER.md:33 "repeated until ... absorbed").  With
+    # g = 0.999999 every scatter leaves the direction unchanged to ~1e-3 rad, so the photon flies straight down in
+    # many flights (mean free path 5-60 m) and the total path must still follow 1 - exp(-sum a_i dz_i), a CDF built
+    # from the table only.  Charging the budget for the wrong stretch of ice (e.g. evaluating the optical depth
+    # after the position advance) fails this with p = 0.
+    ice = W.ice_layered(cos_cherenkov=1.0, g=0.999999)
+    z0 = 495.0
+    r = O.propagate(FAR, ice, W.pencil_beam([0, 0, z0], [0, 0, -1], 2.0e5), seed=11, want_fates=True, brute_force=True)
+    f = r.fates
+    assert f["n_flights"].mean() > 3.0  # the budget really is carried over several flights
+    # straight down: the Henyey-Greenstein tail leaves a few 1e-5 of the photons with one sizeable deflection
+    assert np.quantile(np.abs(f["path_m"] - (z0 - f["z"])), 0.999) < 1e-3
+    assert stats.kstest(f["path_m"], _vertical_tau_cdf(ice, z0)).pvalue > 1e-3
+
+
+def test_layered_proportional_tables_flights_geometric_whatever_the_path():
+    # If abs_len = 4 scat_len in EVERY layer, each interaction is an absorption with probability
+    # a/(a+b) = 1/5 wherever it happens and whatever the direction: flights per photon are geometric with mean
+    # exactly 5 in any layered ice.  Only correct carry-over of the absorption budget between flights and across
+    # layer boundaries gives that (a mis-ordered step 8 gives 4.56).  C1's cascades, the real Cherenkov cone, g = 0.9.
+    ice = W.ice_layered()
+    ice.abs_len = (4.0 * ice.scat_len.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(ice.abs_len.astype(np.float64), 4.0 * ice.scat_len.astype(np.float64))  # x4 is exact in fp32
+    src = W.sources_c1().subset(slice(0, 40))
+    src.src[:, 7] = 0.5  # GeV: 5000 photons per cascade
+    r = O.propagate(FAR, ice, src, seed=13, want_fates=True, brute_force=True)
+    n = r.fates["n_flights"].astype(np.int64)
+    assert len(n) == 40 * 5000 and r.aborted == 0 and r.hit == 0
+    assert n.mean() == pytest.approx(5.0, abs=4 * math.sqrt(20.0 / len(n)))
+    kmax = 40
+    obs = np.bincount(np.minimum(n, kmax), minlength=kmax + 1)[1:]
+    p = 0.2 * 0.8 ** np.arange(kmax)
+    p[-1] = 0.8 ** (kmax - 1)
+    chi2 = ((obs - len(n) * p) ** 2 / (len(n) * p)).sum()
+    assert stats.chi2.sf(chi2, kmax - 1) > 1e-3
+    # and the layers are really visited: the photons end in many different layers
+    assert len(np.unique(np.floor((500.0 - r.fates["z"]) / 10.0))) > 30
+
+
 def test_causality_and_brute_force_on_single_string():
     # C0 geometry with oversized DOMs (1.5 m) so that there are enough hits to look at
     geo, ice = W.geometry_single_string(radius=1.5), W.ice_homogeneous()
