@@ -97,6 +97,8 @@ struct pp_handle {
   Sizes sz;
   HostGeometry hg;
   LaunchParams base{};  // medium + geometry filled in once
+  std::vector<unsigned char> image;  // shared-memory tables as the kernel stages them (LaunchParams::smem_image)
+  uint64_t image_bytes = 0;
 
   // memory
   void* dev_ws = nullptr; bool own_dev = false;
@@ -307,6 +309,113 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
   out->fast_ok = true;
 }
 
+// Medium and geometry constants of a handle and the image of the shared-memory tables (a4, a5; layout in
+// pp_types.h).  Host only: pp_workspace_size() needs the image size, pp_create() uploads the image.
+int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg) {
+  LaunchParams& B = h->base;
+  const double scat_scale = (cfg->flags & PP_FLAG_EFFECTIVE_SCATTERING) ? 1.0 - (double)ice->g : 1.0;
+  if (!(scat_scale > 0.0)) return PP_E_INVAL;
+  const uint32_t nl = ice->n_layers;
+  std::vector<LayerRec> layers(nl + 1);
+  for (uint32_t i = 0; i < nl; ++i) {
+    // R-20: an effective scattering length is turned into the geometric mean free path here, once
+    const double ls = (double)ice->scat_len[i] * scat_scale;
+    layers[i].la = ice->abs_len[i]; layers[i].lb = (float)ls;
+    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / ls);
+  }
+  layers[nl] = layers[nl - 1];
+  B.n_layers = nl; B.last_layer = (int32_t)nl - 1;
+  B.z_top = ice->z_top; B.dz_layer = ice->dz; B.inv_dz_layer = (float)(1.0 / (double)ice->dz);
+  const double g = ice->g;
+  B.hg_one_minus_g = (float)(1.0 - g); B.hg_two_g = (float)(2.0 * g); B.hg_one_minus_g2 = (float)(1.0 - g * g);
+  B.one_minus_cos_c = (float)(1.0 - (double)ice->cos_cherenkov);
+  B.inv_v = (double)ice->n_group / kC;
+  B.inv_c = (float)(1.0 / kC);
+  {
+    uint32_t k0 = (uint32_t)cfg->seed, k1 = (uint32_t)(cfg->seed >> 32);
+    for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  }
+  B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
+  B.tile_photons = kTilePhotons;
+  const uint32_t ns = (uint32_t)h->hg.strings.size();
+  B.n_strings = ns; B.n_dom = geo->n_dom;
+  B.nx = h->hg.nx; B.nx_m1 = h->hg.nx - 1u; B.ny_m1 = h->hg.ny - 1u;
+  B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
+  B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
+  B.rm2 = B.radius_margin * B.radius_margin;
+  B.xy_cap2 = h->hg.xy_cap * h->hg.xy_cap; B.inv_xy_cap = 1.0f / h->hg.xy_cap;
+  // ---- a4: tables of the direct layer walk (pp_types.h) ----
+  std::vector<uint16_t> inv_tab[2];
+  {
+    std::vector<double> cum[2] = {std::vector<double>(nl + 1, 0.0), std::vector<double>(nl + 1, 0.0)};  // B, A
+    for (uint32_t i = 0; i < nl; ++i) {
+      cum[0][i + 1] = cum[0][i] + (double)ice->dz / ((double)ice->scat_len[i] * scat_scale);
+      cum[1][i + 1] = cum[1][i] + (double)ice->dz / (double)ice->abs_len[i];
+    }
+    for (uint32_t i = 0; i <= nl; ++i) {
+      const float bh = (float)cum[0][i], ah = (float)cum[1][i];
+      layers[i].Bh = bh; layers[i].Ah = ah;
+      layers[i].Bl = (float)(cum[0][i] - (double)bh); layers[i].Al = (float)(cum[1][i] - (double)ah);
+    }
+    layers[nl].Bh = layers[nl].Ah = INFINITY; layers[nl].Bl = layers[nl].Al = 0.0f;
+    B.walk_loop = 0;
+    for (int t = 0; t < 2; ++t) {
+      // bin width: just under the thinnest layer, so that a bin holds at most one boundary; coarser (and the
+      // kernel then loops) if that would need more than kMaxWalkInv bins
+      double thin = 1e300;
+      for (uint32_t i = 0; i < nl; ++i) thin = std::min(thin, cum[t][i + 1] - cum[t][i]);
+      const double top = nl > 1 ? cum[t][nl - 1] : 0.0;  // cumulative depth at the upper edge of the last layer
+      double step = 0.99 * thin;
+      if (top / step + 3.0 > (double)kMaxWalkInv) { step = top / ((double)kMaxWalkInv - 3.0); B.walk_loop = 1; }
+      const uint32_t m = (uint32_t)std::ceil(top / step) + 1;  // bins 0..m
+      inv_tab[t].resize(m + 1);
+      uint32_t j = 0;
+      for (uint32_t b = 0; b <= m; ++b) {
+        // a lower bound of the layer for every depth that can land in bin b (index rounding slack 4e-3 bins)
+        const double x = ((double)b - 4e-3) * step;
+        while (j + 1 < nl && (double)(t == 0 ? layers[j + 1].Bh : layers[j + 1].Ah) <= x) ++j;
+        inv_tab[t][b] = (uint16_t)j;
+      }
+      (t == 0 ? B.m_b : B.m_a) = m;
+      (t == 0 ? B.k_b : B.k_a) = (float)(1.0 / step);
+    }
+  }
+  // ---- the image ----
+  std::vector<float2> str_xy(ns + 1);
+  std::vector<float4> str_a(ns);
+  std::vector<uint2> str_b(ns);
+  for (uint32_t i = 0; i < ns; ++i) {
+    const StringRec& r = h->hg.strings[i];
+    str_xy[i] = make_float2(r.x, r.y);
+    str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
+    str_b[i] = make_uint2(r.n, r.base);
+  }
+  str_xy[ns] = make_float2(NAN, NAN);  // what an empty cell names: fails the pre-filter
+  std::vector<uint16_t> cell(h->hg.cell_sid);
+  for (auto& c : cell) if (c == kNoString) c = (uint16_t)ns;
+  std::vector<unsigned char>& img = h->image;
+  img.clear();
+  auto put = [&](const void* src, size_t bytes) {
+    const size_t off = (img.size() + 15) & ~(size_t)15;
+    img.resize(off + bytes, 0);
+    if (bytes) std::memcpy(img.data() + off, src, bytes);
+    return (uint32_t)off;
+  };
+  put(layers.data(), layers.size() * sizeof(LayerRec));
+  B.off_inv_b = put(inv_tab[0].data(), inv_tab[0].size() * sizeof(uint16_t));
+  B.off_inv_a = put(inv_tab[1].data(), inv_tab[1].size() * sizeof(uint16_t));
+  B.off_str_xy = put(str_xy.data(), str_xy.size() * sizeof(float2));
+  B.off_cell = put(cell.data(), cell.size() * sizeof(uint16_t));
+  B.off_str_a = put(str_a.data(), str_a.size() * sizeof(float4));
+  B.off_str_b = put(str_b.data(), str_b.size() * sizeof(uint2));
+  img.resize((img.size() + 15) & ~(size_t)15, 0);
+  h->image_bytes = img.size();
+  B.smem_image_bytes = (uint32_t)img.size();
+  B.off_wsrc = (uint32_t)img.size();
+  h->smem = img.size() + (size_t)propagate_warps_per_block() * sizeof(SrcRec);
+  return PP_OK;
+}
+
 void fill_sizes(const pp_config& cfg, int n_sm, Sizes* s) {
   s->target = cfg.launch_photons_target ? cfg.launch_photons_target : 100000000ull;
   const uint64_t src_bytes = cfg.source_ring_bytes ? cfg.source_ring_bytes : (64ull << 20);
@@ -322,14 +431,8 @@ void fill_sizes(const pp_config& cfg, int n_sm, Sizes* s) {
 uint64_t carve_device(pp_handle* h, void* base) {
   Carver c(base);
   const HostGeometry& g = h->hg;
-  auto* d_ice = c.take<IceLayer>(h->ice.n_layers);
-  h->base.walk = c.take<float4>(h->ice.n_layers + 1);
-  h->base.inv_b = c.take<uint16_t>(kMaxWalkInv);
-  h->base.inv_a = c.take<uint16_t>(kMaxWalkInv);
-  auto* d_strings = c.take<StringRec>(std::max<size_t>(1, g.strings.size()));
-  auto* d_dom = c.take<float4>(g.dom_xyzw.size());
-  auto* d_cell = c.take<uint16_t>(g.cell_sid.size());
-  h->base.ice = d_ice; h->base.strings = d_strings; h->base.dom_xyzw = d_dom; h->base.cell_sid = d_cell;
+  h->base.smem_image = c.take<uint4>(h->image_bytes / 16);
+  h->base.dom_xyzw = c.take<float4>(g.dom_xyzw.size());
   for (int i = 0; i < 2; ++i) {
     Slot& s = h->slot[i];
     s.d_src = c.take<SrcRec>(h->sz.cap_src);
@@ -743,6 +846,8 @@ int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config
   build_geometry(geo, tmp.brute, &tmp.hg);
   if (!tmp.brute && !tmp.hg.fast_ok) return PP_E_UNSUPPORTED;
   fill_sizes(*cfg, n_sm, &tmp.sz);
+  rc = build_tables(&tmp, geo, ice, cfg);
+  if (rc != PP_OK) return rc;
   if (device_bytes) *device_bytes = carve_device(&tmp, nullptr);
   if (pinned_bytes) *pinned_bytes = carve_pinned(&tmp, nullptr);
   return PP_OK;
@@ -770,6 +875,8 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   build_geometry(geo, h->brute, &h->hg);
   if (!h->brute && !h->hg.fast_ok) return bail(PP_E_UNSUPPORTED);
   fill_sizes(*cfg, h->n_sm, &h->sz);
+  rc = build_tables(h, geo, ice, cfg);
+  if (rc != PP_OK) return bail(rc);
   h->hitq_budget = 1ull << 30;
 
   // ---- workspaces ----
@@ -804,84 +911,16 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   }
   if (cudaEventCreate(&h->ev_base) != cudaSuccess || cudaEventCreate(&h->ev_job) != cudaSuccess) return bail(PP_E_CUDA);
 
-  // ---- medium and geometry constants ----
+  // ---- tables and constants to the device ----
   LaunchParams& B = h->base;
-  const double scat_scale = (cfg->flags & PP_FLAG_EFFECTIVE_SCATTERING) ? 1.0 - (double)ice->g : 1.0;
-  if (!(scat_scale > 0.0)) return bail(PP_E_INVAL);
-  std::vector<IceLayer> layers(ice->n_layers);
-  for (uint32_t i = 0; i < ice->n_layers; ++i) {
-    // R-20: an effective scattering length is turned into the geometric mean free path here, once
-    const double ls = (double)ice->scat_len[i] * scat_scale;
-    layers[i].la = ice->abs_len[i]; layers[i].lb = (float)ls;
-    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / ls);
-  }
-  B.n_layers = ice->n_layers; B.z_top = ice->z_top; B.dz_layer = ice->dz; B.inv_dz_layer = (float)(1.0 / (double)ice->dz);
-  const double g = ice->g;
-  B.hg_one_minus_g = (float)(1.0 - g); B.hg_two_g = (float)(2.0 * g); B.hg_one_minus_g2 = (float)(1.0 - g * g);
-  B.one_minus_cos_c = (float)(1.0 - (double)ice->cos_cherenkov);
-  B.inv_v = (double)ice->n_group / kC;
-  B.inv_c = (float)(1.0 / kC);
-  {
-    uint32_t k0 = (uint32_t)cfg->seed, k1 = (uint32_t)(cfg->seed >> 32);
-    for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
-  }
-  B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
-  B.tile_photons = kTilePhotons;
-  B.n_strings = (uint32_t)h->hg.strings.size(); B.n_dom = geo->n_dom;
-  B.nx = h->hg.nx; B.ny = h->hg.ny; B.cell_ox = h->hg.cell_ox; B.cell_oy = h->hg.cell_oy; B.inv_cell = h->hg.inv_cell;
-  B.radius = geo->radius; B.radius_margin = geo->radius + 5e-3f;
-  B.xy_cap2 = h->hg.xy_cap * h->hg.xy_cap; B.inv_xy_cap = 1.0f / h->hg.xy_cap;
-  // ---- a4: tables of the direct layer walk (pp_types.h) ----
-  const uint32_t nl = ice->n_layers;
-  std::vector<float4> walk(nl + 1);
-  std::vector<uint16_t> inv_tab[2];
-  {
-    std::vector<double> cum[2] = {std::vector<double>(nl + 1, 0.0), std::vector<double>(nl + 1, 0.0)};  // B, A
-    for (uint32_t i = 0; i < nl; ++i) {
-      cum[0][i + 1] = cum[0][i] + (double)ice->dz / ((double)ice->scat_len[i] * scat_scale);
-      cum[1][i + 1] = cum[1][i] + (double)ice->dz / (double)ice->abs_len[i];
-    }
-    for (uint32_t i = 0; i <= nl; ++i) {
-      const float bh = (float)cum[0][i], ah = (float)cum[1][i];
-      walk[i] = make_float4(bh, ah, (float)(cum[0][i] - (double)bh), (float)(cum[1][i] - (double)ah));
-    }
-    walk[nl].x = walk[nl].y = INFINITY; walk[nl].z = walk[nl].w = 0.0f;
-    B.walk_loop = 0;
-    for (int t = 0; t < 2; ++t) {
-      // bin width: just under the thinnest layer, so that a bin holds at most one boundary; coarser (and the
-      // kernel then loops) if that would need more than kMaxWalkInv bins
-      double thin = 1e300;
-      for (uint32_t i = 0; i < nl; ++i) thin = std::min(thin, cum[t][i + 1] - cum[t][i]);
-      const double top = nl > 1 ? cum[t][nl - 1] : 0.0;  // cumulative depth at the upper edge of the last layer
-      double step = 0.99 * thin;
-      if (top / step + 3.0 > (double)kMaxWalkInv) { step = top / ((double)kMaxWalkInv - 3.0); B.walk_loop = 1; }
-      const uint32_t m = (uint32_t)std::ceil(top / step) + 1;  // bins 0..m
-      inv_tab[t].resize(m + 1);
-      uint32_t j = 0;
-      for (uint32_t b = 0; b <= m; ++b) {
-        // a lower bound of the layer for every depth that can land in bin b (index rounding slack 4e-3 bins)
-        const double x = ((double)b - 4e-3) * step;
-        while (j + 1 < nl && (double)walk[j + 1].x * (t == 0) + (double)walk[j + 1].y * (t == 1) <= x) ++j;
-        inv_tab[t][b] = (uint16_t)j;
-      }
-      (t == 0 ? B.m_b : B.m_a) = m;
-      (t == 0 ? B.k_b : B.k_a) = (float)(1.0 / step);
-    }
-  }
   auto up = [&](const void* dst, const void* src, size_t bytes) {
     return bytes == 0 || cudaMemcpy(const_cast<void*>(dst), src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
-  if (!up(B.ice, layers.data(), layers.size() * sizeof(IceLayer)) ||
-      !up(B.walk, walk.data(), walk.size() * sizeof(float4)) ||
-      !up(B.inv_b, inv_tab[0].data(), inv_tab[0].size() * sizeof(uint16_t)) ||
-      !up(B.inv_a, inv_tab[1].data(), inv_tab[1].size() * sizeof(uint16_t)) ||
-      !up(B.strings, h->hg.strings.data(), h->hg.strings.size() * sizeof(StringRec)) ||
-      !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)) ||
-      !up(B.cell_sid, h->hg.cell_sid.data(), h->hg.cell_sid.size() * sizeof(uint16_t)))
+  if (!up(B.smem_image, h->image.data(), h->image.size()) ||
+      !up(B.dom_xyzw, h->hg.dom_xyzw.data(), h->hg.dom_xyzw.size() * sizeof(float4)))
     return bail(PP_E_CUDA);
 
   // ---- persistent grid: every SM filled to the kernel's occupancy ----
-  h->smem = propagate_smem_layout(&B);
   {
     // make the opt-in dynamic shared memory size known before asking for the occupancy
     int bps = 0;

@@ -78,6 +78,14 @@ __device__ __forceinline__ float neg_log_uniform(float u) {
   return fmaf(e, -8.262958317573066e-08f, r);  // -ln2 / 2^23
 }
 
+// -ln(u) for the absorption budget (once per photon): one MUFU.LG2; absolute error <= 2^-21.4, which moves the
+// absorption point by <= 4e-7 lambda_abs.  u is a normal number (R-3): no denormal handling.
+__device__ __forceinline__ float neg_log_fast(float u) {
+  float l;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(u));
+  return l * -0.693147182464599609375f;
+}
+
 // (sin, cos) of 2 pi u for u in (0, 1): j = rint(4u) picks the quadrant, f = 4u - j in [-1/2, 1/2] is exact,
 // sin and cos of f pi/2 from degree-7/8 minimax fits (errors 2.4e-8 / 1e-8, fitted for this file), then the
 // quadrant swap and signs from the two low bits of j.

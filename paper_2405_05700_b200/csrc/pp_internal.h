@@ -18,7 +18,7 @@ cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint
 cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_cum, cudaStream_t st);
 cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
                          uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st);
-size_t propagate_smem_layout(LaunchParams* P);  // fills the off_* fields, returns the dynamic shared memory size
+int propagate_warps_per_block();
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st);
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm);
 

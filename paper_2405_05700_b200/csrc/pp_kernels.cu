@@ -16,6 +16,7 @@ static_assert(sizeof(SrcRec) == 48, "SrcRec layout");
 static_assert(sizeof(pp_hit) == 32, "pp_hit layout");
 static_assert(sizeof(pp_fate) == 40, "pp_fate layout");
 static_assert(sizeof(WorkItem) == 24, "WorkItem layout");
+static_assert(sizeof(LayerRec) == 32, "LayerRec layout");
 
 // =============================================================================================
 // a2  Source expansion
@@ -101,9 +102,9 @@ __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_
 #define PP_BLOCK_THREADS 256
 #endif
 constexpr int kBlockThreads = PP_BLOCK_THREADS;
+constexpr int kMaxDevices = 64;
 
-// Shared-memory tables, staged once per launch (offsets in LaunchParams::off_*):
-// [IceLayer x n_layers][float4 walk x (n_layers + 1)][float4 x n_str][uint2 x n_str][u16 inv_b][u16 inv_a][u16 x cells]
+// Shared-memory tables: one image built by the host (LaunchParams::smem_image), copied verbatim by every CTA.
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -202,48 +203,82 @@ __device__ __forceinline__ float segment_fraction(const LaunchParams& P, float u
   return fmaf(x - (float)i, f1 - f0, f0);
 }
 
-// kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18) is compiled in
+// Fetch the next work item of the launch for a warp (lane 0 talks to the queues; rare: once per tile).
+// Returns the warp-uniform (t_next, t_end, s_cur, resume list not yet empty); t_next == t_end means no work is left.
+__device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, bool use_resume) {
+  Status* const st = P.status;
+  unsigned long long a = 0, b = 0;
+  uint32_t sh = 0, res_left = use_resume ? 1u : 0u;
+  if (lane == 0 && *(volatile unsigned int*)&st->stop == 0u) {
+    if (use_resume) {
+      const unsigned r = atomicAdd(&st->resume_counter, 1u);
+      if (r < P.n_resume_in) {
+        const WorkItem w = P.resume_in[r];
+        a = w.g0; b = w.g1; sh = w.src;
+      } else {
+        res_left = 0u;
+      }
+    }
+    if (a == b) {
+      const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
+      if (j < P.n_tiles) {
+        a = P.g_begin + j * P.tile_photons;
+        b = min(a + (unsigned long long)P.tile_photons, P.g_end);
+        sh = __ldg(&P.tile_src[j]);
+        if (*(volatile unsigned int*)&st->stop != 0u) {
+          // the ring filled up while we were fetching: hand the whole tile to the next launch
+          const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+          if (o < P.resume_cap) P.resume_out[o] = WorkItem{a, b, sh, 0u}; else atomicExch(&st->error, 1u);
+          a = b = 0;
+        }
+      }
+    }
+  }
+  uint4 r;
+  r.x = __shfl_sync(0xffffffffu, (uint32_t)(a - P.g_begin), 0);
+  r.y = __shfl_sync(0xffffffffu, (uint32_t)(b - P.g_begin), 0);
+  r.z = __shfl_sync(0xffffffffu, sh, 0);
+  r.w = __shfl_sync(0xffffffffu, res_left, 0);
+  return r;
+}
+
+// kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18, wavelength bins R-21, emission
+// smearing R-22) is compiled in
 template <bool kBrute, bool kFates, bool kExt>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // table offsets come from the constant bank (LaunchParams), not from registers
-  IceLayer* const s_ice = reinterpret_cast<IceLayer*>(smem_raw);
-  float4* const s_walk = reinterpret_cast<float4*>(smem_raw + P.off_walk);
-  float4* const s_str_a = reinterpret_cast<float4*>(smem_raw + P.off_str_a);
-  uint2* const s_str_b = reinterpret_cast<uint2*>(smem_raw + P.off_str_b);
-  uint16_t* const s_inv_b = reinterpret_cast<uint16_t*>(smem_raw + P.off_inv_b);
-  uint16_t* const s_inv_a = reinterpret_cast<uint16_t*>(smem_raw + P.off_inv_a);
-  uint16_t* const s_cell = reinterpret_cast<uint16_t*>(smem_raw + P.off_cell);
-
-  // ---- stage the medium and the DOM lookup in shared memory (a4, a5) ----
-  for (uint32_t i = threadIdx.x; i < P.n_layers; i += blockDim.x) s_ice[i] = P.ice[i];
-  for (uint32_t i = threadIdx.x; i <= P.n_layers; i += blockDim.x) s_walk[i] = P.walk[i];
-  for (uint32_t i = threadIdx.x; i <= P.m_b; i += blockDim.x) s_inv_b[i] = P.inv_b[i];
-  for (uint32_t i = threadIdx.x; i <= P.m_a; i += blockDim.x) s_inv_a[i] = P.inv_a[i];
-  if (!kBrute) {
-    for (uint32_t i = threadIdx.x; i < P.n_strings; i += blockDim.x) {
-      const StringRec r = P.strings[i];
-      s_str_a[i] = make_float4(r.x, r.y, r.z0, r.inv_pitch);
-      s_str_b[i] = make_uint2(r.n, r.base);
-    }
-    const uint32_t n_cell = P.nx * P.ny;
-    for (uint32_t i = threadIdx.x; i < n_cell; i += blockDim.x) s_cell[i] = P.cell_sid[i];
+  // ---- stage the medium and the DOM lookup in shared memory (a4, a5): one verbatim copy of the host-built image ----
+  {
+    uint4* const dst = reinterpret_cast<uint4*>(smem_raw);
+    const uint32_t n16 = P.smem_image_bytes >> 4;
+    for (uint32_t i = threadIdx.x; i < n16; i += blockDim.x) dst[i] = __ldg(P.smem_image + i);
   }
   __syncthreads();
-  const float4* const lay = reinterpret_cast<const float4*>(s_ice);  // (a, b, 1/a, 1/b) per layer
+  // layer records at offset 0: coefficients (a, b, 1/a, 1/b) of layer i, cumulative depths at boundary i
+  auto lay = [&](int i) { return *reinterpret_cast<const float4*>(smem_raw + (uint32_t)i * 32u); };
+  auto walk = [&](int i) { return *reinterpret_cast<const float4*>(smem_raw + (uint32_t)i * 32u + 16u); };
+  auto walk_B = [&](int i) { return *reinterpret_cast<const float*>(smem_raw + (uint32_t)i * 32u + 16u); };
+  auto walk_A = [&](int i) { return *reinterpret_cast<const float*>(smem_raw + (uint32_t)i * 32u + 20u); };
+  const uint16_t* const s_inv_b = reinterpret_cast<const uint16_t*>(smem_raw + P.off_inv_b);
+  const uint16_t* const s_inv_a = reinterpret_cast<const uint16_t*>(smem_raw + P.off_inv_a);
+  const float2* const s_str_xy = reinterpret_cast<const float2*>(smem_raw + P.off_str_xy);
+  const uint16_t* const s_cell = reinterpret_cast<const uint16_t*>(smem_raw + P.off_cell);
+  // the warp's current source record (a2): staged once per (tile, source) run, read by the lanes that refill
+  float4* const my_src = reinterpret_cast<float4*>(smem_raw + P.off_wsrc) + 3u * (threadIdx.x >> 5);
 
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
   Status* const st = P.status;
   const float inf = __int_as_float(0x7f800000);
 
-  // ---- warp-uniform work state: photons [t_next, t_end) of the launch (numbered from g_begin) ----
-  uint32_t t_next = 0, t_end = 0, s_cur = 0;
+  // ---- warp-uniform work state: photons [t_next, t_end) of the launch (numbered from g_begin) are this warp's
+  // current work item; [t_next, run_end) of them belong to source s_cur, whose photon 0 is launch photon pbase ----
+  uint32_t t_next = 0, t_end = 0, run_end = 0, s_cur = 0, pbase = 0;
   bool refill_ok = true;   // false once the queues are empty or the hit ring filled up
   bool use_resume = P.n_resume_in > 0;
   uint32_t w_started = 0, w_hits = 0, w_flights = 0;
 
-  // ---- per-lane photon state ----
+  // ---- per-lane photon state (a dead lane keeps computing on its stale state; nothing it produces is used) ----
   bool alive = false;
   float phx = 0, phy = 0, phz = 0, plx = 0, ply = 0, plz = 0;  // position, two-float (hi + lo)
   float dx = 0, dy = 0, dz = 1;
@@ -256,62 +291,42 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     // =========================== refill dead lanes (a2 -> a3) ===========================
     const unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
     if (need_mask != 0u && refill_ok) {
-      if (t_next == t_end) {
-        // fetch the next work item: resume list first, then fresh tiles
-        unsigned long long a = 0, b = 0;
-        uint32_t sh = 0, res_left = use_resume ? 1u : 0u;
-        if (lane == 0 && *(volatile unsigned int*)&st->stop == 0u) {
-          if (use_resume) {
-            const unsigned r = atomicAdd(&st->resume_counter, 1u);
-            if (r < P.n_resume_in) {
-              const WorkItem w = P.resume_in[r];
-              a = w.g0; b = w.g1; sh = w.src;
-            } else {
-              res_left = 0u;
-            }
-          }
-          if (a == b) {
-            const unsigned long long j = atomicAdd(&st->tile_counter, 1ull);
-            if (j < P.n_tiles) {
-              a = P.g_begin + j * P.tile_photons;
-              b = min(a + (unsigned long long)P.tile_photons, P.g_end);
-              sh = __ldg(&P.tile_src[j]);
-              if (*(volatile unsigned int*)&st->stop != 0u) {
-                // the ring filled up while we were fetching: hand the whole tile to the next launch
-                const unsigned o = atomicAdd(&st->n_resume_out, 1u);
-                if (o < P.resume_cap) P.resume_out[o] = WorkItem{a, b, sh, 0u}; else atomicExch(&st->error, 1u);
-                a = b = 0;
-              }
-            }
-          }
+      if (t_next == run_end) {
+        // a new run: the next source of the current work item, or a new work item (resume list first, then tiles)
+        if (t_next == t_end) {
+          const uint4 wk = fetch_work(P, lane, use_resume);
+          t_next = wk.x; t_end = wk.y; s_cur = wk.z; use_resume = wk.w != 0u;
+        } else {
+          ++s_cur;
         }
-        t_next = __shfl_sync(0xffffffffu, (uint32_t)(a - P.g_begin), 0);
-        t_end = __shfl_sync(0xffffffffu, (uint32_t)(b - P.g_begin), 0);
-        s_cur = __shfl_sync(0xffffffffu, sh, 0);
-        use_resume = __shfl_sync(0xffffffffu, res_left, 0) != 0u;
-        if (t_next == t_end) refill_ok = false;
+        if (t_next != t_end) {
+          uint32_t hi;
+          while ((hi = __ldg(&P.cum_rel[s_cur + 1])) <= t_next) ++s_cur;  // skips sources without photons
+          pbase = __ldg(&P.cum_rel[s_cur]);  // mod 2^32: right for the launch's first (split) source too
+          run_end = min(t_end, hi);
+          __syncwarp();
+          if (lane < 3u) my_src[lane] = __ldg(reinterpret_cast<const float4*>(P.src + s_cur) + lane);
+          __syncwarp();
+        } else {
+          run_end = t_end;
+          refill_ok = false;
+        }
       }
-      if (t_next != t_end) {
+      if (t_next != run_end) {
         // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
         const uint32_t r = t_next + __popc(need_mask & lt);
-        uint32_t s_new = s_cur;
-        if (!alive && r < t_end) {
-          uint32_t s = s_cur;
-          while (r >= __ldg(&P.cum_rel[s + 1])) ++s;
-          s_new = s;
-          const float4* rp = reinterpret_cast<const float4*>(P.src + s);
-          const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
-          const uint2 r2 = __ldg(reinterpret_cast<const uint2*>(rp + 2));
+        if (!alive && r < run_end) {
+          const float4 r0 = my_src[0], r1 = my_src[1];
+          const uint2 r2 = *reinterpret_cast<const uint2*>(my_src + 2);
           phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
           dx = r0.w; dy = r1.x; dz = r1.y;
           Lh = 0.0f; Ll = 0.0f;
           ev = r2.x; sid = r2.y;
-          pidx = r - __ldg(&P.cum_rel[s]);  // mod 2^32: right for the launch's first (split) source too
-          k = 0; s_mine = s;
+          pidx = r - pbase;
+          k = 0; s_mine = s_cur;
           alive = true;
         }
-        s_cur = __reduce_max_sync(0xffffffffu, s_new);
-        const uint32_t take = min((uint32_t)__popc(need_mask), t_end - t_next);
+        const uint32_t take = min((uint32_t)__popc(need_mask), run_end - t_next);
         t_next += take;
         w_started += take;
       }
@@ -319,220 +334,220 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
     if (alive_mask == 0u) {
       if (!refill_ok) break;
-      continue;  // the tile ran out exactly here: fetch the next one
+      continue;  // the run ended exactly here: start the next one
     }
     w_flights += __popc(alive_mask);  // every live lane flies once per iteration
 
-    bool hit = false, done = false, aborted = false;
-    uint32_t hit_dom = 0xFFFFFFFFu;
-    if (alive) {
-      // =========================== a7': Philox block k of this photon ===========================
-      uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
-      philox4x32_10(c0, c1, c2, c3, P.rk);
-      const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
-      const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
-      // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
-      const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
-      const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
-      if (kExt && P.has_segments != 0u && k == 0) {
-        // R-18: a source with a length emits from a point uniform along it; u_hg is free on flight 0
-        const float ell = segment_fraction(P, u_hg) * __ldg(&P.src[s_mine].length);
-        const float nx_ = fmaf(dx, ell, phx); plx += fmaf(dx, ell, phx - nx_); phx = nx_;
-        const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
-        const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
-      }
-      if (kExt && P.emit_on != 0u && k == 0) {
-        // R-22: the axis the photon is emitted about = the source axis deflected by an HG(g_axis) polar angle
-        uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0x20000000u;
-        philox4x32_10(e0, e1, e2, e3, P.rk);
-        rotate(dx, dy, dz, hg_one_minus_cos(uniform_from_word(e0), P.emit_one_minus_g, P.emit_two_g, P.emit_one_minus_g2),
-               uniform_from_word(e1));
-      }
-      rotate(dx, dy, dz, m, u_az);
-      // =========================== a3: absorption budget (once per photon) ======================
-      float tau_new = -__logf(u_abs);
-      if (kExt && P.spec_n != 0u && k == 0) {
-        // R-21: the photon's wavelength bin from the spare bits of block 0.  Both optical-depth budgets are kept in
-        // units of the unscaled ice table: tau_a is divided by abs_scale once, sc_b = 1 / scat_scale multiplies
-        // every tau_s.
-        const uint32_t j = spectrum_bin_from_words(P, c0, c1, c2);
-        tau_new *= P.spec_inv_a[j];
-        sc_b = P.spec_inv_b[j];
-      }
-      tau_a = (k == 0) ? tau_new : tau_a;
-      // =========================== a4: optical depth to the next scatter ========================
-      float tau_s = neg_log_uniform(u_dist);
-      if (kExt && P.spec_n != 0u) tau_s *= sc_b;
-      // =========================== a4: layer walk in vertical optical depth ======================
-      // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
-      // so the budgets are scaled by w = |d_z| once and the walk works in vertical metres.
-      const float w = fmaxf(fabsf(dz), 1e-9f);
-      const float inv_w = fast_rcp(w);
-      const bool up = dz > 0.0f;
-      const int last = (int)P.n_layers - 1;
-      int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
-      li = max(0, min(li, last));
-      const float zb = P.z_top - P.dz_layer * (float)(li + (up ? 0 : 1));
-      const bool open = up ? (li == 0) : (li == last);  // no boundary ahead: the end layers are infinite (R-6)
-      const float h0 = open ? inf : fabsf(zb - phz);    // vertical distance to the first boundary
-      float Ts = tau_s * w, Ta = tau_a * w, Vb = 0.0f;
-      float4 L4 = lay[li];
-      {
-        const float t1 = fmaf(-L4.y, h0, Ts), t2 = fmaf(-L4.x, h0, Ta);
-        if (fminf(t1, t2) > 0.0f) {
-          // The flight leaves layer li through boundary i1 with budgets t1, t2 left.  Direct walk: the cumulative
-          // depths X at which the budgets run out name the layers js, ja (inverse table + one step); the nearer
-          // one is where the flight ends, and the budgets left at its entry boundary jb come from the two-float
-          // cumulative sums, so their error is relative to the budget, not to the cumulative depth.
-          const int i1 = li + (up ? 0 : 1);
-          const float4 W1 = s_walk[i1];
-          const float Xs = up ? W1.x - t1 : W1.x + t1, Xa = up ? W1.y - t2 : W1.y + t2;
-          int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
-          int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
-          js += (s_walk[js + 1].x <= Xs) ? 1 : 0;
-          ja += (s_walk[ja + 1].y <= Xa) ? 1 : 0;
-          if (P.walk_loop) {
-            while (s_walk[js + 1].x <= Xs) ++js;
-            while (s_walk[ja + 1].y <= Xa) ++ja;
-          }
-          const int lj = up ? min(max(js, ja), li - 1) : max(min(js, ja), li + 1);
-          const int jb = lj + (up ? 1 : 0);
-          const float4 Wb = s_walk[jb];
-          Ts = t1 - fabsf((Wb.x - W1.x) + (Wb.z - W1.z));
-          Ta = t2 - fabsf((Wb.y - W1.y) + (Wb.w - W1.w));
-          Vb = fmaf(P.dz_layer, (float)abs(jb - i1), h0);
-          L4 = lay[lj];
+    // =========================== a7': Philox block k of this photon ===========================
+    uint32_t c0 = pidx, c1 = sid, c2 = ev, c3 = k;
+    philox4x32_10(c0, c1, c2, c3, P.rk);
+    const float u_az = uniform_from_word(c0), u_hg = uniform_from_word(c1);
+    const float u_dist = uniform_from_word(c2), u_abs = uniform_from_word(c3);
+    // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
+    const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
+    const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
+    if (kExt && P.has_segments != 0u && k == 0) {
+      // R-18: a source with a length emits from a point uniform along it; u_hg is free on flight 0
+      const float ell = segment_fraction(P, u_hg) * __ldg(&P.src[s_mine].length);
+      const float nx_ = fmaf(dx, ell, phx); plx += fmaf(dx, ell, phx - nx_); phx = nx_;
+      const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
+      const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
+    }
+    if (kExt && P.emit_on != 0u && k == 0) {
+      // R-22: the axis the photon is emitted about = the source axis deflected by an HG(g_axis) polar angle
+      uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0x20000000u;
+      philox4x32_10(e0, e1, e2, e3, P.rk);
+      rotate(dx, dy, dz, hg_one_minus_cos(uniform_from_word(e0), P.emit_one_minus_g, P.emit_two_g, P.emit_one_minus_g2),
+             uniform_from_word(e1));
+    }
+    rotate(dx, dy, dz, m, u_az);
+    // =========================== a3: absorption budget (once per photon) ======================
+    float tau_new = neg_log_fast(u_abs);
+    if (kExt && P.spec_n != 0u && k == 0) {
+      // R-21: the photon's wavelength bin from the spare bits of block 0.  Both optical-depth budgets are kept in
+      // units of the unscaled ice table: tau_a is divided by abs_scale once, sc_b = 1 / scat_scale multiplies
+      // every tau_s.
+      const uint32_t j = spectrum_bin_from_words(P, c0, c1, c2);
+      tau_new *= P.spec_inv_a[j];
+      sc_b = P.spec_inv_b[j];
+    }
+    tau_a = (k == 0) ? tau_new : tau_a;
+    // =========================== a4: optical depth to the next scatter ========================
+    float tau_s = neg_log_uniform(u_dist);
+    if (kExt && P.spec_n != 0u) tau_s *= sc_b;
+    // =========================== a4: layer walk in vertical optical depth ======================
+    // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
+    // so the budgets are scaled by w = |d_z| once and the walk works in vertical metres.
+    const float w = fmaxf(fabsf(dz), 1e-9f);
+    const float inv_w = fast_rcp(w);
+    const bool up = dz > 0.0f;
+    const int last = P.last_layer;
+    int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
+    li = max(0, min(li, last));
+    const int i1 = li + (up ? 0 : 1);                   // boundary ahead
+    const float zb = fmaf(-P.dz_layer, (float)i1, P.z_top);
+    const bool open = up ? (li == 0) : (li == last);  // no boundary ahead: the end layers are infinite (R-6)
+    const float h0 = open ? inf : fabsf(zb - phz);    // vertical distance to the first boundary
+    float Ts = tau_s * w, Ta = tau_a * w, Vb = 0.0f;
+    float4 L4 = lay(li);
+    {
+      const float t1 = fmaf(-L4.y, h0, Ts), t2 = fmaf(-L4.x, h0, Ta);
+      if (fminf(t1, t2) > 0.0f) {
+        // The flight leaves layer li through boundary i1 with budgets t1, t2 left.  Direct walk: the cumulative
+        // depths X at which the budgets run out name the layers js, ja (inverse table + one step); the nearer
+        // one is where the flight ends, and the budgets left at its entry boundary jb come from the two-float
+        // cumulative sums, so their error is relative to the budget, not to the cumulative depth.
+        const float4 W1 = walk(i1);
+        const float sgn = up ? -1.0f : 1.0f;
+        const float Xs = fmaf(sgn, t1, W1.x), Xa = fmaf(sgn, t2, W1.y);
+        int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
+        int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
+        js += (walk_B(js + 1) <= Xs) ? 1 : 0;
+        ja += (walk_A(ja + 1) <= Xa) ? 1 : 0;
+        if (P.walk_loop) {
+          while (js < last && walk_B(js + 1) <= Xs) ++js;
+          while (ja < last && walk_A(ja + 1) <= Xa) ++ja;
         }
+        const int lj = up ? min(max(js, ja), li - 1) : max(min(js, ja), li + 1);
+        const int jb = lj + (up ? 1 : 0);
+        const float4 Wb = walk(jb);
+        Ts = t1 - fabsf((Wb.x - W1.x) + (Wb.z - W1.z));
+        Ta = t2 - fabsf((Wb.y - W1.y) + (Wb.w - W1.w));
+        Vb = fmaf(P.dz_layer, (float)abs(jb - i1), h0);
+        L4 = lay(lj);
       }
-      const float vs = Ts * L4.w, va = Ta * L4.z;  // vertical distance left in the final layer
-      const bool absorbed = va <= vs;
-      const float v_in = fminf(vs, va);
-      const float s = (Vb + v_in) * inv_w;
-      tau_a = fmaxf(0.0f, fmaf(-L4.x, v_in, Ta)) * inv_w;
-      // =========================== a5: DOM intersection on [0, s] ===============================
-      Best best{inf, 0xFFFFFFFFu};
-      if (kBrute) {
-        best = test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
-      } else {
-        // the one line of DOMs a piece of flight no longer than xy_cap in the xy-plane can meet is named by the
-        // cell of the piece's xy midpoint; a longer flight is looked up piece by piece
-        const float rho2 = fmaf(dx, dx, dy * dy);
-        const float sxy2 = s * s * rho2;
-        float ds = s;
-        int n_ch = 1;
-        bool all_lines = false;  // a flight of more than 64 pieces (far longer than the detector is wide)
-        if (sxy2 > P.xy_cap2) {
-          const float f = floorf(fast_sqrt(sxy2) * P.inv_xy_cap) + 1.0f;
-          all_lines = f > 64.0f;
-          n_ch = all_lines ? 1 : (int)f;
-          ds = s * fast_rcp(f);
-        }
-        const float rm2 = fmaf(P.radius_margin * P.radius_margin, rho2, 1e-12f);
-        float tm = 0.5f * ds;
+    }
+    const float vs = Ts * L4.w, va = Ta * L4.z;  // vertical distance left in the final layer
+    const bool absorbed = va <= vs;
+    const float v_in = fminf(vs, va);
+    const float s = (Vb + v_in) * inv_w;
+    tau_a = fmaxf(0.0f, fmaf(-L4.x, v_in, Ta)) * inv_w;
+    // =========================== a5: DOM intersection on [0, s] ===============================
+    Best best{inf, 0xFFFFFFFFu};
+    if (kBrute) {
+      if (alive) best = test_all_doms(P, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+    } else {
+      // the one line of DOMs a piece of flight no longer than xy_cap in the xy-plane can meet is named by the
+      // cell of the piece's xy midpoint; a longer flight is looked up piece by piece
+      const float rho2 = fmaf(dx, dx, dy * dy);
+      const float sxy2 = s * s * rho2;
+      float ds = s;
+      int n_ch = 1;
+      bool all_lines = false;  // a flight of more than 64 pieces (far longer than the detector is wide)
+      if (sxy2 > P.xy_cap2) {
+        const float f = floorf(fast_sqrt(sxy2) * P.inv_xy_cap) + 1.0f;
+        all_lines = f > 64.0f;
+        n_ch = all_lines ? 1 : (int)f;
+        ds = s * fast_rcp(f);
+      }
+      const float rm2 = fmaf(P.rm2, rho2, 1e-12f);
+      float tm = 0.5f * ds;
 #pragma unroll 1
-        for (;;) {
-          // cell of the piece's midpoint; the saturating conversion sends negative coordinates to cell 0
-          const uint32_t cx = min(__float2uint_rz(fmaf(fmaf(tm, dx, phx), P.inv_cell, P.cell_ox)), P.nx - 1u);
-          const uint32_t cy = min(__float2uint_rz(fmaf(fmaf(tm, dy, phy), P.inv_cell, P.cell_oy)), P.ny - 1u);
-          const uint32_t si = s_cell[cy * P.nx + cx];
-          if (si != kNoString) {
-            const float4 sa = s_str_a[si];
-            const float cr = fmaf(sa.x - phx, dy, -(sa.y - phy) * dx);
-            if (cr * cr <= rm2)
-              best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
-          }
-          if (--n_ch <= 0) break;
-          tm += ds;
-        }
-        if (all_lines) {
-          for (uint32_t si = 0; si < P.n_strings; ++si)
-            best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
-        }
+      for (;;) {
+        // cell of the piece's midpoint; the saturating conversion sends negative coordinates to cell 0.  An empty
+        // cell names the NaN entry of the line table, which fails the pre-filter.
+        const uint32_t cx = min(__float2uint_rz(fmaf(fmaf(tm, dx, phx), P.inv_cell, P.cell_ox)), P.nx_m1);
+        const uint32_t cy = min(__float2uint_rz(fmaf(fmaf(tm, dy, phy), P.inv_cell, P.cell_oy)), P.ny_m1);
+        const uint32_t si = s_cell[cy * P.nx + cx];
+        const float2 sxy = s_str_xy[si];
+        const float cr = fmaf(sxy.x - phx, dy, -(sxy.y - phy) * dx);
+        if (cr * cr <= rm2 && alive)
+          best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+        if (--n_ch <= 0) break;
+        tm += ds;
       }
-      hit = best.t <= s;
-      hit_dom = best.dom;
-      // =========================== a6: advance / terminate ======================================
-      const float adv = hit ? best.t : s;
-      {
-        // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
-        // more fma (exact unless |p| << |d*adv| ulp-wise, where it is negligible anyway)
-        const float nx_ = fmaf(dx, adv, phx); plx += fmaf(dx, adv, phx - nx_); phx = nx_;
-        const float ny_ = fmaf(dy, adv, phy); ply += fmaf(dy, adv, phy - ny_); phy = ny_;
-        const float nz_ = fmaf(dz, adv, phz); plz += fmaf(dz, adv, phz - nz_); phz = nz_;
-        const float nl = Lh + adv; Ll += adv - (nl - Lh); Lh = nl;
+      if (all_lines && alive) {
+        for (uint32_t si = 0; si < P.n_strings; ++si)
+          best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
       }
-      k += 1u;  // k counts the free flights started = index of the next Philox block
-      aborted = !hit && !absorbed && k >= P.max_flights;
-      done = hit || absorbed || aborted;
     }
+    bool hit = alive && best.t <= s;
+    const uint32_t hit_dom = best.dom;
+    // =========================== a6: advance / terminate ======================================
+    const float adv = hit ? best.t : s;
+    {
+      // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
+      // more fma (exact unless |p| << |d*adv| ulp-wise, where it is negligible anyway)
+      const float nx_ = fmaf(dx, adv, phx); plx += fmaf(dx, adv, phx - nx_); phx = nx_;
+      const float ny_ = fmaf(dy, adv, phy); ply += fmaf(dy, adv, phy - ny_); phy = ny_;
+      const float nz_ = fmaf(dz, adv, phz); plz += fmaf(dz, adv, phz - nz_); phz = nz_;
+      const float nl = Lh + adv; Ll += adv - (nl - Lh); Lh = nl;
+    }
+    k += 1u;  // k counts the free flights started = index of the next Philox block
+    const bool aborted = alive && !hit && !absorbed && k >= P.max_flights;
+    const bool done = hit || absorbed || aborted;
 
-    // =========================== a8: hit write (warp-aggregated) ================================
+    // =========================== a8: hit write (warp-aggregated); rare =============================
     bool deferred = false, rejected = false;
-    unsigned hit_mask = __ballot_sync(0xffffffffu, hit);
-    float weight = 1.0f;
-    if (kExt && P.acc_mode != 0u && hit_mask) {
-      // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z; rare path ----
-      if (hit) {
-        float pa = 0.0f;
-        for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
-        pa = fminf(fmaxf(pa, 0.0f), 1.0f);
-        if (P.spec_n != 0u) pa = fminf(1.0f, pa * P.spec_acc[spectrum_bin(P, pidx, sid, ev)]);  // R-21
-        if (P.acc_mode == 1u) {
-          uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | (k - 1u);  // k was advanced: the hit flight is k - 1
-          philox4x32_10(a0, a1, a2, a3, P.rk);
-          rejected = !(uniform_from_word(a0) < pa);
-        } else {
-          weight = pa;
-          rejected = !(pa > 0.0f);
-        }
-        hit = !rejected;
-      }
-      const unsigned rej_mask = __ballot_sync(0xffffffffu, rejected);
-      if (rej_mask && (int)lane == __ffs(rej_mask) - 1) atomicAdd(&st->photons_rejected, (unsigned long long)__popc(rej_mask));
-      hit_mask &= ~rej_mask;
-    }
+    unsigned hit_mask = __ballot_sync(0xffffffffu, hit || aborted);
     if (hit_mask) {
-      const unsigned n_hit = __popc(hit_mask);
-      unsigned base = 0;
-      const int leader = __ffs(hit_mask) - 1;
-      if ((int)lane == leader) base = atomicAdd(&st->hit_count, n_hit);
-      base = __shfl_sync(0xffffffffu, base, leader);
-      if (hit) {
-        const unsigned slot = base + __popc(hit_mask & lt);
-        if (slot < P.ring_cap) {
-          double t0 = (double)__ldg(&P.src[s_mine].t);
-          if (kExt && P.has_segments != 0u) {
-            // R-18: emitted l / c after the source time; l is recomputed from block 0 instead of being carried
-            uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0u;
-            philox4x32_10(e0, e1, e2, e3, P.rk);
-            t0 += (double)(segment_fraction(P, uniform_from_word(e1)) * __ldg(&P.src[s_mine].length)) * (double)P.inv_c;
+      if (aborted) atomicAdd(&st->photons_aborted, 1ull);  // never in practice (R-10)
+      hit_mask = __ballot_sync(0xffffffffu, hit);
+      float weight = 1.0f;
+      if (kExt && P.acc_mode != 0u && hit_mask) {
+        // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z ----
+        if (hit) {
+          float pa = 0.0f;
+          for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
+          pa = fminf(fmaxf(pa, 0.0f), 1.0f);
+          if (P.spec_n != 0u) pa = fminf(1.0f, pa * P.spec_acc[spectrum_bin(P, pidx, sid, ev)]);  // R-21
+          if (P.acc_mode == 1u) {
+            uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | (k - 1u);  // k was advanced: the hit flight is k - 1
+            philox4x32_10(a0, a1, a2, a3, P.rk);
+            rejected = !(uniform_from_word(a0) < pa);
+          } else {
+            weight = pa;
+            rejected = !(pa > 0.0f);
           }
-          pp_hit h;
-          h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
-          double inv_v = P.inv_v;
-          if (kExt && P.spec_n != 0u) inv_v = P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)];  // R-21
-          h.time_ns = t0 + ((double)Lh + (double)Ll) * inv_v;
-          h.weight = weight; h.n_scatter = k - 1;
-          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
-          const uint4* srcv = reinterpret_cast<const uint4*>(&h);
-          dst[0] = srcv[0];
-          dst[1] = srcv[1];
-        } else {
-          // ring full: this photon is replayed from scratch by the next launch (counter-based RNG)
-          deferred = true;
-          const unsigned long long g = __ldg(&P.cum[s_mine]) + pidx;
-          const unsigned o = atomicAdd(&st->n_resume_out, 1u);
-          if (o < P.resume_cap) P.resume_out[o] = WorkItem{g, g + 1, s_mine, 0u}; else atomicExch(&st->error, 1u);
-          atomicExch(&st->stop, 1u);
+          hit = !rejected;
         }
+        const unsigned rej_mask = __ballot_sync(0xffffffffu, rejected);
+        if (rej_mask && (int)lane == __ffs(rej_mask) - 1) atomicAdd(&st->photons_rejected, (unsigned long long)__popc(rej_mask));
+        hit_mask &= ~rej_mask;
       }
-      const unsigned def_mask = __ballot_sync(0xffffffffu, deferred);
-      w_hits += n_hit - __popc(def_mask);
-      if (def_mask) {
-        // the replay will count these photons (and their flights) again: take them out here
-        refill_ok = false;
-        w_started -= __popc(def_mask);
-        w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
+      if (hit_mask) {
+        const unsigned n_hit = __popc(hit_mask);
+        unsigned base = 0;
+        const int leader = __ffs(hit_mask) - 1;
+        if ((int)lane == leader) base = atomicAdd(&st->hit_count, n_hit);
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (hit) {
+          const unsigned slot = base + __popc(hit_mask & lt);
+          if (slot < P.ring_cap) {
+            double t0 = (double)__ldg(&P.src[s_mine].t);
+            if (kExt && P.has_segments != 0u) {
+              // R-18: emitted l / c after the source time; l is recomputed from block 0 instead of being carried
+              uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0u;
+              philox4x32_10(e0, e1, e2, e3, P.rk);
+              t0 += (double)(segment_fraction(P, uniform_from_word(e1)) * __ldg(&P.src[s_mine].length)) * (double)P.inv_c;
+            }
+            pp_hit h;
+            h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
+            double inv_v = P.inv_v;
+            if (kExt && P.spec_n != 0u) inv_v = P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)];  // R-21
+            h.time_ns = t0 + ((double)Lh + (double)Ll) * inv_v;
+            h.weight = weight; h.n_scatter = k - 1;
+            uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
+            const uint4* srcv = reinterpret_cast<const uint4*>(&h);
+            dst[0] = srcv[0];
+            dst[1] = srcv[1];
+          } else {
+            // ring full: this photon is replayed from scratch by the next launch (counter-based RNG)
+            deferred = true;
+            const unsigned long long g = __ldg(&P.cum[s_mine]) + pidx;
+            const unsigned o = atomicAdd(&st->n_resume_out, 1u);
+            if (o < P.resume_cap) P.resume_out[o] = WorkItem{g, g + 1, s_mine, 0u}; else atomicExch(&st->error, 1u);
+            atomicExch(&st->stop, 1u);
+          }
+        }
+        const unsigned def_mask = __ballot_sync(0xffffffffu, deferred);
+        w_hits += n_hit - __popc(def_mask);
+        if (def_mask) {
+          // the replay will count these photons (and their flights) again: take them out here
+          refill_ok = false;
+          w_started -= __popc(def_mask);
+          w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
+        }
       }
     }
 
@@ -551,10 +566,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         reinterpret_cast<pp_fate*>(P.fates)[g] = f;
       }
     }
-    if (done) {
-      alive = false;
-      if (aborted) atomicAdd(&st->photons_aborted, 1ull);  // never in practice (R-10)
-    }
+    alive = alive && !done;
   }
 
   // ---- leftovers of a stopped warp go to the next launch; fold the counters ----
@@ -599,26 +611,18 @@ cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsign
   return cudaGetLastError();
 }
 
-size_t propagate_smem_layout(LaunchParams* P) {
-  auto up16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
-  const size_t n_str = P->n_strings ? P->n_strings : 1;
-  size_t o = up16(sizeof(IceLayer) * P->n_layers);
-  P->off_walk = (uint32_t)o; o = up16(o + sizeof(float4) * (P->n_layers + 1));
-  P->off_str_a = (uint32_t)o; o = up16(o + sizeof(float4) * n_str);
-  P->off_str_b = (uint32_t)o; o = up16(o + sizeof(uint2) * n_str);
-  P->off_inv_b = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (P->m_b + 1));
-  P->off_inv_a = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (P->m_a + 1));
-  P->off_cell = (uint32_t)o; o = up16(o + sizeof(uint16_t) * (size_t)P->nx * P->ny);
-  return o;
-}
-
 template <bool B, bool F, bool A>
 static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
-  static std::atomic<size_t> attr_smem{0};  // opt-in dynamic shared memory size set so far
-  if (smem > attr_smem.load()) {
-    cudaError_t e = cudaFuncSetAttribute(propagate_kernel<B, F, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // opt-in dynamic shared memory size set so far, per device (the attribute is per device and per function)
+  static std::atomic<size_t> attr_smem[kMaxDevices];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (smem > attr_smem[dev].load()) {
+    e = cudaFuncSetAttribute(propagate_kernel<B, F, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_smem.store(smem);
+    attr_smem[dev].store(smem);
   }
   propagate_kernel<B, F, A><<<grid, kBlockThreads, smem, st>>>(P);
   g_launches++;
@@ -639,6 +643,8 @@ cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int 
     default: return launch_prop_t<true, true, true>(P, grid, smem, st);
   }
 }
+
+int propagate_warps_per_block() { return kBlockThreads / 32; }
 
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
   // all variants are compiled for the same launch bounds; the leanest and the fullest bracket the rest

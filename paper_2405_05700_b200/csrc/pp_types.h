@@ -1,6 +1,7 @@
 // Records shared by the host side (pp_api.cpp) and the kernels (pp_kernels.cu) of the library.
 // Not part of the public ABI.  Product code: shares nothing with oracle/.
 #pragma once
+#include <cstddef>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -51,11 +52,38 @@ constexpr int kMinTilePhotons = 32;
 constexpr int kMaxStringsSmem = 512;
 constexpr float kPoleRho2 = 1e-10f;  // R-9
 constexpr uint32_t kMaxWalkInv = 4096;  // entries per inverse walk table (device and shared memory)
-constexpr uint16_t kNoString = 0xFFFFu;  // cell-table entry: no line of DOMs within reach of this cell
+constexpr uint16_t kNoString = 0xFFFFu;  // host-side marker while the cell table is built: no line within reach
 
-// Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).
+// One record per layer boundary i (= upper edge of layer i), i = 0..n_layers; 32 B, shared memory (a4).
+// The first half is layer i's coefficients, the second half the cumulative vertical optical depth at the boundary as
+// two-float sums (B scattering, A absorption).  Record n_layers repeats the last layer's coefficients and holds +inf
+// in the hi parts (only ever compared against).
+struct __align__(16) LayerRec {
+  float a, b, la, lb;     // 1/m, 1/m, m, m
+  float Bh, Ah, Bl, Al;
+};
+
+// Everything a propagation launch needs.  Passed by value (kernel parameter space = constant bank).  The fields the
+// loop touches every iteration sit in 16-byte groups so that one constant load fetches a group.
 struct LaunchParams {
-  // work
+  // ---- hot groups (each 16 B, 16 B aligned) ----
+  uint32_t rk[10][2];                                   // Philox round keys (5 groups)
+  float hg_one_minus_g, hg_two_g, hg_one_minus_g2;      // 1-g, 2g, 1-g^2
+  float one_minus_cos_c;                                // 1 - cos(theta_c)
+  float z_top, inv_dz_layer, dz_layer;
+  int32_t last_layer;                                   // n_layers - 1
+  float k_b, k_a;                                       // inverse-table index = cumulative depth * k
+  uint32_t m_b, m_a;                                    // largest inverse-table index
+  uint32_t off_inv_b, off_inv_a, off_str_xy, off_cell;  // byte offsets into dynamic shared memory (layer records at 0)
+  float inv_cell, cell_ox, cell_oy;                     // cell coordinate = x * inv_cell + cell_ox
+  float rm2;                                            // radius_margin^2 (pre-filter)
+  uint32_t nx_m1, ny_m1, nx;
+  float xy_cap2;                                        // (longest piece of flight looked up at once, xy)^2
+  float inv_xy_cap;
+  uint32_t max_flights;
+  uint32_t ring_cap;
+  uint32_t walk_loop;
+  // ---- work ----
   const SrcRec* src;
   const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons (batch-global photon numbers)
   const uint32_t* cum_rel;        // [n_src + 1] cum[s] - g_begin as 32 bits: wraps below 0 (only the launch's first
@@ -64,34 +92,34 @@ struct LaunchParams {
   unsigned long long g_begin, g_end;
   uint32_t n_src, n_tiles;
   uint32_t tile_photons;          // photons per fresh tile of this launch: kMinTilePhotons..kTilePhotons, a power of two
+  uint32_t n_resume_in, resume_cap;
   const WorkItem* resume_in;
   WorkItem* resume_out;
-  uint32_t n_resume_in, resume_cap;
   Status* status;
   void* ring;         // pp_hit[ring_cap]
-  uint32_t ring_cap;
-  uint32_t max_flights;
   void* fates;        // pp_fate[g_end] or nullptr
-  // medium
-  const IceLayer* ice;  // [n_layers]
-  // Direct layer walk (a4): cumulative vertical optical depth at the layer boundaries, boundary i = upper edge of
-  // layer i, as two-float sums {B_hi, A_hi, B_lo, A_lo} (B scattering, A absorption); entry n_layers holds +inf in
-  // the hi parts (only ever compared against).  inv_b / inv_a map a quantised cumulative depth to a layer j0 such
-  // that the layer holding that depth is j0 or j0 + 1 (or beyond, when walk_loop is set for a coarse table).
-  const float4* walk;     // [n_layers + 1]
-  const uint16_t* inv_b;  // [m_b + 1]
-  const uint16_t* inv_a;  // [m_a + 1]
-  uint32_t m_b, m_a;      // largest table index
-  float k_b, k_a;         // table index = cumulative depth * k
-  uint32_t walk_loop;
-  // byte offsets of the tables in dynamic shared memory (ice table at 0)
-  uint32_t off_walk, off_str_a, off_str_b, off_inv_b, off_inv_a, off_cell;
+  // ---- tables ----
+  // Image of the shared-memory tables, copied verbatim into dynamic shared memory by every CTA (smem_image_bytes, a
+  // multiple of 16): [LayerRec x (n_layers + 1)] [u16 inv_b x (m_b + 1)] [u16 inv_a x (m_a + 1)]
+  // [float2 line xy x (n_strings + 1)] [u16 cell x (nx ny)] [float4 line (x, y, z0, 1/pitch) x n_strings]
+  // [uint2 line (n, base) x n_strings].  After the image: one 48-byte SrcRec slot per warp (off_wsrc).
+  //  * inv_b / inv_a map a quantised cumulative depth to a layer j0 such that the layer holding that depth is j0 or
+  //    j0 + 1 (or beyond, when walk_loop is set for a coarse table).
+  //  * cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter disc
+  //    can be met by a piece of flight whose xy midpoint lies in that cell; n_strings if none: that entry of the line
+  //    xy table holds NaN, so the pre-filter fails without a branch.  Unique because a piece is at most xy_cap long in
+  //    xy (longer flights are looked up piece by piece), and xy_cap < (smallest distance between two lines)
+  //    - 2 radius_margin - cell diagonal; the outermost ring of cells is empty, so the cell index may simply be
+  //    clamped into the grid.
+  const uint4* smem_image;
+  uint32_t smem_image_bytes;
+  uint32_t off_wsrc, off_str_a, off_str_b;
   uint32_t n_layers;
-  float z_top, dz_layer, inv_dz_layer;
-  float hg_one_minus_g, hg_two_g, hg_one_minus_g2;  // 1-g, 2g, 1-g^2
-  float one_minus_cos_c;                             // 1 - cos(theta_c)
+  uint32_t n_strings, n_dom;
+  const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
+  float radius, radius_margin;       // radius_margin = R + safety used by the pre-filter
   double inv_v;                                      // n_group / c  [ns/m]
-  uint32_t rk[10][2];                                // Philox round keys
+  // ---- optional physics (kExt variant only) ----
   // DOM acceptance (pp_set_acceptance, R-17): mode 0 off, 1 probabilistic, 2 weighted
   uint32_t acc_mode, acc_n;
   // wavelength bins (pp_set_spectrum, R-21): 0 = monochromatic
@@ -107,21 +135,10 @@ struct LaunchParams {
   uint32_t has_segments;  // some source of this launch has length > 0 (R-18)
   float inv_c;            // 1 / c  [ns/m]
   float acc_coef[8];
-  // geometry
-  const StringRec* strings;  // [n_strings]
-  const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id
-  // cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter
-  // disc can be met by a piece of flight whose xy midpoint lies in that cell (kNoString if none).  Unique because
-  // a piece is at most xy_cap long in xy (longer flights are looked up piece by piece), and xy_cap < (smallest
-  // distance between two lines) - 2 radius_margin - cell diagonal; the outermost ring of cells is empty, so the
-  // cell index may simply be clamped into the grid.
-  const uint16_t* cell_sid;  // [nx*ny]
-  uint32_t n_strings, n_dom;
-  uint32_t nx, ny;
-  float cell_ox, cell_oy, inv_cell;  // cell coordinate = x * inv_cell + cell_ox
-  float radius, radius_margin;       // radius_margin = R + safety used by the pre-filter
-  // a flight longer than xy_cap metres in the xy-plane is looked up in the cell table in chunks of at most xy_cap
-  float xy_cap2, inv_xy_cap;  // xy_cap^2, 1/xy_cap
 };
+static_assert(offsetof(LaunchParams, hg_one_minus_g) % 16 == 0 && offsetof(LaunchParams, z_top) % 16 == 0 &&
+              offsetof(LaunchParams, k_b) % 16 == 0 && offsetof(LaunchParams, off_inv_b) % 16 == 0 &&
+              offsetof(LaunchParams, inv_cell) % 16 == 0 && offsetof(LaunchParams, nx_m1) % 16 == 0 &&
+              offsetof(LaunchParams, inv_xy_cap) % 16 == 0, "hot parameter groups must be 16-byte aligned");
 
 }  // namespace pp
