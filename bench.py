@@ -36,17 +36,68 @@ WORKLOAD = "C1: BASELINE.json configs[1], 200 cascades E^-1 1 GeV-10 TeV on a 1 
 INSTR_PER_FLIGHT_FILE = os.path.join(ROOT, "profiles", "instr_per_flight.json")
 
 
-def load_instr_per_flight(library_version):
-    """The per-unit figure of the roofline; only valid for the library version it was measured on."""
+KERNEL_SOURCES = ["pp_kernels.cu", "pp_device.cuh", "pp_types.h"]
+FIXED_BUDGET_INSTR_PER_FLIGHT = 240.0  # ~220-260 thread instructions per scattering step
+
+
+def kernel_source_hash():
+    """SHA-256 over the kernel sources and the nvcc flags: what the stored instructions-per-flight was measured on."""
+    import hashlib
+    from paper_2405_05700_b200 import build as pp_build
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(pp_build.CSRC, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read() + b"\0")
+    h.update(" ".join(pp_build.NVCC_FLAGS + os.environ.get("PP_NVCC_EXTRA", "").split()).encode())
+    return h.hexdigest()
+
+
+def load_instr_per_flight():
+    """The per-unit figure of the roofline.  Valid only for the exact kernel sources + flags it was measured on:
+    returns (None, ..., reason) if the stored SHA-256 differs from the sources in the tree."""
     try:
         with open(INSTR_PER_FLIGHT_FILE) as f:
             d = json.load(f)
-        if d.get("library") != library_version:
-            return None, None, f"stale: measured on {d.get('library')!r}, library is {library_version!r}", None
+        have = kernel_source_hash()
+        if d.get("kernel_sources_sha256") != have:
+            return None, None, (f"stale: profiles/instr_per_flight.json was measured on sources {str(d.get('kernel_sources_sha256'))[:12]}, "
+                                f"the tree holds {have[:12]}; re-measure (bench.py --update-instr-per-flight)"), None
         return float(d["thread_instructions_per_flight"]), d.get("dram_bytes_per_launch"), d.get("source", ""), \
             d.get("fp32_flops_per_flight")
-    except Exception:
-        return None, None, "", None
+    except Exception as e:
+        return None, None, f"unreadable: {e!r}", None
+
+
+def update_instr_per_flight(args):
+    """`bench.py --update-instr-per-flight NCU.csv --flights N [--fp32-per-thread-instr X]`: store the per-unit figure
+    from an ncu --csv log of `bench.py --steps 1 --warmup 0 --no-cpu-baseline` taken with the metrics
+    smsp__thread_inst_executed.sum, smsp__inst_executed.sum, dram__bytes_read.sum, dram__bytes_write.sum (all propagate
+    launches of the run; N = flights those launches simulated, printed by the same bench line)."""
+    import csv
+    tot = {}
+    n_launch = 0
+    with open(args.update_instr_per_flight) as f:
+        rows = [r for r in csv.reader(f) if len(r) > 5]
+    hdr = rows[0]
+    i_k, i_m, i_v = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value")
+    for r in rows[1:]:
+        if "propagate_kernel" not in r[i_k]:
+            continue
+        v = float(r[i_v].replace(",", ""))
+        tot[r[i_m]] = tot.get(r[i_m], 0.0) + v
+        n_launch += r[i_m] == "smsp__inst_executed.sum"
+    thr, warp = tot["smsp__thread_inst_executed.sum"], tot["smsp__inst_executed.sum"]
+    d = {"thread_instructions_per_flight": thr / args.flights, "warp_instructions_per_flight": warp / args.flights,
+         "mean_active_lanes": thr / warp,
+         "fp32_flops_per_flight": (args.fp32_per_thread_instr * thr / args.flights) if args.fp32_per_thread_instr else None,
+         "dram_bytes_per_launch": (tot.get("dram__bytes_read.sum", 0.0) + tot.get("dram__bytes_write.sum", 0.0)) / max(1, n_launch),
+         "propagate_launches": n_launch, "flights": args.flights, "kernel_sources_sha256": kernel_source_hash(),
+         "kernel": "pp::propagate_kernel<false,false,false>", "source": args.note}
+    with open(INSTR_PER_FLIGHT_FILE, "w") as f:
+        json.dump(d, f, indent=2)
+        f.write("\n")
+    print(json.dumps(d))
+    return 0
 
 
 def measured_peaks():
@@ -109,11 +160,12 @@ def workload():
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ------------------------------------------------------------------------------------------------
-def oracle_rate(geo, ice, src, seed, budget_s):
-    """Times the oracle, as it stands, on a strided sample of the workload sized for ~budget_s."""
+def oracle_rate(geo, ice, src, seed, budget_s, n_threads=0):
+    """Times the oracle, as it stands, on a strided sample of the workload sized for ~budget_s (n_threads = 0: all
+    host cores)."""
     from oracle import oracle as O
     t = time.perf_counter()
-    r = O.propagate(geo, ice, src, seed=seed, stride=8192)
+    r = O.propagate(geo, ice, src, seed=seed, stride=8192, n_threads=n_threads)
     dt = time.perf_counter() - t
     rate = r.photons / max(dt, 1e-9)
     total = sum(O.photon_count(e, ice.photons_per_GeV) for e in src.src[:, 7])
@@ -121,7 +173,7 @@ def oracle_rate(geo, ice, src, seed, budget_s):
     while stride > 1 and (total / (stride // 2)) / rate < budget_s:
         stride //= 2
     t = time.perf_counter()
-    r = O.propagate(geo, ice, src, seed=seed, stride=stride)
+    r = O.propagate(geo, ice, src, seed=seed, stride=stride, n_threads=n_threads)
     dt = time.perf_counter() - t
     return {"photons": r.photons, "seconds": dt, "value": r.photons / dt, "flights_per_s": r.flights / dt,
             "stride": stride, "hits": r.hit}
@@ -234,6 +286,28 @@ def run_ours(args):
     st_e2e = prop.stats()
     e2e_launches = st_e2e.launches - st_after.launches
 
+    # ---- device-busy fraction THROUGH THE BATCHING SERVER (north_star: >= 90 %; "> 90 %", PAPER.md:86
+    # 45 % -> 80 %): C2 x 10 re-numbered replicas shipped by 8 producer threads in blocks of 8192 sources through
+    # pp_submit while one consumer collects; repeated until >= 0.4 s of wall time is covered ----
+    server = None
+    if world == 1 and not args.no_server_leg:
+        c2, packed, n_events = pack_stream_blocks(10, 8, 8192)
+        with B.Propagator(geo, ice, seed=seed, launch_photons_target=target) as sp:
+            sp.run(c2.src, c2.event_id, c2.source_id)  # warm-up
+            tot = {"wall_s": 0.0, "photons": 0, "kernel_s": 0.0, "launches": 0, "hits": 0}
+            reps = 0
+            while tot["wall_s"] < 0.4 and reps < 20:
+                r = stream_job(sp, packed)
+                for k_ in tot:
+                    tot[k_] += r[k_]
+                reps += 1
+        server = {"device_busy_frac": tot["kernel_s"] / tot["wall_s"], "photons_per_s": tot["photons"] / tot["wall_s"],
+                  "threads": 8, "launches": tot["launches"], "jobs": reps, "photons": tot["photons"], "wall_s": tot["wall_s"],
+                  "hits": tot["hits"],
+                  "workload": f"C2 x 10 replicas of {n_events} events ({sum(len(b) for b in packed)} blocks of >= 8192 sources) "
+                              "per job through pp_submit / pp_collect",
+                  "paper": "GPU utilisation > 90 % (PAPER.md:5); 45 % -> 80 % (PAPER.md:86); hardware not stated"}
+
     # ---- max over ranks ----
     tmax, wsum = replicas.reduce_results(dist, torch.device("cuda", local), {"dev_ms": dev_ms, "e2e_s": e2e_s},
                                          {"photons": float(photons)})
@@ -244,7 +318,7 @@ def run_ours(args):
     if rank == 0:
         peaks = measured_peaks()
         clocks = clk.summary()
-        ipf, dram_bytes, ipf_src, fpf = load_instr_per_flight(B.version())
+        ipf, dram_bytes, ipf_src, fpf = load_instr_per_flight()
         sm_max = peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         roofline = None
@@ -263,6 +337,10 @@ def run_ours(args):
                                        "MEASURED_PEAKS.json sm_max_mhz)",
                         "frac_at_observed_clock": (achieved / (n_sm * 4 * 32 * clocks["sm_mhz"] * 1e-3)
                                                    if clocks.get("sm_mhz") else None)}
+            # the same flights/s against a FIXED instruction budget per flight (~240): unlike
+            # `frac`, this one cannot rise by executing more instructions per flight
+            roofline["frac_fixed_budget"] = flights * FIXED_BUDGET_INSTR_PER_FLIGHT / (busy_ms * 1e-3) / 1e9 / peak
+            roofline["fixed_budget_thread_instructions_per_flight"] = FIXED_BUDGET_INSTR_PER_FLIGHT
             if fpf:
                 # the metric's "% of SM FP32 roofline": FP32 flops (FFMA = 2, FMUL/FADD = 1) per flight from the same
                 # ncu capture, against SMs x 128 lanes x 2 x f; capped near 30 % by the integer/control share of the mix
@@ -272,10 +350,13 @@ def run_ours(args):
                                     "fp32_flops_per_flight": float(fpf)}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            o = oracle_rate(geo, ice, src, 0, 15.0)
+            o = oracle_rate(geo, ice, src, 0, 12.0)
+            o1 = oracle_rate(geo, ice, src, 0, 6.0, n_threads=1)  # 1 thread and all cores
             cpu = {"value": o["value"], "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
                    "sample": f"C1 photons with photon_idx % {o['stride']} == 0 ({o['photons']} photons, {o['seconds']:.1f} s)",
-                   "flights_per_s": o["flights_per_s"]}
+                   "flights_per_s": o["flights_per_s"],
+                   "one_thread": {"value": o1["value"], "cores": 1, "flights_per_s": o1["flights_per_s"],
+                                  "sample": f"photon_idx % {o1['stride']} == 0 ({o1['photons']} photons, {o1['seconds']:.1f} s)"}}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
@@ -290,7 +371,9 @@ def run_ours(args):
                         "h2d_bytes_per_step": int(len(src) * 48 + 0),
                         "d2h_bytes_per_step": int(e2e_hits / args.steps * 32 + e2e_launches / args.steps * 64),
                         "hits_per_step": e2e_hits / args.steps},
-                "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+                "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "server": server, "cpu_baseline": cpu}
+        if roofline is None:
+            line["roofline_note"] = ipf_src or "no per-unit figure"
         print(json.dumps(line))
     prop.close()
     if dist is not None:
@@ -335,6 +418,81 @@ def run_sweep(args):
     return 0
 
 
+def pack_stream_blocks(replicas, n_thr, block_sources):
+    """C2 re-numbered `replicas` times and dealt to `n_thr` clients: client t owns events g with g % n_thr == t of
+    every replica and ships a block whenever >= block_sources sources have piled up (blocks end on event boundaries)."""
+    from paper_2405_05700_b200 import binding as B
+    from paper_2405_05700_b200 import workloads as W
+    src = W.sources_c2()
+    order = np.argsort(src.event_id, kind="stable")
+    rec = B.pack_sources(src.src[order])
+    ev, sid = src.event_id[order], src.source_id[order]
+    n_events = int(ev.max()) + 1
+    first = np.searchsorted(ev, np.arange(n_events + 1))  # sources of event g: [first[g], first[g+1])
+    blocks = [[] for _ in range(n_thr)]
+    for t in range(n_thr):
+        cur, cur_n = [], 0
+        for r in range(replicas):
+            for g in range(t, n_events, n_thr):
+                a, b = int(first[g]), int(first[g + 1])
+                if b > a:
+                    cur.append((r, a, b))
+                    cur_n += b - a
+                if cur_n >= block_sources:
+                    blocks[t].append(cur)
+                    cur, cur_n = [], 0
+        if cur:
+            blocks[t].append(cur)
+    packed = [[(np.concatenate([rec[a:b] for _, a, b in blk]),
+                np.concatenate([ev[a:b] + np.uint32(r * n_events) for r, a, b in blk]),
+                np.concatenate([sid[a:b] for _, a, b in blk])) for blk in bl] for bl in blocks]
+    return src, packed, n_events
+
+
+def stream_job(prop, packed):
+    """Producer threads (the paper's propagation clients) ship their packed blocks through pp_submit
+    while one consumer thread collects hits; returns wall seconds, photons, kernel-busy seconds, launches, hits between
+    the first submit and the drain."""
+    import torch
+    st0 = prop.stats()
+
+    def producer(t):
+        for r_, e_, s_ in packed[t]:
+            prop.submit(r_, e_, s_)
+
+    n_hits = [0]
+    done = threading.Event()
+
+    def consumer():
+        while True:
+            h = prop.collect(1 << 20, block=True)
+            if len(h) == 0:
+                if done.is_set():
+                    return
+                time.sleep(0.0005)
+                continue
+            n_hits[0] += len(h)
+
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    cons = threading.Thread(target=consumer)
+    cons.start()
+    th = [threading.Thread(target=producer, args=(t,)) for t in range(len(packed))]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    prop.flush()
+    done.set()
+    cons.join()
+    n_hits[0] += len(prop.collect_all())
+    wall = time.perf_counter() - t0
+    st1 = prop.stats()
+    return {"wall_s": wall, "photons": int(st1.photons_done - st0.photons_done),
+            "kernel_s": (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3, "launches": int(st1.launches - st0.launches),
+            "hits": int(n_hits[0]), "source_ring_high_water": int(st1.source_ring_high_water)}
+
+
 def run_stream(args):
     """BASELINE.json configs[2] through the batching server.  `--threads` producer threads play the paper's
     propagation clients: each owns a share of the events of `--replicas` re-numbered replicas of
@@ -348,75 +506,17 @@ def run_stream(args):
     from paper_2405_05700_b200 import workloads as W
     torch.cuda.set_device(0)
     geo, ice = W.geometry_full(), W.ice_layered()
-    src = W.sources_c2()
-    order = np.argsort(src.event_id, kind="stable")
-    rec = B.pack_sources(src.src[order])
-    ev, sid = src.event_id[order], src.source_id[order]
-    n_events = int(ev.max()) + 1
-    first = np.searchsorted(ev, np.arange(n_events + 1))  # sources of event g: [first[g], first[g+1])
     replicas, n_thr = args.replicas, max(1, args.threads)
-    # client t owns events g with g % n_thr == t of every replica; its blocks end on event boundaries
-    blocks = [[] for _ in range(n_thr)]
-    for t in range(n_thr):
-        cur, cur_n = [], 0
-        for r in range(replicas):
-            for g in range(t, n_events, n_thr):
-                a, b = int(first[g]), int(first[g + 1])
-                if b > a:
-                    cur.append((r, a, b))
-                    cur_n += b - a
-                if cur_n >= args.block_sources:
-                    blocks[t].append(cur)
-                    cur, cur_n = [], 0
-        if cur:
-            blocks[t].append(cur)
-    packed = [[(np.concatenate([rec[a:b] for _, a, b in blk]),
-                np.concatenate([ev[a:b] + np.uint32(r * n_events) for r, a, b in blk]),
-                np.concatenate([sid[a:b] for _, a, b in blk])) for blk in bl] for bl in blocks]
+    src, packed, n_events = pack_stream_blocks(replicas, n_thr, args.block_sources)
     with B.Propagator(geo, ice, seed=0, launch_photons_target=10 ** 8) as prop:
         prop.run(src.src, src.event_id, src.source_id)  # warm-up
-        st0 = prop.stats()
-
-        def producer(t):
-            for r_, e_, s_ in packed[t]:
-                prop.submit(r_, e_, s_)
-
-        n_hits = [0]
-        done = threading.Event()
-
-        def consumer():
-            while True:
-                h = prop.collect(1 << 20, block=True)
-                if len(h) == 0:
-                    if done.is_set():
-                        return
-                    time.sleep(0.0005)
-                    continue
-                n_hits[0] += len(h)
-
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        cons = threading.Thread(target=consumer)
-        cons.start()
-        th = [threading.Thread(target=producer, args=(t,)) for t in range(n_thr)]
-        for t in th:
-            t.start()
-        for t in th:
-            t.join()
-        prop.flush()
-        done.set()
-        cons.join()
-        n_hits[0] += len(prop.collect_all())
-        wall = time.perf_counter() - t0
-        st1 = prop.stats()
-    ph = st1.photons_done - st0.photons_done
-    busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+        r = stream_job(prop, packed)
     print(json.dumps({"mode": "stream", "workload": f"C2 x {replicas} replicas of {n_events} events, shipped in blocks of >= "
                       f"{args.block_sources} sources by {n_thr} client threads", "threads": n_thr,
-                      "blocks": sum(len(b) for b in blocks), "sources": int(len(src) * replicas), "photons": int(ph),
-                      "launches": st1.launches - st0.launches, "photons_per_s": ph / wall, "device_busy_frac": busy / wall,
-                      "wall_s": wall, "kernel_s": busy, "hits": n_hits[0],
-                      "source_ring_high_water": st1.source_ring_high_water}), flush=True)
+                      "blocks": sum(len(b) for b in packed), "sources": int(len(src) * replicas), "photons": r["photons"],
+                      "launches": r["launches"], "photons_per_s": r["photons"] / r["wall_s"],
+                      "device_busy_frac": r["kernel_s"] / r["wall_s"], "wall_s": r["wall_s"], "kernel_s": r["kernel_s"],
+                      "hits": r["hits"], "source_ring_high_water": r["source_ring_high_water"]}), flush=True)
     return 0
 
 
@@ -571,6 +671,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-server-leg", action="store_true", help="skip the device-busy-through-the-server leg")
+    ap.add_argument("--update-instr-per-flight", default="", metavar="NCU_CSV",
+                    help="store profiles/instr_per_flight.json from an ncu --csv log (see update_instr_per_flight)")
+    ap.add_argument("--flights", type=float, default=0.0, help="with --update-instr-per-flight: flights the launches simulated")
+    ap.add_argument("--fp32-per-thread-instr", type=float, default=0.0,
+                    help="with --update-instr-per-flight: FP32 flops per thread instruction from the ncu source page")
+    ap.add_argument("--note", default="", help="with --update-instr-per-flight: where the numbers come from")
     ap.add_argument("--ext", action="store_true", help="C1 with the optional physics on (report mode)")
     ap.add_argument("--c4", action="store_true", help="C4 memory-bounded extreme event (report mode)")
     ap.add_argument("--sweep", action="store_true", help="C3 launch-size sweep (report mode)")
@@ -581,6 +688,8 @@ def main():
     ap.add_argument("--ipc-clients", type=int, default=0, help="with --stream: N client processes over include/pp_ipc.h")
     ap.add_argument("--block-sources", type=int, default=8192, help="sources a client queues before it ships a block")
     args = ap.parse_args()
+    if args.update_instr_per_flight:
+        return update_instr_per_flight(args)
     if args.impl == "reference":
         return run_reference(args)
     if args.ext:

@@ -154,8 +154,12 @@ int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config
 /* Builds the DOM lookup and ice tables, uploads them, starts the batching server thread. */
 int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, pp_handle** out);
 
-/* Enqueues n light sources ("a block of steps").  event_ids[n] required; source_ids may be
- * NULL, in which case source i of this call gets id i.  Thread-safe: any number of threads may submit
+/* Enqueues n light sources ("a block of steps").  event_ids[n] required.
+ * (event_id, source_id) MUST BE UNIQUE for the life of the handle: the pair is part of the Philox counter (R-3), so
+ * two sources that share it draw the same random numbers -- perfectly correlated photons, duplicated hits, no error.
+ * source_ids may be NULL: a source then gets the handle's running record number (the count of sources submitted
+ * before it, pp_stats.sources_submitted, mod 2^32), which is unique across calls.  Results are reproducible from run
+ * to run only with explicit ids or a fixed submit order.  Thread-safe: any number of threads may submit
  * concurrently.  Copies before returning.  Blocks while the source ring is full unless
  * PP_FLAG_NONBLOCKING_SUBMIT.  Sources with N == 0 photons are accepted and ignored. */
 int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids, const uint32_t* source_ids,
@@ -235,8 +239,8 @@ const char* pp_last_error(pp_handle* h);
 void pp_destroy(pp_handle* h);
 
 /* ---- device-resident path (what bench.py times as `value`, and what the parity tests drive) ----
- * Inputs already in HBM: d_sources[n] (pp_source), d_event_ids[n], d_source_ids[n] (nullable: index)
- * are DEVICE pointers.  Runs source expansion + propagation for ALL photons of the n sources in
+ * Inputs already in HBM: d_sources[n] (pp_source), d_event_ids[n], d_source_ids[n] (nullable: the running
+ * record number as in pp_submit) are DEVICE pointers.  Runs source expansion + propagation for ALL photons of the n sources in
  * launches of at most launch_photons_target photons, alternating between the two streams,
  * synchronously; hits go through the bounded device hit ring to the pp_collect queue.  Needs an
  * idle server (PP_E_STATE otherwise) and n <= source ring capacity (PP_E_NOMEM otherwise).

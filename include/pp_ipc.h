@@ -13,9 +13,17 @@
  * (so launches mix the sources of all clients); its dispatch thread routes every collected hit to the client that
  * submitted the hit's event.
  *
- * Contract: event ids are global -- an event belongs to the client that first submits a source of it, until the
- * server next runs dry (nothing queued, in flight or uncollected anywhere: the owner table is emptied then); two
- * clients submitting the same event id at the same time is a caller error (its hits all go to the first).  The
+ * Contract: event ids are global -- an event belongs to the client that first submits a source of it, for as long as
+ * a block of that client holding sources of the event is in the server (the owner table forgets an event when the
+ * last such block is complete and its hits are routed, so the table stays as small as the work in flight); two
+ * clients submitting the same event id at the same time is a caller error (its hits all go to the first).
+ * (event_id, source_id) must be unique for the life of the server, as in pp.h: two sources with the same pair draw
+ * the same random numbers.  source_ids == NULL numbers a client's sources with its running record count.
+ *
+ * A client that falls behind with pp_ipc_collect never holds up the others: hits its ring has no room for are parked
+ * in the server, and while more than four rings' worth is parked the server takes no more sources from that client
+ * (it then blocks in pp_ipc_submit).  A client whose process has died (checked with kill(pid, 0), so server and
+ * clients must share a pid namespace) is treated as closed: its hits are dropped and its slot is handed out again.  The
  * hits a client receives are exactly the hits of its events, and, as everywhere in pp.h, they do not depend on how
  * many clients there are, on block sizes or on timing.
  *
@@ -43,7 +51,8 @@ typedef struct pp_ipc_config {
 
 /* The server's back end: where blocks go and hits come from.  pp_ipc_server_create() binds it to a pp_handle
  * (submit = pp_submit_segments, flush = pp_flush, collect = pp_collect with block = 0, completed =
- * pp_stats.sources_completed); tests on a machine without a GPU bind it to pp_ipc_echo_backend(). */
+ * pp_stats.sources_completed); tests on a machine without a GPU bind it to a host-only back end of their own
+ * (tests/echo_backend.cpp) through pp_ipc_server_create_backend(). */
 typedef struct pp_ipc_backend {
   void* ctx;
   int (*submit)(void* ctx, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
@@ -70,13 +79,11 @@ typedef struct pp_ipc_server_stats {
   uint64_t sources_ingested;
   uint64_t hits_routed;
   uint64_t hits_unrouted;    /* hits of an event no client had announced (must be 0) */
+  uint64_t hits_dropped;     /* hits of clients that had left (closed, or their process died) */
+  uint64_t clients_dropped;  /* clients the server declared gone because their process no longer exists */
+  uint64_t events_tracked;   /* entries of the event-owner table right now (bounded by the events in flight) */
 } pp_ipc_server_stats;
 int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out);
-
-/* Host-only test back end: every source yields, at the next flush, one hit {event_id, source_id, photon_idx =
- * its photon count at 1e4 photons/GeV, dom_id = 0, time_ns = t_ns + length, weight = energy}.  The returned
- * pointer stays valid for the life of the process; each call makes an independent instance. */
-const pp_ipc_backend* pp_ipc_echo_backend(void);
 
 /* ---- client side (any process; no CUDA call inside) ---- */
 /* Attaches to the segment and claims a client slot -- one a former client has left, else a fresh one (PP_E_NOMEM if
@@ -93,7 +100,8 @@ int pp_ipc_flush(pp_ipc_client* c);
  * drains on its own: it does not wait for other clients' work (the server tracks completion block by block, in the
  * order it handed the blocks to the GPU server). */
 int pp_ipc_collect(pp_ipc_client* c, pp_hit* out, size_t cap, size_t* n_out, int block);
-/* Detaches.  Hits not yet collected are dropped; the slot is handed out again once the server has next run dry. */
+/* Detaches.  Hits not yet collected are dropped; the slot is handed out again once the blocks this client shipped
+ * are complete (other clients' work does not delay that). */
 void pp_ipc_client_close(pp_ipc_client* c);
 
 #ifdef __cplusplus

@@ -411,8 +411,7 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
   img.resize((img.size() + 15) & ~(size_t)15, 0);
   h->image_bytes = img.size();
   B.smem_image_bytes = (uint32_t)img.size();
-  B.off_wsrc = (uint32_t)img.size();
-  h->smem = img.size() + (size_t)propagate_warps_per_block() * sizeof(SrcRec);
+  h->smem = img.size();
   return PP_OK;
 }
 
@@ -999,7 +998,7 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
       SrcRec& r = h->ring[(h->ring_head + j) % h->sz.cap_src];
       r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
       r.event_id = event_ids[i];
-      r.source_id = source_ids ? source_ids[i] : (uint32_t)i;
+      r.source_id = source_ids ? source_ids[i] : (uint32_t)(h->st.sources_submitted + j);  // running record number
       r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
       r.length = lengths ? lengths[i] : 0.0f;
       ph += r.n_photons;
@@ -1171,12 +1170,14 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
   if (n == 0) return PP_OK;
   if (!d_sources || !d_event_ids) return fail(h, PP_E_INVAL, "null device pointer");
   if (n > h->sz.cap_src) return fail(h, PP_E_NOMEM, "more sources than the source ring holds; raise source_ring_bytes");
+  uint32_t sid_base = 0;  // source ids when d_source_ids is NULL: the handle's running record number
   {
     std::unique_lock<std::mutex> lk(h->mu);
     if (h->shutdown) return PP_E_STATE;
     if (!idle_locked(h) || h->ring_launch != h->ring_head)
       return fail(h, PP_E_STATE, "pp_run_resident needs an idle server (flush and collect first)");
     h->resident_active = true;
+    sid_base = (uint32_t)h->st.sources_submitted;
     if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
   }
   auto leave = [&](int rc) {
@@ -1193,7 +1194,7 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
   cudaError_t e = cudaEventRecord(h->ev_job, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->d_res_overflow, 0, sizeof(unsigned int), st);
   if (e == cudaSuccess)
-    e = launch_ingest(d_sources, d_event_ids, d_source_ids, (uint32_t)n, h->ice.photons_per_GeV, h->d_res_src,
+    e = launch_ingest(d_sources, d_event_ids, d_source_ids, sid_base, (uint32_t)n, h->ice.photons_per_GeV, h->d_res_src,
                       h->d_res_overflow, st);
   if (e == cudaSuccess) e = launch_scan(h->d_res_src, (uint32_t)n, h->d_res_cum, st);
   if (e == cudaSuccess)

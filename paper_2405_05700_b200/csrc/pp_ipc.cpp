@@ -4,6 +4,7 @@
 #include "../../include/pp_ipc.h"
 
 #include <fcntl.h>
+#include <signal.h>
 #include <sys/mman.h>
 #include <sys/stat.h>
 #include <unistd.h>
@@ -12,6 +13,7 @@
 #include <atomic>
 #include <chrono>
 #include <cmath>
+#include <cerrno>
 #include <cstring>
 #include <deque>
 #include <mutex>
@@ -56,6 +58,7 @@ struct ClientCtl {
   std::atomic<uint64_t> flush_seq;      // client: src_head at its last flush request
   std::atomic<uint64_t> flushed_seq;    // server: flush requests honoured up to here
   std::atomic<uint64_t> completed_seq;  // server: sources before it are propagated and their hits are in the hit ring
+  std::atomic<uint32_t> pid;            // client: its process id (the server checks that a stalled client still exists)
 };
 static_assert(sizeof(ClientCtl) <= kCtlBytes, "ctl");
 static_assert(std::atomic<uint64_t>::is_always_lock_free, "address-free atomics needed in shared memory");
@@ -74,6 +77,7 @@ struct Segment {
   }
 };
 
+using Clock = std::chrono::steady_clock;
 inline void nap(int us) { std::this_thread::sleep_for(std::chrono::microseconds(us)); }
 
 // ---- back end bound to a pp_handle ----
@@ -101,50 +105,6 @@ int h_completed(void* ctx, uint64_t* n_sources) {
   return rc;
 }
 
-// ---- host-only echo back end (tests without a GPU) ----
-struct Echo {
-  std::mutex mu;
-  std::vector<pp_hit> pending, ready;
-  uint64_t flushed = 0;  // sources whose hit has been made available
-};
-int e_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
-  Echo* e = static_cast<Echo*>(ctx);
-  std::lock_guard<std::mutex> g(e->mu);
-  for (size_t i = 0; i < n; ++i) {
-    pp_hit h{};
-    uint64_t cnt = 0;
-    pp_photon_count(s[i].energy_GeV, 1.0e4f, &cnt);
-    h.event_id = ev[i]; h.source_id = sid ? sid[i] : (uint32_t)i; h.photon_idx = (uint32_t)cnt; h.dom_id = 0;
-    h.time_ns = (double)s[i].t_ns + (len ? (double)len[i] : 0.0); h.weight = s[i].energy_GeV; h.n_scatter = 0;
-    e->pending.push_back(h);
-  }
-  return PP_OK;
-}
-int e_flush(void* ctx) {
-  Echo* e = static_cast<Echo*>(ctx);
-  std::lock_guard<std::mutex> g(e->mu);
-  e->ready.insert(e->ready.end(), e->pending.begin(), e->pending.end());
-  e->flushed += e->pending.size();
-  e->pending.clear();
-  return PP_OK;
-}
-int e_completed(void* ctx, uint64_t* n_sources) {
-  Echo* e = static_cast<Echo*>(ctx);
-  std::lock_guard<std::mutex> g(e->mu);
-  *n_sources = e->flushed;
-  return PP_OK;
-}
-int e_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
-  Echo* e = static_cast<Echo*>(ctx);
-  std::lock_guard<std::mutex> g(e->mu);
-  const size_t n = std::min(cap, e->ready.size());
-  std::memcpy(out, e->ready.data(), n * sizeof(pp_hit));
-  e->ready.erase(e->ready.begin(), e->ready.begin() + (long)n);
-  *n_out = n;
-  *drained = (n == 0 && e->pending.empty() && e->ready.empty()) ? 1 : 0;
-  return PP_OK;
-}
-
 }  // namespace
 
 struct pp_ipc_server {
@@ -153,14 +113,26 @@ struct pp_ipc_server {
   pp_ipc_backend be{};
   std::thread ingest, dispatch;
   std::atomic<bool> stop{false};
+  // event id -> owning client slot, with the number of that client's blocks holding sources of the event that are
+  // handed to the back end and not yet complete; the entry goes when the count drops to zero
+  struct Owner { uint32_t client, blocks; };
   std::mutex map_mu;
-  std::unordered_map<uint32_t, uint32_t> owner;  // event id -> client slot
-  std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0};
-  std::atomic<uint32_t> ingest_busy{0};  // a block is between "events announced" and "handed to the back end"
-  struct Block { uint32_t client; uint64_t tail_after, global_end; };
+  std::unordered_map<uint32_t, Owner> owner;
+  std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0}, dropped{0}, clients_dropped{0};
+  struct Block { uint32_t client; uint64_t tail_after, global_end; std::vector<uint32_t> events; };
   std::mutex fifo_mu;
   std::deque<Block> fifo;       // blocks handed to the back end, in order, not yet known to be complete
   uint64_t base_completed = 0;  // the back end's completed count when the server started
+  // per client slot
+  struct PerClient {
+    std::deque<pp_hit> parked;             // dispatch thread only: hits waiting for room in the client's hit ring
+    uint64_t pending_completed = 0;        // dispatch thread only: completed_seq to publish once `parked` is empty
+    std::atomic<uint64_t> parked_n{0};     // read by the ingest thread: a client far behind is not ingested from
+    std::atomic<uint32_t> blocks_in_flight{0};
+    Clock::time_point last_alive_check{};
+  };
+  std::vector<PerClient> pc;
+  uint64_t park_cap = 0;  // hits parked per client above which the server stops taking that client's sources
 
   std::atomic<int> error{PP_OK};
 };
@@ -184,7 +156,10 @@ void ingest_main(pp_ipc_server* s) {
       ClientCtl* ctl = s->seg.ctl(c);
       const uint64_t head = ctl->src_head.load(std::memory_order_acquire);
       uint64_t tail = ctl->src_tail.load(std::memory_order_relaxed);
-      if (head != tail) {
+      // a client that does not read its hits gets no more work done for it: its source ring fills up and it blocks
+      // in pp_ipc_submit, which bounds what the server has to park for it
+      const bool behind = s->pc[c].parked_n.load(std::memory_order_acquire) > s->park_cap;
+      if (head != tail && !behind) {
         const size_t n = (size_t)std::min<uint64_t>(head - tail, kIngestChunk);
         const SrcSlot* ring = s->seg.src_ring(c);
         bool any_len = false;
@@ -193,23 +168,31 @@ void ingest_main(pp_ipc_server* s) {
           src[i] = r.s; len[i] = r.length; ev[i] = r.event_id; sid[i] = r.source_id;
           any_len |= r.length != 0.0f;
         }
-        s->ingest_busy.store(1);
+        pp_ipc_server::Block blk{c, tail + n, 0, {}};
         {
           std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
           uint32_t last = ~ev[0];
-          for (size_t i = 0; i < n; ++i)
-            if (ev[i] != last) { s->owner.emplace(ev[i], c); last = ev[i]; }
+          for (size_t i = 0; i < n; ++i) {
+            if (ev[i] == last) continue;
+            last = ev[i];
+            if (std::find(blk.events.begin(), blk.events.end(), last) != blk.events.end()) continue;
+            auto it = s->owner.find(last);
+            if (it == s->owner.end()) it = s->owner.emplace(last, pp_ipc_server::Owner{c, 0}).first;
+            if (it->second.client == c) { it->second.blocks++; blk.events.push_back(last); }  // else: caller error (pp_ipc.h)
+          }
+        }
+        s->pc[c].blocks_in_flight++;
+        {
+          // the block is in the fifo before the back end sees it, so that "complete" can never overtake it
+          std::lock_guard<std::mutex> g(s->fifo_mu);
+          blk.global_end = s->sources.load() + n;
+          s->fifo.push_back(std::move(blk));
         }
         const int rc = s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
         if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
         s->blocks++; s->sources += n;
         tail += n;
-        {
-          std::lock_guard<std::mutex> g(s->fifo_mu);
-          s->fifo.push_back({c, tail, s->sources.load()});
-        }
         ctl->src_tail.store(tail, std::memory_order_release);
-        s->ingest_busy.store(0);
         progressed = true;
       }
       const uint64_t fs = ctl->flush_seq.load(std::memory_order_acquire);
@@ -224,17 +207,60 @@ void ingest_main(pp_ipc_server* s) {
   }
 }
 
+// A client is gone if it closed, or if its process no longer exists (it was killed: PAPER.md:47 names jobs that die
+// at their memory limit).  The existence check costs a system call, so it is made at most every 10 ms per client and
+// only for a client the server is waiting for.
+bool client_gone(pp_ipc_server* s, uint32_t c) {
+  ClientCtl* ctl = s->seg.ctl(c);
+  const uint32_t st = ctl->state.load(std::memory_order_acquire);
+  if (st == kClosed || st == kRecycled) return true;
+  auto& pc = s->pc[c];
+  const auto now = Clock::now();
+  if (now - pc.last_alive_check < std::chrono::milliseconds(10)) return false;
+  pc.last_alive_check = now;
+  const uint32_t pid = ctl->pid.load(std::memory_order_acquire);
+  if (pid != 0 && kill((pid_t)pid, 0) != 0 && errno == ESRCH) {
+    uint32_t expect = kAttached;
+    if (ctl->state.compare_exchange_strong(expect, kClosed, std::memory_order_acq_rel)) s->clients_dropped++;
+    return true;
+  }
+  return false;
+}
+
+// Move parked hits of client c into its ring as far as there is room; drop them if the client is gone.
+void drain_parked(pp_ipc_server* s, uint32_t c) {
+  auto& pc = s->pc[c];
+  ShmHeader* H = s->seg.hdr();
+  ClientCtl* ctl = s->seg.ctl(c);
+  if (!pc.parked.empty()) {
+    const uint64_t head = ctl->hit_head.load(std::memory_order_relaxed);
+    const uint64_t space = H->hit_cap - (head - ctl->hit_tail.load(std::memory_order_acquire));
+    if (space > 0) {
+      pp_hit* ring = s->seg.hit_ring(c);
+      const size_t m = (size_t)std::min<uint64_t>(space, pc.parked.size());
+      for (size_t q = 0; q < m; ++q) ring[(head + q) % H->hit_cap] = pc.parked[q];
+      pc.parked.erase(pc.parked.begin(), pc.parked.begin() + (long)m);
+      ctl->hit_head.store(head + m, std::memory_order_release);
+      s->routed += m;
+    } else if (client_gone(s, c)) {
+      s->dropped += pc.parked.size();
+      pc.parked.clear();
+    }
+    pc.parked_n.store(pc.parked.size(), std::memory_order_release);
+  }
+  if (pc.parked.empty() && pc.pending_completed > ctl->completed_seq.load(std::memory_order_relaxed))
+    ctl->completed_seq.store(pc.pending_completed, std::memory_order_release);  // its hits are all in the ring now
+}
+
 void dispatch_main(pp_ipc_server* s) {
   ShmHeader* H = s->seg.hdr();
   const size_t cap = 1 << 16;
   std::vector<pp_hit> buf(cap);
-  std::vector<uint64_t> snap(H->max_clients);
   while (!s->stop.load()) {
     const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
-    for (uint32_t c = 0; c < n_slots; ++c) snap[c] = s->seg.ctl(c)->src_tail.load(std::memory_order_acquire);
-    const uint64_t sources_before = s->sources.load();
+    for (uint32_t c = 0; c < n_slots; ++c) drain_parked(s, c);
     // how many sources (in hand-over order) were complete BEFORE the collect below: their hits are already queued,
-    // so once that collect comes back empty they have all been routed
+    // so once that collect comes back empty they have all been routed (or parked)
     uint64_t n_complete = 0;
     if (s->be.completed) {
       uint64_t v = 0;
@@ -247,67 +273,85 @@ void dispatch_main(pp_ipc_server* s) {
     const int rc = s->be.collect(s->be.ctx, buf.data(), cap, &n, &drained);
     if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
     size_t i = 0;
-    while (i < n && !s->stop.load()) {
+    while (i < n) {
       // route a run of hits of one event in one go
       uint32_t c = ~0u;
       {
         std::lock_guard<std::mutex> g(s->map_mu);
         auto it = s->owner.find(buf[i].event_id);
-        if (it != s->owner.end()) c = it->second;
+        if (it != s->owner.end()) c = it->second.client;
       }
       size_t j = i + 1;
       while (j < n && buf[j].event_id == buf[i].event_id) ++j;
       if (c == ~0u) { s->unrouted += j - i; i = j; continue; }
+      auto& pc = s->pc[c];
       ClientCtl* ctl = s->seg.ctl(c);
-      pp_hit* ring = s->seg.hit_ring(c);
-      while (i < j && !s->stop.load()) {
-        if (ctl->state.load(std::memory_order_acquire) == kClosed) { i = j; break; }  // nobody will read them
+      const uint32_t st = ctl->state.load(std::memory_order_acquire);
+      if (st == kClosed || st == kRecycled) { s->dropped += j - i; i = j; continue; }  // nobody will read them
+      if (pc.parked.empty()) {
+        // straight into the client's ring as far as there is room ...
+        pp_hit* ring = s->seg.hit_ring(c);
         const uint64_t head = ctl->hit_head.load(std::memory_order_relaxed);
         const uint64_t space = H->hit_cap - (head - ctl->hit_tail.load(std::memory_order_acquire));
-        if (space == 0) { nap(50); continue; }  // back-pressure: the client is behind
         const size_t m = (size_t)std::min<uint64_t>(space, j - i);
         for (size_t q = 0; q < m; ++q) ring[(head + q) % H->hit_cap] = buf[i + q];
-        ctl->hit_head.store(head + m, std::memory_order_release);
+        if (m) ctl->hit_head.store(head + m, std::memory_order_release);
         s->routed += m;
         i += m;
       }
+      if (i < j) {
+        // ... the rest is parked: a client that is behind (or dead) never holds up the routing for the others
+        pc.parked.insert(pc.parked.end(), buf.begin() + (long)i, buf.begin() + (long)j);
+        pc.parked_n.store(pc.parked.size(), std::memory_order_release);
+        i = j;
+      }
     }
     if (n == 0) {
+      // per-client completion, block by block: a client drains without waiting for the others.  A block is complete
+      // once the back end says so (n_complete, read before the collect that came back empty: its hits are routed).
+      std::vector<pp_ipc_server::Block> done;
       {
-        // per-client completion, block by block: a client drains without waiting for the others
         std::lock_guard<std::mutex> g(s->fifo_mu);
-        while (!s->fifo.empty() && s->fifo.front().global_end <= n_complete) {
-          const pp_ipc_server::Block b = s->fifo.front();
+        // `drained` covers back ends without a completed() call: everything handed over before the collect is done
+        const uint64_t upto = drained ? std::max<uint64_t>(n_complete, s->sources.load()) : n_complete;
+        while (!s->fifo.empty() && s->fifo.front().global_end <= upto &&
+               s->fifo.front().tail_after <= s->seg.ctl(s->fifo.front().client)->src_tail.load(std::memory_order_acquire)) {
+          done.push_back(std::move(s->fifo.front()));
           s->fifo.pop_front();
-          ClientCtl* ctl = s->seg.ctl(b.client);
-          if (b.tail_after > ctl->completed_seq.load(std::memory_order_relaxed))
-            ctl->completed_seq.store(b.tail_after, std::memory_order_release);
         }
       }
-      if (drained) {
-        for (uint32_t c = 0; c < n_slots; ++c) {
-          ClientCtl* ctl = s->seg.ctl(c);
-          if (snap[c] > ctl->completed_seq.load(std::memory_order_relaxed))
-            ctl->completed_seq.store(snap[c], std::memory_order_release);
-        }
-        // Forget the event owners once nothing can still produce a hit: the back end was drained at the collect
-        // above, and no block has been announced or ingested since the snapshot taken before it (the ingest thread
-        // needs map_mu to announce, so it cannot slip in while the map is cleared).
+      if (!done.empty()) {
         std::lock_guard<std::mutex> g(s->map_mu);
-        if (s->ingest_busy.load() == 0 && s->sources.load() == sources_before) {
-          s->owner.clear();
-          // the server is dry: slots of clients that have left can be handed out again.  The ring counters are
-          // absolute and simply carry on; hits the old client never read are skipped.
-          std::lock_guard<std::mutex> gf(s->fifo_mu);
-          if (s->fifo.empty())
-            for (uint32_t c = 0; c < n_slots; ++c) {
-              ClientCtl* ctl = s->seg.ctl(c);
-              if (ctl->state.load(std::memory_order_acquire) != kClosed) continue;
-              if (ctl->src_head.load(std::memory_order_acquire) != ctl->src_tail.load(std::memory_order_acquire)) continue;
-              ctl->hit_tail.store(ctl->hit_head.load(std::memory_order_relaxed), std::memory_order_release);
-              ctl->state.store(kRecycled, std::memory_order_release);
-            }
+        for (const auto& b : done)
+          for (uint32_t e : b.events) {
+            auto it = s->owner.find(e);
+            if (it != s->owner.end() && it->second.client == b.client && --it->second.blocks == 0) s->owner.erase(it);
+          }
+      }
+      for (const auto& b : done) {
+        auto& pc = s->pc[b.client];
+        pc.pending_completed = std::max(pc.pending_completed, b.tail_after);
+        pc.blocks_in_flight--;
+        drain_parked(s, b.client);
+      }
+      // a slot is handed out again once its client has left and nothing of it is in the server any more.  The ring
+      // counters are absolute and simply carry on; hits the old client never read are skipped.
+      for (uint32_t c = 0; c < n_slots; ++c) {
+        ClientCtl* ctl = s->seg.ctl(c);
+        if (ctl->state.load(std::memory_order_acquire) != kClosed) continue;
+        auto& pc = s->pc[c];
+        if (!pc.parked.empty()) { s->dropped += pc.parked.size(); pc.parked.clear(); pc.parked_n.store(0); }
+        if (pc.blocks_in_flight.load() != 0) continue;
+        const uint64_t head = ctl->src_head.load(std::memory_order_acquire);
+        if (head != ctl->src_tail.load(std::memory_order_acquire)) {
+          // sources it shipped and the server never took: nobody wants their hits
+          ctl->src_tail.store(head, std::memory_order_release);
         }
+        ctl->hit_tail.store(ctl->hit_head.load(std::memory_order_relaxed), std::memory_order_release);
+        ctl->flushed_seq.store(ctl->flush_seq.load(std::memory_order_relaxed), std::memory_order_relaxed);
+        pc.pending_completed = 0;
+        ctl->pid.store(0, std::memory_order_relaxed);
+        ctl->state.store(kRecycled, std::memory_order_release);
       }
       nap(100);
     }
@@ -334,11 +378,6 @@ int map_segment(const char* name, bool create, size_t bytes, Segment* seg) {
 
 extern "C" {
 
-const pp_ipc_backend* pp_ipc_echo_backend(void) {
-  auto* be = new pp_ipc_backend{new Echo(), e_submit, e_flush, e_collect, e_completed};  // lives as long as the process
-  return be;
-}
-
 int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name, const pp_ipc_config* cfg,
                                  pp_ipc_server** out) {
   if (!be || !be->submit || !be->flush || !be->collect || !shm_name || shm_name[0] != '/' || !out) return PP_E_INVAL;
@@ -362,6 +401,8 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
   H->client_stride = stride; H->total_bytes = total;
   for (uint32_t c = 0; c < max_clients; ++c) new (s->seg.ctl(c)) ClientCtl();  // ftruncate zero-filled the rings
   H->next_slot.store(0);
+  s->pc = std::vector<pp_ipc_server::PerClient>(max_clients);
+  s->park_cap = 4 * hit_cap;
   H->magic = kMagic;
   H->server_alive.store(1, std::memory_order_release);
   if (s->be.completed) s->be.completed(s->be.ctx, &s->base_completed);  // the back end must be drained at this point
@@ -393,6 +434,11 @@ int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out) {
   out->clients_attached = std::min(s->seg.hdr()->next_slot.load(), s->seg.hdr()->max_clients);
   out->blocks_ingested = s->blocks.load(); out->sources_ingested = s->sources.load();
   out->hits_routed = s->routed.load(); out->hits_unrouted = s->unrouted.load();
+  out->hits_dropped = s->dropped.load(); out->clients_dropped = s->clients_dropped.load();
+  {
+    std::lock_guard<std::mutex> g(s->map_mu);
+    out->events_tracked = s->owner.size();
+  }
   return s->error.load();
 }
 
@@ -420,6 +466,7 @@ int pp_ipc_client_open(const char* shm_name, pp_ipc_client** out) {
     c->seg.ctl(slot)->state.store(kAttached, std::memory_order_release);
   }
   c->slot = slot;
+  c->seg.ctl(slot)->pid.store((uint32_t)getpid(), std::memory_order_release);
   *out = c;
   return PP_OK;
 }
@@ -450,7 +497,7 @@ int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengt
     for (size_t q = 0; q < m; ++q, ++i) {
       SrcSlot& r = ring[(head + q) % H->src_cap];
       r.s = sources[i]; r.length = lengths ? lengths[i] : 0.0f; r.event_id = event_ids[i];
-      r.source_id = source_ids ? source_ids[i] : (uint32_t)i; r.pad = 0;
+      r.source_id = source_ids ? source_ids[i] : (uint32_t)(head + q); r.pad = 0;  // the client's running record number
     }
     ctl->src_head.store(head + m, std::memory_order_release);
   }

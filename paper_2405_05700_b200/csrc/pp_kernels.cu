@@ -33,7 +33,8 @@ __host__ __device__ inline unsigned long long photon_count(float energy, float y
 
 // Resident path only: build SrcRec[] from the caller's device arrays and count photons.
 __global__ void ingest_kernel(const pp_source* __restrict__ s, const uint32_t* __restrict__ ev,
-                              const uint32_t* __restrict__ sid, uint32_t n, float yield, SrcRec* __restrict__ out,
+                              const uint32_t* __restrict__ sid, uint32_t sid_base, uint32_t n, float yield,
+                              SrcRec* __restrict__ out,
                               unsigned int* __restrict__ overflow) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -42,7 +43,7 @@ __global__ void ingest_kernel(const pp_source* __restrict__ s, const uint32_t* _
   if (cnt > 0xFFFFFFFFull) { atomicExch(overflow, 1u); cnt = 0; }
   SrcRec r;
   r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
-  r.event_id = ev[i]; r.source_id = sid ? sid[i] : i; r.n_photons = (uint32_t)cnt; r.length = 0.0f;
+  r.event_id = ev[i]; r.source_id = sid ? sid[i] : sid_base + i; r.n_photons = (uint32_t)cnt; r.length = 0.0f;
   out[i] = r;
 }
 
@@ -264,7 +265,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   const float2* const s_str_xy = reinterpret_cast<const float2*>(smem_raw + P.off_str_xy);
   const uint16_t* const s_cell = reinterpret_cast<const uint16_t*>(smem_raw + P.off_cell);
   // the warp's current source record (a2): staged once per (tile, source) run, read by the lanes that refill
-  float4* const my_src = reinterpret_cast<float4*>(smem_raw + P.off_wsrc) + 3u * (threadIdx.x >> 5);
+  __shared__ float4 s_wsrc[kBlockThreads / 32][3];
+  const unsigned wslot = threadIdx.x >> 5;
 
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
@@ -305,7 +307,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           pbase = __ldg(&P.cum_rel[s_cur]);  // mod 2^32: right for the launch's first (split) source too
           run_end = min(t_end, hi);
           __syncwarp();
-          if (lane < 3u) my_src[lane] = __ldg(reinterpret_cast<const float4*>(P.src + s_cur) + lane);
+          if (lane < 3u) s_wsrc[wslot][lane] = __ldg(reinterpret_cast<const float4*>(P.src + s_cur) + lane);
           __syncwarp();
         } else {
           run_end = t_end;
@@ -316,8 +318,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
         const uint32_t r = t_next + __popc(need_mask & lt);
         if (!alive && r < run_end) {
-          const float4 r0 = my_src[0], r1 = my_src[1];
-          const uint2 r2 = *reinterpret_cast<const uint2*>(my_src + 2);
+          const float4 r0 = s_wsrc[wslot][0], r1 = s_wsrc[wslot][1];
+          const uint2 r2 = *reinterpret_cast<const uint2*>(&s_wsrc[wslot][2]);
           phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
           dx = r0.w; dy = r1.x; dz = r1.y;
           Lh = 0.0f; Ll = 0.0f;
@@ -588,10 +590,10 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
 static std::atomic<uint64_t> g_launches{0};
 uint64_t kernel_launch_count() { return g_launches.load(); }
 
-cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint32_t* d_sid, uint32_t n, float yield,
-                          SrcRec* d_out, unsigned int* d_overflow, cudaStream_t st) {
+cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint32_t* d_sid, uint32_t sid_base, uint32_t n,
+                          float yield, SrcRec* d_out, unsigned int* d_overflow, cudaStream_t st) {
   if (n == 0) return cudaSuccess;
-  ingest_kernel<<<(n + 255) / 256, 256, 0, st>>>(d_s, d_ev, d_sid, n, yield, d_out, d_overflow);
+  ingest_kernel<<<(n + 255) / 256, 256, 0, st>>>(d_s, d_ev, d_sid, sid_base, n, yield, d_out, d_overflow);
   g_launches++;
   return cudaGetLastError();
 }
@@ -643,8 +645,6 @@ cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int 
     default: return launch_prop_t<true, true, true>(P, grid, smem, st);
   }
 }
-
-int propagate_warps_per_block() { return kBlockThreads / 32; }
 
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
   // all variants are compiled for the same launch bounds; the leanest and the fullest bracket the rest

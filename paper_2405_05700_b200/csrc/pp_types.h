@@ -102,7 +102,7 @@ struct LaunchParams {
   // Image of the shared-memory tables, copied verbatim into dynamic shared memory by every CTA (smem_image_bytes, a
   // multiple of 16): [LayerRec x (n_layers + 1)] [u16 inv_b x (m_b + 1)] [u16 inv_a x (m_a + 1)]
   // [float2 line xy x (n_strings + 1)] [u16 cell x (nx ny)] [float4 line (x, y, z0, 1/pitch) x n_strings]
-  // [uint2 line (n, base) x n_strings].  After the image: one 48-byte SrcRec slot per warp (off_wsrc).
+  // [uint2 line (n, base) x n_strings].
   //  * inv_b / inv_a map a quantised cumulative depth to a layer j0 such that the layer holding that depth is j0 or
   //    j0 + 1 (or beyond, when walk_loop is set for a coarse table).
   //  * cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter disc
@@ -113,7 +113,7 @@ struct LaunchParams {
   //    clamped into the grid.
   const uint4* smem_image;
   uint32_t smem_image_bytes;
-  uint32_t off_wsrc, off_str_a, off_str_b;
+  uint32_t off_str_a, off_str_b;
   uint32_t n_layers;
   uint32_t n_strings, n_dom;
   const float4* dom_xyzw;    // [n_dom] sorted by (string, k); w = bit pattern of the public dom_id

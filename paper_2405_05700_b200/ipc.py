@@ -12,7 +12,7 @@ import numpy as np
 from .binding import HIT_DTYPE, PP_OK, PPError, load_library, pack_sources, SOURCE_DTYPE
 
 EXPORTS = ["pp_ipc_server_create", "pp_ipc_server_create_backend", "pp_ipc_server_destroy", "pp_ipc_server_get_stats",
-           "pp_ipc_echo_backend", "pp_ipc_client_open", "pp_ipc_submit", "pp_ipc_flush", "pp_ipc_collect",
+           "pp_ipc_client_open", "pp_ipc_submit", "pp_ipc_flush", "pp_ipc_collect",
            "pp_ipc_client_close"]
 
 
@@ -23,7 +23,8 @@ class _IpcConfig(C.Structure):
 
 class _IpcStats(C.Structure):
     _fields_ = [("clients_attached", C.c_uint64), ("blocks_ingested", C.c_uint64), ("sources_ingested", C.c_uint64),
-                ("hits_routed", C.c_uint64), ("hits_unrouted", C.c_uint64)]
+                ("hits_routed", C.c_uint64), ("hits_unrouted", C.c_uint64), ("hits_dropped", C.c_uint64),
+                ("clients_dropped", C.c_uint64), ("events_tracked", C.c_uint64)]
 
 
 _declared = False
@@ -42,7 +43,6 @@ def _lib():
         L.pp_ipc_server_destroy.argtypes = [vp]
         L.pp_ipc_server_get_stats.restype = C.c_int
         L.pp_ipc_server_get_stats.argtypes = [vp, C.POINTER(_IpcStats)]
-        L.pp_ipc_echo_backend.restype = vp
         L.pp_ipc_client_open.restype = C.c_int
         L.pp_ipc_client_open.argtypes = [C.c_char_p, C.POINTER(vp)]
         L.pp_ipc_submit.restype = C.c_int
@@ -58,15 +58,16 @@ def _lib():
 
 
 class IpcServer:
-    """pp_ipc_server_create over a Propagator (``propagator=None, echo=True``: the host-only echo back end)."""
+    """pp_ipc_server_create over a Propagator, or pp_ipc_server_create_backend over ``backend`` (the address of a
+    ``pp_ipc_backend`` struct that outlives the server; the CPU tests pass their host-only echo back end)."""
 
     def __init__(self, propagator, name: str, *, max_clients: int = 16, source_ring_bytes: int = 0,
-                 hit_ring_bytes: int = 0, echo: bool = False):
+                 hit_ring_bytes: int = 0, backend=None):
         self._L = _lib()
         cfg = _IpcConfig(int(max_clients), 0, int(source_ring_bytes), int(hit_ring_bytes))
         s = C.c_void_p()
-        if echo:
-            rc = self._L.pp_ipc_server_create_backend(self._L.pp_ipc_echo_backend(), name.encode(), C.byref(cfg), C.byref(s))
+        if backend is not None:
+            rc = self._L.pp_ipc_server_create_backend(C.c_void_p(backend), name.encode(), C.byref(cfg), C.byref(s))
         else:
             self._prop = propagator  # keep the handle alive
             rc = self._L.pp_ipc_server_create(propagator._h, name.encode(), C.byref(cfg), C.byref(s))

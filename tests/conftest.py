@@ -11,13 +11,27 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: longer statistical test")
-    # a fresh checkout has no binaries: build the CUDA library (nvcc cross-compiles without a GPU) and the oracle
-    # once if they are missing; an existing build is left alone (rebuild with __graft_entry__.build())
+    # build the CUDA library (nvcc cross-compiles without a GPU) and the oracle; both builders compare modification
+    # times, so an up-to-date binary is left alone and a stale one is never what the tests exercise
     from paper_2405_05700_b200 import build as pp_build
-    if not os.path.exists(pp_build.LIB):
-        pp_build.build(force=True)
+    pp_build.build()
     from oracle import oracle as O
     O.build()
+    build_echo_backend()
+
+
+ECHO_LIB = os.path.join(ROOT, "tests", "libpp_echo.so")
+
+
+def build_echo_backend() -> str:
+    """tests/libpp_echo.so: the host-only back end the CPU tests of the multi-process front end plug into
+    pp_ipc_server_create_backend (test infrastructure; not part of libpp.so)."""
+    import subprocess
+    src = os.path.join(ROOT, "tests", "echo_backend.cpp")
+    deps = [src, os.path.join(ROOT, "include", "pp_ipc.h"), os.path.join(ROOT, "include", "pp.h")]
+    if not os.path.exists(ECHO_LIB) or any(os.path.getmtime(d) > os.path.getmtime(ECHO_LIB) for d in deps):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-o", ECHO_LIB, src])
+    return ECHO_LIB
 
 
 def pytest_collection_modifyitems(config, items):

@@ -199,3 +199,30 @@ def test_c4_extreme_event_bounded_memory():
     dom_gpu = np.bincount(sub["dom_id"], minlength=geo.n_dom)
     dom_ref = np.bincount(ref.hits["dom_id"], minlength=geo.n_dom)
     assert np.abs(dom_gpu - dom_ref).sum() <= 0.05 * max(1, dom_ref.sum())
+
+
+def test_null_source_ids_are_unique_across_calls():
+    """one event shipped in two pp_submit calls with source_ids == NULL used to reuse ids 0..n-1, i.e. the
+    same Philox streams twice (duplicated hits).  NULL now means the handle's running record number."""
+    geo, ice = W.geometry_single_string(radius=2.0), W.ice_homogeneous()
+    src = W.sources_c0(seed=0, n_photons=2.0e5, toward_string=True)
+    two = np.concatenate([src.src, src.src])
+    ev = np.zeros(2, np.uint32)
+    with B.Propagator(geo, ice, seed=1) as p:
+        p.submit(two[:1], ev[:1], None)
+        p.submit(two[1:], ev[1:], None)          # the same cascade again, same event, second call
+        h = p.collect_all()
+        assert sorted(np.unique(h["source_id"])) == [0, 1]
+        a, b = h[h["source_id"] == 0], h[h["source_id"] == 1]
+        assert len(a) > 20 and len(b) > 20
+        assert not np.array_equal(np.sort(a["photon_idx"]), np.sort(b["photon_idx"]))  # independent streams
+        # explicit equal ids reproduce the collision the header warns about: identical hits twice
+        p.submit(two[:1], ev[:1], np.array([7], np.uint32))
+        p.submit(two[1:], ev[1:], np.array([7], np.uint32))
+        h2 = p.collect_all()
+        assert len(h2) % 2 == 0 and len(np.unique(h2["photon_idx"])) == len(h2) // 2
+        # the resident path numbers on from the same count
+        d = p.upload(two, ev, None)
+        p.run_resident(*d)
+        h3 = p.drain()
+        assert sorted(np.unique(h3["source_id"])) == [4, 5]

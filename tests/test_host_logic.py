@@ -174,3 +174,32 @@ def test_replica_reduction_single_process():
     from paper_2405_05700_b200 import replicas
     t, w = replicas.reduce_results(None, None, {"x": 3.0}, {"y": 4.0})
     assert t == {"x": 3.0} and w == {"y": 4.0}
+
+
+def test_roofline_constant_goes_stale_when_a_kernel_source_changes(tmp_path, monkeypatch):
+    """bench.py trusts profiles/instr_per_flight.json only for the exact kernel sources + nvcc flags it was measured
+    on (SHA-256): touching a comment in pp_kernels.cu without re-measuring must drop the roofline."""
+    import json
+    import shutil
+    import sys
+    sys.path.insert(0, ROOT) if ROOT not in sys.path else None
+    import bench
+    from paper_2405_05700_b200 import build as pp_build
+    csrc = tmp_path / "csrc"
+    csrc.mkdir()
+    for name in bench.KERNEL_SOURCES:
+        shutil.copy(os.path.join(pp_build.CSRC, name), csrc / name)
+    monkeypatch.setattr(pp_build, "CSRC", str(csrc))
+    monkeypatch.delenv("PP_NVCC_EXTRA", raising=False)
+    f = tmp_path / "instr_per_flight.json"
+    monkeypatch.setattr(bench, "INSTR_PER_FLIGHT_FILE", str(f))
+    f.write_text(json.dumps({"thread_instructions_per_flight": 321.0, "dram_bytes_per_launch": 1.0e6,
+                             "fp32_flops_per_flight": 150.0, "kernel_sources_sha256": bench.kernel_source_hash()}))
+    ipf, dram, note, fpf = bench.load_instr_per_flight()
+    assert ipf == 321.0 and dram == 1.0e6 and fpf == 150.0
+    with open(csrc / "pp_kernels.cu", "a") as g:
+        g.write("// a comment\n")
+    ipf, dram, note, fpf = bench.load_instr_per_flight()
+    assert ipf is None and "stale" in note
+    monkeypatch.setenv("PP_NVCC_EXTRA", "-DPP_MIN_BLOCKS=3")  # different flags are a different kernel too
+    assert bench.load_instr_per_flight()[0] is None

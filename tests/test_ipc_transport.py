@@ -1,5 +1,6 @@
 """The multi-process front end (include/pp_ipc.h, NEXT-3) without a GPU: client processes
-ship blocks through shared memory to a server bound to the host-only echo back end (one hit per source)."""
+ship blocks through shared memory to a server bound to the host-only echo back end of tests/echo_backend.cpp (one hit
+per source), plugged in through pp_ipc_server_create_backend."""
 import multiprocessing as mp
 import os
 
@@ -9,6 +10,24 @@ import pytest
 from paper_2405_05700_b200 import binding as B
 from paper_2405_05700_b200 import ipc
 from paper_2405_05700_b200 import workloads as W
+
+
+def _echo_lib():
+    import ctypes as C
+    from conftest import build_echo_backend
+    L = C.CDLL(build_echo_backend())
+    L.echo_backend_new.restype = C.c_void_p
+    L.echo_set_hits_per_source.argtypes = [C.c_void_p, C.c_uint32]
+    return L
+
+
+def echo_backend(hits_per_source: int = 1) -> int:
+    """Address of a fresh host-only back end (tests/echo_backend.cpp): one hit per source at the next flush."""
+    L = _echo_lib()
+    be = L.echo_backend_new()
+    if hits_per_source != 1:
+        L.echo_set_hits_per_source(be, hits_per_source)
+    return be
 
 
 def _sources(client: int, n_events: int, per_event: int):
@@ -62,7 +81,7 @@ def test_clients_get_exactly_their_events_back(n_clients, ring_kib):
     q = ctx.Queue()
     n_events, per_event, block = 20, 37, 111
     with ipc.IpcServer(None, name, max_clients=n_clients, source_ring_bytes=ring_kib * 1024,
-                       hit_ring_bytes=ring_kib * 1024, echo=True) as srv:
+                       hit_ring_bytes=ring_kib * 1024, backend=echo_backend()) as srv:
         procs = [ctx.Process(target=_client_main, args=(name, c, n_events, per_event, block, q)) for c in range(n_clients)]
         for p in procs:
             p.start()
@@ -85,9 +104,9 @@ def test_open_errors_and_slot_limit():
         ipc.IpcClient(f"/pp_ipc_nobody_{os.getpid()}")
     assert e.value.code == -7  # PP_E_STATE: no server
     name = f"/pp_ipc_test_{os.getpid()}_lim"
-    with ipc.IpcServer(None, name, max_clients=2, echo=True):
+    with ipc.IpcServer(None, name, max_clients=2, backend=echo_backend()):
         with pytest.raises(B.PPError):
-            ipc.IpcServer(None, name, echo=True)  # the segment exists already
+            ipc.IpcServer(None, name, backend=echo_backend())  # the segment exists already
         a, b = ipc.IpcClient(name), ipc.IpcClient(name)
         with pytest.raises(B.PPError) as e:
             ipc.IpcClient(name)
@@ -111,7 +130,7 @@ def test_a_client_drains_without_waiting_for_the_others():
     """Steady state (clients keep queueing steps): client A must see its own work drained while client B
     still has a block in the server that nobody flushed."""
     name = f"/pp_ipc_test_{os.getpid()}_own"
-    with ipc.IpcServer(None, name, max_clients=2, echo=True) as srv:
+    with ipc.IpcServer(None, name, max_clients=2, backend=echo_backend()) as srv:
         a, b = ipc.IpcClient(name), ipc.IpcClient(name)
         sa, ea, ia, la = _sources(0, 5, 11)
         sb, eb, ib, lb = _sources(1, 3, 7)
@@ -140,7 +159,7 @@ def test_slots_are_recycled():
     server has run dry."""
     import time
     name = f"/pp_ipc_test_{os.getpid()}_recycle"
-    with ipc.IpcServer(None, name, max_clients=2, echo=True) as srv:
+    with ipc.IpcServer(None, name, max_clients=2, backend=echo_backend()) as srv:
         keep = ipc.IpcClient(name)
         for round_ in range(5):
             c = None
@@ -170,7 +189,7 @@ def test_server_gone_and_client_gone():
     hits does not wedge the server (its hits are dropped), and the other client still drains."""
     name = f"/pp_ipc_test_{os.getpid()}_gone"
     src, ev, sid, ln = _sources(0, 4, 50)
-    srv = ipc.IpcServer(None, name, max_clients=2, hit_ring_bytes=32 * 8, echo=True)  # hit ring of 8 hits
+    srv = ipc.IpcServer(None, name, max_clients=2, hit_ring_bytes=32 * 8, backend=echo_backend())  # hit ring of 8 hits
     a, b = ipc.IpcClient(name), ipc.IpcClient(name)
     a.submit(src, ev, sid, ln)          # 200 hits will come back into a ring of 8 ...
     a.flush()
@@ -202,3 +221,110 @@ def test_ipc_symbols_are_exported():
     for s in declared:
         assert hasattr(lib, s), s
     assert declared == set(ipc.EXPORTS)
+
+
+def _stuck_client_main(name, q):
+    """Ships work whose hits overflow its hit ring many times over, reads nothing, reports its pid and waits to be
+    killed (jobs die at their memory limit)."""
+    import time
+    src, ev, sid, ln = _sources(7, 4, 50)
+    c = ipc.IpcClient(name)
+    c.submit(src, ev, sid, ln)
+    c.flush()
+    q.put(os.getpid())
+    time.sleep(600)
+
+
+def test_a_killed_client_with_a_full_hit_ring_does_not_wedge_the_server():
+    """a client that dies without closing (SIGKILL) while its hit ring is full used to stall the dispatch
+    thread for ever.  Its hits are parked, the others are served meanwhile, and once its process is gone the server
+    drops them and hands the slot out again."""
+    import signal
+    import time
+    name = f"/pp_ipc_test_{os.getpid()}_kill"
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    # hit ring of 8 hits; every source echoes 40 hits: 200 sources -> 8000 hits against a ring of 8
+    with ipc.IpcServer(None, name, max_clients=2, hit_ring_bytes=32 * 8, backend=echo_backend(40)) as srv:
+        p = ctx.Process(target=_stuck_client_main, args=(name, q))
+        p.start()
+        pid = q.get(timeout=60)
+        b = ipc.IpcClient(name)
+        s2, e2, i2, l2 = _sources(1, 3, 20)
+        t0 = time.time()
+        b.submit(s2, e2, i2, l2)
+        got = b.collect_all()                       # served although the other client's ring is full and unread
+        assert len(got) == 40 * len(e2) and time.time() - t0 < 20
+        assert set(np.unique(got["event_id"])) == set(np.unique(e2))
+        os.kill(pid, signal.SIGKILL)
+        p.join(timeout=30)
+        c = None
+        for _ in range(400):                        # the dead client's slot comes back
+            try:
+                c = ipc.IpcClient(name)
+                break
+            except B.PPError as e:
+                assert e.code == -2
+                time.sleep(0.01)
+        assert c is not None, "the slot of the killed client was never recycled"
+        s3, e3, i3, l3 = _sources(2, 2, 5)
+        c.submit(s3, e3 + np.uint32(9000), i3, l3)
+        assert len(c.collect_all()) == 40 * len(e3)
+        st = srv.stats()
+        assert st["error"] == 0 and st["clients_dropped"] == 1 and st["hits_dropped"] > 0 and st["hits_unrouted"] == 0
+        b.close(), c.close()
+
+
+def test_owner_table_and_slots_stay_bounded_while_the_server_never_runs_dry():
+    """in steady state the server as a whole never runs dry.  One client keeps a block in the
+    server at all times (shipped, never flushed by itself) while others come and go: their events must leave the
+    owner table when their blocks complete, and their slots must be handed out again."""
+    import time
+    name = f"/pp_ipc_test_{os.getpid()}_busy"
+    with ipc.IpcServer(None, name, max_clients=2, backend=echo_backend()) as srv:
+        keep = ipc.IpcClient(name)
+        sk, ek, ik, lk = _sources(9, 2, 5)
+        n_keep = 0
+        for round_ in range(12):
+            keep.submit(sk, ek + np.uint32(50000 + 10 * round_), ik, lk)   # keeps the server from running dry
+            n_keep += len(ek)
+            c = None
+            for _ in range(400):
+                try:
+                    c = ipc.IpcClient(name)
+                    break
+                except B.PPError as e:
+                    assert e.code == -2
+                    time.sleep(0.005)
+            assert c is not None, f"round {round_}: slot not recycled while another client keeps the server busy"
+            src, ev, sid, ln = _sources(round_ % 5, 30, 3)
+            ev = ev + np.uint32(100000 * (round_ + 1))
+            c.submit(src, ev, sid, ln)
+            got = np.sort(c.collect_all(), order=["event_id", "source_id"])   # its flush also launches keep's block
+            assert np.array_equal(got, _expected(src, ev, sid, ln))
+            c.close()
+            st = srv.stats()
+            # at most: this round's 30 events (about to be forgotten) + the keeper's outstanding events
+            assert st["events_tracked"] <= 30 + 2 * (round_ + 1), st
+        assert len(keep.collect_all()) == n_keep
+        for _ in range(200):
+            if srv.stats()["events_tracked"] == 0:
+                break
+            time.sleep(0.005)
+        st = srv.stats()
+        assert st["events_tracked"] == 0 and st["error"] == 0 and st["clients_attached"] == 2
+        keep.close()
+
+
+def test_null_source_ids_do_not_collide_across_submits():
+    """with source_ids == NULL two blocks of one event must not reuse ids 0..n-1 (identical Philox
+    streams): the client's running record number is used."""
+    name = f"/pp_ipc_test_{os.getpid()}_null"
+    with ipc.IpcServer(None, name, max_clients=1, backend=echo_backend()) as srv:
+        with ipc.IpcClient(name) as c:
+            src, ev, sid, ln = _sources(0, 1, 20)
+            c.submit(src[:10], ev[:10], None, ln[:10])
+            c.submit(src[10:], ev[10:], None, ln[10:])
+            got = c.collect_all()
+        assert len(got) == 20 and len(np.unique(got["source_id"])) == 20
+        assert srv.stats()["error"] == 0
