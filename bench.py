@@ -597,6 +597,53 @@ def run_stream_ipc(args):
     return 0
 
 
+def run_multi(args):
+    """`python bench.py --gpus N` WITHOUT torchrun: ONE server process, N devices behind one front (include/pp_multi.h,
+    NEXT-4): C1 is shipped through pp_multi_submit, dealt in batches of 1e8 photons to the least-loaded device, and
+    collected through one pp_multi_collect.  Prints the contract's JSON line (value = whole-job photons/s; wall clock
+    between the first submit and the drain, host buffers in and out).  With `--same-device` all N handles sit on
+    cuda:0 (what a 1-GPU box can run: checks the plumbing, says nothing about scaling)."""
+    import torch
+    from paper_2405_05700_b200 import multi
+    n = args.gpus
+    have = torch.cuda.device_count()
+    devices = [0] * n if args.same_device else list(range(n))
+    if not args.same_device and have < n:
+        raise SystemExit(f"bench.py: --gpus {n} but only {have} CUDA devices (use --same-device for a plumbing check)")
+    geo, ice, src = workload()
+    target = 10 ** 8
+    with multi.MultiFront.over_devices(geo, ice, devices, seed=0, launch_photons_target=target, deal_photons=target) as m:
+        for _ in range(args.warmup):
+            m.run(src.src, src.event_id, src.source_id)
+        for d in set(devices):
+            torch.cuda.synchronize(d)
+        st0 = [p.stats() for p in m._props]
+        hits = 0
+        with ClockSampler(0) as clk:
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                hits += len(m.run(src.src, src.event_id, src.source_id))
+            wall = time.perf_counter() - t0
+        st1 = [p.stats() for p in m._props]
+        mst = m.stats()
+    ph = sum(b.photons_done - a.photons_done for a, b in zip(st0, st1))
+    busy = [(b.kernel_busy_ms - a.kernel_busy_ms) * 1e-3 for a, b in zip(st0, st1)]
+    print(json.dumps({"metric": METRIC, "value": ph / wall, "unit": UNIT, "n_gpus": n, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps, "higher_is_better": True,
+                      "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": WORKLOAD, "parallelism": f"one server process, {n} devices behind one front "
+                                 "(pp_multi.h): replicas only, no collective", "devices": devices,
+                                 "deal_photons": target, "photons_per_step": ph / args.steps},
+                      "device_busy_frac_per_device": [b / wall for b in busy],
+                      "photons_per_device": [b.photons_done - a.photons_done for a, b in zip(st0, st1)],
+                      "batches_per_device": mst["batches"], "hits_per_step": hits / args.steps,
+                      "e2e": {"value": ph / wall, "unit": UNIT, "h2d_bytes_per_step": int(len(src) * 48),
+                              "d2h_bytes_per_step": int(hits / args.steps * 32)},
+                      "gpu_launches": int(sum(b.launches - a.launches for a, b in zip(st0, st1))),
+                      "clocks": clk.summary(), "roofline": None, "cpu_baseline": None}))
+    return 0
+
+
 def run_c4(args):
     """BASELINE.json configs[4]: one 1e8 GeV bundle (500 muons, ~5e9 photons) with the hit ring capped at 2 GB, and
     the same event with a 256 KiB ring (stop/replay relaunches all the time): time, device memory, hits."""
@@ -671,6 +718,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--same-device", action="store_true",
+                    help="with --gpus N and no torchrun: put all N handles of the multi-device front on cuda:0")
     ap.add_argument("--no-server-leg", action="store_true", help="skip the device-busy-through-the-server leg")
     ap.add_argument("--update-instr-per-flight", default="", metavar="NCU_CSV",
                     help="store profiles/instr_per_flight.json from an ncu --csv log (see update_instr_per_flight)")
@@ -700,6 +749,8 @@ def main():
         return run_sweep(args)
     if args.stream:
         return run_stream_ipc(args) if args.ipc_clients > 0 else run_stream(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return run_multi(args)  # one server process, N devices (NEXT-4); under torchrun: N independent replicas
     return run_ours(args)
 
 

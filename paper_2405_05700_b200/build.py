@@ -12,9 +12,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpp.so")
-SOURCES = ["pp_kernels.cu", "pp_api.cpp", "pp_ipc.cpp"]
+SOURCES = ["pp_kernels.cu", "pp_api.cpp", "pp_ipc.cpp", "pp_multi.cpp"]
 DEPS = SOURCES + ["pp_device.cuh", "pp_types.h", "pp_internal.h", os.path.join("..", "..", "include", "pp.h"),
-                  os.path.join("..", "..", "include", "pp_ipc.h")]
+                  os.path.join("..", "..", "include", "pp_ipc.h"), os.path.join("..", "..", "include", "pp_multi.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

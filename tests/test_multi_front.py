@@ -1,0 +1,123 @@
+"""Several devices behind one server (include/pp_multi.h, NEXT-4) without a GPU: the front deals
+batches to host-only echo back ends (tests/echo_backend.cpp), one per "device"."""
+import os
+import re
+import threading
+
+import numpy as np
+import pytest
+
+from paper_2405_05700_b200 import binding as B
+from paper_2405_05700_b200 import ipc
+from paper_2405_05700_b200 import multi
+
+from test_ipc_transport import _expected, _sources, echo_backend
+
+ORDER = ["event_id", "source_id"]
+
+
+def test_multi_symbols_are_exported():
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(root, "include", "pp_multi.h")).read(), flags=re.S)
+    declared = set(re.findall(r"\b(pp_multi_[a-z_]+)\s*\(", hdr))
+    lib = B.load_library()
+    for s in declared:
+        assert hasattr(lib, s), s
+    assert declared == set(multi.EXPORTS)
+
+
+@pytest.mark.parametrize("n_dev", [1, 2, 3])
+def test_every_source_comes_back_once_and_the_load_is_shared(n_dev):
+    src, ev, sid, ln = _sources(0, 40, 25)               # 1000 sources of 1e3-1e5 photons
+    tot = sum(B.photon_count(e) for e in src[:, 7])
+    with multi.MultiFront(backends=[echo_backend() for _ in range(n_dev)], photons_per_GeV=1.0e4,
+                          deal_photons=tot // 20) as m:
+        got = []
+        for a in range(0, len(ev), 90):                   # blocks that do not line up with the batches
+            m.submit(src[a:a + 90], ev[a:a + 90], sid[a:a + 90], ln[a:a + 90])
+            got.append(m.collect(block=False).copy())
+        got.append(m.collect_all())
+        st = m.stats()
+    hits = np.sort(np.concatenate(got), order=ORDER)
+    assert np.array_equal(hits, _expected(src, ev, sid, ln))
+    assert st["sources_submitted"] == st["sources_completed"] == 1000 and st["sources_staged"] == 0
+    assert st["photons_submitted"] == tot == sum(st["photons"]) and st["photons_outstanding"] == [0] * n_dev
+    assert sum(st["batches"]) >= 19
+    if n_dev > 1:
+        # the echo back end completes a batch at once, so all devices look idle and the first one would get
+        # everything if ties were not the only thing deciding; what must hold: nobody got more than everything
+        assert max(st["photons"]) <= tot
+
+
+def test_least_loaded_device_gets_the_next_batch():
+    """Back end 0 never completes anything until flushed by hand (its flush is a no-op here): the front must send the
+    following batches to the other device."""
+    import ctypes as C
+    be0, be1 = echo_backend(), echo_backend()
+    # wrap back end 0 so that its flush does nothing: its batches stay outstanding
+    b0 = multi.Backend()
+    C.memmove(C.byref(b0), C.c_void_p(be0), C.sizeof(multi.Backend))
+    real_flush = b0.flush
+    NOFLUSH = C.CFUNCTYPE(C.c_int, C.c_void_p)(lambda ctx: 0)
+    b0.flush = C.cast(NOFLUSH, C.c_void_p).value
+    src, ev, sid, ln = _sources(1, 10, 10)
+    tot = sum(B.photon_count(e) for e in src[:, 7])
+    with multi.MultiFront(backends=[C.addressof(b0), be1], photons_per_GeV=1.0e4, deal_photons=tot // 10) as m:
+        m.submit(src, ev, sid, ln)
+        m.flush()
+        st = m.stats()
+        assert st["batches"][0] == 1 and st["batches"][1] >= 8, st      # one batch stuck on device 0, the rest on 1
+        assert st["photons_outstanding"][0] > 0 and st["photons_outstanding"][1] == 0
+        assert st["sources_completed"] == 0                               # the FIRST batch is the stuck one
+        # release device 0
+        C.CFUNCTYPE(C.c_int, C.c_void_p)(real_flush)(b0.ctx)
+        hits = np.sort(np.concatenate([m.collect_all()]), order=ORDER)
+        assert np.array_equal(hits, _expected(src, ev, sid, ln))
+        assert m.stats()["sources_completed"] == 100
+
+
+def test_null_ids_are_numbered_by_the_front_and_submit_is_thread_safe():
+    src, ev, sid, ln = _sources(2, 8, 50)
+    with multi.MultiFront(backends=[echo_backend(), echo_backend()], photons_per_GeV=1.0e4, deal_photons=10 ** 6) as m:
+        def work(t):
+            for a in range(t * 100, (t + 1) * 100, 20):
+                m.submit(src[a:a + 20], ev[a:a + 20], None, ln[a:a + 20])
+        th = [threading.Thread(target=work, args=(t,)) for t in range(4)]
+        [t.start() for t in th]
+        [t.join() for t in th]
+        hits = m.collect_all()
+    assert len(hits) == 400 and sorted(hits["source_id"]) == list(range(400))   # unique across devices and calls
+
+
+def test_front_rejects_bad_input():
+    with pytest.raises(B.PPError):
+        multi.MultiFront(backends=[], photons_per_GeV=1.0e4)
+    with pytest.raises(B.PPError):
+        multi.MultiFront(backends=[echo_backend()], photons_per_GeV=0.0)
+    with multi.MultiFront(backends=[echo_backend()], photons_per_GeV=1.0e4) as m:
+        src, ev, sid, ln = _sources(3, 1, 2)
+        big = src.copy()
+        big[0, 7] = 1.0e9                                  # 1e13 photons: more than 2^32 - 1 in one source
+        with pytest.raises(B.PPError) as e:
+            m.submit(big, ev, sid, ln)
+        assert e.value.code == -4 and m.stats()["sources_submitted"] == 0   # nothing was staged
+        assert len(m.collect(block=True)) == 0             # nothing outstanding: drained at once
+
+
+def test_client_processes_in_front_of_two_devices():
+    """pp_multi_backend: the multi-process server (pp_ipc.h) drives the front, which drives two "devices"."""
+    name = f"/pp_multi_test_{os.getpid()}"
+    with multi.MultiFront(backends=[echo_backend(), echo_backend()], photons_per_GeV=1.0e4, deal_photons=3 * 10 ** 5) as m:
+        with ipc.IpcServer(None, name, max_clients=2, backend=m.backend_address()) as srv:
+            a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+            sa, ea, ia, la = _sources(0, 6, 30)
+            sb, eb, ib, lb = _sources(1, 4, 45)
+            a.submit(sa, ea, ia, la)
+            b.submit(sb, eb, ib, lb)
+            ga = np.sort(a.collect_all(), order=ORDER)
+            gb = np.sort(b.collect_all(), order=ORDER)
+            assert np.array_equal(ga, _expected(sa, ea, ia, la)) and np.array_equal(gb, _expected(sb, eb, ib, lb))
+            assert srv.stats()["error"] == 0 and srv.stats()["hits_unrouted"] == 0
+            a.close(), b.close()
+        st = m.stats()
+        assert sum(st["batches"]) >= 2 and st["sources_completed"] == 360
