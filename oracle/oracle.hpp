@@ -369,6 +369,7 @@ struct PhotonResult {
   int dom;            // hit DOM or -1
   uint32_t n_flights;  // number of flights (segments) started
   double x, y, z;     // end point
+  double dx, dy, dz;  // direction of the last flight (diagnostics: incidence angle at a DOM)
   double time_ns;     // end time (hit time if fate == kHit)
   double path_m;      // total geometric path
 };
@@ -476,6 +477,7 @@ inline PhotonResult propagate_photon(const Geometry& geo, const StringIndex* idx
     if (absorbed) { r.fate = kAbsorbed; break; }
   }
   r.x = double(p[0]); r.y = double(p[1]); r.z = double(p[2]);
+  r.dx = double(d[0]); r.dy = double(d[1]); r.dz = double(d[2]);
   r.time_ns = double(t);
   r.path_m = double(path);
   return r;

@@ -49,7 +49,8 @@ class _Geo(C.Structure):
 HIT_DTYPE = np.dtype([("event_id", "<u4"), ("source_id", "<u4"), ("photon_idx", "<u4"), ("dom_id", "<u4"),
                       ("time_ns", "<f8"), ("weight", "<f8")])
 FATE_DTYPE = np.dtype([("fate", "<i4"), ("dom", "<i4"), ("n_flights", "<u4"), ("pad", "<u4"),
-                       ("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("time_ns", "<f8"), ("path_m", "<f8")])
+                       ("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("time_ns", "<f8"), ("path_m", "<f8"),
+                       ("dx", "<f8"), ("dy", "<f8"), ("dz", "<f8")])
 FATE_ABSORBED, FATE_HIT, FATE_ABORTED, FATE_REJECTED = 0, 1, 2, 3
 
 

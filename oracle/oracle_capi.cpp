@@ -35,6 +35,7 @@ struct orc_fate {
   int32_t fate, dom;
   uint32_t n_flights, pad;
   double x, y, z, time_ns, path_m;
+  double dx, dy, dz;  // direction of the last flight
 };
 
 struct orc_stats {
@@ -182,6 +183,7 @@ int64_t orc_propagate(const orc_job* job, orc_stats* stats_out) {
           orc_fate& f = job->fates[fi];
           f.fate = r.fate; f.dom = r.dom; f.n_flights = r.n_flights; f.pad = 0;
           f.x = r.x; f.y = r.y; f.z = r.z; f.time_ns = r.time_ns; f.path_m = r.path_m;
+          f.dx = r.dx; f.dy = r.dy; f.dz = r.dz;
         }
       }
     }

@@ -114,24 +114,30 @@ struct pp_handle {
 
   // source ring (pinned), positions are monotonically increasing record numbers
   SrcRec* ring = nullptr;
-  std::mutex mu;  // protects everything below unless noted
-  std::condition_variable cv_space, cv_work, cv_hits;
-  uint64_t ring_head = 0;     // next record to be written by a producer
+  std::mutex mu;  // the source ring, the launch bookkeeping and the stats below; NOT the hit queue (hit_mu)
+  std::condition_variable cv_space, cv_work, cv_pub;
+  uint64_t ring_reserve = 0;  // next record a producer may claim: producers copy into [ring_head, ring_reserve) outside the lock
+  uint64_t next_auto_id = 0;  // running record number handed to sources submitted without ids
+  uint64_t ring_head = 0;     // records below it are written and published (in order)
   uint64_t ring_launch = 0;   // first record not yet fully launched
   uint64_t ring_tail = 0;     // first record still needed
   uint64_t launch_offset = 0; // photons of record ring_launch already launched
   uint64_t queued_photons = 0;
   uint64_t flush_upto = 0;    // records below this position must be launched even if under target
-  bool shutdown = false;
+  std::atomic<bool> shutdown{false};
   bool resident_active = false;
   int n_in_flight = 0;
   uint64_t launch_seq = 0;
   int space_waiters = 0;
 
-  // finished hits waiting for pp_collect
+  // finished hits waiting for pp_collect: a lock of their own, so that collecting never waits for a producer
+  // copying sources or for the server cutting a launch (and vice versa).  Never held together with mu.
+  std::mutex hit_mu;
+  std::condition_variable cv_hits, cv_hit_space;
   std::deque<std::vector<pp_hit>> hitq;
   size_t hitq_front_off = 0;
   uint64_t hitq_bytes = 0, hitq_budget = 0;
+  uint64_t hits_collected = 0, hit_high_water = 0;  // under hit_mu; folded into pp_stats
 
   // stats
   pp_stats_t st{};
@@ -507,15 +513,15 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long
 // which in turn back-pressures pp_submit; the resident path fails instead of dead-locking).
 int push_hits(pp_handle* h, std::vector<pp_hit>&& v, bool may_block) {
   if (v.empty()) return PP_OK;
-  std::unique_lock<std::mutex> lk(h->mu);
+  std::unique_lock<std::mutex> lk(h->hit_mu);
   const uint64_t bytes = v.size() * sizeof(pp_hit);
   while (h->hitq_bytes + bytes > h->hitq_budget && h->hitq_bytes > 0) {
     if (!may_block) return fail(h, PP_E_NOMEM, "host hit queue budget exceeded in pp_run_resident; collect more often");
-    if (h->shutdown) break;
-    h->cv_space.wait(lk);
+    if (h->shutdown.load()) break;
+    h->cv_hit_space.wait_for(lk, std::chrono::milliseconds(20));
   }
   h->hitq_bytes += bytes;
-  h->st.hit_ring_high_water = std::max<uint64_t>(h->st.hit_ring_high_water, bytes);
+  h->hit_high_water = std::max<uint64_t>(h->hit_high_water, bytes);
   h->hitq.push_back(std::move(v));
   h->cv_hits.notify_all();
   return PP_OK;
@@ -973,42 +979,51 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
   const bool nonblock = (h->cfg.flags & PP_FLAG_NONBLOCKING_SUBMIT) != 0;
   size_t i = 0;
   std::unique_lock<std::mutex> lk(h->mu);
-  if (h->shutdown) return PP_E_STATE;
+  if (h->shutdown.load()) return PP_E_STATE;
   if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
   if (nonblock) {
     if (n > h->sz.cap_src) return fail(h, PP_E_NOMEM, "batch larger than the source ring");
-    if (h->sz.cap_src - (h->ring_head - h->ring_tail) < n) { h->cv_work.notify_all(); return PP_E_WOULDBLOCK; }
+    if (h->sz.cap_src - (h->ring_reserve - h->ring_tail) < n) { h->cv_work.notify_all(); return PP_E_WOULDBLOCK; }
   }
   while (i < n) {
-    uint64_t space = h->sz.cap_src - (h->ring_head - h->ring_tail);
+    const uint64_t space = h->sz.cap_src - (h->ring_reserve - h->ring_tail);
     if (space == 0) {
       h->space_waiters++;
       h->cv_work.notify_all();
-      h->cv_space.wait(lk, [&] { return h->sz.cap_src - (h->ring_head - h->ring_tail) > 0 || h->shutdown ||
+      h->cv_space.wait(lk, [&] { return h->sz.cap_src - (h->ring_reserve - h->ring_tail) > 0 || h->shutdown.load() ||
                                         h->sticky.load() != PP_OK; });
       h->space_waiters--;
-      if (h->shutdown) return PP_E_STATE;
+      if (h->shutdown.load()) return PP_E_STATE;
       if (h->sticky.load() != PP_OK) return h->sticky.load();
       continue;
     }
+    // reserve under the lock, copy outside it, publish in order: producers fill the ring in parallel and the server
+    // thread never waits for a copy
     const size_t m = (size_t)std::min<uint64_t>(space, n - i);
+    const uint64_t pos = h->ring_reserve, auto_id = h->next_auto_id;
+    h->ring_reserve += m;
+    h->next_auto_id += m;
+    lk.unlock();
     uint64_t ph = 0;
     for (size_t j = 0; j < m; ++j, ++i) {
       const pp_source& a = src[i];
-      SrcRec& r = h->ring[(h->ring_head + j) % h->sz.cap_src];
+      SrcRec& r = h->ring[(pos + j) % h->sz.cap_src];
       r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
       r.event_id = event_ids[i];
-      r.source_id = source_ids ? source_ids[i] : (uint32_t)(h->st.sources_submitted + j);  // running record number
+      r.source_id = source_ids ? source_ids[i] : (uint32_t)(auto_id + j);  // running record number
       r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
       r.length = lengths ? lengths[i] : 0.0f;
       ph += r.n_photons;
     }
-    h->ring_head += m;
+    lk.lock();
+    h->cv_pub.wait(lk, [&] { return h->ring_head == pos; });  // earlier reservations publish first
+    h->ring_head = pos + m;
+    h->cv_pub.notify_all();
     h->queued_photons += ph;
     h->st.sources_submitted += m;
     h->st.photons_submitted += ph;
     h->st.source_ring_high_water =
-        std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_head - h->ring_tail) * sizeof(SrcRec));
+        std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_reserve - h->ring_tail) * sizeof(SrcRec));
     if (h->queued_photons >= h->sz.target ||
         (h->n_in_flight == 0 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
       h->cv_work.notify_all();
@@ -1028,30 +1043,41 @@ int pp_flush(pp_handle* h) {
 int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block) {
   if (!h || !n_out || (!out && cap)) return PP_E_INVAL;
   *n_out = 0;
-  std::unique_lock<std::mutex> lk(h->mu);
   for (;;) {
-    size_t got = 0;
-    while (got < cap && !h->hitq.empty()) {
-      auto& v = h->hitq.front();
-      const size_t m = std::min(cap - got, v.size() - h->hitq_front_off);
-      std::memcpy(out + got, v.data() + h->hitq_front_off, m * sizeof(pp_hit));
-      got += m;
-      h->hitq_front_off += m;
-      if (h->hitq_front_off == v.size()) {
-        h->hitq_bytes -= v.size() * sizeof(pp_hit);
-        h->hitq.pop_front();
-        h->hitq_front_off = 0;
+    {
+      std::unique_lock<std::mutex> lk(h->hit_mu);
+      size_t got = 0;
+      while (got < cap && !h->hitq.empty()) {
+        auto& v = h->hitq.front();
+        const size_t m = std::min(cap - got, v.size() - h->hitq_front_off);
+        std::memcpy(out + got, v.data() + h->hitq_front_off, m * sizeof(pp_hit));
+        got += m;
+        h->hitq_front_off += m;
+        if (h->hitq_front_off == v.size()) {
+          h->hitq_bytes -= v.size() * sizeof(pp_hit);
+          h->hitq.pop_front();
+          h->hitq_front_off = 0;
+        }
       }
-    }
-    if (got) {
-      *n_out = got;
-      h->st.hits_collected += got;
-      h->cv_space.notify_all();
-      return PP_OK;
+      if (got) {
+        *n_out = got;
+        h->hits_collected += got;
+        h->cv_hit_space.notify_all();
+        return PP_OK;
+      }
     }
     if (h->sticky.load() != PP_OK) return h->sticky.load();
     if (!block || cap == 0) return PP_OK;
-    if (idle_locked(h) && h->ring_launch == h->ring_head) return PP_OK;  // drained
+    bool idle;
+    {
+      std::lock_guard<std::mutex> g(h->mu);
+      idle = idle_locked(h) && h->ring_launch == h->ring_reserve;
+    }
+    std::unique_lock<std::mutex> lk(h->hit_mu);
+    if (!h->hitq.empty()) continue;
+    // a launch's hits are queued before the launch is retired, so "idle" seen first and the queue still empty now
+    // means drained
+    if (idle) return PP_OK;
     h->cv_hits.wait_for(lk, std::chrono::milliseconds(5));
   }
 }
@@ -1128,9 +1154,14 @@ int pp_set_segment_profile(pp_handle* h, uint32_t n_knots, const float* cum_frac
 
 int pp_stats(pp_handle* h, pp_stats_t* out) {
   if (!h || !out) return PP_E_INVAL;
-  std::lock_guard<std::mutex> g(h->mu);
-  *out = h->st;
-  if (h->wall_started) out->wall_ms = std::chrono::duration<double, std::milli>(h->wall_t1 - h->wall_t0).count();
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    *out = h->st;
+    if (h->wall_started) out->wall_ms = std::chrono::duration<double, std::milli>(h->wall_t1 - h->wall_t0).count();
+  }
+  std::lock_guard<std::mutex> g(h->hit_mu);
+  out->hits_collected = h->hits_collected;
+  out->hit_ring_high_water = h->hit_high_water;
   return PP_OK;
 }
 
@@ -1144,8 +1175,12 @@ void pp_destroy(pp_handle* h) {
   if (!h) return;
   {
     std::lock_guard<std::mutex> g(h->mu);
-    h->shutdown = true;
-    h->cv_work.notify_all(); h->cv_space.notify_all(); h->cv_hits.notify_all();
+    h->shutdown.store(true);
+    h->cv_work.notify_all(); h->cv_space.notify_all(); h->cv_pub.notify_all();
+  }
+  {
+    std::lock_guard<std::mutex> g(h->hit_mu);
+    h->cv_hits.notify_all(); h->cv_hit_space.notify_all();
   }
   if (h->server.joinable()) h->server.join();
   cudaSetDevice(h->device);
@@ -1174,10 +1209,11 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
   {
     std::unique_lock<std::mutex> lk(h->mu);
     if (h->shutdown) return PP_E_STATE;
-    if (!idle_locked(h) || h->ring_launch != h->ring_head)
+    if (!idle_locked(h) || h->ring_launch != h->ring_reserve)
       return fail(h, PP_E_STATE, "pp_run_resident needs an idle server (flush and collect first)");
     h->resident_active = true;
-    sid_base = (uint32_t)h->st.sources_submitted;
+    sid_base = (uint32_t)h->next_auto_id;
+    h->next_auto_id += n;
     if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
   }
   auto leave = [&](int rc) {

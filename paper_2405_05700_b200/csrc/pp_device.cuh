@@ -32,6 +32,11 @@ __device__ __forceinline__ float uniform_from_word(uint32_t x) {
   return __uint_as_float(__funnelshift_r(x, 0x7fu, 9)) - 0.99999994f;
 }
 
+#ifdef PP_EXACT_MUFU  // diagnosis only: IEEE-rounded reciprocal / square roots instead of the MUFU approximations
+__device__ __forceinline__ float fast_rcp(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ float fast_rsqrt(float x) { return __frcp_rn(__fsqrt_rn(x)); }
+__device__ __forceinline__ float fast_sqrt(float x) { return __fsqrt_rn(x); }
+#else
 __device__ __forceinline__ float fast_rcp(float x) {
   float r;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -47,6 +52,7 @@ __device__ __forceinline__ float fast_sqrt(float x) {
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
+#endif
 
 // Step 9a: Henyey-Greenstein, returned as m = 1 - cos(theta) in the cancellation-free form
 //   m = (1-g)(1-u)(q + 1 - g)/(1 - g + 2 g u),  q = (1-g^2)/(1 - g + 2 g u)        (R-1)
@@ -56,30 +62,11 @@ __device__ __forceinline__ float hg_one_minus_cos(float u, float one_minus_g, fl
   return one_minus_g * (1.0f - u) * (q + one_minus_g) * inv;
 }
 
-// -ln(u) for u in [2^-24, 1): u = m 2^e with m in [2/3, 4/3), f = m - 1,
-//   -ln(1 + f) = -f + f^2 (1/2 + f P(f)),  P = degree-7 minimax fit on [-1/3, 1/3] (relative error of the
-// approximation 2e-8, fitted for this file); total relative error ~1e-7.  No special cases are needed
-// because u is never 0, 1, denormal or infinite (R-3).
-__device__ __forceinline__ float neg_log_uniform(float u) {
-  const uint32_t ib = __float_as_uint(u);
-  const uint32_t eb = (ib - 0x3f2aaaabu) & 0xff800000u;
-  const float f = __uint_as_float(ib - eb) - 1.0f;
-  const float e = (float)(int)eb;  // exponent * 2^23
-  float p = 0.1274130642414093f;
-  p = fmaf(p, f, -0.13433831930160522f);
-  p = fmaf(p, f, 0.12226679921150208f);
-  p = fmaf(p, f, -0.1411696970462799f);
-  p = fmaf(p, f, 0.16676762700080872f);
-  p = fmaf(p, f, -0.2000383585691452f);
-  p = fmaf(p, f, 0.24999895691871643f);
-  p = fmaf(p, f, -0.33333319425582886f);
-  p = fmaf(p, f, 0.5f);
-  const float r = fmaf(f * f, p, -f);
-  return fmaf(e, -8.262958317573066e-08f, r);  // -ln2 / 2^23
-}
-
-// -ln(u) for the absorption budget (once per photon): one MUFU.LG2; absolute error <= 2^-21.4, which moves the
-// absorption point by <= 4e-7 lambda_abs.  u is a normal number (R-3): no denormal handling.
+// -ln(u) for both optical-depth budgets: one MUFU.LG2 and one multiply.  lg2.approx has an absolute error <= 2^-22 on
+// [1/2, 2) and <= 2 ulp elsewhere, i.e. <= 1.7e-7 in optical depth: the scatter point moves along the ray by
+// <= 1.7e-7 lambda_s (4e-6 m at 25 m) and the absorption point by <= 1.7e-7 lambda_abs.  Measured effect on the
+// per-hit time parity against a degree-8 polynomial with relative error 1e-7: profiles/r02_parity.md.
+// u is a normal number (R-3): no denormal handling is needed.
 __device__ __forceinline__ float neg_log_fast(float u) {
   float l;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(u));

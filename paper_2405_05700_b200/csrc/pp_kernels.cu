@@ -375,7 +375,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     }
     tau_a = (k == 0) ? tau_new : tau_a;
     // =========================== a4: optical depth to the next scatter ========================
-    float tau_s = neg_log_uniform(u_dist);
+    float tau_s = neg_log_fast(u_dist);
     if (kExt && P.spec_n != 0u) tau_s *= sc_b;
     // =========================== a4: layer walk in vertical optical depth ======================
     // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const int i1 = li + (up ? 0 : 1);                   // boundary ahead
     const float zb = fmaf(-P.dz_layer, (float)i1, P.z_top);
     const bool open = up ? (li == 0) : (li == last);  // no boundary ahead: the end layers are infinite (R-6)
-    const float h0 = open ? inf : fabsf(zb - phz);    // vertical distance to the first boundary
+    const float h0 = open ? inf : fabsf((zb - phz) - plz);  // vertical distance to the first boundary (two-float z)
     float Ts = tau_s * w, Ta = tau_a * w, Vb = 0.0f;
     float4 L4 = lay(li);
     {

@@ -165,6 +165,7 @@ def test_c3_launch_size_sweep_same_hits():
     o = O.propagate(geo, ice, src, seed=3, stride=8)
     c = compare_hits(ref[ref["photon_idx"] % 8 == 0], o.hits, o.photons)
     assert c["frac_all"] >= 0.999, c
+    assert c["n_union"] > 10 and (1.0 - c["frac_hit"]) * c["n_union"] <= 2.0, c  # few hits: at most two outliers
 
 
 def test_c4_extreme_event_bounded_memory():
@@ -195,6 +196,7 @@ def test_c4_extreme_event_bounded_memory():
     assert 0.9e7 < ref.photons < 1.1e7
     sub = hits[hits["photon_idx"] % 500 == 0]
     c = compare_hits(sub, ref.hits, ref.photons)
+    # ~100 hits in the subsample: too few for the 0.99 gate of the large samples (profiles/r02_parity.md)
     assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.95, c
     dom_gpu = np.bincount(sub["dom_id"], minlength=geo.n_dom)
     dom_ref = np.bincount(ref.hits["dom_id"], minlength=geo.n_dom)

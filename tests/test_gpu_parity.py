@@ -61,7 +61,7 @@ def test_c0_brute_force_lookup_equals_cell_grid(seed):
     assert np.array_equal(f_fast, f_brute)
     ref = O.propagate(geo, ice, src, seed=seed, brute_force=True)
     c = compare_hits(h_fast, ref.hits, 200000)
-    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.98, c
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.99, c
 
 
 def test_layered_full_detector_every_photon():
@@ -72,9 +72,12 @@ def test_layered_full_detector_every_photon():
     hits, fates, st = gpu_run_resident(geo, ice, src, 0, want_fates=True)
     ref = O.propagate(geo, ice, src, seed=0, want_fates=True, brute_force=True)
     assert st.photons_done == ref.photons == 180000 and st.flights == ref.flights
-    check_fates(fates, ref.fates, min_same=0.99999)
+    frac_t, n_hit = check_fates(fates, ref.fates, min_same=0.99999)
     c = compare_hits(hits, ref.hits, ref.photons)
     assert c["frac_all"] >= 0.999, c
+    # real-size DOMs: only a handful of the 1.8e5 photons hit (P ~ 4e-5), so frac_all alone would pass even if every
+    # hit time were wrong; the hits that exist must agree in time as well (at most one outlier among so few)
+    assert n_hit == c["n_union"] == len(hits) and (1.0 - frac_t) * n_hit <= 1.0, (frac_t, n_hit, c)
 
 
 def test_layered_oversized_doms_many_hits():
@@ -89,12 +92,14 @@ def test_layered_oversized_doms_many_hits():
     assert n_hit > 2000
     c = compare_hits(hits, ref.hits, ref.photons)
     assert c["frac_all"] >= 0.999, c
-    assert c["frac_hit"] >= 0.98, c  # expected ~99 % (grazing-incidence amplification)
+    assert c["frac_hit"] >= 0.99, c  # measured 0.997 (profiles/r02_parity.md)
+    assert frac_t >= 0.99
 
 
 def test_c1_full_size_sampled_against_oracle():
     """C1 at full size (~1.96e9 photons, the bench configuration and launch geometry); the oracle replays
-    the deterministic subsample photon_idx % 256 == 0 photon by photon."""
+    the deterministic subsample photon_idx % 64 == 0 photon by photon (> 1000 hits, so the per-hit gate of
+    SURVEY reading 13 applies: >= 99 % of the photons that hit agree in DOM and within 1e-3 ns)."""
     geo, ice, src = W.geometry_full(), W.ice_layered(), W.sources_c1()
     hits, st = gpu_run(geo, ice, src, 0, launch_photons_target=10 ** 8)
     n_ph = total_photons(src, ice)
@@ -102,13 +107,13 @@ def test_c1_full_size_sampled_against_oracle():
     assert st.photons_done == st.photons_absorbed + st.photons_hit == st.photons_submitted
     assert len(hits) == st.photons_hit
     assert 4.5 < st.flights / st.photons_done < 6.0
-    stride = 256
+    stride = 64
     ref = O.propagate(geo, ice, src, seed=0, stride=stride)
     sub = hits[hits["photon_idx"] % stride == 0]
     c = compare_hits(sub, ref.hits, ref.photons)
-    assert c["n_ref"] > 150
+    assert c["n_union"] > 1000
     assert c["frac_all"] >= 0.999, c
-    assert c["frac_hit"] >= 0.97, c
+    assert c["frac_hit"] >= 0.99, c
     # causality on every one of the ~8e4 hits: arrival no earlier than straight-line flight at c/n
     v = W.C_VACUUM / float(np.float32(ice.n_group))
     s = src.src[hits["source_id"]]
@@ -122,12 +127,12 @@ def test_c1_full_size_sampled_against_oracle():
 
 def test_c2_per_event_hit_lists():
     """C2 (muon-bundle events, heavy-tailed photon counts, tiny cascades) through pp_submit from 8 threads;
-    per-event hit lists against the oracle on the 60 largest + 140 random events."""
+    per-event hit lists against the oracle on every event (> 1000 hits: per-hit gate 0.99)."""
     import threading
     geo, ice, src = W.geometry_full(), W.ice_layered(), W.sources_c2()
     per_event = np.bincount(src.event_id, weights=src.src[:, 7].astype(np.float64))
     rng = np.random.default_rng(0)
-    ev_sel = np.union1d(np.argsort(per_event)[-3:], rng.choice(len(per_event), 300, replace=False))
+    ev_sel = np.arange(len(per_event))
     with B.Propagator(geo, ice, seed=2, launch_photons_target=3 * 10 ** 7, source_ring_bytes=8 << 20) as p:
         n, nt = len(src), 8
         bounds = np.linspace(0, n, nt * 8 + 1).astype(int)
@@ -148,9 +153,9 @@ def test_c2_per_event_hit_lists():
     sub = hits[np.isin(hits["event_id"], ev_sel)]
     c = compare_hits(sub, ref.hits, ref.photons)
     assert c["frac_all"] >= 0.999, c
-    assert c["n_ref"] > 30 and c["frac_hit"] >= 0.95, c
+    assert c["n_union"] > 1000 and c["frac_hit"] >= 0.99, c
     # per-event counts identical up to the rare fp32/fp64 decision flips counted above
-    for e in ev_sel[-3:]:
+    for e in np.argsort(per_event)[-3:]:
         assert abs(int((sub["event_id"] == e).sum()) - int((ref.hits["event_id"] == e).sum())) <= 2
 
 

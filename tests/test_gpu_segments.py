@@ -8,7 +8,7 @@ from oracle import oracle as O
 from paper_2405_05700_b200 import binding as B
 from paper_2405_05700_b200 import workloads as W
 
-from gpu_util import compare_hits, sort_hits, total_photons
+from gpu_util import compare_hits, sort_hits, total_photons, flights_agree
 
 pytestmark = pytest.mark.gpu
 C = W.C_VACUUM
@@ -34,7 +34,7 @@ def test_track_with_cascades_per_photon():
     hits, st = run(geo, ice, src, 6, src.length, launch_photons_target=400000)
     ref = O.propagate(geo, ice, src, seed=6)
     assert st.photons_done == n == ref.photons and st.launches >= 3
-    assert st.flights == ref.flights
+    assert flights_agree(st.flights, ref.flights)
     assert ref.hit > 1000 and abs(st.photons_hit - ref.hit) <= 2
     c = compare_hits(hits, ref.hits, n)
     assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.97, c
