@@ -2,6 +2,11 @@
 
 nvcc cross-compiles for sm_100a without a GPU; the resulting ``libpp.so`` sits next to this file
 (git-ignored, but it travels to the GPU box with the repo snapshot).
+
+Developer knob: the environment variable ``PP_NVCC_EXTRA`` is appended to the nvcc command line (e.g.
+``-DPP_MIN_BLOCKS=3`` for an occupancy experiment).  It is part of the hash ``bench.py`` stores with the measured
+instructions per flight, so a library built with extra flags never borrows the roofline constant of the default
+build.  The product build uses none.
 """
 from __future__ import annotations
 

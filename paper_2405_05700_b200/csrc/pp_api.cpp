@@ -26,6 +26,9 @@ namespace {
 
 constexpr double kC = 0.299792458;  // m/ns
 constexpr size_t kStageBytes = 4u << 20;  // pinned D2H staging chunk per slot (x2)
+constexpr size_t kHeadBytes = 128;        // the Status record sits this far in front of the hit ring (device and pinned)
+constexpr uint64_t kFirstHits = 2048;     // hits read back in the same copy as the Status record (64 KiB)
+static_assert(sizeof(Status) <= kHeadBytes, "Status must fit the ring head");
 using Clock = std::chrono::steady_clock;
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -72,7 +75,8 @@ struct Slot {
   WorkItem* d_resume[2] = {nullptr, nullptr};
   pp_hit* d_ring = nullptr;
   // pinned host
-  Status* h_status = nullptr;     // D2H target
+  Status* h_status = nullptr;     // D2H target; the first kFirstHits hits of the ring follow at kHeadBytes
+  pp_hit* h_first = nullptr;
   Status* h_status_in = nullptr;  // H2D source for relaunches
   unsigned char* h_stage[2] = {nullptr, nullptr};
   cudaEvent_t ev_h2d = nullptr, ev_k0 = nullptr, ev_k1 = nullptr, ev_done = nullptr, ev_stage[2] = {nullptr, nullptr};
@@ -262,10 +266,8 @@ void build_geometry(const pp_geometry* geo, bool brute, HostGeometry* out) {
     for (size_t j = i + 1; j < ns; ++j)
       d_min = std::min(d_min, std::hypot((double)xy[i].first - xy[j].first, (double)xy[i].second - xy[j].second));
   const double Rm = (double)geo->radius + 5e-3, slack = 0.02;
-  double L_max = 100.0;  // tuning knob PP_XY_CAP (metres)
-  if (const char* e = std::getenv("PP_XY_CAP")) { const double v = std::atof(e); if (v >= 1.0 && v <= 1.0e4) L_max = v; }
-  double cell_div = 6.0;  // tuning knob PP_CELL_DIV: cells per smallest line distance
-  if (const char* e = std::getenv("PP_CELL_DIV")) { const double v = std::atof(e); if (v >= 2.0 && v <= 64.0) cell_div = v; }
+  const double L_max = 100.0;   // longest piece of flight looked up at once (metres); measured optimum for the 125 m grid
+  const double cell_div = 6.0;  // cells per smallest line distance (finer tables gained 0.4 %: profiles/r01_v6.md)
   double cell = ns > 1 ? d_min / cell_div : 32.0;
   double L = ns > 1 ? std::min(L_max, d_min - 2.0 * (Rm + slack) - cell * std::sqrt(2.0) - slack) : L_max;
   double x0 = 1e30, x1 = -1e30, y0 = 1e30, y1 = -1e30;
@@ -444,10 +446,12 @@ uint64_t carve_device(pp_handle* h, void* base) {
     s.d_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
     s.d_cum_rel = c.take<uint32_t>(h->sz.cap_src + 1);
     s.d_tile_src = c.take<uint32_t>(h->sz.max_tiles);
-    s.d_status = c.take<Status>(1);
     s.d_resume[0] = c.take<WorkItem>(h->sz.resume_cap);
     s.d_resume[1] = c.take<WorkItem>(h->sz.resume_cap);
-    s.d_ring = c.take<pp_hit>(h->sz.ring_cap);
+    // [Status | pad to kHeadBytes | pp_hit x ring_cap]: one device-to-host copy brings the status and the first hits
+    unsigned char* sr = c.take<unsigned char>(kHeadBytes + h->sz.ring_cap * sizeof(pp_hit));
+    s.d_status = reinterpret_cast<Status*>(sr);
+    s.d_ring = reinterpret_cast<pp_hit*>(sr ? sr + kHeadBytes : nullptr);
   }
   h->d_res_src = c.take<SrcRec>(h->sz.cap_src);
   h->d_res_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
@@ -460,7 +464,9 @@ uint64_t carve_pinned(pp_handle* h, void* base) {
   h->ring = c.take<SrcRec>(h->sz.cap_src);
   for (int i = 0; i < 2; ++i) {
     Slot& s = h->slot[i];
-    s.h_status = c.take<Status>(1);
+    unsigned char* hs = c.take<unsigned char>(kHeadBytes + kFirstHits * sizeof(pp_hit));
+    s.h_status = reinterpret_cast<Status*>(hs);
+    s.h_first = reinterpret_cast<pp_hit*>(hs ? hs + kHeadBytes : nullptr);
     s.h_status_in = c.take<Status>(1);
     s.h_stage[0] = c.take<unsigned char>(kStageBytes);
     s.h_stage[1] = c.take<unsigned char>(kStageBytes);
@@ -474,10 +480,17 @@ uint64_t carve_pinned(pp_handle* h, void* base) {
 // launch engine
 // ---------------------------------------------------------------------------------------------
 
+// a9, first part: the Status record and the first kFirstHits hits of the ring in ONE device-to-host copy (they are
+// contiguous on both sides): a launch with few hits -- every small launch -- needs no second copy.
+cudaError_t read_back_head(pp_handle* h, Slot& s) {
+  const size_t bytes = kHeadBytes + (size_t)std::min<uint64_t>(kFirstHits, h->sz.ring_cap) * sizeof(pp_hit);
+  return cudaMemcpyAsync(s.h_status, s.d_status, bytes, cudaMemcpyDeviceToHost, s.stream);
+}
+
 // Enqueue tiles + propagate (+ status read-back) for photons [g_begin, g_end) of the batch
 // (src, cum, n_src), which must already be (or be enqueued to become) resident on slot.stream.
-int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long long* cum, uint32_t n_src,
-                   uint64_t g_begin, uint64_t g_end, pp_fate* fates, bool has_segments) {
+int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, unsigned long long* cum, uint32_t n_src,
+                   uint64_t g_begin, uint64_t g_end, pp_fate* fates, bool has_segments, bool need_scan) {
   const uint64_t n_ph = g_end - g_begin;
   // tile size: 1024 photons for large launches; a small launch is cut finer so that every resident warp gets work
   // (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3)
@@ -486,7 +499,14 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long
   while (tile > (uint32_t)kMinTilePhotons && n_ph / tile < want_tiles) tile >>= 1;
   const uint32_t n_tiles = (uint32_t)((n_ph + tile - 1) / tile);
   if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");
-  PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, tile, s.d_tile_src, s.d_cum_rel, s.stream));
+  // a2: prefix sums (unless the batch is scanned already), tile -> source table, launch-relative prefix sums; the
+  // status record is cleared by the same kernel.  Small launches do all of it in one single-CTA kernel.
+  if (need_scan && n_src <= kPrologueMax && n_tiles <= kPrologueMax) {
+    PP_CUDA(h, launch_prologue(src, n_src, cum, g_begin, n_tiles, tile, s.d_tile_src, s.d_cum_rel, s.d_status, s.stream));
+  } else {
+    if (need_scan) PP_CUDA(h, launch_scan(src, n_src, cum, s.stream));
+    PP_CUDA(h, launch_tiles(cum, n_src, g_begin, n_tiles, tile, s.d_tile_src, s.d_cum_rel, s.d_status, s.stream));
+  }
   LaunchParams P = h->base;
   P.src = src; P.cum = cum; P.cum_rel = s.d_cum_rel; P.tile_src = s.d_tile_src;
   P.g_begin = g_begin; P.g_end = g_end; P.n_src = n_src; P.n_tiles = n_tiles; P.tile_photons = tile;
@@ -498,11 +518,10 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, const unsigned long
   P.fates = fates;
   s.fates = fates != nullptr;
   s.P = P;
-  PP_CUDA(h, cudaMemsetAsync(s.d_status, 0, sizeof(Status), s.stream));
   PP_CUDA(h, cudaEventRecord(s.ev_k0, s.stream));
   PP_CUDA(h, launch_propagate(P, h->brute, s.fates, h->grid, h->smem, s.stream));
   PP_CUDA(h, cudaEventRecord(s.ev_k1, s.stream));
-  PP_CUDA(h, cudaMemcpyAsync(s.h_status, s.d_status, sizeof(Status), cudaMemcpyDeviceToHost, s.stream));
+  PP_CUDA(h, read_back_head(h, s));
   PP_CUDA(h, cudaEventRecord(s.ev_done, s.stream));
   s.in_flight = true;
   s.seq = ++h->launch_seq;
@@ -539,24 +558,28 @@ int finish_slot(pp_handle* h, Slot& s, bool may_block) {
   const uint64_t n_valid = std::min<uint64_t>(hs.hit_count, h->sz.ring_cap);
   std::vector<pp_hit> hits(n_valid);
   {
+    // the first hits came with the status record; the rest through the two staging chunks, two copies in flight
+    const uint64_t n_first = std::min<uint64_t>(n_valid, kFirstHits);
+    std::memcpy(hits.data(), s.h_first, n_first * sizeof(pp_hit));
     const uint64_t per = kStageBytes / sizeof(pp_hit);
-    uint64_t issued = 0, done = 0;
-    int b = 0;
+    uint64_t issued = n_first, done = n_first;
+    uint64_t n_issued = 0, n_done = 0;
     uint64_t cnt[2] = {0, 0};
     while (done < n_valid) {
-      // keep up to two chunk copies in flight
-      while (issued < n_valid && issued - done < 2 * per) {
-        const int bi = (int)((issued / per) & 1);
+      while (issued < n_valid && n_issued - n_done < 2) {
+        const int bi = (int)(n_issued & 1);
         cnt[bi] = std::min<uint64_t>(per, n_valid - issued);
         PP_CUDA(h, cudaMemcpyAsync(s.h_stage[bi], s.d_ring + issued, cnt[bi] * sizeof(pp_hit), cudaMemcpyDeviceToHost,
                                    s.stream));
         PP_CUDA(h, cudaEventRecord(s.ev_stage[bi], s.stream));
         issued += cnt[bi];
+        n_issued++;
       }
+      const int b = (int)(n_done & 1);
       PP_CUDA(h, cudaEventSynchronize(s.ev_stage[b]));
       std::memcpy(hits.data() + done, s.h_stage[b], cnt[b] * sizeof(pp_hit));
       done += cnt[b];
-      b ^= 1;
+      n_done++;
     }
   }
   {
@@ -599,7 +622,7 @@ int finish_slot(pp_handle* h, Slot& s, bool may_block) {
     PP_CUDA(h, cudaEventRecord(s.ev_k0, s.stream));
     PP_CUDA(h, launch_propagate(P, h->brute, s.fates, h->grid, h->smem, s.stream));
     PP_CUDA(h, cudaEventRecord(s.ev_k1, s.stream));
-    PP_CUDA(h, cudaMemcpyAsync(s.h_status, s.d_status, sizeof(Status), cudaMemcpyDeviceToHost, s.stream));
+    PP_CUDA(h, read_back_head(h, s));
     PP_CUDA(h, cudaEventRecord(s.ev_done, s.stream));
     std::lock_guard<std::mutex> g(h->mu);
     h->st.relaunches += 1;
@@ -736,11 +759,10 @@ void server_main(pp_handle* h) {
           if (e == cudaSuccess && first < n_src)
             e = cudaMemcpyAsync(s.d_src + first, h->ring, (n_src - first) * sizeof(SrcRec), cudaMemcpyHostToDevice, s.stream);
           if (e == cudaSuccess) e = cudaEventRecord(s.ev_h2d, s.stream);
-          if (e == cudaSuccess) e = launch_scan(s.d_src, n_src, s.d_cum, s.stream);
           if (e != cudaSuccess) rc = fail(h, PP_E_CUDA, std::string("upload: ") + cudaGetErrorString(e));
           bool seg = false;  // any track segment among the records of this launch?
           for (uint32_t q = 0; q < n_src && !seg; ++q) seg = h->ring[(rec_a + q) % cap].length > 0.0f;
-          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg);
+          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg, true);
           if (rc == PP_OK && cudaEventSynchronize(s.ev_h2d) != cudaSuccess) rc = fail(h, PP_E_CUDA, "upload sync failed");
         }
         lk.lock();
@@ -1043,6 +1065,9 @@ int pp_flush(pp_handle* h) {
 int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block) {
   if (!h || !n_out || (!out && cap)) return PP_E_INVAL;
   *n_out = 0;
+  // a blocking caller first polls for a short while (a small launch is back within ~0.1 ms, less than a sleep and
+  // wake-up costs), then sleeps on the condition variable
+  const auto spin_until = Clock::now() + std::chrono::microseconds(200);
   for (;;) {
     {
       std::unique_lock<std::mutex> lk(h->hit_mu);
@@ -1078,6 +1103,7 @@ int pp_collect(pp_handle* h, pp_hit* out, size_t cap, size_t* n_out, int block) 
     // a launch's hits are queued before the launch is retired, so "idle" seen first and the queue still empty now
     // means drained
     if (idle) return PP_OK;
+    if (Clock::now() < spin_until) { lk.unlock(); std::this_thread::yield(); continue; }
     h->cv_hits.wait_for(lk, std::chrono::milliseconds(5));
   }
 }
@@ -1257,7 +1283,7 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
     rc = drain_slot(h, s, false);
     if (rc != PP_OK) break;
     const uint64_t g1 = std::min(total, g0 + h->sz.target);
-    rc = enqueue_launch(h, s, h->d_res_src, h->d_res_cum, (uint32_t)n, g0, g1, d_fates, false);
+    rc = enqueue_launch(h, s, h->d_res_src, h->d_res_cum, (uint32_t)n, g0, g1, d_fates, false, false);
     which ^= 1;
   }
   // retire in launch order

@@ -16,8 +16,15 @@ uint64_t kernel_launch_count();
 cudaError_t launch_ingest(const pp_source* d_s, const uint32_t* d_ev, const uint32_t* d_sid, uint32_t sid_base, uint32_t n,
                           float yield, SrcRec* d_out, unsigned int* d_overflow, cudaStream_t st);
 cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_cum, cudaStream_t st);
+// tiles + cum_rel for photons [g_begin, ...) of a scanned batch; also clears *d_status for the launch that follows
 cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
-                         uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st);
+                         uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, Status* d_status,
+                         cudaStream_t st);
+// scan + tiles + cum_rel + status in one single-CTA kernel: small launches only (n_src, n_tiles <= kPrologueMax)
+constexpr uint32_t kPrologueMax = 4096;
+cudaError_t launch_prologue(const SrcRec* d_src, uint32_t n_src, unsigned long long* d_cum, unsigned long long g_begin,
+                            uint32_t n_tiles, uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel,
+                            Status* d_status, cudaStream_t st);
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st);
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm);
 

@@ -78,15 +78,9 @@ __global__ void __launch_bounds__(1024) scan_kernel(const SrcRec* __restrict__ s
 // tile_src[j] = index of the source that holds batch-global photon g_begin + j * tile_photons,
 // i.e. the last s with cum[s] <= g (sources with zero photons are skipped by construction); and
 // cum_rel[s] = cum[s] - g_begin in 32 bits for the refill (see LaunchParams::cum_rel).
-__global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_t n_src, unsigned long long g_begin,
-                             uint32_t n_tiles, uint32_t tile_photons, uint32_t* __restrict__ tile_src,
-                             uint32_t* __restrict__ cum_rel) {
-  const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j <= n_src) {
-    const unsigned long long c = cum[j];
-    cum_rel[j] = c < g_begin ? (uint32_t)(c - g_begin) : (uint32_t)min(c - g_begin, 0xFFFFFFFFull);
-  }
-  if (j >= n_tiles) return;
+__device__ __forceinline__ void tile_entry(const unsigned long long* __restrict__ cum, uint32_t n_src,
+                                           unsigned long long g_begin, uint32_t tile_photons, uint32_t j,
+                                           uint32_t* __restrict__ tile_src) {
   const unsigned long long g = g_begin + (unsigned long long)j * tile_photons;
   uint32_t lo = 0, hi = n_src;  // invariant: cum[lo] <= g < cum[hi]
   while (hi - lo > 1) {
@@ -95,6 +89,55 @@ __global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_
   }
   tile_src[j] = lo;
 }
+__device__ __forceinline__ uint32_t rel32(unsigned long long c, unsigned long long g_begin) {
+  return c < g_begin ? (uint32_t)(c - g_begin) : (uint32_t)min(c - g_begin, 0xFFFFFFFFull);
+}
+
+// Also clears the launch's Status record (the propagation kernel that follows on the stream counts from zero).
+__global__ void tiles_kernel(const unsigned long long* __restrict__ cum, uint32_t n_src, unsigned long long g_begin,
+                             uint32_t n_tiles, uint32_t tile_photons, uint32_t* __restrict__ tile_src,
+                             uint32_t* __restrict__ cum_rel, Status* __restrict__ status) {
+  const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j == 0 && status) *status = Status{};
+  if (j <= n_src) cum_rel[j] = rel32(cum[j], g_begin);
+  if (j < n_tiles) tile_entry(cum, n_src, g_begin, tile_photons, j, tile_src);
+}
+
+// Small launches (a few thousand sources and tiles; C3's 1e5-photon end): scan + tiles + status in ONE kernel of one
+// CTA, so that the fixed cost of a launch is one kernel less (small batches underuse the GPU; what can
+// be saved is the host-side latency around the kernel).
+__global__ void __launch_bounds__(1024) prologue_kernel(const SrcRec* __restrict__ src, uint32_t n_src,
+                                                        unsigned long long* __restrict__ cum, unsigned long long g_begin,
+                                                        uint32_t n_tiles, uint32_t tile_photons,
+                                                        uint32_t* __restrict__ tile_src, uint32_t* __restrict__ cum_rel,
+                                                        Status* __restrict__ status) {
+  __shared__ unsigned long long part[1024];
+  const uint32_t t = threadIdx.x;
+  const uint32_t per = (n_src + 1023u) / 1024u;
+  const uint32_t lo = min(n_src, t * per), hi = min(n_src, lo + per);
+  unsigned long long s = 0;
+  for (uint32_t i = lo; i < hi; ++i) s += src[i].n_photons;
+  part[t] = s;
+  __syncthreads();
+  for (uint32_t off = 1; off < 1024; off <<= 1) {
+    unsigned long long v = (t >= off) ? part[t - off] : 0ull;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  unsigned long long run = (t == 0) ? 0ull : part[t - 1];
+  for (uint32_t i = lo; i < hi; ++i) {
+    cum[i] = run;
+    cum_rel[i] = rel32(run, g_begin);
+    run += src[i].n_photons;
+  }
+  if (t == 1023) { cum[n_src] = part[1023]; cum_rel[n_src] = rel32(part[1023], g_begin); }
+  if (t == 0) *status = Status{};
+  __threadfence_block();
+  __syncthreads();
+  for (uint32_t j = t; j < n_tiles; j += 1024u) tile_entry(cum, n_src, g_begin, tile_photons, j, tile_src);
+}
+
 
 // =============================================================================================
 // a3-a8  Persistent propagation kernel
@@ -605,10 +648,19 @@ cudaError_t launch_scan(const SrcRec* d_src, uint32_t n, unsigned long long* d_c
 }
 
 cudaError_t launch_tiles(const unsigned long long* d_cum, uint32_t n_src, unsigned long long g_begin, uint32_t n_tiles,
-                         uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, cudaStream_t st) {
-  if (n_tiles == 0) return cudaSuccess;
-  const uint32_t n_thr = max(n_tiles, n_src + 1);
-  tiles_kernel<<<(n_thr + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, tile_photons, d_tile_src, d_cum_rel);
+                         uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel, Status* d_status,
+                         cudaStream_t st) {
+  const uint32_t n_thr = max(max(n_tiles, n_src + 1), 1u);
+  tiles_kernel<<<(n_thr + 255) / 256, 256, 0, st>>>(d_cum, n_src, g_begin, n_tiles, tile_photons, d_tile_src, d_cum_rel,
+                                                      d_status);
+  g_launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prologue(const SrcRec* d_src, uint32_t n_src, unsigned long long* d_cum, unsigned long long g_begin,
+                            uint32_t n_tiles, uint32_t tile_photons, uint32_t* d_tile_src, uint32_t* d_cum_rel,
+                            Status* d_status, cudaStream_t st) {
+  prologue_kernel<<<1, 1024, 0, st>>>(d_src, n_src, d_cum, g_begin, n_tiles, tile_photons, d_tile_src, d_cum_rel, d_status);
   g_launches++;
   return cudaGetLastError();
 }
