@@ -47,7 +47,11 @@ struct ShmHeader {
 };
 static_assert(sizeof(ShmHeader) <= kHeaderBytes, "header");
 
-enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3 };  // kRecycled: closed, emptied, claimable again
+// Life of a slot: kAttached (a client owns it) -> kClosed (the client left, or its process is gone) -> kQuiesced (the
+// ingest thread has seen that and will not touch the slot's source ring again) -> kRecycled (the dispatch thread has
+// emptied it: claimable again).  Only the ingest thread moves a slot out of kClosed, so the dispatch thread never
+// recycles a slot while a block of it is being handed to the back end.
+enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3, kQuiesced = 4 };
 
 struct ClientCtl {
   std::atomic<uint32_t> state;
@@ -154,6 +158,22 @@ void ingest_main(pp_ipc_server* s) {
     const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
     for (uint32_t c = 0; c < n_slots; ++c) {
       ClientCtl* ctl = s->seg.ctl(c);
+      const uint32_t state = ctl->state.load(std::memory_order_acquire);
+      if (state == kClosed) {
+        // the client has left: sources it shipped and the server never took are skipped (nobody wants their hits),
+        // and from here on this thread leaves the slot alone until a new client has attached
+        ctl->src_tail.store(ctl->src_head.load(std::memory_order_acquire), std::memory_order_release);
+        ctl->flushed_seq.store(ctl->flush_seq.load(std::memory_order_relaxed), std::memory_order_relaxed);
+        if (s->pc[c].blocks_in_flight.load() != 0) {
+          // blocks of it that the back end still holds must complete for the slot to come back
+          const int rc = s->be.flush(s->be.ctx);
+          if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
+        }
+        uint32_t expect = kClosed;
+        ctl->state.compare_exchange_strong(expect, kQuiesced, std::memory_order_acq_rel);
+        continue;
+      }
+      if (state != kAttached) continue;
       const uint64_t head = ctl->src_head.load(std::memory_order_acquire);
       uint64_t tail = ctl->src_tail.load(std::memory_order_relaxed);
       // a client that does not read its hits gets no more work done for it: its source ring fills up and it blocks
@@ -213,7 +233,7 @@ void ingest_main(pp_ipc_server* s) {
 bool client_gone(pp_ipc_server* s, uint32_t c) {
   ClientCtl* ctl = s->seg.ctl(c);
   const uint32_t st = ctl->state.load(std::memory_order_acquire);
-  if (st == kClosed || st == kRecycled) return true;
+  if (st != kAttached) return true;
   auto& pc = s->pc[c];
   const auto now = Clock::now();
   if (now - pc.last_alive_check < std::chrono::milliseconds(10)) return false;
@@ -287,7 +307,7 @@ void dispatch_main(pp_ipc_server* s) {
       auto& pc = s->pc[c];
       ClientCtl* ctl = s->seg.ctl(c);
       const uint32_t st = ctl->state.load(std::memory_order_acquire);
-      if (st == kClosed || st == kRecycled) { s->dropped += j - i; i = j; continue; }  // nobody will read them
+      if (st != kAttached) { s->dropped += j - i; i = j; continue; }  // nobody will read them
       if (pc.parked.empty()) {
         // straight into the client's ring as far as there is room ...
         pp_hit* ring = s->seg.hit_ring(c);
@@ -338,18 +358,15 @@ void dispatch_main(pp_ipc_server* s) {
       // counters are absolute and simply carry on; hits the old client never read are skipped.
       for (uint32_t c = 0; c < n_slots; ++c) {
         ClientCtl* ctl = s->seg.ctl(c);
-        if (ctl->state.load(std::memory_order_acquire) != kClosed) continue;
+        const uint32_t st = ctl->state.load(std::memory_order_acquire);
+        if (st == kAttached) { client_gone(s, c); continue; }  // a client whose process was killed is closed here
+        if (st != kQuiesced) continue;                         // the ingest thread has not let go of the slot yet
         auto& pc = s->pc[c];
         if (!pc.parked.empty()) { s->dropped += pc.parked.size(); pc.parked.clear(); pc.parked_n.store(0); }
         if (pc.blocks_in_flight.load() != 0) continue;
-        const uint64_t head = ctl->src_head.load(std::memory_order_acquire);
-        if (head != ctl->src_tail.load(std::memory_order_acquire)) {
-          // sources it shipped and the server never took: nobody wants their hits
-          ctl->src_tail.store(head, std::memory_order_release);
-        }
         ctl->hit_tail.store(ctl->hit_head.load(std::memory_order_relaxed), std::memory_order_release);
-        ctl->flushed_seq.store(ctl->flush_seq.load(std::memory_order_relaxed), std::memory_order_relaxed);
         pc.pending_completed = 0;
+        ctl->completed_seq.store(ctl->src_head.load(std::memory_order_acquire), std::memory_order_release);
         ctl->pid.store(0, std::memory_order_relaxed);
         ctl->state.store(kRecycled, std::memory_order_release);
       }
