@@ -92,7 +92,7 @@ def update_instr_per_flight(args):
          "fp32_flops_per_flight": (args.fp32_per_thread_instr * thr / args.flights) if args.fp32_per_thread_instr else None,
          "dram_bytes_per_launch": (tot.get("dram__bytes_read.sum", 0.0) + tot.get("dram__bytes_write.sum", 0.0)) / max(1, n_launch),
          "propagate_launches": n_launch, "flights": args.flights, "kernel_sources_sha256": kernel_source_hash(),
-         "kernel": "pp::propagate_kernel<false,false,false>", "source": args.note}
+         "kernel": "pp::propagate_kernel<false,false,false,false>", "source": args.note}
     with open(INSTR_PER_FLIGHT_FILE, "w") as f:
         json.dump(d, f, indent=2)
         f.write("\n")
@@ -329,7 +329,7 @@ def run_ours(args):
             achieved = flights * ipf / (busy_ms * 1e-3) / 1e9
             roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-level)",
                         "frac": achieved / peak, "traffic": dram_bytes,
-                        "kernel": "pp::propagate_kernel<false,false,false>",
+                        "kernel": "pp::propagate_kernel<false,false,false,false>",
                         "kernel_ms_per_launch": busy_ms / max(1, n_prop_launches),
                         "units_per_launch": {"flights": flights / max(1, n_prop_launches)},
                         "thread_instructions_per_flight": ipf, "per_unit_source": ipf_src,

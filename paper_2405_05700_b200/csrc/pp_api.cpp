@@ -410,6 +410,15 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
     return (uint32_t)off;
   };
   put(layers.data(), layers.size() * sizeof(LayerRec));
+  {
+    std::vector<LayerRec> rec_b(layers);
+    for (uint32_t i = 0; i < nl; ++i) {
+      const LayerRec& lo = layers[std::min(i + 1, nl - 1)];  // finite at the bottom edge (pp_types.h)
+      rec_b[i].Bh = lo.Bh; rec_b[i].Ah = lo.Ah; rec_b[i].Bl = lo.Bl; rec_b[i].Al = lo.Al;
+    }
+    rec_b[nl] = rec_b[nl - 1];
+    B.off_rec_b = put(rec_b.data(), rec_b.size() * sizeof(LayerRec));
+  }
   B.off_inv_b = put(inv_tab[0].data(), inv_tab[0].size() * sizeof(uint16_t));
   B.off_inv_a = put(inv_tab[1].data(), inv_tab[1].size() * sizeof(uint16_t));
   B.off_str_xy = put(str_xy.data(), str_xy.size() * sizeof(float2));
@@ -495,7 +504,7 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, unsigned long long*
   // tile size: 1024 photons for large launches; a small launch is cut finer so that every resident warp gets work
   // (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3)
   uint32_t tile = kTilePhotons;
-  const uint64_t want_tiles = (uint64_t)h->grid * 8ull * 4ull;  // 8 warps per CTA
+  const uint64_t want_tiles = (uint64_t)h->grid * (uint64_t)propagate_warps_per_block() * 4ull;
   while (tile > (uint32_t)kMinTilePhotons && n_ph / tile < want_tiles) tile >>= 1;
   const uint32_t n_tiles = (uint32_t)((n_ph + tile - 1) / tile);
   if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");

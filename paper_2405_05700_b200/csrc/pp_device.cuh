@@ -54,6 +54,13 @@ __device__ __forceinline__ float fast_sqrt(float x) {
 }
 #endif
 
+// (a == b) ? x : y as one compare and one select whose operands are evaluated unconditionally
+__device__ __forceinline__ float select_eq(int a, int b, float x, float y) {
+  float r;
+  asm("{ .reg .pred p; setp.eq.s32 p, %1, %2; selp.f32 %0, %3, %4, p; }" : "=f"(r) : "r"(a), "r"(b), "f"(x), "f"(y));
+  return r;
+}
+
 // Step 9a: Henyey-Greenstein, returned as m = 1 - cos(theta) in the cancellation-free form
 //   m = (1-g)(1-u)(q + 1 - g)/(1 - g + 2 g u),  q = (1-g^2)/(1 - g + 2 g u)        (R-1)
 __device__ __forceinline__ float hg_one_minus_cos(float u, float one_minus_g, float two_g, float one_minus_g2) {

@@ -27,6 +27,7 @@ cudaError_t launch_prologue(const SrcRec* d_src, uint32_t n_src, unsigned long l
                             Status* d_status, cudaStream_t st);
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st);
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm);
+int propagate_warps_per_block();  // warps of one CTA of the propagation kernel
 
 // Step 1 on the host (same arithmetic as the device's, exact in fp64).
 inline unsigned long long host_photon_count(float energy, float yield) {

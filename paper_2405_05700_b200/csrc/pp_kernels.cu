@@ -7,7 +7,7 @@
 #include "pp_device.cuh"
 
 #ifndef PP_MIN_BLOCKS
-#define PP_MIN_BLOCKS 4  // resident CTAs of 256 threads per SM the propagation kernel is compiled for
+#define PP_MIN_BLOCKS 1  // resident CTAs per SM the propagation kernel is compiled for (one CTA of 1024 threads)
 #endif
 
 namespace pp {
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(1024) prologue_kernel(const SrcRec* __restrict
 // a3-a8  Persistent propagation kernel
 // =============================================================================================
 #ifndef PP_BLOCK_THREADS
-#define PP_BLOCK_THREADS 256
+#define PP_BLOCK_THREADS 1024  // 64 registers per thread either way; one big CTA per SM stages the tables once (+1 %)
 #endif
 constexpr int kBlockThreads = PP_BLOCK_THREADS;
 constexpr int kMaxDevices = 64;
@@ -191,12 +191,14 @@ __device__ __noinline__ Best test_string(const LaunchParams& P, uint32_t si, flo
   const float rho2 = fmaf(dx, dx, dy * dy);
   float ta = 0.0f, tb = s;
   if (rho2 > 1e-12f) {
-    const float inv = 1.0f / rho2;
+    // (approximate reciprocal and square root: the interval only selects candidate DOMs, and Rm carries a margin
+    // five orders of magnitude above their error)
+    const float inv = fast_rcp(rho2);
     const float tc = fmaf(ax, dx, ay * dy) * inv;
     const float cr = fmaf(ax, dy, -ay * dx);
     const float h2 = fmaf(Rm * Rm, rho2, -cr * cr);
     if (h2 < 0.0f) return best;
-    const float h = sqrtf(h2) * inv;
+    const float h = fast_sqrt(h2) * inv;
     ta = fmaxf(0.0f, tc - h);
     tb = fminf(s, tc + h);
     if (ta > tb) return best;
@@ -287,8 +289,9 @@ __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, b
 }
 
 // kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18, wavelength bins R-21, emission
-// smearing R-22) is compiled in
-template <bool kBrute, bool kFates, bool kExt>
+// smearing R-22) is compiled in.  kLoop: the inverse walk tables are coarser than the thinnest layer (pathological
+// ice, LaunchParams::walk_loop), so the layer found may be several layers short
+template <bool kBrute, bool kFates, bool kExt, bool kLoop>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // ---- stage the medium and the DOM lookup in shared memory (a4, a5): one verbatim copy of the host-built image ----
@@ -310,8 +313,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   // the warp's current source record (a2): staged once per (tile, source) run, read by the lanes that refill
   __shared__ float4 s_wsrc[kBlockThreads / 32][3];
   const unsigned wslot = threadIdx.x >> 5;
+  uint32_t wsrc_addr;  // shared-window address of this warp's record, pinned in a register (not rematerialised)
+  asm volatile("mov.u32 %0, %1;" : "=r"(wsrc_addr) : "r"((uint32_t)__cvta_generic_to_shared(&s_wsrc[wslot][0])));
 
-  const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = lanemask_lt();
   Status* const st = P.status;
   const float inf = __int_as_float(0x7f800000);
@@ -332,55 +336,59 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   float sc_b = 1.0f;  // kExt only: 1 / scat_scale of the photon's wavelength bin (R-21)
   uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
 
+  // A new run (rare: once per source of a work item): the next source of the current work item, or a new work item
+  // (resume list first, then tiles).  Leaves t_next < run_end, or refill_ok = false when no work is left.
+  auto next_run = [&]() {
+    if (t_next == t_end) {
+      const uint4 wk = fetch_work(P, __popc(lt), use_resume);
+      t_next = wk.x; t_end = wk.y; s_cur = wk.z; use_resume = wk.w != 0u;
+      w_started += t_end - t_next;  // counted per work item; what is handed back at the end is taken out again
+    } else {
+      ++s_cur;
+    }
+    if (t_next != t_end) {
+      uint32_t hi;
+      while ((hi = __ldg(&P.cum_rel[s_cur + 1])) <= t_next) ++s_cur;  // skips sources without photons
+      pbase = __ldg(&P.cum_rel[s_cur]);  // mod 2^32: right for the launch's first (split) source too
+      run_end = min(t_end, hi);
+      __syncwarp();
+      if (__popc(lt) < 3) s_wsrc[wslot][__popc(lt)] = __ldg(reinterpret_cast<const float4*>(P.src + s_cur) + __popc(lt));
+      __syncwarp();
+    } else {
+      run_end = t_end;
+      refill_ok = false;
+    }
+  };
+  next_run();
+
   for (;;) {
     // =========================== refill dead lanes (a2 -> a3) ===========================
-    const unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
-    if (need_mask != 0u && refill_ok) {
-      if (t_next == run_end) {
-        // a new run: the next source of the current work item, or a new work item (resume list first, then tiles)
-        if (t_next == t_end) {
-          const uint4 wk = fetch_work(P, lane, use_resume);
-          t_next = wk.x; t_end = wk.y; s_cur = wk.z; use_resume = wk.w != 0u;
-        } else {
-          ++s_cur;
-        }
-        if (t_next != t_end) {
-          uint32_t hi;
-          while ((hi = __ldg(&P.cum_rel[s_cur + 1])) <= t_next) ++s_cur;  // skips sources without photons
-          pbase = __ldg(&P.cum_rel[s_cur]);  // mod 2^32: right for the launch's first (split) source too
-          run_end = min(t_end, hi);
-          __syncwarp();
-          if (lane < 3u) s_wsrc[wslot][lane] = __ldg(reinterpret_cast<const float4*>(P.src + s_cur) + lane);
-          __syncwarp();
-        } else {
-          run_end = t_end;
-          refill_ok = false;
-        }
+    // t_next < run_end whenever refill_ok: the next run is fetched as soon as the current one is used up, and a
+    // refill that uses it up goes on with the next one, so lanes stay dead only when the launch has run dry
+    unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
+    while (need_mask != 0u && refill_ok) {
+      // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
+      const uint32_t r = t_next + __popc(need_mask & lt);
+      if (!alive && r < run_end) {
+        float4 r0; float2 r1; uint2 r2;
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w) : "r"(wsrc_addr));
+        asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+16];" : "=f"(r1.x), "=f"(r1.y) : "r"(wsrc_addr));
+        asm volatile("ld.shared.v2.u32 {%0,%1}, [%2+32];" : "=r"(r2.x), "=r"(r2.y) : "r"(wsrc_addr));
+        phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
+        dx = r0.w; dy = r1.x; dz = r1.y;
+        Lh = 0.0f; Ll = 0.0f;
+        ev = r2.x; sid = r2.y;
+        pidx = r - pbase;
+        k = 0; s_mine = s_cur;
+        alive = true;
       }
-      if (t_next != run_end) {
-        // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
-        const uint32_t r = t_next + __popc(need_mask & lt);
-        if (!alive && r < run_end) {
-          const float4 r0 = s_wsrc[wslot][0], r1 = s_wsrc[wslot][1];
-          const uint2 r2 = *reinterpret_cast<const uint2*>(&s_wsrc[wslot][2]);
-          phx = r0.x; phy = r0.y; phz = r0.z; plx = ply = plz = 0.0f;
-          dx = r0.w; dy = r1.x; dz = r1.y;
-          Lh = 0.0f; Ll = 0.0f;
-          ev = r2.x; sid = r2.y;
-          pidx = r - pbase;
-          k = 0; s_mine = s_cur;
-          alive = true;
-        }
-        const uint32_t take = min((uint32_t)__popc(need_mask), run_end - t_next);
-        t_next += take;
-        w_started += take;
-      }
+      t_next = min(t_next + (uint32_t)__popc(need_mask), run_end);
+      if (t_next != run_end) break;
+      next_run();
+      need_mask = __ballot_sync(0xffffffffu, !alive);
     }
     const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
-    if (alive_mask == 0u) {
-      if (!refill_ok) break;
-      continue;  // the run ended exactly here: start the next one
-    }
+    if (alive_mask == 0u) break;  // nothing left to refill from
     w_flights += __popc(alive_mask);  // every live lane flies once per iteration
 
     // =========================== a7': Philox block k of this photon ===========================
@@ -427,41 +435,41 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const float inv_w = fast_rcp(w);
     const bool up = dz > 0.0f;
     const int last = P.last_layer;
+    // Direct walk, branch-free.  h0 is the vertical distance to the boundary ahead, i1; the flight reaches it with
+    // budgets t1, t2 left (negative: it ends before).  With B(i), A(i) the cumulative vertical optical depths at the
+    // boundaries (two-float sums), the cumulative depths X at which the budgets run out name the layers js, ja
+    // (inverse table + one compare-and-step); the nearer one, clamped to the photon's side of its own layer, is the
+    // layer lj where the flight ends.  lj = li (always so in an end layer with no boundary ahead, R-6): the budgets
+    // are spent in layer li, as they are.  Otherwise the budgets left at lj's entry boundary come from the two-float
+    // sums, so their error is relative to the budget, not to the cumulative depth.  Coefficients and sums come from
+    // one record each at the start and at the end (LayerRec, pp_types.h).
+    const float sgn = up ? -1.0f : 1.0f;
     int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
     li = max(0, min(li, last));
-    const int i1 = li + (up ? 0 : 1);                   // boundary ahead
-    const float zb = fmaf(-P.dz_layer, (float)i1, P.z_top);
-    const bool open = up ? (li == 0) : (li == last);  // no boundary ahead: the end layers are infinite (R-6)
-    const float h0 = open ? inf : fabsf((zb - phz) - plz);  // vertical distance to the first boundary (two-float z)
-    float Ts = tau_s * w, Ta = tau_a * w, Vb = 0.0f;
-    float4 L4 = lay(li);
-    {
-      const float t1 = fmaf(-L4.y, h0, Ts), t2 = fmaf(-L4.x, h0, Ta);
-      if (fminf(t1, t2) > 0.0f) {
-        // The flight leaves layer li through boundary i1 with budgets t1, t2 left.  Direct walk: the cumulative
-        // depths X at which the budgets run out name the layers js, ja (inverse table + one step); the nearer
-        // one is where the flight ends, and the budgets left at its entry boundary jb come from the two-float
-        // cumulative sums, so their error is relative to the budget, not to the cumulative depth.
-        const float4 W1 = walk(i1);
-        const float sgn = up ? -1.0f : 1.0f;
-        const float Xs = fmaf(sgn, t1, W1.x), Xa = fmaf(sgn, t2, W1.y);
-        int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
-        int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
-        js += (walk_B(js + 1) <= Xs) ? 1 : 0;
-        ja += (walk_A(ja + 1) <= Xa) ? 1 : 0;
-        if (P.walk_loop) {
-          while (js < last && walk_B(js + 1) <= Xs) ++js;
-          while (ja < last && walk_A(ja + 1) <= Xa) ++ja;
-        }
-        const int lj = up ? min(max(js, ja), li - 1) : max(min(js, ja), li + 1);
-        const int jb = lj + (up ? 1 : 0);
-        const float4 Wb = walk(jb);
-        Ts = t1 - fabsf((Wb.x - W1.x) + (Wb.z - W1.z));
-        Ta = t2 - fabsf((Wb.y - W1.y) + (Wb.w - W1.w));
-        Vb = fmaf(P.dz_layer, (float)abs(jb - i1), h0);
-        L4 = lay(lj);
-      }
+    const int i1 = li + (up ? 0 : 1);
+    const float h0 = fabsf((fmaf(-P.dz_layer, (float)i1, P.z_top) - phz) - plz);  // two-float z
+    const unsigned char* const rec0 = smem_raw + (up ? 0u : P.off_rec_b) + (uint32_t)li * 32u;
+    const float4 L0 = *reinterpret_cast<const float4*>(rec0), W1 = *reinterpret_cast<const float4*>(rec0 + 16);
+    const float Ts0 = tau_s * w, Ta0 = tau_a * w;
+    const float t1 = fmaf(-L0.y, h0, Ts0), t2 = fmaf(-L0.x, h0, Ta0);
+    const float Xs = fmaf(sgn, t1, W1.x), Xa = fmaf(sgn, t2, W1.y);
+    const float xs_l = fmaf(sgn, t1, W1.z), xa_l = fmaf(sgn, t2, W1.w);  // lo parts of the two-float X
+    int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
+    int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
+    js += (walk_B(js + 1) <= Xs) ? 1 : 0;
+    ja += (walk_A(ja + 1) <= Xa) ? 1 : 0;
+    if (kLoop) {
+      while (js < last && walk_B(js + 1) <= Xs) ++js;
+      while (ja < last && walk_A(ja + 1) <= Xa) ++ja;
     }
+    const int lj = up ? min(max(js, ja), li) : max(min(js, ja), li);
+    const unsigned char* const rec1 = smem_raw + (up ? P.off_rec_b : 0u) + (uint32_t)lj * 32u;
+    const float4 L4 = *reinterpret_cast<const float4*>(rec1), Wb = *reinterpret_cast<const float4*>(rec1 + 16);
+    // (selects through select_eq: the compiler would otherwise branch around the three right-hand sides, and nearly
+    // every warp holds lanes of both kinds)
+    const float Ts = select_eq(lj, li, Ts0, sgn * ((W1.x - Wb.x) + (xs_l - Wb.z)));
+    const float Ta = select_eq(lj, li, Ta0, sgn * ((W1.y - Wb.y) + (xa_l - Wb.w)));
+    const float Vb = select_eq(lj, li, 0.0f, fmaf(P.dz_layer, (float)(abs(lj - li) - 1), h0));
     const float vs = Ts * L4.w, va = Ta * L4.z;  // vertical distance left in the final layer
     const bool absorbed = va <= vs;
     const float v_in = fminf(vs, va);
@@ -478,12 +486,18 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       const float sxy2 = s * s * rho2;
       float ds = s;
       int n_ch = 1;
-      bool all_lines = false;  // a flight of more than 64 pieces (far longer than the detector is wide)
       if (sxy2 > P.xy_cap2) {
         const float f = floorf(fast_sqrt(sxy2) * P.inv_xy_cap) + 1.0f;
-        all_lines = f > 64.0f;
-        n_ch = all_lines ? 1 : (int)f;
-        ds = s * fast_rcp(f);
+        if (f > 64.0f) {
+          // a flight of more than 64 pieces (far longer than the detector is wide): every line, here in the rare
+          // path; the one look-up below then repeats a line already tested, which changes nothing
+          if (alive)
+            for (uint32_t si = 0; si < P.n_strings; ++si)
+              best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
+        } else {
+          n_ch = (int)f;
+          ds = s * fast_rcp(f);
+        }
       }
       const float rm2 = fmaf(P.rm2, rho2, 1e-12f);
       float tm = 0.5f * ds;
@@ -500,10 +514,6 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
         if (--n_ch <= 0) break;
         tm += ds;
-      }
-      if (all_lines && alive) {
-        for (uint32_t si = 0; si < P.n_strings; ++si)
-          best = test_string(P, si, phx, phy, phz, plx, ply, plz, dx, dy, dz, s, best);
       }
     }
     bool hit = alive && best.t <= s;
@@ -547,14 +557,14 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
           hit = !rejected;
         }
         const unsigned rej_mask = __ballot_sync(0xffffffffu, rejected);
-        if (rej_mask && (int)lane == __ffs(rej_mask) - 1) atomicAdd(&st->photons_rejected, (unsigned long long)__popc(rej_mask));
+        if (rej_mask && __popc(lt) == __ffs(rej_mask) - 1) atomicAdd(&st->photons_rejected, (unsigned long long)__popc(rej_mask));
         hit_mask &= ~rej_mask;
       }
       if (hit_mask) {
         const unsigned n_hit = __popc(hit_mask);
         unsigned base = 0;
         const int leader = __ffs(hit_mask) - 1;
-        if ((int)lane == leader) base = atomicAdd(&st->hit_count, n_hit);
+        if (__popc(lt) == leader) base = atomicAdd(&st->hit_count, n_hit);
         base = __shfl_sync(0xffffffffu, base, leader);
         if (hit) {
           const unsigned slot = base + __popc(hit_mask & lt);
@@ -615,8 +625,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   }
 
   // ---- leftovers of a stopped warp go to the next launch; fold the counters ----
-  if (lane == 0) {
+  if (lt == 0u) {
     if (t_next < t_end) {
+      w_started -= t_end - t_next;
       const unsigned o = atomicAdd(&st->n_resume_out, 1u);
       if (o < P.resume_cap) P.resume_out[o] = WorkItem{P.g_begin + t_next, P.g_begin + t_end, s_cur, 0u};
       else atomicExch(&st->error, 1u);
@@ -665,47 +676,71 @@ cudaError_t launch_prologue(const SrcRec* d_src, uint32_t n_src, unsigned long l
   return cudaGetLastError();
 }
 
-template <bool B, bool F, bool A>
-static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
-  // opt-in dynamic shared memory size set so far, per device (the attribute is per device and per function)
+// Opt-in dynamic shared memory size of one kernel variant: raised when a handle needs more than any before it on
+// this device (the attribute is per device and per function; it is never lowered).
+template <bool B, bool F, bool A, bool L>
+static cudaError_t ensure_smem(size_t smem) {
   static std::atomic<size_t> attr_smem[kMaxDevices];
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
   if (smem > attr_smem[dev].load()) {
-    e = cudaFuncSetAttribute(propagate_kernel<B, F, A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(propagate_kernel<B, F, A, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_smem[dev].store(smem);
   }
-  propagate_kernel<B, F, A><<<grid, kBlockThreads, smem, st>>>(P);
+  return cudaSuccess;
+}
+
+template <bool B, bool F, bool A, bool L>
+static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
+  const cudaError_t e = ensure_smem<B, F, A, L>(smem);
+  if (e != cudaSuccess) return e;
+  propagate_kernel<B, F, A, L><<<grid, kBlockThreads, smem, st>>>(P);
   g_launches++;
   return cudaGetLastError();
 }
 
-// the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use)
+// the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use, coarse walk tables)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  const int v = (brute ? 4 : 0) | (fates ? 2 : 0) | ((P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u) ? 1 : 0);
+  const bool ext = P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u;
+  const int v = (P.walk_loop ? 8 : 0) | (brute ? 4 : 0) | (fates ? 2 : 0) | (ext ? 1 : 0);
   switch (v) {
-    case 0: return launch_prop_t<false, false, false>(P, grid, smem, st);
-    case 1: return launch_prop_t<false, false, true>(P, grid, smem, st);
-    case 2: return launch_prop_t<false, true, false>(P, grid, smem, st);
-    case 3: return launch_prop_t<false, true, true>(P, grid, smem, st);
-    case 4: return launch_prop_t<true, false, false>(P, grid, smem, st);
-    case 5: return launch_prop_t<true, false, true>(P, grid, smem, st);
-    case 6: return launch_prop_t<true, true, false>(P, grid, smem, st);
-    default: return launch_prop_t<true, true, true>(P, grid, smem, st);
+    case 0: return launch_prop_t<false, false, false, false>(P, grid, smem, st);
+    case 1: return launch_prop_t<false, false, true, false>(P, grid, smem, st);
+    case 2: return launch_prop_t<false, true, false, false>(P, grid, smem, st);
+    case 3: return launch_prop_t<false, true, true, false>(P, grid, smem, st);
+    case 4: return launch_prop_t<true, false, false, false>(P, grid, smem, st);
+    case 5: return launch_prop_t<true, false, true, false>(P, grid, smem, st);
+    case 6: return launch_prop_t<true, true, false, false>(P, grid, smem, st);
+    case 7: return launch_prop_t<true, true, true, false>(P, grid, smem, st);
+    case 8: return launch_prop_t<false, false, false, true>(P, grid, smem, st);
+    case 9: return launch_prop_t<false, false, true, true>(P, grid, smem, st);
+    case 10: return launch_prop_t<false, true, false, true>(P, grid, smem, st);
+    case 11: return launch_prop_t<false, true, true, true>(P, grid, smem, st);
+    case 12: return launch_prop_t<true, false, false, true>(P, grid, smem, st);
+    case 13: return launch_prop_t<true, false, true, true>(P, grid, smem, st);
+    case 14: return launch_prop_t<true, true, false, true>(P, grid, smem, st);
+    default: return launch_prop_t<true, true, true, true>(P, grid, smem, st);
   }
+}
+
+int propagate_warps_per_block() { return kBlockThreads / 32; }
+
+template <bool B, bool F, bool A, bool L>
+static cudaError_t occupancy_t(size_t smem, int* n) {
+  const cudaError_t e = ensure_smem<B, F, A, L>(smem);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, propagate_kernel<B, F, A, L>, kBlockThreads, smem);
 }
 
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
   // all variants are compiled for the same launch bounds; the leanest and the fullest bracket the rest
   int a = 0, b = 0;
-  cudaError_t e = brute ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, propagate_kernel<true, true, true>, kBlockThreads, smem)
-                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, propagate_kernel<false, true, true>, kBlockThreads, smem);
+  cudaError_t e = brute ? occupancy_t<true, true, true, true>(smem, &a) : occupancy_t<false, true, true, true>(smem, &a);
   if (e != cudaSuccess) return e;
-  e = brute ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, propagate_kernel<true, false, false>, kBlockThreads, smem)
-            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, propagate_kernel<false, false, false>, kBlockThreads, smem);
+  e = brute ? occupancy_t<true, false, false, false>(smem, &b) : occupancy_t<false, false, false, false>(smem, &b);
   (void)fates;
   *blocks_per_sm = a < b ? a : b;
   return e;

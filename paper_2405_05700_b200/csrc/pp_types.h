@@ -57,7 +57,11 @@ constexpr uint16_t kNoString = 0xFFFFu;  // host-side marker while the cell tabl
 // One record per layer boundary i (= upper edge of layer i), i = 0..n_layers; 32 B, shared memory (a4).
 // The first half is layer i's coefficients, the second half the cumulative vertical optical depth at the boundary as
 // two-float sums (B scattering, A absorption).  Record n_layers repeats the last layer's coefficients and holds +inf
-// in the hi parts (only ever compared against).
+// in the hi parts (only ever compared against).  A second array (LaunchParams::off_rec_b) pairs layer i's
+// coefficients with the sums at its LOWER boundary i + 1 (record n_layers - 1 and n_layers: the finite sums of
+// boundary n_layers - 1, never used for arithmetic), so that a flight reads the coefficients of a layer and the sums
+// of the boundary it faces (start) or entered through (end) from ONE record: the first array going up at the start
+// and down at the end, the second one otherwise.
 struct __align__(16) LayerRec {
   float a, b, la, lb;     // 1/m, 1/m, m, m
   float Bh, Ah, Bl, Al;
@@ -82,7 +86,7 @@ struct LaunchParams {
   float inv_xy_cap;
   uint32_t max_flights;
   uint32_t ring_cap;
-  uint32_t walk_loop;
+  uint32_t off_rec_b;                                   // byte offset of the second layer-record array (below)
   // ---- work ----
   const SrcRec* src;
   const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons (batch-global photon numbers)
@@ -113,6 +117,7 @@ struct LaunchParams {
   //    clamped into the grid.
   const uint4* smem_image;
   uint32_t smem_image_bytes;
+  uint32_t walk_loop;        // the inverse walk tables are coarse (host: picks the kLoop kernel variant)
   uint32_t off_str_a, off_str_b;
   uint32_t n_layers;
   uint32_t n_strings, n_dom;

@@ -80,6 +80,34 @@ def test_layered_full_detector_every_photon():
     assert n_hit == c["n_union"] == len(hits) and (1.0 - frac_t) * n_hit <= 1.0, (frac_t, n_hit, c)
 
 
+def test_coarse_walk_tables_clear_and_dense_layers():
+    """Ice whose layers differ by four orders of magnitude in optical thickness (a few nearly clear 5 m layers, a few
+    very dense ones): the inverse walk tables cannot resolve the thinnest layer within their size limit, so the
+    library takes the kernel variant that steps on from the table entry (LaunchParams::walk_loop).  Every photon
+    compared, R = 2 m DOMs."""
+    rng = np.random.default_rng(77)
+    n = 200
+    lam_s = rng.uniform(15.0, 60.0, n)
+    lam_a = rng.uniform(60.0, 250.0, n)
+    clear = rng.choice(n, 12, replace=False)
+    dense = rng.choice(np.setdiff1d(np.arange(n), clear), 8, replace=False)
+    lam_s[clear], lam_a[clear] = 5000.0, 10000.0
+    lam_s[dense], lam_a[dense] = 0.5, 40.0
+    ice = W.Ice(abs_len=lam_a.astype(np.float32), scat_len=lam_s.astype(np.float32), z_top=500.0, dz=5.0)
+    geo = W.geometry_full(radius=2.0)
+    src = W.sources_c1().subset(slice(0, 100))
+    src.src[:, 7] = 0.2
+    hits, fates, st = gpu_run_resident(geo, ice, src, 9, want_fates=True)
+    ref = O.propagate(geo, ice, src, seed=9, want_fates=True)
+    assert st.photons_done == ref.photons == 200000
+    assert st.flights == ref.flights or abs(st.flights - ref.flights) < 1e-5 * ref.flights
+    # (absorption lengths of 10 km in the clear layers: the absorption point moves by up to 4e-7 of that, see check_fates)
+    frac_t, n_hit = check_fates(fates, ref.fates, min_same=0.9999, pos_tol=2e-2)
+    assert n_hit > 500
+    c = compare_hits(hits, ref.hits, ref.photons)
+    assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.98, c
+
+
 def test_layered_oversized_doms_many_hits():
     """Same with R = 2 m DOMs so that ~1 % of photons hit: the per-hit statistics mean something."""
     geo, ice = W.geometry_full(radius=2.0), W.ice_layered()

@@ -94,5 +94,6 @@ cudaError_t launch_propagate(const LaunchParams& P, bool, bool, int, size_t, cud
 }
 
 cudaError_t propagate_occupancy(bool, bool, size_t, int* blocks_per_sm) { *blocks_per_sm = 2; return cudaSuccess; }
+int propagate_warps_per_block() { return 8; }
 
 }  // namespace pp
