@@ -77,7 +77,10 @@ struct Slot {
   // pinned host
   Status* h_status = nullptr;     // D2H target; the first kFirstHits hits of the ring follow at kHeadBytes
   pp_hit* h_first = nullptr;
-  Status* h_status_in = nullptr;  // H2D source for relaunches
+  Status* h_status_in = nullptr;  // H2D source of the cleared Status record
+  unsigned long long* h_cum = nullptr;  // host-side prologue of a server launch: prefix sums and tile table
+  uint32_t* h_cum_rel = nullptr;
+  uint32_t* h_tile_src = nullptr;
   unsigned char* h_stage[2] = {nullptr, nullptr};
   cudaEvent_t ev_h2d = nullptr, ev_k0 = nullptr, ev_k1 = nullptr, ev_done = nullptr, ev_stage[2] = {nullptr, nullptr};
   // state of the launch in flight
@@ -477,6 +480,9 @@ uint64_t carve_pinned(pp_handle* h, void* base) {
     s.h_status = reinterpret_cast<Status*>(hs);
     s.h_first = reinterpret_cast<pp_hit*>(hs ? hs + kHeadBytes : nullptr);
     s.h_status_in = c.take<Status>(1);
+    s.h_cum = c.take<unsigned long long>(h->sz.cap_src + 1);
+    s.h_cum_rel = c.take<uint32_t>(h->sz.cap_src + 1);
+    s.h_tile_src = c.take<uint32_t>(h->sz.max_tiles);
     s.h_stage[0] = c.take<unsigned char>(kStageBytes);
     s.h_stage[1] = c.take<unsigned char>(kStageBytes);
   }
@@ -496,21 +502,65 @@ cudaError_t read_back_head(pp_handle* h, Slot& s) {
   return cudaMemcpyAsync(s.h_status, s.d_status, bytes, cudaMemcpyDeviceToHost, s.stream);
 }
 
-// Enqueue tiles + propagate (+ status read-back) for photons [g_begin, g_end) of the batch
-// (src, cum, n_src), which must already be (or be enqueued to become) resident on slot.stream.
-int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, unsigned long long* cum, uint32_t n_src,
-                   uint64_t g_begin, uint64_t g_end, pp_fate* fates, bool has_segments, bool need_scan) {
-  const uint64_t n_ph = g_end - g_begin;
-  // tile size: 1024 photons for large launches; a small launch is cut finer so that every resident warp gets work
-  // (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3)
+// Tile size of a launch: 1024 photons for large launches; a small launch is cut finer so that every resident warp
+// gets work (about 4 tiles per warp), which is what sets the latency of a launch the GPU is too big for (C3).
+void pick_tiles(const pp_handle* h, uint64_t n_ph, uint32_t* tile_photons, uint32_t* n_tiles) {
   uint32_t tile = kTilePhotons;
   const uint64_t want_tiles = (uint64_t)h->grid * (uint64_t)propagate_warps_per_block() * 4ull;
   while (tile > (uint32_t)kMinTilePhotons && n_ph / tile < want_tiles) tile >>= 1;
-  const uint32_t n_tiles = (uint32_t)((n_ph + tile - 1) / tile);
+  *tile_photons = tile;
+  *n_tiles = (uint32_t)std::min<uint64_t>((n_ph + tile - 1) / tile, 0xFFFFFFFFull);
+}
+
+// cum[s] - g_begin in 32 bits as the kernels read it (LaunchParams::cum_rel)
+inline uint32_t rel32(uint64_t c, uint64_t g_begin) {
+  return c < g_begin ? (uint32_t)(c - g_begin) : (uint32_t)std::min<uint64_t>(c - g_begin, 0xFFFFFFFFull);
+}
+
+// a2 on the host, for launches cut by the batching server: the server walks the queued records anyway, so it
+// writes the prefix sums, their launch-relative form and the tile -> source table itself, into pinned memory that
+// travels with the records.  A launch then needs no kernel in front of the propagation kernel, which matters because
+// that kernel could not start before the previous launch has left an SM: with the tables uploaded by the copy engine
+// the next launch's CTAs move in as the previous launch's move out.  `count_at(q)` = photons of the launch's q-th
+// record.  Returns the total.
+template <class CountAt>
+uint64_t host_prologue(Slot& s, CountAt count_at, uint32_t n_src, uint64_t g_begin, uint32_t tile, uint32_t n_tiles) {
+  uint64_t run = 0;
+  for (uint32_t q = 0; q < n_src; ++q) {
+    s.h_cum[q] = run; s.h_cum_rel[q] = rel32(run, g_begin);
+    run += count_at(q);
+  }
+  s.h_cum[n_src] = run; s.h_cum_rel[n_src] = rel32(run, g_begin);
+  uint32_t si = 0;  // tile_src[j] = the last source with cum <= the tile's first photon (skips sources without photons)
+  for (uint32_t j = 0; j < n_tiles; ++j) {
+    const uint64_t g = g_begin + (uint64_t)j * tile;
+    while (si + 1 < n_src && s.h_cum[si + 1] <= g) ++si;
+    s.h_tile_src[j] = si;
+  }
+  *s.h_status_in = Status{};
+  return run;
+}
+
+// Enqueue tiles + propagate (+ status read-back) for photons [g_begin, g_end) of the batch
+// (src, cum, n_src), which must already be (or be enqueued to become) resident on slot.stream.
+// `host_tables`: host_prologue() has filled the slot's pinned tables for exactly this launch; they are uploaded
+// instead of being computed by the scan / tiles kernels.
+int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, unsigned long long* cum, uint32_t n_src,
+                   uint64_t g_begin, uint64_t g_end, pp_fate* fates, bool has_segments, bool need_scan,
+                   bool host_tables = false) {
+  const uint64_t n_ph = g_end - g_begin;
+  uint32_t tile = 0, n_tiles = 0;
+  pick_tiles(h, n_ph, &tile, &n_tiles);
   if (n_tiles > h->sz.max_tiles) return fail(h, PP_E_NOMEM, "launch larger than launch_photons_target");
-  // a2: prefix sums (unless the batch is scanned already), tile -> source table, launch-relative prefix sums; the
-  // status record is cleared by the same kernel.  Small launches do all of it in one single-CTA kernel.
-  if (need_scan && n_src <= kPrologueMax && n_tiles <= kPrologueMax) {
+  if (host_tables) {
+    PP_CUDA(h, cudaMemcpyAsync(cum, s.h_cum, ((size_t)n_src + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice, s.stream));
+    PP_CUDA(h, cudaMemcpyAsync(s.d_cum_rel, s.h_cum_rel, ((size_t)n_src + 1) * sizeof(uint32_t), cudaMemcpyHostToDevice, s.stream));
+    PP_CUDA(h, cudaMemcpyAsync(s.d_tile_src, s.h_tile_src, (size_t)n_tiles * sizeof(uint32_t), cudaMemcpyHostToDevice, s.stream));
+    PP_CUDA(h, cudaMemcpyAsync(s.d_status, s.h_status_in, sizeof(Status), cudaMemcpyHostToDevice, s.stream));
+  } else if (need_scan && n_src <= kPrologueMax && n_tiles <= kPrologueMax) {
+    // a2 on the device (resident path): prefix sums (unless the batch is scanned already), tile -> source table,
+    // launch-relative prefix sums; the status record is cleared by the same kernel.  Small launches do all of it in
+    // one single-CTA kernel.
     PP_CUDA(h, launch_prologue(src, n_src, cum, g_begin, n_tiles, tile, s.d_tile_src, s.d_cum_rel, s.d_status, s.stream));
   } else {
     if (need_scan) PP_CUDA(h, launch_scan(src, n_src, cum, s.stream));
@@ -755,6 +805,7 @@ void server_main(pp_handle* h) {
         h->queued_photons -= c.photons;
         if (c.last_partial) { h->ring_launch = rec_a + c.n_rec - 1; h->launch_offset = c.next_offset; }
         else { h->ring_launch = rec_a + c.n_rec; h->launch_offset = 0; }
+        const bool idle_gpu = h->n_in_flight == 0;
         s.in_flight = true;  // reserve
         s.sources_end = h->ring_launch;  // a source split across launches completes with the launch that ends it
         h->n_in_flight++;
@@ -771,7 +822,16 @@ void server_main(pp_handle* h) {
           if (e != cudaSuccess) rc = fail(h, PP_E_CUDA, std::string("upload: ") + cudaGetErrorString(e));
           bool seg = false;  // any track segment among the records of this launch?
           for (uint32_t q = 0; q < n_src && !seg; ++q) seg = h->ring[(rec_a + q) % cap].length > 0.0f;
-          if (rc == PP_OK) rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg, true);
+          uint32_t tile = 0, n_tiles = 0;
+          pick_tiles(h, c.photons, &tile, &n_tiles);
+          // a small launch onto an idle GPU keeps the single prologue kernel (one launch instead of four copies:
+          // 20 us of a 0.15 ms launch, C3); every other launch gets its tables from the host
+          const bool host_tables = !(idle_gpu && n_src <= kPrologueMax && n_tiles <= kPrologueMax);
+          if (rc == PP_OK && host_tables && n_tiles <= h->sz.max_tiles)
+            host_prologue(s, [&](uint32_t q) { return (uint64_t)h->ring[(rec_a + q) % cap].n_photons; }, n_src, c.g_begin,
+                          tile, n_tiles);
+          if (rc == PP_OK)
+            rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg, true, host_tables);
           if (rc == PP_OK && cudaEventSynchronize(s.ev_h2d) != cudaSuccess) rc = fail(h, PP_E_CUDA, "upload sync failed");
         }
         lk.lock();
@@ -825,7 +885,7 @@ bool idle_locked(pp_handle* h) {
 // =============================================================================================
 extern "C" {
 
-const char* pp_version(void) { return "pp 0.4 (sm_100a)"; }
+const char* pp_version(void) { return "pp 0.5 (sm_100a)"; }
 
 int pp_check_inputs(const pp_geometry* geo, const pp_ice* ice, uint32_t flags) {
   std::string why;
