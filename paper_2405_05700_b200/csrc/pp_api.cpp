@@ -90,6 +90,8 @@ struct Slot {
   LaunchParams P;
   uint64_t seq = 0;
   bool fates = false;
+  Clock::time_point t_enq{};  // when the launch was enqueued, and how long it should take once it has the GPU
+  double expect_us = 0.0;
 };
 
 }  // namespace
@@ -135,6 +137,8 @@ struct pp_handle {
   bool resident_active = false;
   int n_in_flight = 0;
   uint64_t launch_seq = 0;
+  double us_per_photon = 7.0e-5;     // running estimate of the kernel time per photon (server thread's polling)
+  Clock::time_point t_last_retire{};
   int space_waiters = 0;
 
   // finished hits waiting for pp_collect: a lock of their own, so that collecting never waits for a producer
@@ -584,6 +588,8 @@ int enqueue_launch(pp_handle* h, Slot& s, const SrcRec* src, unsigned long long*
   PP_CUDA(h, cudaEventRecord(s.ev_done, s.stream));
   s.in_flight = true;
   s.seq = ++h->launch_seq;
+  s.t_enq = Clock::now();
+  s.expect_us = 60.0 + (double)n_ph * h->us_per_photon;
   return PP_OK;
 }
 
@@ -650,9 +656,14 @@ int finish_slot(pp_handle* h, Slot& s, bool may_block) {
     h->st.photons_absorbed += hs.photons_started - hs.photons_hit - hs.photons_aborted - hs.photons_rejected;
     h->st.flights += hs.flights;
     h->st.launches += 1;
-    if (t0 > h->busy_end_ms) h->st.kernel_busy_ms += (double)t1 - t0;
-    else if (t1 > h->busy_end_ms) h->st.kernel_busy_ms += (double)t1 - h->busy_end_ms;
+    // time this launch had the GPU to itself: from the end of the launch before it (its CTAs move in as that one's
+    // move out) or from its own start, whichever is later
+    const double own_ms = std::max(0.0, (double)t1 - std::max((double)t0, h->busy_end_ms));
+    h->st.kernel_busy_ms += own_ms;
     h->busy_end_ms = std::max(h->busy_end_ms, (double)t1);
+    if (hs.photons_started > 1000000ull && own_ms > 0.0)
+      h->us_per_photon = 0.75 * h->us_per_photon + 0.25 * (own_ms * 1e3 / (double)hs.photons_started);
+    h->t_last_retire = Clock::now();
   }
   int rc = push_hits(h, std::move(hits), may_block);
   if (rc != PP_OK) return rc;
@@ -846,16 +857,23 @@ void server_main(pp_handle* h) {
     if (progressed) continue;
     if (h->shutdown && h->n_in_flight == 0 && h->queued_photons == 0) return;
     if (h->n_in_flight > 0 && !h->resident_active) {
-      // nothing launchable and the GPU is busy.  A short launch (C3's 1e5-1e6 photons take 0.1-0.2 ms) would lose
-      // half a sleep period of latency, so first poll the oldest launch's completion event for up to 150 us
-      // (bounded spinning, only while a launch is in flight), then sleep briefly (new sources may arrive).
+      // nothing launchable and the GPU is busy: sleep through most of the time the oldest launch should still take
+      // (a running estimate of the kernel time per photon), then poll its completion event (bounded spinning, only
+      // around the expected end), so that the latency of a launch is not rounded up to a sleep period (C3)
       Slot* oldest = nullptr;
       for (auto& s : h->slot)
         if (s.in_flight && (!oldest || s.seq < oldest->seq)) oldest = &s;
       bool ready = false;
       if (oldest) {
+        const auto t_ref = std::max(oldest->t_enq, h->t_last_retire);
+        const double elapsed = std::chrono::duration<double, std::micro>(Clock::now() - t_ref).count();
+        const double left = oldest->expect_us - elapsed;
+        if (left > 250.0) {
+          h->cv_work.wait_for(lk, std::chrono::microseconds((long)std::min(left - 150.0, 2000.0)));
+          continue;  // new sources may have arrived meanwhile
+        }
         lk.unlock();
-        const auto t_end = Clock::now() + std::chrono::microseconds(150);
+        const auto t_end = Clock::now() + std::chrono::microseconds((long)(std::max(left, 0.0) + 250.0));
         do {
           ready = cudaEventQuery(oldest->ev_done) != cudaErrorNotReady;
           if (!ready) std::this_thread::yield();
