@@ -56,6 +56,40 @@ def test_absorption_and_bin_frequencies():
     assert abs(np.corrcoef(az, is0[:4000].astype(float))[0, 1]) < 0.06
 
 
+def test_wavelength_uniform_is_independent_of_the_blocks_other_uniforms():
+    """R-21 takes the wavelength uniform from the low 9 bits of words 0, 1, 2 of Philox block 0; the four uniforms of
+    R-3 use the top 23 bits of a word.  (a) The two bit sets are disjoint, exactly: changing one never changes the
+    other.  (b) Jointly uniform: chi-square of the 8 x 8 table of (wavelength uniform, each of the four uniforms) over
+    1e5 blocks, and of the wavelength uniform alone."""
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        w = [int(x) for x in rng.integers(0, 2 ** 32, 4)]
+        low = [int(x) for x in rng.integers(0, 512, 4)]
+        w_low = [(a & 0xFFFFFE00) | b for a, b in zip(w, low)]         # other low bits: the four uniforms stay
+        assert [O.uniform(a) for a in w] == [O.uniform(a) for a in w_low]
+        high = [int(x) << 9 for x in rng.integers(0, 2 ** 23, 4)]
+        w_high = [(a & 0x1FF) | b for a, b in zip(w, high)]            # other high bits: the wavelength word stays
+        assert O.spectrum_word(w) == O.spectrum_word(w_high)
+        assert O.spectrum_word(w) == O.spectrum_word((w[0], w[1], w[2], w[3] ^ 0xFFFFFFFF))  # word 3 takes no part
+    n = 100000
+    lam = np.empty(n)
+    u4 = np.empty((n, 4))
+    for i in range(n):
+        w = O.philox4x32_10((i, 3, 7, 0), (21, 0))
+        lam[i] = O.uniform(O.spectrum_word(w))
+        u4[i] = [O.uniform(x) for x in w]
+    from scipy import stats
+    bl = np.minimum((lam * 8).astype(int), 7)
+    assert stats.chisquare(np.bincount(bl, minlength=8)).pvalue > 1e-3
+    for k in range(4):
+        bu = np.minimum((u4[:, k] * 8).astype(int), 7)
+        table = np.zeros((8, 8))
+        np.add.at(table, (bl, bu), 1)
+        chi2, p, _, _ = stats.chi2_contingency(table)
+        assert p > 1e-3, (k, chi2, p)
+        assert abs(np.corrcoef(lam, u4[:, k])[0, 1]) < 4.0 / math.sqrt(n)
+
+
 def test_scattering_scale_and_arrival_times():
     # scattering scaled by (2, 0.5): flights per photon 1 + lambda_a_j / lambda_s_j with lambda_s_j = 25 / scat_scale_j
     n = 200000
