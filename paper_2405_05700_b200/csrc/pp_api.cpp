@@ -90,6 +90,7 @@ struct Slot {
   LaunchParams P;
   uint64_t seq = 0;
   bool fates = false;
+  uint64_t photons = 0;       // photons of the launch in flight (fresh tiles)
   Clock::time_point t_enq{};  // when the launch was enqueued, and how long it should take once it has the GPU
   double expect_us = 0.0;
 };
@@ -136,6 +137,7 @@ struct pp_handle {
   std::atomic<bool> shutdown{false};
   bool resident_active = false;
   int n_in_flight = 0;
+  uint64_t inflight_photons = 0;  // photons of the launches in flight
   uint64_t launch_seq = 0;
   double us_per_photon = 7.0e-5;     // running estimate of the kernel time per photon (server thread's polling)
   Clock::time_point t_last_retire{};
@@ -782,7 +784,7 @@ void server_main(pp_handle* h) {
       lk.lock();
       if (rc != PP_OK) { oldest->in_flight = false; }
       if (!oldest->in_flight) {
-        h->n_in_flight--; h->wall_t1 = Clock::now();
+        h->n_in_flight--; h->inflight_photons -= std::min(h->inflight_photons, oldest->photons); h->wall_t1 = Clock::now();
         // launches retire oldest first and their hits are queued by now: everything before sources_end is complete
         h->st.sources_completed = std::max<uint64_t>(h->st.sources_completed, oldest->sources_end);
         h->cv_hits.notify_all();
@@ -793,9 +795,12 @@ void server_main(pp_handle* h) {
     if (!h->resident_active && h->n_in_flight < 2 && h->sticky.load() == PP_OK) {
       Slot& s = h->slot[next_slot].in_flight ? h->slot[next_slot ^ 1] : h->slot[next_slot];
       Cut c{};
-      // an idle GPU is fed early: with nothing in flight a launch is cut as soon as an eighth of the target is queued
-      // ("to keep the GPU as busy as possible"); with a launch in flight the queue fills to the target
-      const bool idle_feed = h->n_in_flight == 0 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8);
+      // a GPU that is idle, or about to be, is fed early: while less than half a target is in flight, a launch is
+      // cut as soon as an eighth of the target is queued ("to keep the GPU as busy as possible"), so a
+      // job ramps up through launches of growing size instead of waiting for a full one; once enough is in flight
+      // the queue fills to the target
+      const bool idle_feed = h->inflight_photons < h->sz.target / 2 &&
+                             h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8);
       const bool force = h->flush_upto > h->ring_launch || h->space_waiters > 0 || idle_feed;
       bool have = false;
       if (!s.in_flight) {
@@ -805,7 +810,8 @@ void server_main(pp_handle* h) {
           h->cv_space.notify_all();
         } else if (h->queued_photons >= h->sz.target || force) {
           const uint64_t cap = h->sz.cap_src, base = h->ring_launch;
-          have = plan_cut([&](uint64_t i) { return (uint64_t)h->ring[(base + i) % cap].n_photons; },
+          const uint64_t b0 = base % cap;  // (one division, not one per record: a cut walks 2e5 records of C2)
+          have = plan_cut([&](uint64_t i) { const uint64_t k = b0 + i; return (uint64_t)h->ring[k < cap ? k : k - cap].n_photons; },
                           h->ring_head - base, h->launch_offset, h->sz.target, &c);
         }
       }
@@ -820,6 +826,7 @@ void server_main(pp_handle* h) {
         s.in_flight = true;  // reserve
         s.sources_end = h->ring_launch;  // a source split across launches completes with the launch that ends it
         h->n_in_flight++;
+        s.photons = c.photons; h->inflight_photons += c.photons;
         lk.unlock();
         int rc = PP_OK;
         {
@@ -832,21 +839,23 @@ void server_main(pp_handle* h) {
           if (e == cudaSuccess) e = cudaEventRecord(s.ev_h2d, s.stream);
           if (e != cudaSuccess) rc = fail(h, PP_E_CUDA, std::string("upload: ") + cudaGetErrorString(e));
           bool seg = false;  // any track segment among the records of this launch?
-          for (uint32_t q = 0; q < n_src && !seg; ++q) seg = h->ring[(rec_a + q) % cap].length > 0.0f;
+          auto rec = [&](uint32_t q) -> const SrcRec& { const uint64_t k = a + q; return h->ring[k < cap ? k : k - cap]; };
           uint32_t tile = 0, n_tiles = 0;
           pick_tiles(h, c.photons, &tile, &n_tiles);
           // a small launch onto an idle GPU keeps the single prologue kernel (one launch instead of four copies:
           // 20 us of a 0.15 ms launch, C3); every other launch gets its tables from the host
           const bool host_tables = !(idle_gpu && n_src <= kPrologueMax && n_tiles <= kPrologueMax);
           if (rc == PP_OK && host_tables && n_tiles <= h->sz.max_tiles)
-            host_prologue(s, [&](uint32_t q) { return (uint64_t)h->ring[(rec_a + q) % cap].n_photons; }, n_src, c.g_begin,
-                          tile, n_tiles);
+            host_prologue(s, [&](uint32_t q) { const SrcRec& r = rec(q); seg |= r.length > 0.0f; return (uint64_t)r.n_photons; },
+                          n_src, c.g_begin, tile, n_tiles);  // (one pass over the records: sums and the segment flag)
+          else
+            for (uint32_t q = 0; q < n_src && !seg; ++q) seg = rec(q).length > 0.0f;
           if (rc == PP_OK)
             rc = enqueue_launch(h, s, s.d_src, s.d_cum, n_src, c.g_begin, c.g_end, nullptr, seg, true, host_tables);
           if (rc == PP_OK && cudaEventSynchronize(s.ev_h2d) != cudaSuccess) rc = fail(h, PP_E_CUDA, "upload sync failed");
         }
         lk.lock();
-        if (rc != PP_OK) { s.in_flight = false; h->n_in_flight--; }
+        if (rc != PP_OK) { s.in_flight = false; h->n_in_flight--; h->inflight_photons -= std::min(h->inflight_photons, s.photons); }
         // the uploaded records are free again (a split record stays for the next launch)
         h->ring_tail = h->ring_launch;
         h->cv_space.notify_all();
@@ -1114,9 +1123,11 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
     h->next_auto_id += m;
     lk.unlock();
     uint64_t ph = 0;
+    const uint64_t p0 = pos % h->sz.cap_src;
     for (size_t j = 0; j < m; ++j, ++i) {
       const pp_source& a = src[i];
-      SrcRec& r = h->ring[(pos + j) % h->sz.cap_src];
+      const uint64_t kk = p0 + j;
+      SrcRec& r = h->ring[kk < h->sz.cap_src ? kk : kk - h->sz.cap_src];
       r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
       r.event_id = event_ids[i];
       r.source_id = source_ids ? source_ids[i] : (uint32_t)(auto_id + j);  // running record number
@@ -1134,7 +1145,7 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
     h->st.source_ring_high_water =
         std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_reserve - h->ring_tail) * sizeof(SrcRec));
     if (h->queued_photons >= h->sz.target ||
-        (h->n_in_flight == 0 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
+        (h->inflight_photons < h->sz.target / 2 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
       h->cv_work.notify_all();
   }
   return PP_OK;
