@@ -337,8 +337,8 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
   for (uint32_t i = 0; i < nl; ++i) {
     // R-20: an effective scattering length is turned into the geometric mean free path here, once
     const double ls = (double)ice->scat_len[i] * scat_scale;
-    layers[i].la = ice->abs_len[i]; layers[i].lb = (float)ls;
-    layers[i].a = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / ls);
+    layers[i].lb = (float)ls;
+    layers[i].a = layers[i].a2 = (float)(1.0 / (double)ice->abs_len[i]); layers[i].b = (float)(1.0 / ls);
   }
   layers[nl] = layers[nl - 1];
   B.n_layers = nl; B.last_layer = (int32_t)nl - 1;

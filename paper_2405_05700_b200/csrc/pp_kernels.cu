@@ -249,6 +249,32 @@ __device__ __forceinline__ float segment_fraction(const LaunchParams& P, float u
   return fmaf(x - (float)i, f1 - f0, f0);
 }
 
+// Step 6, rare path.  The fast walk only finds where the SCATTERING budget runs out and how much absorption budget is
+// left there; a remainder <= 0 means the photon was absorbed before that point.  Where that was matters only if a DOM
+// was met on the flight (or for the fate dump): walk the absorption budget tau_a forward from the photon, layer by
+// layer.  Returns the distance along the ray to the absorption point.
+__device__ __noinline__ float absorb_distance(const LaunchParams& P, float phz, float plz, float dz, float tau_a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const float w = fmaxf(fabsf(dz), 1e-9f);
+  const int last = P.last_layer;
+  const bool up = dz > 0.0f;
+  int l = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
+  l = max(0, min(l, last));
+  const int i1 = l + (up ? 0 : 1);
+  float h = fabsf((fmaf(-P.dz_layer, (float)i1, P.z_top) - phz) - plz);  // to the boundary ahead (two-float z)
+  float T = tau_a * w, V = 0.0f;                                         // vertical budget, vertical distance so far
+  for (;;) {
+    const float a = *reinterpret_cast<const float*>(smem_raw + (uint32_t)l * 32u);  // absorption coefficient
+    const bool open = up ? (l == 0) : (l == last);  // the end layers are infinite (R-6)
+    const float need = a * h;
+    if (open || T <= need) return (V + T / a) / w;
+    T -= need;
+    V += h;
+    l += up ? -1 : 1;
+    h = P.dz_layer;
+  }
+}
+
 // Fetch the next work item of the launch for a warp (lane 0 talks to the queues; rare: once per tile).
 // Returns the warp-uniform (t_next, t_end, s_cur, resume list not yet empty); t_next == t_end means no work is left.
 __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, bool use_resume) {
@@ -301,13 +327,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     for (uint32_t i = threadIdx.x; i < n16; i += blockDim.x) dst[i] = __ldg(P.smem_image + i);
   }
   __syncthreads();
-  // layer records at offset 0: coefficients (a, b, 1/a, 1/b) of layer i, cumulative depths at boundary i
-  auto lay = [&](int i) { return *reinterpret_cast<const float4*>(smem_raw + (uint32_t)i * 32u); };
-  auto walk = [&](int i) { return *reinterpret_cast<const float4*>(smem_raw + (uint32_t)i * 32u + 16u); };
+  // layer records at offset 0: coefficients (a, b, 1/b, a) of layer i, cumulative depths at boundary i
   auto walk_B = [&](int i) { return *reinterpret_cast<const float*>(smem_raw + (uint32_t)i * 32u + 16u); };
-  auto walk_A = [&](int i) { return *reinterpret_cast<const float*>(smem_raw + (uint32_t)i * 32u + 20u); };
   const uint16_t* const s_inv_b = reinterpret_cast<const uint16_t*>(smem_raw + P.off_inv_b);
-  const uint16_t* const s_inv_a = reinterpret_cast<const uint16_t*>(smem_raw + P.off_inv_a);
   const float2* const s_str_xy = reinterpret_cast<const float2*>(smem_raw + P.off_str_xy);
   const uint16_t* const s_cell = reinterpret_cast<const uint16_t*>(smem_raw + P.off_cell);
   // the warp's current source record (a2): staged once per (tile, source) run, read by the lanes that refill
@@ -436,45 +458,48 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const bool up = dz > 0.0f;
     const int last = P.last_layer;
     // Direct walk, branch-free.  h0 is the vertical distance to the boundary ahead, i1; the flight reaches it with
-    // budgets t1, t2 left (negative: it ends before).  With B(i), A(i) the cumulative vertical optical depths at the
-    // boundaries (two-float sums), the cumulative depths X at which the budgets run out name the layers js, ja
-    // (inverse table + one compare-and-step); the nearer one, clamped to the photon's side of its own layer, is the
-    // layer lj where the flight ends.  lj = li (always so in an end layer with no boundary ahead, R-6): the budgets
-    // are spent in layer li, as they are.  Otherwise the budgets left at lj's entry boundary come from the two-float
-    // sums, so their error is relative to the budget, not to the cumulative depth.  Coefficients and sums come from
-    // one record each at the start and at the end (LayerRec, pp_types.h).
+    // budgets t1 (scattering), t2 (absorption) left (negative: it ends before).  With B(i), A(i) the cumulative
+    // vertical optical depths at the boundaries (two-float sums), the cumulative depth X = B(i1) +- t1 at which the
+    // scattering budget runs out names the layer js (inverse table + one compare-and-step); clamped to the photon's
+    // side of its own layer it is the layer lj where the flight would scatter.  lj = li (always so in an end layer
+    // with no boundary ahead, R-6): the budgets are spent in layer li, as they are.  Otherwise the budgets left at
+    // lj's entry boundary come from the two-float sums, so their error is relative to the budget, not to the
+    // cumulative depth.  Coefficients and sums come from one record each at the start and at the end (LayerRec,
+    // pp_types.h).  The absorption budget is only FOLLOWED to the scatter point: what is left of it there becomes
+    // the new tau_a, and a remainder <= 0 means the photon was absorbed on the way (where exactly is worked out in
+    // the rare path, absorb_distance, when a DOM was met on the flight).
     const float sgn = up ? -1.0f : 1.0f;
     int li = (int)floorf((P.z_top - phz) * P.inv_dz_layer);
     li = max(0, min(li, last));
     const int i1 = li + (up ? 0 : 1);
     const float h0 = fabsf((fmaf(-P.dz_layer, (float)i1, P.z_top) - phz) - plz);  // two-float z
     const unsigned char* const rec0 = smem_raw + (up ? 0u : P.off_rec_b) + (uint32_t)li * 32u;
-    const float4 L0 = *reinterpret_cast<const float4*>(rec0), W1 = *reinterpret_cast<const float4*>(rec0 + 16);
+    const float2 L0 = *reinterpret_cast<const float2*>(rec0);  // a, b of layer li
+    const float4 W1 = *reinterpret_cast<const float4*>(rec0 + 16);
     const float Ts0 = tau_s * w, Ta0 = tau_a * w;
     const float t1 = fmaf(-L0.y, h0, Ts0), t2 = fmaf(-L0.x, h0, Ta0);
-    const float Xs = fmaf(sgn, t1, W1.x), Xa = fmaf(sgn, t2, W1.y);
+    const float Xs = fmaf(sgn, t1, W1.x);
     const float xs_l = fmaf(sgn, t1, W1.z), xa_l = fmaf(sgn, t2, W1.w);  // lo parts of the two-float X
     int js = s_inv_b[min(__float2uint_rz(fmaf(Xs, P.k_b, -1e-3f)), P.m_b)];
-    int ja = s_inv_a[min(__float2uint_rz(fmaf(Xa, P.k_a, -1e-3f)), P.m_a)];
     js += (walk_B(js + 1) <= Xs) ? 1 : 0;
-    ja += (walk_A(ja + 1) <= Xa) ? 1 : 0;
     if (kLoop) {
       while (js < last && walk_B(js + 1) <= Xs) ++js;
-      while (ja < last && walk_A(ja + 1) <= Xa) ++ja;
     }
-    const int lj = up ? min(max(js, ja), li) : max(min(js, ja), li);
+    const int lj = up ? min(js, li) : max(js, li);
     const unsigned char* const rec1 = smem_raw + (up ? P.off_rec_b : 0u) + (uint32_t)lj * 32u;
-    const float4 L4 = *reinterpret_cast<const float4*>(rec1), Wb = *reinterpret_cast<const float4*>(rec1 + 16);
+    const float2 L4 = *reinterpret_cast<const float2*>(rec1 + 8);  // 1/b, a of layer lj
+    const float4 Wb = *reinterpret_cast<const float4*>(rec1 + 16);
     // (selects through select_eq: the compiler would otherwise branch around the three right-hand sides, and nearly
     // every warp holds lanes of both kinds)
     const float Ts = select_eq(lj, li, Ts0, sgn * ((W1.x - Wb.x) + (xs_l - Wb.z)));
     const float Ta = select_eq(lj, li, Ta0, sgn * ((W1.y - Wb.y) + (xa_l - Wb.w)));
     const float Vb = select_eq(lj, li, 0.0f, fmaf(P.dz_layer, (float)(abs(lj - li) - 1), h0));
-    const float vs = Ts * L4.w, va = Ta * L4.z;  // vertical distance left in the final layer
-    const bool absorbed = va <= vs;
-    const float v_in = fminf(vs, va);
-    const float s = (Vb + v_in) * inv_w;
-    tau_a = fmaxf(0.0f, fmaf(-L4.x, v_in, Ta)) * inv_w;
+    const float vs = Ts * L4.x;                   // vertical distance to the scatter point in the final layer
+    const float s = (Vb + vs) * inv_w;            // ... and the flight's length if the photon gets that far
+    const float Ta_left = fmaf(-L4.y, vs, Ta);    // absorption budget left at the scatter point (vertical)
+    const bool absorbed = !(Ta_left > 0.0f);      // ties: absorbed (s_abs <= s_scat)
+    const float tau_a0 = tau_a;                   // (kept for the rare path below)
+    tau_a = Ta_left * inv_w;
     // =========================== a5: DOM intersection on [0, s] ===============================
     Best best{inf, 0xFFFFFFFFu};
     if (kBrute) {
@@ -519,7 +544,13 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     bool hit = alive && best.t <= s;
     const uint32_t hit_dom = best.dom;
     // =========================== a6: advance / terminate ======================================
-    const float adv = hit ? best.t : s;
+    float s_end = s;
+    if (kFates ? (alive && absorbed) : (hit && absorbed)) {
+      // the photon was absorbed before the scatter point: where?  (rare in the lean variant: a DOM was met too)
+      s_end = fminf(s, absorb_distance(P, phz, plz, dz, tau_a0));
+      hit = hit && best.t <= s_end;
+    }
+    const float adv = hit ? best.t : s_end;
     {
       // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
       // more fma (exact unless |p| << |d*adv| ulp-wise, where it is negligible anyway)

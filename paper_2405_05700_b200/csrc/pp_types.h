@@ -63,7 +63,9 @@ constexpr uint16_t kNoString = 0xFFFFu;  // host-side marker while the cell tabl
 // of the boundary it faces (start) or entered through (end) from ONE record: the first array going up at the start
 // and down at the end, the second one otherwise.
 struct __align__(16) LayerRec {
-  float a, b, la, lb;     // 1/m, 1/m, m, m
+  float a, b;             // absorption and scattering coefficients, 1/m: what a flight needs where it starts ...
+  float lb, a2;           // ... and where it ends: the scattering length (m) and the absorption coefficient again,
+                          // so that either pair is one 8-byte load
   float Bh, Ah, Bl, Al;
 };
 
