@@ -119,7 +119,7 @@ typedef struct pp_config {
   void* stream0; /* cudaStream_t */
   void* stream1; /* cudaStream_t */
   uint32_t flags;
-  uint32_t max_flights; /* safety cap on flights per photon (default 100000, R-10) */
+  uint32_t max_flights; /* safety cap on flights per photon (default 100000, R-10); < 2^31 */
   int32_t device;       /* CUDA device ordinal (default: current device) */
   uint32_t reserved;
 } pp_config;

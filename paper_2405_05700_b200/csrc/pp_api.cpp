@@ -352,6 +352,7 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
     uint32_t k0 = (uint32_t)cfg->seed, k1 = (uint32_t)(cfg->seed >> 32);
     for (int r = 0; r < 10; ++r) { B.rk[r][0] = k0; B.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
   }
+  if (cfg->max_flights >= 0x80000000u) return PP_E_INVAL;  // the kernel keeps a flag in the counter's top bit
   B.max_flights = cfg->max_flights ? cfg->max_flights : 100000u;
   B.tile_photons = kTilePhotons;
   const uint32_t ns = (uint32_t)h->hg.strings.size();
@@ -362,7 +363,7 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
   B.rm2 = B.radius_margin * B.radius_margin;
   B.xy_cap2 = h->hg.xy_cap * h->hg.xy_cap; B.inv_xy_cap = 1.0f / h->hg.xy_cap;
   // ---- a4: tables of the direct layer walk (pp_types.h) ----
-  std::vector<uint16_t> inv_tab[2];
+  std::vector<uint16_t> inv_tab;  // layer holding a cumulative SCATTERING depth (the walk follows absorption along)
   {
     std::vector<double> cum[2] = {std::vector<double>(nl + 1, 0.0), std::vector<double>(nl + 1, 0.0)};  // B, A
     for (uint32_t i = 0; i < nl; ++i) {
@@ -376,7 +377,8 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
     }
     layers[nl].Bh = layers[nl].Ah = INFINITY; layers[nl].Bl = layers[nl].Al = 0.0f;
     B.walk_loop = 0;
-    for (int t = 0; t < 2; ++t) {
+    {
+      const int t = 0;
       // bin width: just under the thinnest layer, so that a bin holds at most one boundary; coarser (and the
       // kernel then loops) if that would need more than kMaxWalkInv bins
       double thin = 1e300;
@@ -385,16 +387,16 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
       double step = 0.99 * thin;
       if (top / step + 3.0 > (double)kMaxWalkInv) { step = top / ((double)kMaxWalkInv - 3.0); B.walk_loop = 1; }
       const uint32_t m = (uint32_t)std::ceil(top / step) + 1;  // bins 0..m
-      inv_tab[t].resize(m + 1);
+      inv_tab.resize(m + 1);
       uint32_t j = 0;
       for (uint32_t b = 0; b <= m; ++b) {
         // a lower bound of the layer for every depth that can land in bin b (index rounding slack 4e-3 bins)
         const double x = ((double)b - 4e-3) * step;
-        while (j + 1 < nl && (double)(t == 0 ? layers[j + 1].Bh : layers[j + 1].Ah) <= x) ++j;
-        inv_tab[t][b] = (uint16_t)j;
+        while (j + 1 < nl && (double)layers[j + 1].Bh <= x) ++j;
+        inv_tab[b] = (uint16_t)j;
       }
-      (t == 0 ? B.m_b : B.m_a) = m;
-      (t == 0 ? B.k_b : B.k_a) = (float)(1.0 / step);
+      B.m_b = m;
+      B.k_b = (float)(1.0 / step);
     }
   }
   // ---- the image ----
@@ -428,8 +430,7 @@ int build_tables(pp_handle* h, const pp_geometry* geo, const pp_ice* ice, const 
     rec_b[nl] = rec_b[nl - 1];
     B.off_rec_b = put(rec_b.data(), rec_b.size() * sizeof(LayerRec));
   }
-  B.off_inv_b = put(inv_tab[0].data(), inv_tab[0].size() * sizeof(uint16_t));
-  B.off_inv_a = put(inv_tab[1].data(), inv_tab[1].size() * sizeof(uint16_t));
+  B.off_inv_b = put(inv_tab.data(), inv_tab.size() * sizeof(uint16_t));
   B.off_str_xy = put(str_xy.data(), str_xy.size() * sizeof(float2));
   B.off_cell = put(cell.data(), cell.size() * sizeof(uint16_t));
   B.off_str_a = put(str_a.data(), str_a.size() * sizeof(float4));

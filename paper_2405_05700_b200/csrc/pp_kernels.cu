@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(1024) prologue_kernel(const SrcRec* __restrict
 #endif
 constexpr int kBlockThreads = PP_BLOCK_THREADS;
 constexpr int kMaxDevices = 64;
+constexpr uint32_t kDeadBit = 0x80000000u;  // top bit of a lane's flight counter: the lane holds no photon
 
 // Shared-memory tables: one image built by the host (LaunchParams::smem_image), copied verbatim by every CTA.
 
@@ -350,13 +351,14 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   uint32_t w_started = 0, w_hits = 0, w_flights = 0;
 
   // ---- per-lane photon state (a dead lane keeps computing on its stale state; nothing it produces is used) ----
-  bool alive = false;
   float phx = 0, phy = 0, phz = 0, plx = 0, ply = 0, plz = 0;  // position, two-float (hi + lo)
   float dx = 0, dy = 0, dz = 1;
   float Lh = 0, Ll = 0;  // path length, two-float
   float tau_a = 0;
   float sc_b = 1.0f;  // kExt only: 1 / scat_scale of the photon's wavelength bin (R-21)
-  uint32_t ev = 0, sid = 0, pidx = 0, k = 0, s_mine = 0;
+  // k = flights started so far = index of the next Philox block; its top bit marks a DEAD lane (no register for a
+  // flag; max_flights < 2^31 is checked at pp_create)
+  uint32_t ev = 0, sid = 0, pidx = 0, k = kDeadBit, s_mine = 0;
 
   // A new run (rare: once per source of a work item): the next source of the current work item, or a new work item
   // (resume list first, then tiles).  Leaves t_next < run_end, or refill_ok = false when no work is left.
@@ -387,11 +389,11 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     // =========================== refill dead lanes (a2 -> a3) ===========================
     // t_next < run_end whenever refill_ok: the next run is fetched as soon as the current one is used up, and a
     // refill that uses it up goes on with the next one, so lanes stay dead only when the launch has run dry
-    unsigned need_mask = __ballot_sync(0xffffffffu, !alive);
+    unsigned need_mask = __ballot_sync(0xffffffffu, (int)k < 0);
     while (need_mask != 0u && refill_ok) {
       // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
       const uint32_t r = t_next + __popc(need_mask & lt);
-      if (!alive && r < run_end) {
+      if ((int)k < 0 && r < run_end) {
         float4 r0; float2 r1; uint2 r2;
         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w) : "r"(wsrc_addr));
         asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+16];" : "=f"(r1.x), "=f"(r1.y) : "r"(wsrc_addr));
@@ -401,14 +403,14 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         Lh = 0.0f; Ll = 0.0f;
         ev = r2.x; sid = r2.y;
         pidx = r - pbase;
-        k = 0; s_mine = s_cur;
-        alive = true;
+        k = 0; s_mine = s_cur;  // alive
       }
       t_next = min(t_next + (uint32_t)__popc(need_mask), run_end);
       if (t_next != run_end) break;
       next_run();
-      need_mask = __ballot_sync(0xffffffffu, !alive);
+      need_mask = __ballot_sync(0xffffffffu, (int)k < 0);
     }
+    const bool alive = (int)k >= 0;
     const unsigned alive_mask = __ballot_sync(0xffffffffu, alive);
     if (alive_mask == 0u) break;  // nothing left to refill from
     w_flights += __popc(alive_mask);  // every live lane flies once per iteration
@@ -652,7 +654,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         reinterpret_cast<pp_fate*>(P.fates)[g] = f;
       }
     }
-    alive = alive && !done;
+    k |= done ? kDeadBit : 0u;  // (a dead lane stays dead whatever its stale state says)
   }
 
   // ---- leftovers of a stopped warp go to the next launch; fold the counters ----

@@ -78,9 +78,10 @@ struct LaunchParams {
   float one_minus_cos_c;                                // 1 - cos(theta_c)
   float z_top, inv_dz_layer, dz_layer;
   int32_t last_layer;                                   // n_layers - 1
-  float k_b, k_a;                                       // inverse-table index = cumulative depth * k
-  uint32_t m_b, m_a;                                    // largest inverse-table index
-  uint32_t off_inv_b, off_inv_a, off_str_xy, off_cell;  // byte offsets into dynamic shared memory (layer records at 0)
+  float k_b;                                            // inverse-table index = cumulative scattering depth * k_b
+  uint32_t m_b;                                         // largest inverse-table index
+  uint32_t off_inv_b, off_rec_b;                        // byte offsets into dynamic shared memory (layer records at 0)
+  uint32_t off_str_xy, off_cell, pad0, pad1;
   float inv_cell, cell_ox, cell_oy;                     // cell coordinate = x * inv_cell + cell_ox
   float rm2;                                            // radius_margin^2 (pre-filter)
   uint32_t nx_m1, ny_m1, nx;
@@ -88,7 +89,7 @@ struct LaunchParams {
   float inv_xy_cap;
   uint32_t max_flights;
   uint32_t ring_cap;
-  uint32_t off_rec_b;                                   // byte offset of the second layer-record array (below)
+  uint32_t pad2;
   // ---- work ----
   const SrcRec* src;
   const unsigned long long* cum;  // [n_src + 1] exclusive prefix of n_photons (batch-global photon numbers)
@@ -106,11 +107,11 @@ struct LaunchParams {
   void* fates;        // pp_fate[g_end] or nullptr
   // ---- tables ----
   // Image of the shared-memory tables, copied verbatim into dynamic shared memory by every CTA (smem_image_bytes, a
-  // multiple of 16): [LayerRec x (n_layers + 1)] [u16 inv_b x (m_b + 1)] [u16 inv_a x (m_a + 1)]
+  // multiple of 16): [LayerRec x (n_layers + 1)] [LayerRec x (n_layers + 1), second array] [u16 inv_b x (m_b + 1)]
   // [float2 line xy x (n_strings + 1)] [u16 cell x (nx ny)] [float4 line (x, y, z0, 1/pitch) x n_strings]
   // [uint2 line (n, base) x n_strings].
-  //  * inv_b / inv_a map a quantised cumulative depth to a layer j0 such that the layer holding that depth is j0 or
-  //    j0 + 1 (or beyond, when walk_loop is set for a coarse table).
+  //  * inv_b maps a quantised cumulative scattering depth to a layer j0 such that the layer holding that depth is j0
+  //    or j0 + 1 (or beyond, when walk_loop is set for a coarse table).
   //  * cell table (a5): cell (ix, iy) of a uniform grid over the footprint names THE line of DOMs whose pre-filter disc
   //    can be met by a piece of flight whose xy midpoint lies in that cell; n_strings if none: that entry of the line
   //    xy table holds NaN, so the pre-filter fails without a branch.  Unique because a piece is at most xy_cap long in
@@ -144,7 +145,7 @@ struct LaunchParams {
   float acc_coef[8];
 };
 static_assert(offsetof(LaunchParams, hg_one_minus_g) % 16 == 0 && offsetof(LaunchParams, z_top) % 16 == 0 &&
-              offsetof(LaunchParams, k_b) % 16 == 0 && offsetof(LaunchParams, off_inv_b) % 16 == 0 &&
+              offsetof(LaunchParams, k_b) % 16 == 0 && offsetof(LaunchParams, off_str_xy) % 16 == 0 &&
               offsetof(LaunchParams, inv_cell) % 16 == 0 && offsetof(LaunchParams, nx_m1) % 16 == 0 &&
               offsetof(LaunchParams, inv_xy_cap) % 16 == 0, "hot parameter groups must be 16-byte aligned");
 
