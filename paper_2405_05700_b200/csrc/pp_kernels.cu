@@ -497,7 +497,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const float Ta = select_eq(lj, li, Ta0, sgn * ((W1.y - Wb.y) + (xa_l - Wb.w)));
     const float Vb = select_eq(lj, li, 0.0f, fmaf(P.dz_layer, (float)(abs(lj - li) - 1), h0));
     const float vs = Ts * L4.x;                   // vertical distance to the scatter point in the final layer
-    const float s = (Vb + vs) * inv_w;            // ... and the flight's length if the photon gets that far
+    // ... and the flight's length if the photon gets that far; kept finite (a near-horizontal flight in ice that
+    // hardly scatters overflows), so that "no DOM" (t = inf) never compares as a hit
+    const float s = fminf((Vb + vs) * inv_w, 3.0e38f);
     const float Ta_left = fmaf(-L4.y, vs, Ta);    // absorption budget left at the scatter point (vertical)
     const bool absorbed = !(Ta_left > 0.0f);      // ties: absorbed (s_abs <= s_scat)
     const float tau_a0 = tau_a;                   // (kept for the rare path below)
@@ -543,15 +545,17 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         tm += ds;
       }
     }
-    bool hit = alive && best.t <= s;
+    bool hit = best.t <= s;  // (a dead lane never looks for DOMs: its best.t is inf)
     const uint32_t hit_dom = best.dom;
     // =========================== a6: advance / terminate ======================================
     float s_end = s;
-    if (kFates ? (alive && absorbed) : (hit && absorbed)) {
-      // the photon was absorbed before the scatter point: where?  (rare in the lean variant: a DOM was met too)
+    if (kFates && alive && absorbed) {
+      // the fate dump wants the end point of every absorbed photon: where was it absorbed?
       s_end = fminf(s, absorb_distance(P, phz, plz, dz, tau_a0));
       hit = hit && best.t <= s_end;
     }
+    // (the lean variant asks that question only for a photon that also met a DOM on this flight, in the rare
+    // block below; until then `hit` may hold a DOM that lies behind the absorption point)
     const float adv = hit ? best.t : s_end;
     {
       // compensated position: sum = fl(p + d*adv); the rounding error is recovered with one
@@ -570,6 +574,13 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     unsigned hit_mask = __ballot_sync(0xffffffffu, hit || aborted);
     if (hit_mask) {
       if (aborted) atomicAdd(&st->photons_aborted, 1ull);  // never in practice (R-10)
+      if (!kFates && hit && absorbed) {
+        // absorbed before the scatter point AND a DOM on the way: which came first?  The photon has been advanced to
+        // the DOM already (it is dead either way), so its start height is recovered from there, as a two-float.
+        const float z0 = fmaf(-dz, adv, phz);
+        const float z0l = plz + fmaf(-dz, adv, phz - z0);
+        hit = adv <= absorb_distance(P, z0, z0l, dz, tau_a0);
+      }
       hit_mask = __ballot_sync(0xffffffffu, hit);
       float weight = 1.0f;
       if (kExt && P.acc_mode != 0u && hit_mask) {
