@@ -389,11 +389,16 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     // =========================== refill dead lanes (a2 -> a3) ===========================
     // t_next < run_end whenever refill_ok: the next run is fetched as soon as the current one is used up, and a
     // refill that uses it up goes on with the next one, so lanes stay dead only when the launch has run dry
+    // (no test in front of the loop: nearly every iteration has dead lanes, and with none, or with nothing to refill
+    // from -- run_end == t_next then --, the body assigns nothing and leaves at once)
     unsigned need_mask = __ballot_sync(0xffffffffu, (int)k < 0);
-    while (need_mask != 0u && refill_ok) {
+    for (;;) {
       // ---- a2/a3: initial state of photon r of the launch (fused expansion) ----
-      const uint32_t r = t_next + __popc(need_mask & lt);
-      if ((int)k < 0 && r < run_end) {
+      // (compared as "rank < photons left in the run": t_next + rank may wrap for a warp that holds no work item
+      // in a launch whose first photon is not the first of its source)
+      const uint32_t rank = __popc(need_mask & lt), avail = run_end - t_next;
+      const uint32_t r = t_next + rank;
+      if ((int)k < 0 && rank < avail) {
         float4 r0; float2 r1; uint2 r2;
         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r0.x), "=f"(r0.y), "=f"(r0.z), "=f"(r0.w) : "r"(wsrc_addr));
         asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+16];" : "=f"(r1.x), "=f"(r1.y) : "r"(wsrc_addr));
@@ -405,8 +410,8 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         pidx = r - pbase;
         k = 0; s_mine = s_cur;  // alive
       }
-      t_next = min(t_next + (uint32_t)__popc(need_mask), run_end);
-      if (t_next != run_end) break;
+      t_next += min((uint32_t)__popc(need_mask), avail);
+      if (t_next != run_end || !refill_ok) break;
       next_run();
       need_mask = __ballot_sync(0xffffffffu, (int)k < 0);
     }
@@ -644,6 +649,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         if (def_mask) {
           // the replay will count these photons (and their flights) again: take them out here
           refill_ok = false;
+          run_end = t_next;  // (nothing more is handed out; [t_next, t_end) goes to the resume list at the end)
           w_started -= __popc(def_mask);
           w_flights -= __reduce_add_sync(0xffffffffu, deferred ? k : 0u);
         }

@@ -11,6 +11,12 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: longer statistical test")
+    # a hung kernel or a dead-locked server must fail the run, not stall it: with pytest-timeout installed every test
+    # gets 15 minutes unless the command line says otherwise ('thread' method: works while blocked in a C call)
+    if config.pluginmanager.hasplugin("timeout") and not getattr(config.option, "timeout", None):
+        config.option.timeout = 900.0
+        config.option.timeout_method = "thread"
+        config._env_timeout, config._env_timeout_method = 900.0, "thread"  # (the plugin has read its settings already)
     # build the CUDA library (nvcc cross-compiles without a GPU) and the oracle; both builders compare modification
     # times, so an up-to-date binary is left alone and a stale one is never what the tests exercise
     from paper_2405_05700_b200 import build as pp_build

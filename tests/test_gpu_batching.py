@@ -40,6 +40,19 @@ def test_launch_size_invariance(case, reference_hits, target):
     assert st.launches == -(-n // target)
 
 
+def test_launch_that_starts_a_few_photons_into_a_source():
+    """A launch whose first photon is the 8th of its source, with thousands of warps that get no work item: their
+    (empty) photon range then sits just below 2^32 in launch-relative numbering, where "next photon + lane rank" wraps
+    (regression: such warps once refilled themselves for ever)."""
+    geo, ice = W.geometry_full(radius=2.0), W.ice_layered()
+    src = W.sources_c1().subset(slice(0, 6))
+    src.src[:, 7] = np.array([0.9993, 5.0, 0.0031, 2.0, 0.0007, 1.5], np.float32)  # 9993, 50000, 31, 20000, 7, 15000 photons
+    ref, _ = gpu_run(geo, ice, src, 4)
+    hits, st = gpu_run(geo, ice, src, 4, launch_photons_target=10000)  # launch 2 starts at photon 7 of source 1
+    assert st.photons_done == total_photons(src, ice) and st.launches == -(-st.photons_done // 10000)
+    assert len(ref) > 50 and np.array_equal(hits, ref)
+
+
 def test_resident_path_equals_server_path(case, reference_hits):
     geo, ice, src = case
     hits, _, st = gpu_run_resident(geo, ice, src, 9, launch_photons_target=300000)
