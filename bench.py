@@ -540,13 +540,15 @@ def _ipc_client_main(name, client, n_clients, replicas, block_sources, barrier, 
         n_hits = 0
         with ipc.IpcClient(name) as c:
             barrier.wait()
+            t_first = time.time()  # (wall-clock stamps: comparable across the client processes)
             for r_, e_, s_ in blocks:
                 c.submit(r_, e_, s_)
                 n_hits += len(c.collect(block=False))
             n_hits += len(c.collect_all())
-        q.put((client, n_hits, len(blocks)))
+            t_drained = time.time()
+        q.put((client, n_hits, len(blocks), t_first, t_drained))
     except Exception as e:  # pragma: no cover
-        q.put((client, repr(e), 0))
+        q.put((client, repr(e), 0, 0.0, 0.0))
 
 
 def run_stream_ipc(args):
@@ -588,10 +590,14 @@ def run_stream_ipc(args):
         raise SystemExit(f"ipc client failed: {bad}")
     ph = st1.photons_done - st0.photons_done
     busy = (st1.kernel_busy_ms - st0.kernel_busy_ms) * 1e-3
+    # the job as the clients see it: from the first client's first submit to the last client's drain (the outer clock
+    # also counts the wake-up from the start barrier and the result queue of N Python processes)
+    wall_outer, wall = wall, max(r[4] for r in res) - min(r[3] for r in res)
     print(json.dumps({"mode": "stream-ipc", "workload": f"C2 x {args.replicas} replicas shipped in blocks of {args.block_sources} "
                       f"sources by {n} client processes over shared memory", "client_processes": n,
                       "blocks": int(sum(r[2] for r in res)), "photons": int(ph), "launches": st1.launches - st0.launches,
                       "photons_per_s": ph / wall, "device_busy_frac": busy / wall, "wall_s": wall, "kernel_s": busy,
+                      "wall_s_outer": wall_outer, "device_busy_frac_outer": busy / wall_outer,
                       "hits": int(sum(r[1] for r in res)), "hits_unrouted": ist["hits_unrouted"],
                       "server_blocks_ingested": ist["blocks_ingested"]}), flush=True)
     return 0

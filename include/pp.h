@@ -175,6 +175,21 @@ int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids,
 int pp_submit_segments(pp_handle* h, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
                        const uint32_t* source_ids, size_t n);
 
+/* One light source with everything pp_submit_segments takes for it, as ONE 48-byte record (array of structures). */
+typedef struct pp_packed_source {
+  pp_source s;
+  float length_m;     /* 0 = point source (R-18) */
+  uint32_t event_id;
+  uint32_t source_id;
+  uint32_t reserved;  /* ignored */
+} pp_packed_source;
+
+/* pp_submit_segments for n packed records (HOST): the same checks, the same semantics, explicit source ids; one pass
+ * over one array instead of four.  This is what the multi-process front end (pp_ipc.h) moves from its shared-memory
+ * rings into the handle: at C2's 400 photons per source a B200 consumes 4e7 sources/s ("a block of
+ * steps is sent to the GPU"), which is within sight of what one ingest thread can copy. */
+int pp_submit_packed(pp_handle* h, const pp_packed_source* records, size_t n);
+
 /* Longitudinal profile of extended sources (NEXT-2, reading R-23): where along its length a source of
  * pp_submit_segments emits.  The offset of a photon becomes l = L F(u) with the same u as above and F piecewise
  * linear through the n_knots values cum_fraction[i] at u = i / (n_knots - 1): an inverse cumulative distribution given

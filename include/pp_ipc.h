@@ -62,6 +62,9 @@ typedef struct pp_ipc_backend {
                                             everything submitted before this call has been propagated and handed out */
   int (*completed)(void* ctx, uint64_t* n_sources); /* the first n_sources sources, in submit order, are fully
                                             propagated and their hits can be collected (pp_stats.sources_completed) */
+  int (*submit_packed)(void* ctx, const pp_packed_source* records, size_t n); /* optional (may be NULL): the same as
+                                            submit for packed records (pp_submit_packed); the ingest thread then hands
+                                            the ring's records over as they lie, in one pass */
 } pp_ipc_backend;
 
 /* Creates (O_CREAT | O_EXCL) the shared-memory segment `shm_name` ("/name"), and starts the ingest and dispatch

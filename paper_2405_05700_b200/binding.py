@@ -69,7 +69,7 @@ class _Stats(C.Structure):
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
            "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum",
-           "pp_set_emission_smearing", "pp_set_segment_profile"]
+           "pp_set_emission_smearing", "pp_set_segment_profile", "pp_submit_packed"]
 
 
 class _LaunchPlan(C.Structure):
@@ -98,6 +98,8 @@ def load_library(path: str = LIB_PATH):
     L.pp_submit.argtypes = [vp, vp, vp, vp, C.c_size_t]
     L.pp_submit_segments.restype = C.c_int
     L.pp_submit_segments.argtypes = [vp, vp, vp, vp, vp, C.c_size_t]
+    L.pp_submit_packed.restype = C.c_int
+    L.pp_submit_packed.argtypes = [vp, vp, C.c_size_t]
     L.pp_flush.restype = C.c_int
     L.pp_flush.argtypes = [vp]
     L.pp_collect.restype = C.c_int
@@ -180,6 +182,24 @@ def plan_launches(photon_counts, target: int):
         if rc != PP_OK:
             raise PPError(rc, "pp_debug_plan_launches")
         return [(int(b.first_source), int(b.n_sources), int(b.g_begin), int(b.g_end)) for b in buf[: n_out.value]]
+
+
+# pp_packed_source (include/pp.h): a source with its length and ids as one 48-byte record
+PACKED_DTYPE = np.dtype([("src", np.float32, (8,)), ("length_m", np.float32), ("event_id", np.uint32),
+                         ("source_id", np.uint32), ("reserved", np.uint32)])
+assert PACKED_DTYPE.itemsize == 48
+
+
+def pack_records(sources, event_ids, source_ids, lengths=None) -> np.ndarray:
+    """float32 [n, 8] rows + ids (+ lengths) -> pp_packed_source records."""
+    a = np.ascontiguousarray(sources, dtype=np.float32).reshape(-1, 8)
+    out = np.zeros(a.shape[0], PACKED_DTYPE)
+    out["src"] = a
+    out["event_id"] = event_ids
+    out["source_id"] = source_ids
+    if lengths is not None:
+        out["length_m"] = lengths
+    return out
 
 
 def pack_sources(src: np.ndarray) -> np.ndarray:
@@ -294,6 +314,11 @@ class Propagator:
             rc = self._L.pp_submit_segments(self._h, rec.ctypes.data, ln.ctypes.data, ev.ctypes.data,
                                             None if sid is None else sid.ctypes.data, rec.shape[0])
         self._check(rc, self._h)
+
+    def submit_packed(self, records):
+        """pp_submit_packed: PACKED_DTYPE [n] records (see pack_records); host buffer; thread-safe."""
+        rec = np.ascontiguousarray(records, dtype=PACKED_DTYPE)
+        self._check(self._L.pp_submit_packed(self._h, rec.ctypes.data, rec.shape[0]), self._h)
 
     def set_acceptance(self, mode: str = "off", coef=()):
         """pp_set_acceptance: ``mode`` in ACCEPTANCE_MODES; ``coef`` = polynomial coefficients in d_z."""

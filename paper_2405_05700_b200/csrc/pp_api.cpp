@@ -1076,23 +1076,27 @@ int pp_submit(pp_handle* h, const pp_source* src, const uint32_t* event_ids, con
   return pp_submit_segments(h, src, nullptr, event_ids, source_ids, n);
 }
 
-int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths, const uint32_t* event_ids,
-                       const uint32_t* source_ids, size_t n) {
-  if (!h) return PP_E_INVAL;
-  if (h->sticky.load() != PP_OK) return h->sticky.load();
-  if (n == 0) return PP_OK;
-  if (!src || !event_ids) return fail(h, PP_E_INVAL, "null sources or event_ids");
+}  // extern "C"
+
+namespace {
+// One light source as the submit path sees it, whatever the caller's layout.
+struct SrcView { const pp_source* s; float length; uint32_t event_id; bool has_id; uint32_t source_id; };
+
+// pp_submit / pp_submit_segments / pp_submit_packed: `at(i)` is the i-th source of the call.
+template <class At>
+int submit_generic(pp_handle* h, size_t n, At at) {
   const float yield = h->ice.photons_per_GeV;
   // validate everything before enqueueing anything
   for (size_t i = 0; i < n; ++i) {
-    const pp_source& a = src[i];
-    const float v[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
-    for (float f : v)
+    const SrcView v = at(i);
+    const pp_source& a = *v.s;
+    const float f8[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
+    for (float f : f8)
       if (!std::isfinite(f)) return fail(h, PP_E_INVAL, "non-finite field in source " + std::to_string(i));
     const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
     if (std::fabs(n2 - 1.0) > 1e-4) return fail(h, PP_E_INVAL, "source direction is not a unit vector");
     if (a.energy_GeV < 0.0f) return fail(h, PP_E_INVAL, "negative source energy");
-    if (lengths && !(std::isfinite(lengths[i]) && lengths[i] >= 0.0f)) return fail(h, PP_E_INVAL, "bad source length");
+    if (!(std::isfinite(v.length) && v.length >= 0.0f)) return fail(h, PP_E_INVAL, "bad source length");
     if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
       return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
   }
@@ -1127,14 +1131,15 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
     uint64_t ph = 0;
     const uint64_t p0 = pos % h->sz.cap_src;
     for (size_t j = 0; j < m; ++j, ++i) {
-      const pp_source& a = src[i];
+      const SrcView v = at(i);
+      const pp_source& a = *v.s;
       const uint64_t kk = p0 + j;
       SrcRec& r = h->ring[kk < h->sz.cap_src ? kk : kk - h->sz.cap_src];
       r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
-      r.event_id = event_ids[i];
-      r.source_id = source_ids ? source_ids[i] : (uint32_t)(auto_id + j);  // running record number
+      r.event_id = v.event_id;
+      r.source_id = v.has_id ? v.source_id : (uint32_t)(auto_id + j);  // running record number
       r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
-      r.length = lengths ? lengths[i] : 0.0f;
+      r.length = v.length;
       ph += r.n_photons;
     }
     lk.lock();
@@ -1151,6 +1156,30 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
       h->cv_work.notify_all();
   }
   return PP_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths, const uint32_t* event_ids,
+                       const uint32_t* source_ids, size_t n) {
+  if (!h) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  if (n == 0) return PP_OK;
+  if (!src || !event_ids) return fail(h, PP_E_INVAL, "null sources or event_ids");
+  return submit_generic(h, n, [&](size_t i) {
+    return SrcView{src + i, lengths ? lengths[i] : 0.0f, event_ids[i], source_ids != nullptr, source_ids ? source_ids[i] : 0u};
+  });
+}
+
+int pp_submit_packed(pp_handle* h, const pp_packed_source* recs, size_t n) {
+  if (!h) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  if (n == 0) return PP_OK;
+  if (!recs) return fail(h, PP_E_INVAL, "null records");
+  return submit_generic(h, n, [&](size_t i) {
+    return SrcView{&recs[i].s, recs[i].length_m, recs[i].event_id, true, recs[i].source_id};
+  });
 }
 
 int pp_flush(pp_handle* h) {

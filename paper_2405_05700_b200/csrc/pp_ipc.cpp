@@ -14,6 +14,7 @@
 #include <chrono>
 #include <cmath>
 #include <cerrno>
+#include <cstddef>
 #include <cstring>
 #include <deque>
 #include <mutex>
@@ -36,6 +37,10 @@ struct SrcSlot {  // 48 B
   uint32_t event_id, source_id, pad;
 };
 static_assert(sizeof(SrcSlot) == 48, "SrcSlot layout");
+static_assert(sizeof(pp_packed_source) == sizeof(SrcSlot) && offsetof(pp_packed_source, length_m) == offsetof(SrcSlot, length) &&
+              offsetof(pp_packed_source, event_id) == offsetof(SrcSlot, event_id) &&
+              offsetof(pp_packed_source, source_id) == offsetof(SrcSlot, source_id),
+              "a ring slot is a pp_packed_source");
 
 struct ShmHeader {
   uint64_t magic;
@@ -87,6 +92,9 @@ inline void nap(int us) { std::this_thread::sleep_for(std::chrono::microseconds(
 // ---- back end bound to a pp_handle ----
 int h_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
   return pp_submit_segments(static_cast<pp_handle*>(ctx), s, len, ev, sid, n);
+}
+int h_submit_packed(void* ctx, const pp_packed_source* recs, size_t n) {
+  return pp_submit_packed(static_cast<pp_handle*>(ctx), recs, n);
 }
 int h_flush(void* ctx) { return pp_flush(static_cast<pp_handle*>(ctx)); }
 int h_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
@@ -180,21 +188,28 @@ void ingest_main(pp_ipc_server* s) {
       // in pp_ipc_submit, which bounds what the server has to park for it
       const bool behind = s->pc[c].parked_n.load(std::memory_order_acquire) > s->park_cap;
       if (head != tail && !behind) {
-        const size_t n = (size_t)std::min<uint64_t>(head - tail, kIngestChunk);
         const SrcSlot* ring = s->seg.src_ring(c);
+        const uint64_t t0 = tail % H->src_cap;
+        // a back end that takes packed records gets them as they lie in the ring (one contiguous span per pass)
+        const bool packed = s->be.submit_packed != nullptr;
+        const size_t n = (size_t)std::min<uint64_t>(std::min<uint64_t>(head - tail, kIngestChunk),
+                                                    packed ? H->src_cap - t0 : kIngestChunk);
         bool any_len = false;
-        for (size_t i = 0; i < n; ++i) {
-          const SrcSlot& r = ring[(tail + i) % H->src_cap];
-          src[i] = r.s; len[i] = r.length; ev[i] = r.event_id; sid[i] = r.source_id;
-          any_len |= r.length != 0.0f;
-        }
+        if (!packed)
+          for (size_t i = 0; i < n; ++i) {
+            const uint64_t k = t0 + i;
+            const SrcSlot& r = ring[k < H->src_cap ? k : k - H->src_cap];
+            src[i] = r.s; len[i] = r.length; ev[i] = r.event_id; sid[i] = r.source_id;
+            any_len |= r.length != 0.0f;
+          }
         pp_ipc_server::Block blk{c, tail + n, 0, {}};
         {
           std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
-          uint32_t last = ~ev[0];
+          uint32_t last = ~(packed ? ring[t0].event_id : ev[0]);
           for (size_t i = 0; i < n; ++i) {
-            if (ev[i] == last) continue;
-            last = ev[i];
+            const uint32_t e = packed ? ring[t0 + i].event_id : ev[i];
+            if (e == last) continue;
+            last = e;
             if (std::find(blk.events.begin(), blk.events.end(), last) != blk.events.end()) continue;
             auto it = s->owner.find(last);
             if (it == s->owner.end()) it = s->owner.emplace(last, pp_ipc_server::Owner{c, 0}).first;
@@ -208,7 +223,8 @@ void ingest_main(pp_ipc_server* s) {
           blk.global_end = s->sources.load() + n;
           s->fifo.push_back(std::move(blk));
         }
-        const int rc = s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
+        const int rc = packed ? s->be.submit_packed(s->be.ctx, reinterpret_cast<const pp_packed_source*>(ring + t0), n)
+                              : s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
         if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
         s->blocks++; s->sources += n;
         tail += n;
@@ -431,7 +447,7 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
 
 int pp_ipc_server_create(pp_handle* h, const char* shm_name, const pp_ipc_config* cfg, pp_ipc_server** out) {
   if (!h) return PP_E_INVAL;
-  const pp_ipc_backend be{h, h_submit, h_flush, h_collect, h_completed};
+  const pp_ipc_backend be{h, h_submit, h_flush, h_collect, h_completed, h_submit_packed};
   return pp_ipc_server_create_backend(&be, shm_name, cfg, out);
 }
 

@@ -285,7 +285,7 @@ int pp_multi_get_stats(pp_multi* m, pp_multi_stats* out) {
 
 int pp_multi_backend(pp_multi* m, pp_ipc_backend* out) {
   if (!m || !out) return PP_E_INVAL;
-  *out = pp_ipc_backend{m, m_submit, m_flush, m_collect, m_completed};
+  *out = pp_ipc_backend{m, m_submit, m_flush, m_collect, m_completed, nullptr};
   return PP_OK;
 }
 

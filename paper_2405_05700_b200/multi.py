@@ -26,7 +26,7 @@ class _MultiStats(C.Structure):
 class Backend(C.Structure):
     """pp_ipc_backend (include/pp_ipc.h)."""
     _fields_ = [("ctx", C.c_void_p), ("submit", C.c_void_p), ("flush", C.c_void_p), ("collect", C.c_void_p),
-                ("completed", C.c_void_p)]
+                ("completed", C.c_void_p), ("submit_packed", C.c_void_p)]
 
 
 _declared = False

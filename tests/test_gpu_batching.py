@@ -53,6 +53,22 @@ def test_launch_that_starts_a_few_photons_into_a_source():
     assert len(ref) > 50 and np.array_equal(hits, ref)
 
 
+def test_packed_records_equal_separate_arrays(case, reference_hits):
+    """pp_submit_packed (one 48-byte record per source: what the multi-process front end hands over) gives the hits of
+    pp_submit; bad records are rejected before anything is queued."""
+    geo, ice, src = case
+    rec = B.pack_records(src.src, src.event_id, src.source_id)
+    with B.Propagator(geo, ice, seed=9) as p:
+        for part in np.array_split(rec, 7):
+            p.submit_packed(part)
+        hits = sort_hits(p.collect_all())
+        bad = rec[:3].copy()
+        bad["src"][1, 3] = 2.0  # not a unit direction
+        with pytest.raises(B.PPError):
+            p.submit_packed(bad)
+    assert np.array_equal(hits, reference_hits)
+
+
 def test_resident_path_equals_server_path(case, reference_hits):
     geo, ice, src = case
     hits, _, st = gpu_run_resident(geo, ice, src, 9, launch_photons_target=300000)
