@@ -576,8 +576,8 @@ def run_stream_ipc(args):
                      for c in range(n)]
             for p in procs:
                 p.start()
+            st0 = prop.stats()  # (before the start signal: the server is idle now, and the clients start at once)
             barrier.wait()  # every client has packed its blocks and attached
-            st0 = prop.stats()
             t0 = time.perf_counter()
             res = [q.get(timeout=600) for _ in procs]
             wall = time.perf_counter() - t0

@@ -1086,20 +1086,39 @@ struct SrcView { const pp_source* s; float length; uint32_t event_id; bool has_i
 template <class At>
 int submit_generic(pp_handle* h, size_t n, At at) {
   const float yield = h->ice.photons_per_GeV;
-  // validate everything before enqueueing anything
+  // validate everything before enqueueing anything.  First a branch-free pass that only says whether ANY source is
+  // bad and keeps the photon counts (the multi-process front end pushes 4e7 sources/s through here); the slow pass
+  // that names the offender runs only if there is one.
+  thread_local std::vector<uint32_t> counts;
+  if (counts.size() < n) counts.resize(n);
+  uint32_t bad = 0;
   for (size_t i = 0; i < n; ++i) {
     const SrcView v = at(i);
     const pp_source& a = *v.s;
-    const float f8[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
-    for (float f : f8)
-      if (!std::isfinite(f)) return fail(h, PP_E_INVAL, "non-finite field in source " + std::to_string(i));
+    uint32_t w[8];
+    std::memcpy(w, &a, sizeof w);  // x, y, z, dx, dy, dz, t, E
+    uint32_t nonfinite = 0;
+    for (int q = 0; q < 8; ++q) nonfinite |= (uint32_t)((w[q] & 0x7f800000u) == 0x7f800000u);
     const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
-    if (std::fabs(n2 - 1.0) > 1e-4) return fail(h, PP_E_INVAL, "source direction is not a unit vector");
-    if (a.energy_GeV < 0.0f) return fail(h, PP_E_INVAL, "negative source energy");
-    if (!(std::isfinite(v.length) && v.length >= 0.0f)) return fail(h, PP_E_INVAL, "bad source length");
-    if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
-      return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
+    const unsigned long long cnt = host_photon_count(a.energy_GeV, yield);
+    counts[i] = (uint32_t)cnt;
+    bad |= nonfinite | (uint32_t)(std::fabs(n2 - 1.0) > 1e-4) | (uint32_t)(a.energy_GeV < 0.0f) |
+           (uint32_t)!(v.length >= 0.0f && v.length <= 3.0e38f) | (uint32_t)(cnt > 0xFFFFFFFFull);
   }
+  if (bad)
+    for (size_t i = 0; i < n; ++i) {
+      const SrcView v = at(i);
+      const pp_source& a = *v.s;
+      const float f8[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
+      for (float f : f8)
+        if (!std::isfinite(f)) return fail(h, PP_E_INVAL, "non-finite field in source " + std::to_string(i));
+      const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
+      if (std::fabs(n2 - 1.0) > 1e-4) return fail(h, PP_E_INVAL, "source direction is not a unit vector");
+      if (a.energy_GeV < 0.0f) return fail(h, PP_E_INVAL, "negative source energy");
+      if (!(std::isfinite(v.length) && v.length >= 0.0f)) return fail(h, PP_E_INVAL, "bad source length");
+      if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
+        return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
+    }
   const bool nonblock = (h->cfg.flags & PP_FLAG_NONBLOCKING_SUBMIT) != 0;
   size_t i = 0;
   std::unique_lock<std::mutex> lk(h->mu);
@@ -1138,7 +1157,7 @@ int submit_generic(pp_handle* h, size_t n, At at) {
       r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
       r.event_id = v.event_id;
       r.source_id = v.has_id ? v.source_id : (uint32_t)(auto_id + j);  // running record number
-      r.n_photons = (uint32_t)host_photon_count(a.energy_GeV, yield);
+      r.n_photons = counts[i];
       r.length = v.length;
       ph += r.n_photons;
     }
