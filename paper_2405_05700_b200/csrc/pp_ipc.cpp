@@ -509,13 +509,22 @@ int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengt
   if (!c) return PP_E_INVAL;
   if (n == 0) return PP_OK;
   if (!sources || !event_ids) return PP_E_INVAL;
-  for (size_t i = 0; i < n; ++i) {  // the cheap checks here, so that a bad block never reaches the shared ring
-    const pp_source& a = sources[i];
-    const float v[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
-    for (float f : v) if (!std::isfinite(f)) return PP_E_INVAL;
-    if (a.energy_GeV < 0.0f || (lengths && !(std::isfinite(lengths[i]) && lengths[i] >= 0.0f))) return PP_E_INVAL;
-    const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
-    if (std::fabs(n2 - 1.0) > 1e-4) return PP_E_INVAL;
+  {
+    // the cheap checks here, so that a bad block never reaches the shared ring (one branch-free pass: a client ships
+    // millions of sources per second)
+    uint32_t bad = 0;
+    for (size_t i = 0; i < n; ++i) {
+      const pp_source& a = sources[i];
+      uint32_t w[8];
+      std::memcpy(w, &a, sizeof w);  // x, y, z, dx, dy, dz, t, E
+      uint32_t nonfinite = 0;
+      for (int q = 0; q < 8; ++q) nonfinite |= (uint32_t)((w[q] & 0x7f800000u) == 0x7f800000u);
+      const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
+      const float len = lengths ? lengths[i] : 0.0f;
+      bad |= nonfinite | (uint32_t)(a.energy_GeV < 0.0f) | (uint32_t)!(len >= 0.0f && len <= 3.0e38f) |
+             (uint32_t)(std::fabs(n2 - 1.0) > 1e-4);
+    }
+    if (bad) return PP_E_INVAL;
   }
   ShmHeader* H = c->seg.hdr();
   ClientCtl* ctl = c->seg.ctl(c->slot);
