@@ -1086,14 +1086,9 @@ struct SrcView { const pp_source* s; float length; uint32_t event_id; bool has_i
 template <class At>
 int submit_generic(pp_handle* h, size_t n, At at) {
   const float yield = h->ice.photons_per_GeV;
-  // validate everything before enqueueing anything.  First a branch-free pass that only says whether ANY source is
-  // bad and keeps the photon counts (the multi-process front end pushes 4e7 sources/s through here); the slow pass
-  // that names the offender runs only if there is one.
-  thread_local std::vector<uint32_t> counts;
-  if (counts.size() < n) counts.resize(n);
-  uint32_t bad = 0;
-  for (size_t i = 0; i < n; ++i) {
-    const SrcView v = at(i);
+  const uint64_t cap = h->sz.cap_src;
+  // the checks of one source, branch-free: non-zero = bad; also gives its photon count
+  auto check = [&](const SrcView& v, uint32_t* count) -> uint32_t {
     const pp_source& a = *v.s;
     uint32_t w[8];
     std::memcpy(w, &a, sizeof w);  // x, y, z, dx, dy, dz, t, E
@@ -1101,11 +1096,12 @@ int submit_generic(pp_handle* h, size_t n, At at) {
     for (int q = 0; q < 8; ++q) nonfinite |= (uint32_t)((w[q] & 0x7f800000u) == 0x7f800000u);
     const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
     const unsigned long long cnt = host_photon_count(a.energy_GeV, yield);
-    counts[i] = (uint32_t)cnt;
-    bad |= nonfinite | (uint32_t)(std::fabs(n2 - 1.0) > 1e-4) | (uint32_t)(a.energy_GeV < 0.0f) |
+    *count = (uint32_t)cnt;
+    return nonfinite | (uint32_t)(std::fabs(n2 - 1.0) > 1e-4) | (uint32_t)(a.energy_GeV < 0.0f) |
            (uint32_t)!(v.length >= 0.0f && v.length <= 3.0e38f) | (uint32_t)(cnt > 0xFFFFFFFFull);
-  }
-  if (bad)
+  };
+  // the slow pass that names the offender (runs only if there is one)
+  auto name_offender = [&]() -> int {
     for (size_t i = 0; i < n; ++i) {
       const SrcView v = at(i);
       const pp_source& a = *v.s;
@@ -1119,6 +1115,78 @@ int submit_generic(pp_handle* h, size_t n, At at) {
       if (host_photon_count(a.energy_GeV, yield) > 0xFFFFFFFFull)
         return fail(h, PP_E_OVERFLOW, "source " + std::to_string(i) + " has more than 2^32-1 photons");
     }
+    return fail(h, PP_E_INVAL, "bad source");
+  };
+  auto write_rec = [&](uint64_t p0, size_t j, const SrcView& v, uint32_t count, uint64_t auto_id) {
+    const pp_source& a = *v.s;
+    const uint64_t kk = p0 + j;
+    SrcRec& r = h->ring[kk < cap ? kk : kk - cap];
+    r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
+    r.event_id = v.event_id;
+    r.source_id = v.has_id ? v.source_id : (uint32_t)(auto_id + j);  // running record number
+    r.n_photons = count;
+    r.length = v.length;
+  };
+  auto publish = [&](std::unique_lock<std::mutex>& lk, uint64_t pos, size_t m, uint64_t ph) {  // lk held
+    h->cv_pub.wait(lk, [&] { return h->ring_head == pos; });  // earlier reservations publish first
+    h->ring_head = pos + m;
+    h->cv_pub.notify_all();
+    h->queued_photons += ph;
+    h->st.sources_submitted += m;
+    h->st.photons_submitted += ph;
+    h->st.source_ring_high_water =
+        std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_reserve - h->ring_tail) * sizeof(SrcRec));
+    if (h->queued_photons >= h->sz.target ||
+        (h->inflight_photons < h->sz.target / 2 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
+      h->cv_work.notify_all();
+  };
+  // Everything is validated before anything is enqueued.
+  // Fast path: the whole call fits into the ring right now.  ONE pass checks, counts and copies into reserved slots
+  // that nobody can see yet (the multi-process front end pushes 4e7 sources/s through here); a bad source takes the
+  // reservation back (always possible for a lone producer such as that front end; if other producers have reserved
+  // behind it meanwhile, the slots are published as sources without photons, which the server drops).
+  {
+    std::unique_lock<std::mutex> lk(h->mu);
+    if (h->shutdown.load()) return PP_E_STATE;
+    if ((h->sz.cap_src - (h->ring_reserve - h->ring_tail)) >= n) {
+      if (!h->wall_started) { h->wall_started = true; h->wall_t0 = Clock::now(); h->wall_t1 = h->wall_t0; }
+      const uint64_t pos = h->ring_reserve, auto_id = h->next_auto_id, p0 = pos % cap;
+      h->ring_reserve += n;
+      h->next_auto_id += n;
+      lk.unlock();
+      uint32_t bad = 0;
+      uint64_t ph = 0;
+      for (size_t j = 0; j < n; ++j) {
+        const SrcView v = at(j);
+        uint32_t cnt;
+        bad |= check(v, &cnt);
+        write_rec(p0, j, v, cnt, auto_id);
+        ph += cnt;
+      }
+      if (bad) {
+        for (size_t j = 0; j < n; ++j) { const uint64_t kk = p0 + j; h->ring[kk < cap ? kk : kk - cap].n_photons = 0u; }
+        ph = 0;
+      }
+      lk.lock();
+      if (bad && h->ring_reserve == pos + n) {
+        h->ring_reserve = pos; h->next_auto_id = auto_id;  // nobody reserved behind us: as if nothing had happened
+        lk.unlock();
+        return name_offender();
+      }
+      publish(lk, pos, n, ph);
+      if (bad) { lk.unlock(); return name_offender(); }
+      return PP_OK;
+    }
+  }
+  // General path (the call does not fit into the ring at once): a checking pass that keeps the photon counts, then
+  // the copy in as many pieces as the ring has room for.
+  thread_local std::vector<uint32_t> counts;
+  if (counts.size() < n) counts.resize(n);
+  {
+    uint32_t bad = 0;
+    for (size_t i = 0; i < n; ++i) bad |= check(at(i), &counts[i]);
+    if (bad) return name_offender();
+  }
   const bool nonblock = (h->cfg.flags & PP_FLAG_NONBLOCKING_SUBMIT) != 0;
   size_t i = 0;
   std::unique_lock<std::mutex> lk(h->mu);
@@ -1148,31 +1216,13 @@ int submit_generic(pp_handle* h, size_t n, At at) {
     h->next_auto_id += m;
     lk.unlock();
     uint64_t ph = 0;
-    const uint64_t p0 = pos % h->sz.cap_src;
+    const uint64_t p0 = pos % cap;
     for (size_t j = 0; j < m; ++j, ++i) {
-      const SrcView v = at(i);
-      const pp_source& a = *v.s;
-      const uint64_t kk = p0 + j;
-      SrcRec& r = h->ring[kk < h->sz.cap_src ? kk : kk - h->sz.cap_src];
-      r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
-      r.event_id = v.event_id;
-      r.source_id = v.has_id ? v.source_id : (uint32_t)(auto_id + j);  // running record number
-      r.n_photons = counts[i];
-      r.length = v.length;
-      ph += r.n_photons;
+      write_rec(p0, j, at(i), counts[i], auto_id);
+      ph += counts[i];
     }
     lk.lock();
-    h->cv_pub.wait(lk, [&] { return h->ring_head == pos; });  // earlier reservations publish first
-    h->ring_head = pos + m;
-    h->cv_pub.notify_all();
-    h->queued_photons += ph;
-    h->st.sources_submitted += m;
-    h->st.photons_submitted += ph;
-    h->st.source_ring_high_water =
-        std::max<uint64_t>(h->st.source_ring_high_water, (h->ring_reserve - h->ring_tail) * sizeof(SrcRec));
-    if (h->queued_photons >= h->sz.target ||
-        (h->inflight_photons < h->sz.target / 2 && h->queued_photons >= std::max<uint64_t>(1, h->sz.target / 8)))
-      h->cv_work.notify_all();
+    publish(lk, pos, m, ph);
   }
   return PP_OK;
 }
