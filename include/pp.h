@@ -161,7 +161,10 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
  * before it, pp_stats.sources_submitted, mod 2^32), which is unique across calls.  Results are reproducible from run
  * to run only with explicit ids or a fixed submit order.  Thread-safe: any number of threads may submit
  * concurrently.  Copies before returning.  Blocks while the source ring is full unless
- * PP_FLAG_NONBLOCKING_SUBMIT.  Sources with N == 0 photons are accepted and ignored. */
+ * PP_FLAG_NONBLOCKING_SUBMIT.  Sources with N == 0 photons are accepted and ignored.  A call with a bad source
+ * (non-finite field, direction not a unit vector, negative energy or length, more than 2^32 - 1 photons) fails as a
+ * whole with PP_E_INVAL / PP_E_OVERFLOW: none of its sources is propagated.  (If other threads were submitting at the
+ * same moment, the failed call may still be counted in pp_stats.sources_submitted, as sources without photons.) */
 int pp_submit(pp_handle* h, const pp_source* sources, const uint32_t* event_ids, const uint32_t* source_ids,
               size_t n);
 
