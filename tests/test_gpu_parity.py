@@ -108,6 +108,9 @@ def test_coarse_walk_tables_clear_and_dense_layers():
     # photons cross layers with a 0.5 m scattering length: hundreds of flights each, so more of the hits pass the
     # 1e-3 ns mark than in C1's ice (measured frac_hit 0.972)
     assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.95, c
+    # the same through the server path: the lean kernel variant (no fate dump), several launches
+    hits2, st2 = gpu_run(geo, ice, src, 9, launch_photons_target=70000)
+    assert st2.launches == 3 and np.array_equal(hits2, hits)
 
 
 def test_layered_oversized_doms_many_hits():
