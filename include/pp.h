@@ -191,7 +191,10 @@ typedef struct pp_packed_source {
  * over one array instead of four.  This is what the multi-process front end (pp_ipc.h) moves from its shared-memory
  * rings into the handle: at C2's 400 photons per source a B200 consumes 4e7 sources/s ("a block of
  * steps is sent to the GPU"), which is within sight of what one ingest thread can copy. */
-int pp_submit_packed(pp_handle* h, const pp_packed_source* records, size_t n);
+int pp_submit_packed(pp_handle* h, const pp_packed_source* records, size_t n, uint64_t* records_end);
+/* records_end (nullable): receives the number of sources submitted to the handle up to and including the last one of
+ * this call, in submit order -- the value pp_stats.sources_completed has reached when all of them are propagated.
+ * (With several threads submitting, that is how each of them learns where its sources sit in the common order.) */
 
 /* Longitudinal profile of extended sources (NEXT-2, reading R-23): where along its length a source of
  * pp_submit_segments emits.  The offset of a photon becomes l = L F(u) with the same u as above and F piecewise

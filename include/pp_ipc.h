@@ -44,7 +44,8 @@ typedef struct pp_ipc_client pp_ipc_client;
 
 typedef struct pp_ipc_config {
   uint32_t max_clients;       /* client slots in the segment (default 16) */
-  uint32_t reserved;
+  uint32_t ingest_threads;    /* threads that move blocks from the rings into the back end (default 2; 1 for a back
+                                 end without submit_packed) */
   uint64_t source_ring_bytes; /* per client, client -> server (default 4 MiB = 87 381 sources) */
   uint64_t hit_ring_bytes;    /* per client, server -> client (default 4 MiB = 131 072 hits) */
 } pp_ipc_config;
@@ -62,9 +63,11 @@ typedef struct pp_ipc_backend {
                                             everything submitted before this call has been propagated and handed out */
   int (*completed)(void* ctx, uint64_t* n_sources); /* the first n_sources sources, in submit order, are fully
                                             propagated and their hits can be collected (pp_stats.sources_completed) */
-  int (*submit_packed)(void* ctx, const pp_packed_source* records, size_t n); /* optional (may be NULL): the same as
-                                            submit for packed records (pp_submit_packed); the ingest thread then hands
-                                            the ring's records over as they lie, in one pass */
+  int (*submit_packed)(void* ctx, const pp_packed_source* records, size_t n, uint64_t* records_end); /* optional
+                                            (may be NULL): the same as submit for packed records (pp_submit_packed,
+                                            which also says where the call's last record sits in the back end's submit
+                                            order); the ingest threads then hand the rings' records over as they lie,
+                                            in one pass, several clients at a time */
 } pp_ipc_backend;
 
 /* Creates (O_CREAT | O_EXCL) the shared-memory segment `shm_name` ("/name"), and starts the ingest and dispatch

@@ -99,7 +99,7 @@ def load_library(path: str = LIB_PATH):
     L.pp_submit_segments.restype = C.c_int
     L.pp_submit_segments.argtypes = [vp, vp, vp, vp, vp, C.c_size_t]
     L.pp_submit_packed.restype = C.c_int
-    L.pp_submit_packed.argtypes = [vp, vp, C.c_size_t]
+    L.pp_submit_packed.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_uint64)]
     L.pp_flush.restype = C.c_int
     L.pp_flush.argtypes = [vp]
     L.pp_collect.restype = C.c_int
@@ -318,7 +318,9 @@ class Propagator:
     def submit_packed(self, records):
         """pp_submit_packed: PACKED_DTYPE [n] records (see pack_records); host buffer; thread-safe."""
         rec = np.ascontiguousarray(records, dtype=PACKED_DTYPE)
-        self._check(self._L.pp_submit_packed(self._h, rec.ctypes.data, rec.shape[0]), self._h)
+        end = C.c_uint64(0)
+        self._check(self._L.pp_submit_packed(self._h, rec.ctypes.data, rec.shape[0], C.byref(end)), self._h)
+        return int(end.value)  # sources submitted to the handle up to and including this call's last one
 
     def set_acceptance(self, mode: str = "off", coef=()):
         """pp_set_acceptance: ``mode`` in ACCEPTANCE_MODES; ``coef`` = polynomial coefficients in d_z."""

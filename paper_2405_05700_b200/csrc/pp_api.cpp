@@ -1084,7 +1084,7 @@ struct SrcView { const pp_source* s; float length; uint32_t event_id; bool has_i
 
 // pp_submit / pp_submit_segments / pp_submit_packed: `at(i)` is the i-th source of the call.
 template <class At>
-int submit_generic(pp_handle* h, size_t n, At at) {
+int submit_generic(pp_handle* h, size_t n, At at, uint64_t* records_end = nullptr) {
   const float yield = h->ice.photons_per_GeV;
   const uint64_t cap = h->sz.cap_src;
   // the checks of one source, branch-free: non-zero = bad; also gives its photon count
@@ -1175,6 +1175,7 @@ int submit_generic(pp_handle* h, size_t n, At at) {
       }
       publish(lk, pos, n, ph);
       if (bad) { lk.unlock(); return name_offender(); }
+      if (records_end) *records_end = pos + n;
       return PP_OK;
     }
   }
@@ -1223,6 +1224,7 @@ int submit_generic(pp_handle* h, size_t n, At at) {
     }
     lk.lock();
     publish(lk, pos, m, ph);
+    if (records_end) *records_end = pos + m;
   }
   return PP_OK;
 }
@@ -1241,14 +1243,17 @@ int pp_submit_segments(pp_handle* h, const pp_source* src, const float* lengths,
   });
 }
 
-int pp_submit_packed(pp_handle* h, const pp_packed_source* recs, size_t n) {
+int pp_submit_packed(pp_handle* h, const pp_packed_source* recs, size_t n, uint64_t* records_end) {
   if (!h) return PP_E_INVAL;
   if (h->sticky.load() != PP_OK) return h->sticky.load();
-  if (n == 0) return PP_OK;
+  if (n == 0) {
+    if (records_end) { std::lock_guard<std::mutex> g(h->mu); *records_end = h->ring_reserve; }
+    return PP_OK;
+  }
   if (!recs) return fail(h, PP_E_INVAL, "null records");
   return submit_generic(h, n, [&](size_t i) {
     return SrcView{&recs[i].s, recs[i].length_m, recs[i].event_id, true, recs[i].source_id};
-  });
+  }, records_end);
 }
 
 int pp_flush(pp_handle* h) {

@@ -93,8 +93,8 @@ inline void nap(int us) { std::this_thread::sleep_for(std::chrono::microseconds(
 int h_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
   return pp_submit_segments(static_cast<pp_handle*>(ctx), s, len, ev, sid, n);
 }
-int h_submit_packed(void* ctx, const pp_packed_source* recs, size_t n) {
-  return pp_submit_packed(static_cast<pp_handle*>(ctx), recs, n);
+int h_submit_packed(void* ctx, const pp_packed_source* recs, size_t n, uint64_t* records_end) {
+  return pp_submit_packed(static_cast<pp_handle*>(ctx), recs, n, records_end);
 }
 int h_flush(void* ctx) { return pp_flush(static_cast<pp_handle*>(ctx)); }
 int h_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
@@ -123,7 +123,8 @@ struct pp_ipc_server {
   Segment seg;
   std::string name;
   pp_ipc_backend be{};
-  std::thread ingest, dispatch;
+  std::vector<std::thread> ingest;  // thread t serves the client slots c with c % ingest.size() == t
+  std::thread dispatch;
   std::atomic<bool> stop{false};
   // event id -> owning client slot, with the number of that client's blocks holding sources of the event that are
   // handed to the back end and not yet complete; the entry goes when the count drops to zero
@@ -133,7 +134,8 @@ struct pp_ipc_server {
   std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0}, dropped{0}, clients_dropped{0};
   struct Block { uint32_t client; uint64_t tail_after, global_end; std::vector<uint32_t> events; };
   std::mutex fifo_mu;
-  std::deque<Block> fifo;       // blocks handed to the back end, in order, not yet known to be complete
+  std::deque<Block> fifo;       // blocks handed to the back end, not yet known to be complete: in hand-over order with
+                                // one ingest thread, in any order with several (global_end then comes from the back end)
   uint64_t base_completed = 0;  // the back end's completed count when the server started
   // per client slot
   struct PerClient {
@@ -156,7 +158,7 @@ struct pp_ipc_client {
 
 namespace {
 
-void ingest_main(pp_ipc_server* s) {
+void ingest_main(pp_ipc_server* s, uint32_t me, uint32_t n_thr) {
   ShmHeader* H = s->seg.hdr();
   std::vector<pp_source> src(kIngestChunk);
   std::vector<float> len(kIngestChunk);
@@ -164,7 +166,7 @@ void ingest_main(pp_ipc_server* s) {
   while (!s->stop.load()) {
     bool progressed = false;
     const uint32_t n_slots = std::min(H->next_slot.load(std::memory_order_acquire), H->max_clients);
-    for (uint32_t c = 0; c < n_slots; ++c) {
+    for (uint32_t c = me; c < n_slots; c += n_thr) {
       ClientCtl* ctl = s->seg.ctl(c);
       const uint32_t state = ctl->state.load(std::memory_order_acquire);
       if (state == kClosed) {
@@ -217,14 +219,26 @@ void ingest_main(pp_ipc_server* s) {
           }
         }
         s->pc[c].blocks_in_flight++;
-        {
-          // the block is in the fifo before the back end sees it, so that "complete" can never overtake it
-          std::lock_guard<std::mutex> g(s->fifo_mu);
-          blk.global_end = s->sources.load() + n;
-          s->fifo.push_back(std::move(blk));
+        int rc;
+        if (packed) {
+          // the back end says where the block's last record sits in its submit order; the block joins the list after
+          // the hand-over (a block that is complete before it is listed is simply found complete at the next look)
+          uint64_t end = 0;
+          rc = s->be.submit_packed(s->be.ctx, reinterpret_cast<const pp_packed_source*>(ring + t0), n, &end);
+          if (rc == PP_OK) {
+            blk.global_end = end - s->base_completed;
+            std::lock_guard<std::mutex> g(s->fifo_mu);
+            s->fifo.push_back(std::move(blk));
+          }
+        } else {
+          {
+            // one ingest thread: the block is in the list before the back end sees it, in hand-over order
+            std::lock_guard<std::mutex> g(s->fifo_mu);
+            blk.global_end = s->sources.load() + n;
+            s->fifo.push_back(std::move(blk));
+          }
+          rc = s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
         }
-        const int rc = packed ? s->be.submit_packed(s->be.ctx, reinterpret_cast<const pp_packed_source*>(ring + t0), n)
-                              : s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
         if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
         s->blocks++; s->sources += n;
         tail += n;
@@ -350,10 +364,16 @@ void dispatch_main(pp_ipc_server* s) {
         std::lock_guard<std::mutex> g(s->fifo_mu);
         // `drained` covers back ends without a completed() call: everything handed over before the collect is done
         const uint64_t upto = drained ? std::max<uint64_t>(n_complete, s->sources.load()) : n_complete;
-        while (!s->fifo.empty() && s->fifo.front().global_end <= upto &&
-               s->fifo.front().tail_after <= s->seg.ctl(s->fifo.front().client)->src_tail.load(std::memory_order_acquire)) {
-          done.push_back(std::move(s->fifo.front()));
-          s->fifo.pop_front();
+        for (auto it = s->fifo.begin(); it != s->fifo.end();) {
+          if (it->global_end <= upto &&
+              it->tail_after <= s->seg.ctl(it->client)->src_tail.load(std::memory_order_acquire)) {
+            done.push_back(std::move(*it));
+            it = s->fifo.erase(it);
+          } else if (s->ingest.size() == 1) {
+            break;  // hand-over order: nothing behind an incomplete block is complete
+          } else {
+            ++it;
+          }
         }
       }
       if (!done.empty()) {
@@ -439,7 +459,12 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
   H->magic = kMagic;
   H->server_alive.store(1, std::memory_order_release);
   if (s->be.completed) s->be.completed(s->be.ctx, &s->base_completed);  // the back end must be drained at this point
-  s->ingest = std::thread(ingest_main, s);
+  {
+    uint32_t n_thr = s->be.submit_packed ? (cfg && cfg->ingest_threads ? cfg->ingest_threads : 2u) : 1u;
+    n_thr = std::max(1u, std::min(n_thr, std::min(max_clients, 16u)));
+    s->ingest.reserve(n_thr);  // (dispatch_main reads ingest.size(): all threads exist before it starts)
+    for (uint32_t t = 0; t < n_thr; ++t) s->ingest.emplace_back(ingest_main, s, t, n_thr);
+  }
   s->dispatch = std::thread(dispatch_main, s);
   *out = s;
   return PP_OK;
@@ -454,7 +479,7 @@ int pp_ipc_server_create(pp_handle* h, const char* shm_name, const pp_ipc_config
 void pp_ipc_server_destroy(pp_ipc_server* s) {
   if (!s) return;
   s->stop.store(true);
-  if (s->ingest.joinable()) s->ingest.join();
+  for (auto& t : s->ingest) if (t.joinable()) t.join();
   if (s->dispatch.joinable()) s->dispatch.join();
   s->seg.hdr()->server_alive.store(0, std::memory_order_release);
   munmap(s->seg.base, s->seg.bytes);

@@ -17,7 +17,7 @@ EXPORTS = ["pp_ipc_server_create", "pp_ipc_server_create_backend", "pp_ipc_serve
 
 
 class _IpcConfig(C.Structure):
-    _fields_ = [("max_clients", C.c_uint32), ("reserved", C.c_uint32), ("source_ring_bytes", C.c_uint64),
+    _fields_ = [("max_clients", C.c_uint32), ("ingest_threads", C.c_uint32), ("source_ring_bytes", C.c_uint64),
                 ("hit_ring_bytes", C.c_uint64)]
 
 
