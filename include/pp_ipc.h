@@ -9,7 +9,7 @@
  * (no CUDA needed in them) attach to a POSIX shared-memory segment by name.  Per client the segment holds one
  * single-producer/single-consumer ring of light sources (client -> server) and one of hits (server -> client), both
  * bounded: a client that runs ahead of the GPU blocks in pp_ipc_submit, which is what keeps every process's memory
- * predictable.  The server's ingest thread moves blocks from the rings into pp_submit_segments
+ * predictable.  The server's ingest threads move blocks from the rings into the handle (pp_submit_packed)
  * (so launches mix the sources of all clients); its dispatch thread routes every collected hit to the client that
  * submitted the hit's event.
  *

@@ -53,8 +53,8 @@ struct ShmHeader {
 static_assert(sizeof(ShmHeader) <= kHeaderBytes, "header");
 
 // Life of a slot: kAttached (a client owns it) -> kClosed (the client left, or its process is gone) -> kQuiesced (the
-// ingest thread has seen that and will not touch the slot's source ring again) -> kRecycled (the dispatch thread has
-// emptied it: claimable again).  Only the ingest thread moves a slot out of kClosed, so the dispatch thread never
+// slot's ingest thread has seen that and will not touch the slot's source ring again) -> kRecycled (the dispatch thread has
+// emptied it: claimable again).  Only the ingest thread that serves a slot moves it out of kClosed, so the dispatch thread never
 // recycles a slot while a block of it is being handed to the back end.
 enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3, kQuiesced = 4 };
 
