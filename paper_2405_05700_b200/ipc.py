@@ -6,6 +6,7 @@ any other process and needs neither CUDA nor torch.  Argument marshalling only.
 from __future__ import annotations
 
 import ctypes as C
+import threading
 
 import numpy as np
 
@@ -123,10 +124,13 @@ class IpcClient:
         self._check(self._L.pp_ipc_flush(self._c), "pp_ipc_flush")
 
     def collect(self, cap: int = 1 << 16, block: bool = True) -> np.ndarray:
-        out = np.empty(cap, dtype=HIT_DTYPE)
+        tls = self.__dict__.setdefault("_collect_tls", threading.local())  # one landing buffer per calling thread
+        out = getattr(tls, "buf", None)
+        if out is None or out.shape[0] < cap:
+            out = tls.buf = np.empty(cap, dtype=HIT_DTYPE)
         n = C.c_size_t(0)
         self._check(self._L.pp_ipc_collect(self._c, out.ctypes.data, cap, C.byref(n), 1 if block else 0), "pp_ipc_collect")
-        return out[: n.value]
+        return out[: n.value].copy()
 
     def collect_all(self) -> np.ndarray:
         """flush, then collect until this client's work is drained."""
@@ -136,7 +140,7 @@ class IpcClient:
             h = self.collect(block=True)
             if len(h) == 0:
                 break
-            parts.append(h.copy())
+            parts.append(h)
         return np.concatenate(parts) if parts else np.empty(0, dtype=HIT_DTYPE)
 
     def close(self):

@@ -4,6 +4,7 @@ PAPER.md:33 "embarrassingly parallel").  Argument marshalling only.
 from __future__ import annotations
 
 import ctypes as C
+import threading
 
 import numpy as np
 
@@ -103,11 +104,14 @@ class MultiFront:
         self._check(self._L.pp_multi_flush(self._m), "pp_multi_flush")
 
     def collect(self, cap: int = 1 << 20, block: bool = True) -> np.ndarray:
-        out = np.empty(cap, dtype=HIT_DTYPE)
+        tls = self.__dict__.setdefault("_collect_tls", threading.local())  # one landing buffer per calling thread
+        out = getattr(tls, "buf", None)
+        if out is None or out.shape[0] < cap:
+            out = tls.buf = np.empty(cap, dtype=HIT_DTYPE)
         n = C.c_size_t(0)
         self._check(self._L.pp_multi_collect(self._m, out.ctypes.data, cap, C.byref(n), 1 if block else 0),
                     "pp_multi_collect")
-        return out[: n.value]
+        return out[: n.value].copy()
 
     def collect_all(self) -> np.ndarray:
         self.flush()
@@ -116,7 +120,7 @@ class MultiFront:
             h = self.collect(block=True)
             if len(h) == 0:
                 break
-            parts.append(h.copy())
+            parts.append(h)
         return np.concatenate(parts) if parts else np.empty(0, dtype=HIT_DTYPE)
 
     def run(self, sources, event_ids, source_ids=None, lengths=None) -> np.ndarray:

@@ -30,7 +30,7 @@ def test_two_handles_behind_one_front_give_one_handles_hits():
             got = []
             for a in range(0, len(src), 5000):                       # blocks that do not line up with the batches
                 m.submit(src.src[a:a + 5000], src.event_id[a:a + 5000], src.source_id[a:a + 5000])
-                got.append(m.collect(block=False).copy())
+                got.append(m.collect(block=False))
             got.append(m.collect_all())
             st = m.stats()
         hits = sort_hits(np.concatenate(got))
