@@ -571,7 +571,7 @@ def run_stream_ipc(args):
     barrier = ctx.Barrier(n + 1)
     with B.Propagator(geo, ice, seed=0, launch_photons_target=10 ** 8) as prop:
         prop.run(src.src, src.event_id, src.source_id)  # warm-up
-        with ipc.IpcServer(prop, name, max_clients=n) as srv:
+        with ipc.IpcServer(prop, name, max_clients=n, ingest_threads=args.ingest_threads) as srv:
             procs = [ctx.Process(target=_ipc_client_main, args=(name, c, n, args.replicas, args.block_sources, barrier, q))
                      for c in range(n)]
             for p in procs:
@@ -742,6 +742,7 @@ def main():
     ap.add_argument("--replicas", type=int, default=10)
     ap.add_argument("--ipc-clients", type=int, default=0, help="with --stream: N client processes over include/pp_ipc.h")
     ap.add_argument("--block-sources", type=int, default=8192, help="sources a client queues before it ships a block")
+    ap.add_argument("--ingest-threads", type=int, default=0, help="with --ipc-clients: ingest threads of the server (0 = default)")
     args = ap.parse_args()
     if args.update_instr_per_flight:
         return update_instr_per_flight(args)

@@ -44,8 +44,8 @@ typedef struct pp_ipc_client pp_ipc_client;
 
 typedef struct pp_ipc_config {
   uint32_t max_clients;       /* client slots in the segment (default 16) */
-  uint32_t ingest_threads;    /* threads that move blocks from the rings into the back end (default 2; 1 for a back
-                                 end without submit_packed) */
+  uint32_t ingest_threads;    /* threads that move blocks from the rings into the back end (default: one per four
+                                 client slots, 2 to 4; always 1 for a back end without submit_packed) */
   uint64_t source_ring_bytes; /* per client, client -> server (default 4 MiB = 87 381 sources) */
   uint64_t hit_ring_bytes;    /* per client, server -> client (default 4 MiB = 131 072 hits) */
 } pp_ipc_config;

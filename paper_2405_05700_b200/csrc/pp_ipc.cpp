@@ -460,7 +460,8 @@ int pp_ipc_server_create_backend(const pp_ipc_backend* be, const char* shm_name,
   H->server_alive.store(1, std::memory_order_release);
   if (s->be.completed) s->be.completed(s->be.ctx, &s->base_completed);  // the back end must be drained at this point
   {
-    uint32_t n_thr = s->be.submit_packed ? (cfg && cfg->ingest_threads ? cfg->ingest_threads : 2u) : 1u;
+    // default: one ingest thread per four client slots, at least 2, at most 4 (measured with 8 and 16 clients)
+    uint32_t n_thr = s->be.submit_packed ? (cfg && cfg->ingest_threads ? cfg->ingest_threads : std::max(2u, std::min(4u, max_clients / 4u))) : 1u;
     n_thr = std::max(1u, std::min(n_thr, std::min(max_clients, 16u)));
     s->ingest.reserve(n_thr);  // (dispatch_main reads ingest.size(): all threads exist before it starts)
     for (uint32_t t = 0; t < n_thr; ++t) s->ingest.emplace_back(ingest_main, s, t, n_thr);

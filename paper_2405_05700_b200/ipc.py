@@ -63,9 +63,9 @@ class IpcServer:
     ``pp_ipc_backend`` struct that outlives the server; the CPU tests pass their host-only echo back end)."""
 
     def __init__(self, propagator, name: str, *, max_clients: int = 16, source_ring_bytes: int = 0,
-                 hit_ring_bytes: int = 0, backend=None):
+                 hit_ring_bytes: int = 0, backend=None, ingest_threads: int = 0):
         self._L = _lib()
-        cfg = _IpcConfig(int(max_clients), 0, int(source_ring_bytes), int(hit_ring_bytes))
+        cfg = _IpcConfig(int(max_clients), int(ingest_threads), int(source_ring_bytes), int(hit_ring_bytes))
         s = C.c_void_p()
         if backend is not None:
             rc = self._L.pp_ipc_server_create_backend(C.c_void_p(backend), name.encode(), C.byref(cfg), C.byref(s))
