@@ -282,6 +282,50 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
                     const uint32_t* d_source_ids, size_t n, pp_fate* d_fates, uint64_t* photons_out,
                     double* device_ms_out);
 
+/* ---- a small resident run that allocates nothing ----
+ * For whom: code that must not, or cannot, get device memory at the moment it wants photons propagated.  Three such
+ * callers are common.  (1) A plug-in inside a framework whose caching allocator has already taken nearly all of the
+ * device for its own pool: a cudaMalloc next to that pool fails, or succeeds and later makes the framework's own
+ * allocations fail.  (2) A latency-bound loop: cudaMalloc and cudaFree may wait for every kernel running on the device
+ * -- here, for a 100 ms propagation launch of the batching server -- before they return.  (3) A thread in a process
+ * where some other thread is capturing a stream in CUDA's default (global) capture mode: cudaMalloc is refused there
+ * and breaks the capture.  pp_run_resident itself allocates nothing per call either, but it works in the handle's
+ * workspace, needs the server idle, and queues its hits in host memory that grows by allocation; this call touches none
+ * of that.
+ *
+ * What it does: pp_run_resident for a SMALL batch, in one propagation launch, with the hits written straight into the
+ * caller's DEVICE buffer.  Same kernels, same Philox counters: the hits are, record for record, those pp_run_resident
+ * gives for the same handle and sources (their order in d_hits is unspecified, as everywhere).  The handle supplies the
+ * medium, the geometry, the seed and the optional physics set by pp_set_*; its server, queues, workspace and
+ * statistics are neither used nor changed, so the call may run while the server is busy.
+ *   d_sources[n], d_event_ids[n], d_source_ids[n]   DEVICE inputs, all required (no automatic source ids);
+ *   d_hits[hit_cap]                                  DEVICE output, 16-byte aligned (may be NULL if hit_cap == 0);
+ *   n_hits_out, photons_out                          HOST outputs (photons_out nullable);
+ *   stream                                           cudaStream_t the work is enqueued on (NULL: the default stream).
+ * The call returns after the stream has been synchronised: d_hits[0 .. *n_hits_out) is then complete.
+ *
+ * Scratch: the expanded source records, their photon prefix sums, the tile table and the launch's counters live in
+ * ONE statically allocated device array of 512 KiB inside the library image (every GPU on which the library gets
+ * loaded holds it until the process exits), shared by every call on that device, whatever the handle.  Hence:
+ *   - limits: n <= PP_NOALLOC_MAX_SOURCES and at most PP_NOALLOC_MAX_PHOTONS photons in total; beyond either the call
+ *     fails with PP_E_NOMEM and a message that names the limit (pp_last_error), and nothing is written to d_hits;
+ *   - PP_E_NOMEM as well if the batch makes more than hit_cap hits (then d_hits holds an arbitrary hit_cap of them and
+ *     *n_hits_out the number the batch needs at least); PP_E_OVERFLOW for a source of more than 2^32 - 1 photons;
+ *   - the array keeps what the previous call left in it; each call rewrites or clears everything it reads, so calls
+ *     in sequence are independent.  The library does NOT order calls against each other: two calls whose GPU work
+ *     overlaps on one device (two threads, any streams, any handles) race on the array and both results are garbage.
+ *     Serialise them.
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress), with that device
+ *     current; make that first call before any stream capture begins in the process.
+ * No cudaMalloc, cudaFree, cudaHostAlloc or other allocating CUDA call is made, on the first call or later; host
+ * memory is neither allocated nor pinned except for the text of an error message.  The caller's current device is
+ * restored before returning. */
+#define PP_NOALLOC_MAX_SOURCES 4096u
+#define PP_NOALLOC_MAX_PHOTONS 4194304u /* 2^22 */
+int pp_run_resident_noalloc(pp_handle* h, const pp_source* d_sources, const uint32_t* d_event_ids,
+                            const uint32_t* d_source_ids, size_t n, pp_hit* d_hits, size_t hit_cap, size_t* n_hits_out,
+                            uint64_t* photons_out, void* stream);
+
 /* ---- host-only helpers (no CUDA call inside; usable and tested on a machine without a GPU) ----
  * pp_check_inputs: the validation pp_create performs on geometry and ice (PP_E_INVAL), including whether
  * the fast DOM lookup can represent the geometry (PP_E_UNSUPPORTED unless PP_FLAG_BRUTE_FORCE_DOMS).

@@ -70,7 +70,9 @@ class _Stats(C.Structure):
 EXPORTS = ["pp_workspace_size", "pp_create", "pp_submit", "pp_flush", "pp_collect", "pp_stats", "pp_last_error",
            "pp_destroy", "pp_run_resident", "pp_version", "pp_kernel_launch_count", "pp_check_inputs",
            "pp_photon_count", "pp_debug_plan_launches", "pp_set_acceptance", "pp_submit_segments", "pp_set_spectrum",
-           "pp_set_emission_smearing", "pp_set_segment_profile", "pp_submit_packed"]
+           "pp_set_emission_smearing", "pp_set_segment_profile", "pp_submit_packed", "pp_run_resident_noalloc"]
+NOALLOC_MAX_SOURCES = 4096        # PP_NOALLOC_MAX_SOURCES
+NOALLOC_MAX_PHOTONS = 1 << 22     # PP_NOALLOC_MAX_PHOTONS
 
 
 class _LaunchPlan(C.Structure):
@@ -121,6 +123,9 @@ def load_library(path: str = LIB_PATH):
     L.pp_destroy.argtypes = [vp]
     L.pp_run_resident.restype = C.c_int
     L.pp_run_resident.argtypes = [vp, vp, vp, vp, C.c_size_t, vp, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+    L.pp_run_resident_noalloc.restype = C.c_int
+    L.pp_run_resident_noalloc.argtypes = [vp, vp, vp, vp, C.c_size_t, vp, C.c_size_t, C.POINTER(C.c_size_t),
+                                          C.POINTER(C.c_uint64), vp]
     L.pp_version.restype = C.c_char_p
     L.pp_kernel_launch_count.restype = C.c_uint64
     L.pp_check_inputs.restype = C.c_int
@@ -420,6 +425,22 @@ class Propagator:
         if want_fates:
             fates = fates_t.cpu().numpy().view(FATE_DTYPE)[: ph.value]
         return int(ph.value), float(ms.value), fates
+
+    def run_resident_noalloc(self, d_src, d_ev, d_sid, d_hits):
+        """pp_run_resident_noalloc on tensors from :meth:`upload` (source ids required) and a caller-made uint8 CUDA
+        tensor ``d_hits`` of a multiple of 32 bytes that receives the hits.  The library allocates nothing for this
+        call: its scratch is a fixed 512 KiB array inside libpp.so, shared by all calls on the device -- at most
+        NOALLOC_MAX_SOURCES sources / NOALLOC_MAX_PHOTONS photons per call, and never two calls at once.  Runs on
+        torch's current stream and returns after synchronising it: (number of hits now in ``d_hits``, photons)."""
+        torch = self._torch
+        assert d_sid is not None and d_hits.dtype == torch.uint8 and d_hits.is_cuda and d_hits.is_contiguous()
+        n_hits, ph = C.c_size_t(0), C.c_uint64(0)
+        rc = self._L.pp_run_resident_noalloc(self._h, d_src.data_ptr(), d_ev.data_ptr(), d_sid.data_ptr(),
+                                             int(d_src.shape[0]), d_hits.data_ptr(),
+                                             d_hits.numel() // HIT_DTYPE.itemsize, C.byref(n_hits), C.byref(ph),
+                                             torch.cuda.current_stream(self.device).cuda_stream)
+        self._check(rc, self._h)
+        return int(n_hits.value), int(ph.value)
 
     def drain(self, chunk: int = 1 << 20) -> np.ndarray:
         """Collect whatever is ready without flushing (after run_resident)."""

@@ -1507,3 +1507,21 @@ int pp_run_resident(pp_handle* h, const pp_source* d_sources, const uint32_t* d_
 }
 
 }  // extern "C"
+
+// What the entry point without allocations (pp_run_resident_noalloc, pp_kernels.cu) reads from a handle.
+namespace pp {
+
+int handle_launch_info(pp_handle* h, HandleLaunchInfo* out) {
+  if (!h || !out) return PP_E_INVAL;
+  if (h->sticky.load() != PP_OK) return h->sticky.load();
+  std::lock_guard<std::mutex> g(h->mu);  // (pp_set_* write the template under this lock)
+  if (h->shutdown) return PP_E_STATE;
+  out->base = h->base;
+  out->device = h->device; out->grid = h->grid; out->smem = h->smem; out->brute = h->brute;
+  out->photons_per_GeV = h->ice.photons_per_GeV;
+  return PP_OK;
+}
+
+int handle_fail(pp_handle* h, int code, const char* msg) { return fail(h, code, msg ? msg : ""); }
+
+}  // namespace pp

@@ -29,6 +29,19 @@ cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int 
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm);
 int propagate_warps_per_block();  // warps of one CTA of the propagation kernel
 
+// What pp_run_resident_noalloc (pp_kernels.cu) needs to know about a handle (defined in pp_api.cpp, where pp_handle
+// is): a copy of the launch template with the medium, the geometry and the optional physics filled in, and how the
+// handle launches the propagation kernel.  Returns PP_OK, or the handle's sticky error / PP_E_STATE after shutdown.
+struct HandleLaunchInfo {
+  LaunchParams base;
+  int device, grid;
+  size_t smem;
+  bool brute;
+  float photons_per_GeV;
+};
+int handle_launch_info(pp_handle* h, HandleLaunchInfo* out);
+int handle_fail(pp_handle* h, int code, const char* msg);  // records msg for pp_last_error; returns code
+
 // Step 1 on the host (same arithmetic as the device's, exact in fp64).
 inline unsigned long long host_photon_count(float energy, float yield) {
   // floor(E y + 1/2) by truncation: the same integer for a non-negative argument, and no call into libm on a host

@@ -2,6 +2,9 @@
 // propagation kernel (a3-a8).  See DESIGN.md sections 2 and 5.  Product code: shares nothing with oracle/.
 #include <cuda_runtime.h>
 
+#include <cstdio>
+#include <mutex>
+
 #include "../../include/pp.h"
 #include "pp_internal.h"
 #include "pp_device.cuh"
@@ -796,4 +799,201 @@ cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks
   return e;
 }
 
+// =============================================================================================
+// pp_run_resident_noalloc (include/pp.h): a small resident run whose scratch is a static device array
+// =============================================================================================
+// For callers that cannot get device memory when they need photons propagated (a framework's pool owns the device; a
+// latency-bound loop that cannot afford cudaMalloc's wait for running kernels; a process in which a stream is being
+// captured).  Everything pp_run_resident keeps in the handle's workspace for a launch -- expanded source records,
+// prefix sums, tile table, Status -- sits here in one array that is part of the library image.  One array per device,
+// shared by every call: see the rules in pp.h.
+
+constexpr uint32_t kNoallocMaxSrc = PP_NOALLOC_MAX_SOURCES;
+constexpr uint32_t kNoallocMaxPhotons = PP_NOALLOC_MAX_PHOTONS;
+constexpr uint32_t kNoallocMaxTiles = 65536;  // >= 2 x (tiles wanted for a small launch: 4 per resident warp) up to 256 SMs
+
+struct NoallocHead {  // what the host reads back after the prologue
+  unsigned long long total;  // photons of the call
+  unsigned int overflow;     // a source with more than 2^32 - 1 photons
+  unsigned int tile_photons, n_tiles;
+  unsigned int too_big;      // more photons or tiles than the array is laid out for: no tile table was written
+};
+struct NoallocScratch {
+  Status status;  // counters of the propagation launch: cleared by the prologue of every call
+  NoallocHead head;
+  alignas(16) SrcRec src[kNoallocMaxSrc];
+  unsigned long long cum[kNoallocMaxSrc + 1];
+  uint32_t cum_rel[kNoallocMaxSrc + 1];
+  uint32_t tile_src[kNoallocMaxTiles];
+};
+constexpr size_t kNoallocBytes = (sizeof(NoallocScratch) + 255) / 256 * 256;
+static_assert(kNoallocBytes <= (512u << 10), "pp.h promises at most 512 KiB");
+
+// THE scratch.  In host code this name is only a handle for cudaGetSymbolAddress -- not a device address: a kernel given
+// `g_noalloc_scratch` from the host side would fault, or scribble over host memory the GPU can reach.  The device
+// address is looked up once per device in noalloc_scratch() below.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoallocBytes];
+
+// Variant of prologue_kernel for the array above: ingest (build the source records, count photons) + prefix sums +
+// choice of the tile size + tile table + cleared Status, one CTA.  g_begin is 0: the call is one launch.
+// Everything a later kernel of the same call reads is written here first, so nothing left by an earlier call matters.
+__global__ void __launch_bounds__(1024) noalloc_prologue_kernel(NoallocScratch* __restrict__ S,
+                                                                const pp_source* __restrict__ s,
+                                                                const uint32_t* __restrict__ ev,
+                                                                const uint32_t* __restrict__ sid, uint32_t n, float yield,
+                                                                uint32_t want_tiles) {
+  __shared__ unsigned long long part[1024];
+  __shared__ unsigned int s_overflow;
+  const uint32_t t = threadIdx.x;
+  if (t == 0) s_overflow = 0u;
+  __syncthreads();
+  const uint32_t per = (n + 1023u) / 1024u;
+  const uint32_t lo = min(n, t * per), hi = min(n, lo + per);
+  unsigned long long sum = 0;
+  for (uint32_t i = lo; i < hi; ++i) {
+    const pp_source a = s[i];
+    unsigned long long cnt = photon_count(a.energy_GeV, yield);
+    if (cnt > 0xFFFFFFFFull) { s_overflow = 1u; cnt = 0; }
+    SrcRec r;
+    r.x = a.x; r.y = a.y; r.z = a.z; r.dx = a.dx; r.dy = a.dy; r.dz = a.dz; r.t = a.t_ns; r.energy = a.energy_GeV;
+    r.event_id = ev[i]; r.source_id = sid[i]; r.n_photons = (uint32_t)cnt; r.length = 0.0f;
+    S->src[i] = r;
+    sum += cnt;
+  }
+  part[t] = sum;
+  __syncthreads();
+  for (uint32_t off = 1; off < 1024; off <<= 1) {
+    unsigned long long v = (t >= off) ? part[t - off] : 0ull;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  unsigned long long run = (t == 0) ? 0ull : part[t - 1];
+  for (uint32_t i = lo; i < hi; ++i) {
+    S->cum[i] = run;
+    S->cum_rel[i] = rel32(run, 0ull);
+    run += S->src[i].n_photons;  // (this thread wrote it)
+  }
+  const unsigned long long total = part[1023];
+  if (t == 1023) { S->cum[n] = total; S->cum_rel[n] = rel32(total, 0ull); }
+  // tile size as pick_tiles (pp_api.cpp) chooses it for a small launch: about `want_tiles` tiles, 32..1024 photons each
+  uint32_t tile = kTilePhotons;
+  while (tile > (uint32_t)kMinTilePhotons && total / tile < want_tiles) tile >>= 1;
+  const unsigned long long n_tiles = (total + tile - 1) / tile;
+  const bool too_big = total > kNoallocMaxPhotons || n_tiles > kNoallocMaxTiles;
+  if (t == 0) {
+    S->status = Status{};
+    S->head.total = total; S->head.overflow = s_overflow; S->head.tile_photons = tile;
+    S->head.n_tiles = too_big ? 0u : (uint32_t)n_tiles; S->head.too_big = too_big ? 1u : 0u;
+  }
+  __threadfence_block();
+  __syncthreads();  // the tile search reads prefix sums other threads wrote
+  if (!too_big)
+    for (uint32_t j = t; j < (uint32_t)n_tiles; j += 1024u) tile_entry(S->cum, n, 0ull, tile, j, S->tile_src);
+}
+
+// Device address of the array on the CURRENT device; looked up on the first call for that device, kept afterwards.
+static cudaError_t noalloc_scratch(int dev, NoallocScratch** out) {
+  static std::mutex mu;
+  static NoallocScratch* addr[kMaxDevices] = {};
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> g(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    addr[dev] = static_cast<NoallocScratch*>(p);
+  }
+  *out = addr[dev];
+  return cudaSuccess;
+}
+
+static int run_noalloc(pp_handle* h, const HandleLaunchInfo& info, const pp_source* d_sources, const uint32_t* d_event_ids,
+                       const uint32_t* d_source_ids, uint32_t n, pp_hit* d_hits, uint32_t ring_cap, size_t* n_hits_out,
+                       uint64_t* photons_out, cudaStream_t st) {
+  char msg[256];
+  auto cuda_fail = [&](const char* what, cudaError_t e) {
+    snprintf(msg, sizeof msg, "pp_run_resident_noalloc: %s: %s", what, cudaGetErrorString(e));
+    return handle_fail(h, PP_E_CUDA, msg);
+  };
+  NoallocScratch* S = nullptr;  // DEVICE address: only ever used for address arithmetic on the host
+  cudaError_t e = noalloc_scratch(info.device, &S);
+  if (e != cudaSuccess) return cuda_fail("cudaGetSymbolAddress", e);
+  // ---- a2: expansion into the static array; the host needs the totals before it can launch ----
+  const uint32_t want_tiles = (uint32_t)info.grid * (uint32_t)(kBlockThreads / 32) * 4u;
+  noalloc_prologue_kernel<<<1, 1024, 0, st>>>(S, d_sources, d_event_ids, d_source_ids, n, info.photons_per_GeV, want_tiles);
+  g_launches++;
+  e = cudaGetLastError();
+  NoallocHead head{};
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&head, &S->head, sizeof head, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail("expansion", e);
+  if (head.overflow) return handle_fail(h, PP_E_OVERFLOW, "pp_run_resident_noalloc: a source has more than 2^32-1 photons");
+  if (head.too_big) {
+    snprintf(msg, sizeof msg,
+             "pp_run_resident_noalloc: the batch has %llu photons; the static scratch array is laid out for at most %u "
+             "(PP_NOALLOC_MAX_PHOTONS): split the batch or use pp_run_resident",
+             head.total, kNoallocMaxPhotons);
+    return handle_fail(h, PP_E_NOMEM, msg);
+  }
+  if (photons_out) *photons_out = head.total;
+  if (head.total == 0) return PP_OK;
+  // ---- a3-a8: one propagation launch; the hit "ring" is the caller's buffer, and there are no resume lists: a
+  // buffer that fills up makes the kernel stop and flag an error instead of handing work to a next launch ----
+  LaunchParams P = info.base;
+  P.src = S->src; P.cum = S->cum; P.cum_rel = S->cum_rel; P.tile_src = S->tile_src;
+  P.g_begin = 0; P.g_end = head.total; P.n_src = n; P.n_tiles = head.n_tiles; P.tile_photons = head.tile_photons;
+  P.has_segments = 0u;
+  P.resume_in = nullptr; P.resume_out = nullptr; P.n_resume_in = 0; P.resume_cap = 0;
+  P.status = &S->status; P.ring = d_hits; P.ring_cap = ring_cap;
+  P.fates = nullptr;
+  e = launch_propagate(P, info.brute, false, info.grid, info.smem, st);
+  Status hs{};
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&hs, &S->status, sizeof hs, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail("propagation", e);
+  if (hs.stop || hs.error || hs.hit_count > ring_cap) {
+    *n_hits_out = hs.hit_count;
+    snprintf(msg, sizeof msg,
+             "pp_run_resident_noalloc: hit buffer too small: the batch makes at least %u hits, hit_cap is %u", hs.hit_count,
+             ring_cap);
+    return handle_fail(h, PP_E_NOMEM, msg);
+  }
+  if (hs.photons_started != head.total) return handle_fail(h, PP_E_CUDA, "pp_run_resident_noalloc: internal: photons lost");
+  *n_hits_out = hs.hit_count;
+  return PP_OK;
+}
+
 }  // namespace pp
+
+extern "C" int pp_run_resident_noalloc(pp_handle* h, const pp_source* d_sources, const uint32_t* d_event_ids,
+                                       const uint32_t* d_source_ids, size_t n, pp_hit* d_hits, size_t hit_cap,
+                                       size_t* n_hits_out, uint64_t* photons_out, void* stream) {
+  using namespace pp;
+  if (!h || !n_hits_out) return PP_E_INVAL;
+  *n_hits_out = 0;
+  if (photons_out) *photons_out = 0;
+  HandleLaunchInfo info;
+  const int rc = handle_launch_info(h, &info);
+  if (rc != PP_OK) return rc;
+  if (n == 0) return PP_OK;
+  if (!d_sources || !d_event_ids || !d_source_ids)
+    return handle_fail(h, PP_E_INVAL, "pp_run_resident_noalloc: null device pointer (source ids are required here)");
+  if ((hit_cap > 0 && !d_hits) || (reinterpret_cast<uintptr_t>(d_hits) & 15u))
+    return handle_fail(h, PP_E_INVAL, "pp_run_resident_noalloc: d_hits is null or not 16-byte aligned");
+  if (n > kNoallocMaxSrc) {
+    char msg[200];
+    snprintf(msg, sizeof msg,
+             "pp_run_resident_noalloc: %zu sources; the static scratch array is laid out for at most %u "
+             "(PP_NOALLOC_MAX_SOURCES): split the batch or use pp_run_resident", n, kNoallocMaxSrc);
+    return handle_fail(h, PP_E_NOMEM, msg);
+  }
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+  if (cudaSetDevice(info.device) != cudaSuccess) return handle_fail(h, PP_E_CUDA, "pp_run_resident_noalloc: cudaSetDevice");
+  const uint32_t ring_cap = (uint32_t)(hit_cap < 0xFFFFFF00ull ? hit_cap : 0xFFFFFF00ull);
+  const int out = run_noalloc(h, info, d_sources, d_event_ids, d_source_ids, (uint32_t)n, d_hits, ring_cap, n_hits_out,
+                              photons_out, static_cast<cudaStream_t>(stream));
+  if (prev >= 0 && prev != info.device) cudaSetDevice(prev);
+  return out;
+}
