@@ -62,7 +62,9 @@ typedef struct pp_ipc_backend {
   int (*collect)(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained); /* non-blocking; *drained != 0:
                                             everything submitted before this call has been propagated and handed out */
   int (*completed)(void* ctx, uint64_t* n_sources); /* the first n_sources sources, in submit order, are fully
-                                            propagated and their hits can be collected (pp_stats.sources_completed) */
+                                            propagated and their hits can be collected (pp_stats.sources_completed).
+                                            Optional (may be NULL); when given, the server decides completion on this
+                                            count alone and ignores *drained */
   int (*submit_packed)(void* ctx, const pp_packed_source* records, size_t n, uint64_t* records_end); /* optional
                                             (may be NULL): the same as submit for packed records (pp_submit_packed,
                                             which also says where the call's last record sits in the back end's submit

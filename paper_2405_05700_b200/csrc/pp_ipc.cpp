@@ -311,6 +311,8 @@ void dispatch_main(pp_ipc_server* s) {
     for (uint32_t c = 0; c < n_slots; ++c) drain_parked(s, c);
     // how many sources (in hand-over order) were complete BEFORE the collect below: their hits are already queued,
     // so once that collect comes back empty they have all been routed (or parked)
+    // Both are read BEFORE the collect, never after: a block handed over while the collect was under way (an idle
+    // server, a preempted dispatch thread) is not covered by what that collect reports.
     uint64_t n_complete = 0;
     if (s->be.completed) {
       uint64_t v = 0;
@@ -318,6 +320,8 @@ void dispatch_main(pp_ipc_server* s) {
       if (rc0 != PP_OK) { s->error.store(rc0); s->stop.store(true); break; }
       n_complete = v > s->base_completed ? v - s->base_completed : 0;
     }
+    // (back ends without completed(): the sources whose hand-over had returned by now)
+    const uint64_t handed_before = s->sources.load(std::memory_order_acquire);
     size_t n = 0;
     int drained = 0;
     const int rc = s->be.collect(s->be.ctx, buf.data(), cap, &n, &drained);
@@ -362,8 +366,9 @@ void dispatch_main(pp_ipc_server* s) {
       std::vector<pp_ipc_server::Block> done;
       {
         std::lock_guard<std::mutex> g(s->fifo_mu);
-        // `drained` covers back ends without a completed() call: everything handed over before the collect is done
-        const uint64_t upto = drained ? std::max<uint64_t>(n_complete, s->sources.load()) : n_complete;
+        // a back end with completed() is believed on that count alone; `drained` serves the ones without: everything
+        // whose hand-over had returned before the collect started is done
+        const uint64_t upto = s->be.completed ? n_complete : (drained ? handed_before : 0);
         for (auto it = s->fifo.begin(); it != s->fifo.end();) {
           if (it->global_end <= upto &&
               it->tail_after <= s->seg.ctl(it->client)->src_tail.load(std::memory_order_acquire)) {

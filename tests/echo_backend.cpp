@@ -8,7 +8,10 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <atomic>
+#include <chrono>
 #include <mutex>
+#include <thread>
 #include <vector>
 
 #include "../include/pp_ipc.h"
@@ -22,6 +25,7 @@ struct Echo {
   uint64_t pending_sources = 0;
   uint32_t hits_per_source = 1;
   uint64_t auto_id = 0;
+  std::atomic<uint32_t> collect_delay_us{0};  // a collect that found nothing dawdles this long before it returns
 };
 
 int e_submit(void* ctx, const pp_source* s, const float* len, const uint32_t* ev, const uint32_t* sid, size_t n) {
@@ -64,6 +68,13 @@ int e_collect(void* ctx, pp_hit* out, size_t cap, size_t* n_out, int* drained) {
   e->ready.erase(e->ready.begin(), e->ready.begin() + (long)n);
   *n_out = n;
   *drained = (n == 0 && e->pending.empty() && e->ready.empty()) ? 1 : 0;
+  const uint32_t delay = e->collect_delay_us.load();
+  if (n == 0 && delay) {
+    // the answer above is now stale by `delay`: blocks handed over meanwhile are NOT covered by `drained`
+    e->mu.unlock();
+    std::this_thread::sleep_for(std::chrono::microseconds(delay));
+    e->mu.lock();
+  }
   return PP_OK;
 }
 
@@ -80,6 +91,12 @@ void echo_set_hits_per_source(const pp_ipc_backend* be, uint32_t k) {
   Echo* e = static_cast<Echo*>(be->ctx);
   std::lock_guard<std::mutex> g(e->mu);
   e->hits_per_source = k ? k : 1;
+}
+
+// Makes every empty-handed collect return late: widens the window between "the back end looked" and "the server acts on
+// it" that a preempted dispatch thread opens in production.
+void echo_set_collect_delay_us(const pp_ipc_backend* be, uint32_t us) {
+  static_cast<Echo*>(be->ctx)->collect_delay_us.store(us);
 }
 
 }  // extern "C"

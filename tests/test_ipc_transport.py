@@ -18,6 +18,7 @@ def _echo_lib():
     L = C.CDLL(build_echo_backend())
     L.echo_backend_new.restype = C.c_void_p
     L.echo_set_hits_per_source.argtypes = [C.c_void_p, C.c_uint32]
+    L.echo_set_collect_delay_us.argtypes = [C.c_void_p, C.c_uint32]
     return L
 
 
@@ -328,3 +329,26 @@ def test_null_source_ids_do_not_collide_across_submits():
             got = c.collect_all()
         assert len(got) == 20 and len(np.unique(got["source_id"])) == 20
         assert srv.stats()["error"] == 0
+
+
+def test_a_block_shipped_to_an_idle_server_is_never_declared_complete_before_it_ran():
+    """Regression (round-2 advice): the dispatch thread asked the back end "anything left?" (drained), and only
+    afterwards looked at how many sources had been handed over.  A block that arrived in between -- on an idle server,
+    with the dispatch thread preempted -- was then taken for complete: its client saw "drained" without hits, and the
+    hits turned up later with no owner.  The echo back end's empty-handed collect is made slow here, so that nearly
+    every block lands inside that window; completion must follow the back end's completed count alone."""
+    name = f"/pp_ipc_test_{os.getpid()}_idle"
+    be = echo_backend()
+    _echo_lib().echo_set_collect_delay_us(be, 3000)
+    with ipc.IpcServer(None, name, max_clients=2, backend=be) as srv:
+        total = 0
+        for it in range(25):
+            with ipc.IpcClient(name) as c:
+                src, ev, sid, ln = _sources(it % 7, 3, 5)
+                ev = ev + np.uint32(10000 * it)
+                c.submit(src, ev, sid, ln)
+                got = np.sort(c.collect_all(), order=["event_id", "source_id"])
+                assert np.array_equal(got, _expected(src, ev, sid, ln)), f"iteration {it}: {len(got)} of {len(ev)} hits"
+                total += len(ev)
+        st = srv.stats()
+        assert st["error"] == 0 and st["hits_unrouted"] == 0 and st["hits_routed"] == total
