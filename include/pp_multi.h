@@ -42,7 +42,11 @@ void pp_multi_destroy(pp_multi* m);
 
 /* pp_submit_segments on the front: stages the sources; whenever deal_photons photons are staged, a batch of whole
  * sources is cut and dealt to the least-loaded device (and that device is flushed, so the batch is launched).
- * Thread-safe.  Blocks while the chosen device's source ring is full. */
+ * Thread-safe.  Blocks while the chosen device's source ring is full.  A call with a bad source (pp.h, pp_submit:
+ * non-finite field, direction not a unit vector, negative energy or length, more than 2^32 - 1 photons) fails as a
+ * whole with PP_E_INVAL / PP_E_OVERFLOW before anything is staged.  Should a device still refuse a batch the front has
+ * dealt (a back end with rules of its own), that batch is dropped -- counted as complete, without hits -- and the call
+ * whose deal met it returns the device's code; the sources of other calls are not held up. */
 int pp_multi_submit(pp_multi* m, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
                     const uint32_t* source_ids, size_t n);
 /* Deals whatever is staged (however little) and flushes every device. */

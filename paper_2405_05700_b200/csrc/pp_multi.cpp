@@ -70,6 +70,7 @@ struct pp_multi {
   std::deque<Staged> staged;
   uint64_t staged_photons = 0;
   uint64_t n_submitted = 0, ph_submitted = 0;
+  uint64_t rejected_sources = 0; // sources of batches a back end refused (dropped, counted as complete)
   std::deque<Batch> batches;     // incomplete prefix trimmed as batches complete in order
   size_t batches_base = 0;       // global index of batches.front()
   uint64_t completed_prefix = 0; // sources in the complete prefix of the deal order
@@ -127,6 +128,18 @@ int deal_one(pp_multi* m, uint64_t want) {
   }
   Device& D = m->dev[best];
   rc = D.be.submit(D.be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
+  if (rc == PP_E_INVAL || rc == PP_E_OVERFLOW) {
+    // the device refused the batch as a whole (pp.h: none of its sources is propagated); pp_multi_submit makes the
+    // handle's own checks, so this means a back end with other rules or another light yield.  The batch must not stay
+    // at the head of the queue, where every later deal would meet it again: it is taken out and counted as complete
+    // without hits (so that whoever waits on the completed count is not stuck behind it), and the caller of this deal
+    // gets the code.
+    m->staged.erase(m->staged.begin(), m->staged.begin() + (long)n);
+    m->staged_photons -= ph;
+    m->rejected_sources += n;
+    m->batches.push_back(Batch{best, n, 0, D.dealt_sources, true});
+    return rc;
+  }
   if (rc != PP_OK) return rc;
   rc = D.be.flush(D.be.ctx);  // a dealt batch is a whole launch: do not wait for more
   if (rc != PP_OK) return rc;
@@ -218,10 +231,18 @@ int pp_multi_submit(pp_multi* m, const pp_source* sources, const float* lengths_
   if (!m) return PP_E_INVAL;
   if (n == 0) return PP_OK;
   if (!sources || !event_ids) return PP_E_INVAL;
-  // count photons (and reject what a handle would reject for overflow) before anything is staged
+  // the checks a handle makes on a source (pp.h, pp_submit) and the photon counts, before anything is staged: a bad
+  // call fails as a whole, here and now, in the caller that made it -- not later in some other caller's deal
   std::vector<uint64_t> cnt(n);
   for (size_t i = 0; i < n; ++i) {
-    const int rc = pp_photon_count(sources[i].energy_GeV, m->yield, &cnt[i]);
+    const pp_source& a = sources[i];
+    const float f8[8] = {a.x, a.y, a.z, a.dx, a.dy, a.dz, a.t_ns, a.energy_GeV};
+    for (float f : f8)
+      if (!std::isfinite(f)) return PP_E_INVAL;
+    const double n2 = (double)a.dx * a.dx + (double)a.dy * a.dy + (double)a.dz * a.dz;
+    if (std::fabs(n2 - 1.0) > 1e-4 || a.energy_GeV < 0.0f) return PP_E_INVAL;
+    if (lengths_m && !(std::isfinite(lengths_m[i]) && lengths_m[i] >= 0.0f)) return PP_E_INVAL;
+    const int rc = pp_photon_count(a.energy_GeV, m->yield, &cnt[i]);
     if (rc != PP_OK) return rc;
   }
   std::lock_guard<std::mutex> g(m->mu);

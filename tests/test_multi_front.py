@@ -102,6 +102,52 @@ def test_front_rejects_bad_input():
             m.submit(big, ev, sid, ln)
         assert e.value.code == -4 and m.stats()["sources_submitted"] == 0   # nothing was staged
         assert len(m.collect(block=True)) == 0             # nothing outstanding: drained at once
+        # what a handle would refuse is refused here, in the caller that made the call (round-2 advice)
+        for col, val in ((3, 2.0), (0, np.nan), (6, np.inf), (7, -1.0)):
+            bad = src.copy()
+            bad[1, col] = val
+            with pytest.raises(B.PPError) as e:
+                m.submit(bad, ev, sid, ln)
+            assert e.value.code == -1
+        for val in (-1.0, np.nan):
+            bad_ln = ln.copy()
+            bad_ln[0] = val
+            with pytest.raises(B.PPError) as e:
+                m.submit(src, ev, sid, bad_ln)
+            assert e.value.code == -1
+        assert m.stats()["sources_submitted"] == 0 and m.stats()["sources_staged"] == 0
+        m.submit(src, ev, sid, ln)                         # and a good call after all that goes through
+        assert np.array_equal(np.sort(m.collect_all(), order=ORDER), _expected(src, ev, sid, ln))
+
+
+def test_a_batch_the_device_refuses_does_not_wedge_the_front():
+    """A back end with stricter rules than the front's refuses one batch: that batch is dropped (counted as complete,
+    no hits), the caller whose deal met it gets the code, and everybody else's sources go on."""
+    import ctypes as C
+    be = multi.Backend()
+    C.memmove(C.byref(be), C.c_void_p(echo_backend()), C.sizeof(multi.Backend))
+    SUBMIT = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32), C.c_void_p, C.c_size_t)
+    real = SUBMIT(be.submit)
+
+    def picky(ctx, s, ln, ev, sid, n):
+        if any(ev[i] == 4003 for i in range(n)):
+            return -1
+        return real(ctx, s, ln, ev, sid, n)
+
+    keep = SUBMIT(picky)
+    be.submit = C.cast(keep, C.c_void_p).value
+    src, ev, sid, ln = _sources(4, 6, 5)                   # events 4000..4005, five sources each
+    with multi.MultiFront(backends=[C.addressof(be)], photons_per_GeV=1.0e4, deal_photons=1) as m:
+        ok = ev != 4003
+        m.submit(src[ev < 4003], ev[ev < 4003], sid[ev < 4003], ln[ev < 4003])
+        with pytest.raises(B.PPError) as e:                # deal_photons = 1: every submit deals what it brought
+            m.submit(src[ev == 4003][:1], ev[ev == 4003][:1], sid[ev == 4003][:1], ln[ev == 4003][:1])
+        assert e.value.code == -1
+        m.submit(src[ev > 4003], ev[ev > 4003], sid[ev > 4003], ln[ev > 4003])
+        hits = np.sort(m.collect_all(), order=ORDER)
+        st = m.stats()
+    assert np.array_equal(hits, _expected(src[ok], ev[ok], sid[ok], ln[ok]))
+    assert st["sources_staged"] == 0 and st["sources_completed"] == st["sources_submitted"] == int(ok.sum()) + 1
 
 
 def test_client_processes_in_front_of_two_devices():
