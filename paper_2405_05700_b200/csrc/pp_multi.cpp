@@ -7,6 +7,7 @@
 #include <atomic>
 #include <chrono>
 #include <cmath>
+#include <condition_variable>
 #include <deque>
 #include <mutex>
 #include <thread>
@@ -58,6 +59,7 @@ struct Device {
   uint64_t dealt_sources = 0, dealt_photons = 0, batches = 0;
   uint64_t outstanding = 0;      // photons dealt and not yet complete
   std::deque<size_t> open;       // indices into pp_multi::batches of this device's incomplete batches, in order
+  bool dealing = false;          // a batch is being handed to this device right now, outside pp_multi::mu
 };
 
 }  // namespace
@@ -67,9 +69,11 @@ struct pp_multi {
   uint64_t deal_photons = 100000000ull;
   float yield = 0.0f;
   std::mutex mu;                 // staging, dealing, bookkeeping
+  std::condition_variable cv_dealt;  // a device has finished taking a batch (Device::dealing went false)
   std::deque<Staged> staged;
   uint64_t staged_photons = 0;
   uint64_t n_submitted = 0, ph_submitted = 0;
+  uint64_t n_deals = 0;          // batches cut off the staging queue so far
   uint64_t rejected_sources = 0; // sources of batches a back end refused (dropped, counted as complete)
   std::deque<Batch> batches;     // incomplete prefix trimmed as batches complete in order
   size_t batches_base = 0;       // global index of batches.front()
@@ -106,17 +110,28 @@ int refresh(pp_multi* m) {
 }
 
 // Cut a batch of whole sources holding at least `want` photons (or everything, if less is staged) off the staging
-// queue and hand it to the device with the fewest photons outstanding.  Caller holds m->mu.
-int deal_one(pp_multi* m, uint64_t want) {
-  if (m->staged.empty()) return PP_OK;
-  int rc = refresh(m);
-  if (rc != PP_OK) return rc;
+// queue and hand it to the device with the fewest photons outstanding.  Caller holds m->mu through `lk`; the lock is
+// RELEASED while the device takes the batch: its submit blocks while the device's source ring is full, and the
+// completed count, the drained test of collect, the statistics and every other submitter need m->mu meanwhile (behind
+// the multi-process server a dispatch thread that cannot ask for the completed count stops collecting, and with it
+// the only thing that would ever free the ring).  The batch leaves the staging queue and enters the books before the
+// lock is released; `dealing` keeps a second dealer off the same device until the hand-over is finished, so each
+// device sees its batches in the order of the books.
+int deal_one(pp_multi* m, uint64_t want, std::unique_lock<std::mutex>& lk) {
+  uint32_t best = 0;
+  for (;;) {
+    if (m->staged.empty()) return PP_OK;
+    const int rc0 = refresh(m);
+    if (rc0 != PP_OK) return rc0;
+    bool found = false;
+    for (uint32_t d = 0; d < m->dev.size(); ++d)
+      if (!m->dev[d].dealing && (!found || m->dev[d].outstanding < m->dev[best].outstanding)) { best = d; found = true; }
+    if (found) break;
+    m->cv_dealt.wait(lk);  // every device is taking a batch right now
+  }
   size_t n = 0;
   uint64_t ph = 0;
   while (n < m->staged.size() && (ph < want || n == 0)) ph += m->staged[n++].photons;
-  uint32_t best = 0;
-  for (uint32_t d = 1; d < m->dev.size(); ++d)
-    if (m->dev[d].outstanding < m->dev[best].outstanding) best = d;
   std::vector<pp_source> src(n);
   std::vector<float> len(n);
   std::vector<uint32_t> ev(n), sid(n);
@@ -127,28 +142,34 @@ int deal_one(pp_multi* m, uint64_t want) {
     any_len |= r.length != 0.0f;
   }
   Device& D = m->dev[best];
-  rc = D.be.submit(D.be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
-  if (rc == PP_E_INVAL || rc == PP_E_OVERFLOW) {
-    // the device refused the batch as a whole (pp.h: none of its sources is propagated); pp_multi_submit makes the
-    // handle's own checks, so this means a back end with other rules or another light yield.  The batch must not stay
-    // at the head of the queue, where every later deal would meet it again: it is taken out and counted as complete
-    // without hits (so that whoever waits on the completed count is not stuck behind it), and the caller of this deal
-    // gets the code.
-    m->staged.erase(m->staged.begin(), m->staged.begin() + (long)n);
-    m->staged_photons -= ph;
-    m->rejected_sources += n;
-    m->batches.push_back(Batch{best, n, 0, D.dealt_sources, true});
-    return rc;
-  }
-  if (rc != PP_OK) return rc;
-  rc = D.be.flush(D.be.ctx);  // a dealt batch is a whole launch: do not wait for more
-  if (rc != PP_OK) return rc;
   m->staged.erase(m->staged.begin(), m->staged.begin() + (long)n);
   m->staged_photons -= ph;
   D.dealt_sources += n; D.dealt_photons += ph; D.batches++; D.outstanding += ph;
   m->batches.push_back(Batch{best, n, ph, D.dealt_sources, false});
-  D.open.push_back(m->batches_base + m->batches.size() - 1);
-  return PP_OK;
+  const size_t idx = m->batches_base + m->batches.size() - 1;
+  D.open.push_back(idx);
+  D.dealing = true;
+  m->n_deals++;
+  lk.unlock();
+  int rc = D.be.submit(D.be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
+  if (rc == PP_OK) rc = D.be.flush(D.be.ctx);  // a dealt batch is a whole launch: do not wait for more
+  lk.lock();
+  D.dealing = false;
+  m->cv_dealt.notify_all();
+  if (rc == PP_E_INVAL || rc == PP_E_OVERFLOW) {
+    // the device refused the batch as a whole (pp.h: none of its sources is propagated); pp_multi_submit makes the
+    // handle's own checks, so this means a back end with other rules or another light yield.  The batch is gone from
+    // the staging queue already (left there, every later deal would meet it again); it is taken out of the device's
+    // books and counted as complete without hits, so that whoever waits on the completed count is not stuck behind it,
+    // and the caller of this deal gets the code.  (It is the device's newest batch: nobody else dealt to it meanwhile;
+    // and it cannot have been found complete, since the device never got its sources.)
+    D.dealt_sources -= n; D.dealt_photons -= ph; D.batches--; D.outstanding -= ph;
+    D.open.pop_back();
+    Batch& b = m->batches[idx - m->batches_base];
+    b.photons = 0; b.dev_end = D.dealt_sources; b.complete = true;
+    m->rejected_sources += n;
+  }
+  return rc;
 }
 
 // the front as a pp_ipc_backend
@@ -168,7 +189,20 @@ int collect_once(pp_multi* m, pp_hit* out, size_t cap, size_t* n_out, int* drain
   *drained = 0;
   std::lock_guard<std::mutex> g(m->collect_mu);
   const uint32_t nd = (uint32_t)m->dev.size();
+  // "drained" = every device is, and no source was on its way to one while they were asked: nothing staged, no batch
+  // being handed over, and no batch dealt between the look before and the look after
+  auto quiet = [&]() {
+    bool q = m->staged.empty();
+    for (const Device& D : m->dev) q = q && !D.dealing;
+    return q;
+  };
+  uint64_t deals_before = 0;
   bool all_drained = true;
+  {
+    std::lock_guard<std::mutex> g2(m->mu);
+    deals_before = m->n_deals;
+    all_drained = quiet();
+  }
   for (uint32_t k = 0; k < nd; ++k) {
     Device& D = m->dev[(m->next_dev + k) % nd];
     size_t got = 0;
@@ -184,7 +218,7 @@ int collect_once(pp_multi* m, pp_hit* out, size_t cap, size_t* n_out, int* drain
   }
   if (all_drained) {
     std::lock_guard<std::mutex> g2(m->mu);
-    *drained = m->staged.empty() ? 1 : 0;
+    *drained = (quiet() && m->n_deals == deals_before) ? 1 : 0;
   }
   return PP_OK;
 }
@@ -245,7 +279,7 @@ int pp_multi_submit(pp_multi* m, const pp_source* sources, const float* lengths_
     const int rc = pp_photon_count(a.energy_GeV, m->yield, &cnt[i]);
     if (rc != PP_OK) return rc;
   }
-  std::lock_guard<std::mutex> g(m->mu);
+  std::unique_lock<std::mutex> g(m->mu);
   for (size_t i = 0; i < n; ++i) {
     Staged r;
     r.s = sources[i]; r.length = lengths_m ? lengths_m[i] : 0.0f; r.event_id = event_ids[i];
@@ -257,7 +291,7 @@ int pp_multi_submit(pp_multi* m, const pp_source* sources, const float* lengths_
   m->n_submitted += n;
   for (size_t i = 0; i < n; ++i) m->ph_submitted += cnt[i];
   while (m->staged_photons >= m->deal_photons) {
-    const int rc = deal_one(m, m->deal_photons);
+    const int rc = deal_one(m, m->deal_photons, g);
     if (rc != PP_OK) return rc;
   }
   return PP_OK;
@@ -265,11 +299,12 @@ int pp_multi_submit(pp_multi* m, const pp_source* sources, const float* lengths_
 
 int pp_multi_flush(pp_multi* m) {
   if (!m) return PP_E_INVAL;
-  std::lock_guard<std::mutex> g(m->mu);
+  std::unique_lock<std::mutex> g(m->mu);
   while (!m->staged.empty()) {
-    const int rc = deal_one(m, m->deal_photons);
+    const int rc = deal_one(m, m->deal_photons, g);
     if (rc != PP_OK) return rc;
   }
+  // (a batch another thread is still handing over is flushed by that thread)
   for (auto& D : m->dev) {
     const int rc = D.be.flush(D.be.ctx);
     if (rc != PP_OK) return rc;

@@ -167,3 +167,50 @@ def test_client_processes_in_front_of_two_devices():
             a.close(), b.close()
         st = m.stats()
         assert sum(st["batches"]) >= 2 and st["sources_completed"] == 360
+
+
+def test_the_front_stays_responsive_while_a_device_takes_a_batch_slowly():
+    """A device whose source ring is full blocks in submit (pp.h).  The front hands a batch over OUTSIDE its lock
+    (round-2 advice): meanwhile the statistics and the completed count answer, other callers' batches go to the other
+    device, and "drained" is not reported while a batch is on its way."""
+    import ctypes as C
+    import time
+    b0 = multi.Backend()
+    C.memmove(C.byref(b0), C.c_void_p(echo_backend()), C.sizeof(multi.Backend))
+    SUBMIT = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t)
+    real = SUBMIT(b0.submit)
+    entered, gate = threading.Event(), threading.Event()
+
+    def slow(ctx, s, ln, ev, sid, n):
+        entered.set()
+        gate.wait(20)
+        return real(ctx, s, ln, ev, sid, n)
+
+    keep = SUBMIT(slow)
+    b0.submit = C.cast(keep, C.c_void_p).value
+    s1, e1, i1, l1 = _sources(5, 2, 4)
+    s2, e2, i2, l2 = _sources(6, 3, 3)
+    with multi.MultiFront(backends=[C.addressof(b0), echo_backend()], photons_per_GeV=1.0e4, deal_photons=10 ** 12) as m:
+        t = threading.Thread(target=lambda: (m.submit(s1, e1, i1, l1), m.flush()))  # the flush deals one batch
+        t.start()
+        try:
+            assert entered.wait(10)                           # device 0 is "taking" that batch and will not finish
+            t0 = time.monotonic()
+            st = m.stats()                                    # needs the front's lock
+            assert st["sources_staged"] == 0 and st["photons_outstanding"][0] > 0 and st["sources_completed"] == 0
+            m.submit(s2, e2, i2, l2)
+            m.flush()                                         # dealt to device 1: device 0 is busy
+            got2 = []
+            while len(got2) < len(e2) and time.monotonic() - t0 < 5:
+                got2.extend(m.collect(block=False))
+            assert time.monotonic() - t0 < 5 and len(got2) == len(e2)
+            assert m.stats()["batches"] == [1, 1]
+        finally:
+            gate.set()
+            t.join(10)
+        assert not t.is_alive()
+        got1 = np.sort(m.collect_all(), order=ORDER)
+        st = m.stats()
+    assert np.array_equal(got1, _expected(s1, e1, i1, l1))
+    assert np.array_equal(np.sort(np.array(got2, dtype=B.HIT_DTYPE), order=ORDER), _expected(s2, e2, i2, l2))
+    assert st["sources_completed"] == st["sources_submitted"] == len(e1) + len(e2)
