@@ -206,17 +206,25 @@ void ingest_main(pp_ipc_server* s, uint32_t me, uint32_t n_thr) {
           }
         pp_ipc_server::Block blk{c, tail + n, 0, {}};
         {
-          std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
+          // the block's distinct event ids, found outside the lock (one id per run of equal ids, then sort + unique:
+          // a block of 16384 one-source events costs n log n here, not n^2 comparisons inside the lock the dispatch
+          // thread needs for every run of hits it routes)
+          std::vector<uint32_t>& ids = blk.events;
           uint32_t last = ~(packed ? ring[t0].event_id : ev[0]);
           for (size_t i = 0; i < n; ++i) {
             const uint32_t e = packed ? ring[t0 + i].event_id : ev[i];
-            if (e == last) continue;
-            last = e;
-            if (std::find(blk.events.begin(), blk.events.end(), last) != blk.events.end()) continue;
-            auto it = s->owner.find(last);
-            if (it == s->owner.end()) it = s->owner.emplace(last, pp_ipc_server::Owner{c, 0}).first;
-            if (it->second.client == c) { it->second.blocks++; blk.events.push_back(last); }  // else: caller error (pp_ipc.h)
+            if (e != last) { ids.push_back(e); last = e; }
           }
+          std::sort(ids.begin(), ids.end());
+          ids.erase(std::unique(ids.begin(), ids.end()), ids.end());
+          std::lock_guard<std::mutex> g(s->map_mu);  // announce the events before their hits can exist
+          size_t kept = 0;
+          for (const uint32_t e : ids) {
+            auto it = s->owner.find(e);
+            if (it == s->owner.end()) it = s->owner.emplace(e, pp_ipc_server::Owner{c, 0}).first;
+            if (it->second.client == c) { it->second.blocks++; ids[kept++] = e; }  // else: caller error (pp_ipc.h)
+          }
+          ids.resize(kept);
         }
         s->pc[c].blocks_in_flight++;
         int rc;

@@ -352,3 +352,26 @@ def test_a_block_shipped_to_an_idle_server_is_never_declared_complete_before_it_
                 total += len(ev)
         st = srv.stats()
         assert st["error"] == 0 and st["hits_unrouted"] == 0 and st["hits_routed"] == total
+
+
+def test_a_block_of_one_source_events_with_interleaved_ids():
+    """A block whose sources all belong to different events, some ids recurring out of order within the block: every
+    id is announced once (the owner count per block is 1 however often the id recurs), all hits are routed, and the
+    owner table empties.  (Round-2 advice: the ids are de-duplicated by sort + unique outside the routing lock.)"""
+    import time
+    name = f"/pp_ipc_test_{os.getpid()}_ids"
+    with ipc.IpcServer(None, name, max_clients=1, backend=echo_backend()) as srv:
+        with ipc.IpcClient(name) as c:
+            n = 6000
+            src, _, _, ln = _sources(3, n, 1)
+            ev = (np.arange(n) % 4500 * 7 + 20000).astype(np.uint32)   # 4500 distinct ids, 1500 of them twice, far apart
+            sid = (np.arange(n) // 4500).astype(np.uint32)
+            c.submit(src, ev, sid, ln)
+            got = np.sort(c.collect_all(), order=["event_id", "source_id"])
+            assert np.array_equal(got, _expected(src, ev, sid, ln))
+        for _ in range(200):
+            if srv.stats()["events_tracked"] == 0:
+                break
+            time.sleep(0.005)
+        st = srv.stats()
+        assert st["events_tracked"] == 0 and st["hits_unrouted"] == 0 and st["hits_routed"] == n and st["error"] == 0
