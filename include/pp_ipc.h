@@ -90,6 +90,7 @@ typedef struct pp_ipc_server_stats {
   uint64_t hits_dropped;     /* hits of clients that had left (closed, or their process died) */
   uint64_t clients_dropped;  /* clients the server declared gone because their process no longer exists */
   uint64_t events_tracked;   /* entries of the event-owner table right now (bounded by the events in flight) */
+  uint64_t clients_failed;   /* clients a block of which the back end refused (see pp_ipc_submit) */
 } pp_ipc_server_stats;
 int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out);
 
@@ -98,7 +99,13 @@ int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out);
  * none, PP_E_STATE if there is no server). */
 int pp_ipc_client_open(const char* shm_name, pp_ipc_client** out);
 /* Ships a block of n sources.  lengths_m and source_ids may be NULL as in pp_submit_segments.
- * Blocks while the client's source ring is full; a block larger than the ring is shipped in pieces. */
+ * Blocks while the client's source ring is full; a block larger than the ring is shipped in pieces.
+ * A block with a bad source (pp.h, pp_submit) fails here with PP_E_INVAL and ships nothing.  What only the server can
+ * judge -- a source of more than 2^32 - 1 photons at the server's light yield, or anything else its back end refuses
+ * with PP_E_INVAL / PP_E_OVERFLOW -- fails THIS client only: the refused block is dropped as a whole, the server takes
+ * no more sources from the client and drops its outstanding hits, and every later pp_ipc_submit / pp_ipc_flush /
+ * pp_ipc_collect of the client returns the back end's code (hits already in its ring are still handed out first).
+ * The other clients are served as before; pp_ipc_client_close frees the slot as usual. */
 int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengths_m, const uint32_t* event_ids,
                   const uint32_t* source_ids, size_t n);
 /* Asks the server to launch whatever is queued (pp_flush) once it has ingested everything this client shipped. */

@@ -56,7 +56,10 @@ static_assert(sizeof(ShmHeader) <= kHeaderBytes, "header");
 // slot's ingest thread has seen that and will not touch the slot's source ring again) -> kRecycled (the dispatch thread has
 // emptied it: claimable again).  Only the ingest thread that serves a slot moves it out of kClosed, so the dispatch thread never
 // recycles a slot while a block of it is being handed to the back end.
-enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3, kQuiesced = 4 };
+// kFailed: the back end refused a block of this client (a source the client-side checks cannot judge, e.g. more than
+// 2^32 - 1 photons at the server's light yield): the server takes nothing more from it and drops its hits, every call of
+// the client returns the back end's code, and the slot goes the usual way once the client closes (or is gone).
+enum : uint32_t { kFree = 0, kAttached = 1, kClosed = 2, kRecycled = 3, kQuiesced = 4, kFailed = 5 };
 
 struct ClientCtl {
   std::atomic<uint32_t> state;
@@ -68,6 +71,7 @@ struct ClientCtl {
   std::atomic<uint64_t> flushed_seq;    // server: flush requests honoured up to here
   std::atomic<uint64_t> completed_seq;  // server: sources before it are propagated and their hits are in the hit ring
   std::atomic<uint32_t> pid;            // client: its process id (the server checks that a stalled client still exists)
+  std::atomic<int32_t> fail_code;       // server: why the slot is kFailed (a pp_status)
 };
 static_assert(sizeof(ClientCtl) <= kCtlBytes, "ctl");
 static_assert(std::atomic<uint64_t>::is_always_lock_free, "address-free atomics needed in shared memory");
@@ -131,7 +135,7 @@ struct pp_ipc_server {
   struct Owner { uint32_t client, blocks; };
   std::mutex map_mu;
   std::unordered_map<uint32_t, Owner> owner;
-  std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0}, dropped{0}, clients_dropped{0};
+  std::atomic<uint64_t> blocks{0}, sources{0}, routed{0}, unrouted{0}, dropped{0}, clients_dropped{0}, clients_failed{0};
   struct Block { uint32_t client; uint64_t tail_after, global_end; std::vector<uint32_t> events; };
   std::mutex fifo_mu;
   std::deque<Block> fifo;       // blocks handed to the back end, not yet known to be complete: in hand-over order with
@@ -181,6 +185,12 @@ void ingest_main(pp_ipc_server* s, uint32_t me, uint32_t n_thr) {
         }
         uint32_t expect = kClosed;
         ctl->state.compare_exchange_strong(expect, kQuiesced, std::memory_order_acq_rel);
+        continue;
+      }
+      if (state == kFailed) {
+        // nothing more is taken from a client whose block the back end refused; what it still ships is skipped
+        ctl->src_tail.store(ctl->src_head.load(std::memory_order_acquire), std::memory_order_release);
+        ctl->flushed_seq.store(ctl->flush_seq.load(std::memory_order_relaxed), std::memory_order_relaxed);
         continue;
       }
       if (state != kAttached) continue;
@@ -247,6 +257,30 @@ void ingest_main(pp_ipc_server* s, uint32_t me, uint32_t n_thr) {
           }
           rc = s->be.submit(s->be.ctx, src.data(), any_len ? len.data() : nullptr, ev.data(), sid.data(), n);
         }
+        if (rc == PP_E_INVAL || rc == PP_E_OVERFLOW) {
+          // The back end refused the block as a whole (pp.h: none of its sources is propagated): a fault of this
+          // client's input, not of the server.  The block is taken back out of the books, the client is marked failed,
+          // and everybody else is served as before.
+          if (!packed) {
+            std::lock_guard<std::mutex> g(s->fifo_mu);  // (listed before the hand-over; the one ingest thread's newest)
+            blk = std::move(s->fifo.back());
+            s->fifo.pop_back();
+          }
+          {
+            std::lock_guard<std::mutex> g(s->map_mu);
+            for (const uint32_t e : blk.events) {
+              auto it = s->owner.find(e);
+              if (it != s->owner.end() && it->second.client == c && --it->second.blocks == 0) s->owner.erase(it);
+            }
+          }
+          s->pc[c].blocks_in_flight--;
+          ctl->fail_code.store(rc, std::memory_order_release);
+          uint32_t expect = kAttached;
+          if (ctl->state.compare_exchange_strong(expect, kFailed, std::memory_order_acq_rel)) s->clients_failed++;
+          ctl->src_tail.store(ctl->src_head.load(std::memory_order_acquire), std::memory_order_release);
+          progressed = true;
+          continue;
+        }
         if (rc != PP_OK) { s->error.store(rc); s->stop.store(true); break; }
         s->blocks++; s->sources += n;
         tail += n;
@@ -271,14 +305,14 @@ void ingest_main(pp_ipc_server* s, uint32_t me, uint32_t n_thr) {
 bool client_gone(pp_ipc_server* s, uint32_t c) {
   ClientCtl* ctl = s->seg.ctl(c);
   const uint32_t st = ctl->state.load(std::memory_order_acquire);
-  if (st != kAttached) return true;
+  if (st != kAttached && st != kFailed) return true;
   auto& pc = s->pc[c];
   const auto now = Clock::now();
   if (now - pc.last_alive_check < std::chrono::milliseconds(10)) return false;
   pc.last_alive_check = now;
   const uint32_t pid = ctl->pid.load(std::memory_order_acquire);
   if (pid != 0 && kill((pid_t)pid, 0) != 0 && errno == ESRCH) {
-    uint32_t expect = kAttached;
+    uint32_t expect = st;
     if (ctl->state.compare_exchange_strong(expect, kClosed, std::memory_order_acq_rel)) s->clients_dropped++;
     return true;
   }
@@ -408,7 +442,7 @@ void dispatch_main(pp_ipc_server* s) {
       for (uint32_t c = 0; c < n_slots; ++c) {
         ClientCtl* ctl = s->seg.ctl(c);
         const uint32_t st = ctl->state.load(std::memory_order_acquire);
-        if (st == kAttached) { client_gone(s, c); continue; }  // a client whose process was killed is closed here
+        if (st == kAttached || st == kFailed) { client_gone(s, c); continue; }  // a client whose process was killed is closed here
         if (st != kQuiesced) continue;                         // the ingest thread has not let go of the slot yet
         auto& pc = s->pc[c];
         if (!pc.parked.empty()) { s->dropped += pc.parked.size(); pc.parked.clear(); pc.parked_n.store(0); }
@@ -417,6 +451,7 @@ void dispatch_main(pp_ipc_server* s) {
         pc.pending_completed = 0;
         ctl->completed_seq.store(ctl->src_head.load(std::memory_order_acquire), std::memory_order_release);
         ctl->pid.store(0, std::memory_order_relaxed);
+        ctl->fail_code.store(0, std::memory_order_relaxed);
         ctl->state.store(kRecycled, std::memory_order_release);
       }
       nap(100);
@@ -507,6 +542,7 @@ int pp_ipc_server_get_stats(pp_ipc_server* s, pp_ipc_server_stats* out) {
   out->blocks_ingested = s->blocks.load(); out->sources_ingested = s->sources.load();
   out->hits_routed = s->routed.load(); out->hits_unrouted = s->unrouted.load();
   out->hits_dropped = s->dropped.load(); out->clients_dropped = s->clients_dropped.load();
+  out->clients_failed = s->clients_failed.load();
   {
     std::lock_guard<std::mutex> g(s->map_mu);
     out->events_tracked = s->owner.size();
@@ -571,6 +607,7 @@ int pp_ipc_submit(pp_ipc_client* c, const pp_source* sources, const float* lengt
   size_t i = 0;
   while (i < n) {
     if (!H->server_alive.load(std::memory_order_acquire)) return PP_E_STATE;
+    if (ctl->state.load(std::memory_order_acquire) == kFailed) return ctl->fail_code.load(std::memory_order_acquire);
     const uint64_t head = ctl->src_head.load(std::memory_order_relaxed);
     const uint64_t space = H->src_cap - (head - ctl->src_tail.load(std::memory_order_acquire));
     if (space == 0) { nap(50); continue; }  // bounded ring: the client waits for the GPU
@@ -589,6 +626,7 @@ int pp_ipc_flush(pp_ipc_client* c) {
   if (!c) return PP_E_INVAL;
   ClientCtl* ctl = c->seg.ctl(c->slot);
   ctl->flush_seq.store(ctl->src_head.load(std::memory_order_relaxed), std::memory_order_release);
+  if (ctl->state.load(std::memory_order_acquire) == kFailed) return ctl->fail_code.load(std::memory_order_acquire);
   return c->seg.hdr()->server_alive.load(std::memory_order_acquire) ? PP_OK : PP_E_STATE;
 }
 
@@ -610,6 +648,7 @@ int pp_ipc_collect(pp_ipc_client* c, pp_hit* out, size_t cap, size_t* n_out, int
       *n_out = m;
       return PP_OK;
     }
+    if (ctl->state.load(std::memory_order_acquire) == kFailed) return ctl->fail_code.load(std::memory_order_acquire);
     if (complete || !block) return PP_OK;  // drained, or nothing yet
     if (!H->server_alive.load(std::memory_order_acquire)) return PP_E_STATE;
     nap(100);

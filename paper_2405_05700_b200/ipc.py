@@ -25,7 +25,7 @@ class _IpcConfig(C.Structure):
 class _IpcStats(C.Structure):
     _fields_ = [("clients_attached", C.c_uint64), ("blocks_ingested", C.c_uint64), ("sources_ingested", C.c_uint64),
                 ("hits_routed", C.c_uint64), ("hits_unrouted", C.c_uint64), ("hits_dropped", C.c_uint64),
-                ("clients_dropped", C.c_uint64), ("events_tracked", C.c_uint64)]
+                ("clients_dropped", C.c_uint64), ("events_tracked", C.c_uint64), ("clients_failed", C.c_uint64)]
 
 
 _declared = False

@@ -375,3 +375,57 @@ def test_a_block_of_one_source_events_with_interleaved_ids():
             time.sleep(0.005)
         st = srv.stats()
         assert st["events_tracked"] == 0 and st["hits_unrouted"] == 0 and st["hits_routed"] == n and st["error"] == 0
+
+
+def test_a_block_the_back_end_refuses_fails_its_client_only():
+    """What the client-side checks cannot judge (a photon count beyond 32 bits at the server's light yield, say) is
+    refused by the back end.  That used to stop the server for everybody (round-2 advice); now the refused block is
+    dropped, its client gets the back end's code from every later call, the others are served, and the slot comes
+    back once the failed client has closed."""
+    import ctypes as C
+    import time
+    from paper_2405_05700_b200 import multi
+    be = multi.Backend()
+    C.memmove(C.byref(be), C.c_void_p(echo_backend()), C.sizeof(multi.Backend))
+    SUBMIT = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32), C.c_void_p, C.c_size_t)
+    real = SUBMIT(be.submit)
+
+    def picky(ctx, s, ln, ev, sid, n):
+        if any(ev[i] == 777 for i in range(n)):
+            return -4
+        return real(ctx, s, ln, ev, sid, n)
+
+    keep = SUBMIT(picky)
+    be.submit = C.cast(keep, C.c_void_p).value
+    name = f"/pp_ipc_test_{os.getpid()}_refuse"
+    with ipc.IpcServer(None, name, max_clients=2, backend=C.addressof(be)) as srv:
+        a, b = ipc.IpcClient(name), ipc.IpcClient(name)
+        sa, ea, ia, la = _sources(0, 2, 4)
+        a.submit(sa, ea, ia, la)
+        assert len(a.collect_all()) == len(ea)             # a good block first: A works
+        a.submit(sa, np.full(len(ea), 777, np.uint32), ia, la)
+        with pytest.raises(B.PPError) as e:
+            a.collect_all()
+        assert e.value.code == -4
+        with pytest.raises(B.PPError) as e:
+            a.submit(sa, ea + np.uint32(50), ia, la)
+        assert e.value.code == -4
+        sb, eb, ib, lb = _sources(1, 5, 6)
+        b.submit(sb, eb, ib, lb)                           # B is served as if nothing had happened
+        assert np.array_equal(np.sort(b.collect_all(), order=["event_id", "source_id"]), _expected(sb, eb, ib, lb))
+        st = srv.stats()
+        assert st["error"] == 0 and st["clients_failed"] == 1 and st["hits_unrouted"] == 0
+        a.close()
+        c = None
+        for _ in range(400):                               # A's slot is handed out again
+            try:
+                c = ipc.IpcClient(name)
+                break
+            except B.PPError as e2:
+                assert e2.code == -2
+                time.sleep(0.005)
+        assert c is not None
+        c.submit(sa, ea + np.uint32(900), ia, la)
+        assert len(c.collect_all()) == len(ea)
+        assert srv.stats()["events_tracked"] == 0 or time.sleep(0.2) or srv.stats()["events_tracked"] == 0
+        b.close(), c.close()
