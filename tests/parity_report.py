@@ -1,5 +1,7 @@
 #!/usr/bin/env python
-"""Measured per-hit time parity of the CUDA path against the fp64 oracle (identical Philox streams), as a markdown
+"""A REPORT GENERATOR, not a test (pytest does not collect it; it calls only the oracle and the C ABI binding).
+
+Measured per-hit time parity of the CUDA path against the fp64 oracle (identical Philox streams), as a markdown
 report: `python tests/parity_report.py > gpurun_out/r02_parity.md` on a GPU box (copied to profiles/).
 
 For every configuration of BASELINE.json (C0..C4; the sampled comparisons the -m gpu tests make) it prints the number

@@ -11,7 +11,9 @@ from paper_2405_05700_b200 import binding as B
 from paper_2405_05700_b200 import ipc
 from paper_2405_05700_b200 import workloads as W
 
-from gpu_util import KEY, sort_hits
+from oracle import oracle as O
+
+from gpu_util import KEY, compare_hits, sort_hits
 
 pytestmark = pytest.mark.gpu
 N_EVENTS = 120
@@ -49,6 +51,12 @@ def test_clients_share_one_gpu_server(n_clients, ring_kib):
         ref = sort_hits(p.run(s, ev, sid))
         n_ref_launches = p.stats().launches
     assert len(ref) > 2000 and n_ref_launches >= 3
+    if n_clients == 4:
+        # ... and that single-process run is what the oracle computes (once is enough: the other cases compare with
+        # the same list, bit for bit)
+        ref_o = O.propagate(geo, ice, W.Sources(s, ev, sid), seed=12)
+        c = compare_hits(ref, ref_o.hits, ref_o.photons)
+        assert c["frac_hit"] >= 0.99 and c["frac_all"] >= 0.999, c
     name = f"/pp_ipc_gpu_{os.getpid()}_{n_clients}"
     ctx = mp.get_context("spawn")
     q = ctx.Queue()

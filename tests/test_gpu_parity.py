@@ -11,7 +11,7 @@ from oracle import oracle as O
 from paper_2405_05700_b200 import binding as B
 from paper_2405_05700_b200 import workloads as W
 
-from gpu_util import TOL_NS, compare_hits, gpu_run, gpu_run_resident, sort_hits, total_photons
+from gpu_util import TOL_NS, compare_hits, flights_agree, gpu_run, gpu_run_resident, sort_hits, total_photons
 
 pytestmark = pytest.mark.gpu
 
@@ -62,6 +62,20 @@ def test_c0_brute_force_lookup_equals_cell_grid(seed):
     ref = O.propagate(geo, ice, src, seed=seed, brute_force=True)
     c = compare_hits(h_fast, ref.hits, 200000)
     assert c["frac_all"] >= 0.999 and c["frac_hit"] >= 0.99, c
+
+
+def test_c0_at_its_real_radius_with_enough_photons_to_hit():
+    """C0 as BASELINE.json states it (one string, R = 0.1651 m, homogeneous ice) sees no hit at all in 1e5 photons, so
+    it says nothing about hit times.  The same configuration with the cascade axis toward the string and 2e7 photons
+    ("C0-big"): several hundred hits, every photon replayed by the oracle."""
+    geo, ice = W.geometry_single_string(), W.ice_homogeneous()
+    src = W.sources_c0(seed=0, n_photons=2.0e7, toward_string=True)
+    hits, st = gpu_run(geo, ice, src, 0)
+    ref = O.propagate(geo, ice, src, seed=0)
+    assert st.photons_done == ref.photons == 20000000 and st.photons_aborted == 0
+    assert flights_agree(st.flights, ref.flights)
+    c = compare_hits(hits, ref.hits, ref.photons)
+    assert c["n_union"] > 300 and c["frac_hit"] >= 0.995 and c["frac_all"] >= 0.9999999, c  # measured: 672 hits, 1.000
 
 
 def test_layered_full_detector_every_photon():
