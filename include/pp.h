@@ -103,6 +103,10 @@ typedef struct pp_ice {
                                            (the convention of measured ice tables); the mean free path between
                                            scatters is then lambda_e (1-g) (reading R-20; needs g < 1) */
 
+#define PP_FLAG_DEVICE_ORDINAL 8u /* pp_config.device names a CUDA device ordinal even when it is 0 (without the flag,
+                                     device <= 0 means "the calling thread's current device", so that a zeroed
+                                     pp_config keeps working -- and device 0 cannot be named while another is current) */
+
 /* Sizes and resources.  Zero means "default".  device_workspace / pinned_workspace / streams may be
  * NULL: the library then allocates them itself (cudaMalloc / cudaHostAlloc / cudaStreamCreate) and
  * frees them in pp_destroy.  When given (PyTorch supplies them in the Python binding), they stay
@@ -120,7 +124,8 @@ typedef struct pp_config {
   void* stream1; /* cudaStream_t */
   uint32_t flags;
   uint32_t max_flights; /* safety cap on flights per photon (default 100000, R-10); < 2^31 */
-  int32_t device;       /* CUDA device ordinal (default: current device) */
+  int32_t device;       /* CUDA device ordinal; <= 0: the current device, unless PP_FLAG_DEVICE_ORDINAL makes 0 an
+                           ordinal.  pp_create leaves the caller's current device as it found it. */
   uint32_t reserved;
 } pp_config;
 

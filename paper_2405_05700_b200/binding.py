@@ -23,6 +23,7 @@ ERRORS = {-1: "PP_E_INVAL", -2: "PP_E_NOMEM", -3: "PP_E_CUDA", -4: "PP_E_OVERFLO
 FLAG_BRUTE_FORCE_DOMS = 1
 FLAG_NONBLOCKING_SUBMIT = 2
 FLAG_EFFECTIVE_SCATTERING = 4
+FLAG_DEVICE_ORDINAL = 8
 ACCEPTANCE_MODES = {"off": 0, "probabilistic": 1, "weighted": 2}
 
 SOURCE_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("dx", "<f4"), ("dy", "<f4"), ("dz", "<f4"),
@@ -241,8 +242,9 @@ class Propagator:
     attributes)."""
 
     def __init__(self, geometry, ice, *, seed: int = 0, launch_photons_target: int = 0, hit_ring_bytes: int = 0,
-                 source_ring_bytes: int = 0, flags: int = 0, max_flights: int = 0, device: int = 0,
+                 source_ring_bytes: int = 0, flags: int = 0, max_flights: int = 0, device: int | None = None,
                  use_torch_memory: bool = True):
+        """``device``: a CUDA device ordinal (0 is device 0), or None for torch's current device."""
         import torch  # device memory, pinned memory and streams only
 
         if not torch.cuda.is_available():
@@ -257,8 +259,11 @@ class Propagator:
         cfg.source_ring_bytes = int(source_ring_bytes)
         cfg.flags = int(flags) | (FLAG_EFFECTIVE_SCATTERING if getattr(ice, "effective_scattering", False) else 0)
         cfg.max_flights = int(max_flights)
+        if device is None:
+            device = torch.cuda.current_device()
         cfg.device = int(device)
-        self.device = torch.device("cuda", device if device else torch.cuda.current_device())
+        cfg.flags |= FLAG_DEVICE_ORDINAL
+        self.device = torch.device("cuda", int(device))
         self._keep = []
         if use_torch_memory:
             dev_b, pin_b = C.c_uint64(0), C.c_uint64(0)

@@ -962,7 +962,7 @@ int pp_workspace_size(const pp_geometry* geo, const pp_ice* ice, const pp_config
   if (rc != PP_OK) return rc;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return PP_E_CUDA;
-  if (cfg->device > 0) dev = cfg->device;
+  if (cfg->device > 0 || (cfg->device == 0 && (cfg->flags & PP_FLAG_DEVICE_ORDINAL))) dev = cfg->device;
   int n_sm = 0;
   if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PP_E_CUDA;
   pp_handle tmp;
@@ -991,9 +991,10 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   h->ice = *ice;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { delete h; return PP_E_CUDA; }
-  if (cfg->device > 0) dev = cfg->device;
+  const int callers_dev = dev;  // made current again before pp_create returns, whatever the outcome
+  if (cfg->device > 0 || (cfg->device == 0 && (cfg->flags & PP_FLAG_DEVICE_ORDINAL))) dev = cfg->device;
   h->device = dev;
-  auto bail = [&](int code) { pp_destroy(h); return code; };
+  auto bail = [&](int code) { pp_destroy(h); cudaSetDevice(callers_dev); return code; };
   if (cudaSetDevice(dev) != cudaSuccess) return bail(PP_E_CUDA);
   if (cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(PP_E_CUDA);
   h->brute = (cfg->flags & PP_FLAG_BRUTE_FORCE_DOMS) != 0;
@@ -1068,6 +1069,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   if (cudaEventRecord(h->ev_base, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
   if (cudaEventSynchronize(h->ev_base) != cudaSuccess) return bail(PP_E_CUDA);
   h->server = std::thread(server_main, h);
+  if (callers_dev != dev) cudaSetDevice(callers_dev);
   *out = h;
   return PP_OK;
 }
