@@ -155,6 +155,100 @@ def test_independent_streams_per_dom_chi2_and_mean_times():
     assert abs(zs.mean()) < 4 / math.sqrt(len(zs)) and np.abs(zs).max() < 5.0
 
 
+def _stat_gate(name, geo, ice, src, oracle_kw, n_oracle_photons, min_time_doms, **gpu_kw):
+    """north_star's statistical gate on one configuration AS STATED (real DOM radius, full size on the GPU): GPU seeds
+    0-9 against oracle seeds 100-109, the oracle on a bounded subsample of the photons (`oracle_kw`).  Per seed a
+    two-sample chi^2 over DOMs for samples of unequal size (expected counts scale with the photons tracked; DOMs whose
+    smaller expectation is < 10 are pooled into one bin), summed over the seeds: p > 0.01, at most one seed below 0.01
+    (R-14).  Per-DOM mean arrival times over all seeds: within 0.5 % where the standard error is < 0.1 %, z-scores
+    otherwise (R-15).  The p-values go to gpurun_out/r03_stat_gate.jsonl for profiles/."""
+    import json
+    import os
+    n_g = total_photons(src, ice)
+    n_o = n_oracle_photons
+    chi2_sum, dof_sum, pvals = 0.0, 0, []
+    nd = geo.n_dom
+    acc = {k: np.zeros(nd) for k in ("ng", "sg", "qg", "no", "so", "qo")}
+    for k in range(10):
+        hg, st = gpu_run(geo, ice, src, k, **gpu_kw)
+        ro = O.propagate(geo, ice, src, seed=100 + k, **oracle_kw)
+        assert st.photons_done == n_g and ro.photons == n_o and st.photons_aborted == 0
+        cg = np.bincount(hg["dom_id"], minlength=nd).astype(np.float64)
+        co = np.bincount(ro.hits["dom_id"], minlength=nd).astype(np.float64)
+        big = (cg + co) * min(n_g, n_o) / (n_g + n_o) >= 10.0
+        a = np.concatenate([cg[big], [cg[~big].sum()]])
+        b = np.concatenate([co[big], [co[~big].sum()]])
+        keep = (a + b) > 0
+        chi2 = ((n_o * a - n_g * b) ** 2 / (float(n_g) * float(n_o) * (a + b)))[keep].sum()
+        dof = int(keep.sum())
+        chi2_sum += chi2
+        dof_sum += dof
+        pvals.append(float(stats.chi2.sf(chi2, dof)))
+        for tag, h in (("g", hg), ("o", ro.hits)):
+            t = h["time_ns"].astype(np.float64)
+            acc["n" + tag] += np.bincount(h["dom_id"], minlength=nd)
+            acc["s" + tag] += np.bincount(h["dom_id"], weights=t, minlength=nd)
+            acc["q" + tag] += np.bincount(h["dom_id"], weights=t * t, minlength=nd)
+    p_tot = float(stats.chi2.sf(chi2_sum, dof_sum))
+    sel = (acc["ng"] >= 100) & (acc["no"] >= 100)
+    mg, mo = acc["sg"][sel] / acc["ng"][sel], acc["so"][sel] / acc["no"][sel]
+    vg, vo = acc["qg"][sel] / acc["ng"][sel] - mg ** 2, acc["qo"][sel] / acc["no"][sel] - mo ** 2
+    se = np.sqrt(vg / acc["ng"][sel] + vo / acc["no"][sel])
+    zs = (mg - mo) / se
+    rel = np.abs(mg - mo) / mo
+    tight = se / mo < 1e-3
+    # all hits pooled (the only time comparison the oracle's sample supports where no DOM collects 100 hits)
+    Ng, No = acc["ng"].sum(), acc["no"].sum()
+    Mg, Mo = acc["sg"].sum() / Ng, acc["so"].sum() / No
+    z_all = (Mg - Mo) / math.sqrt((acc["qg"].sum() / Ng - Mg ** 2) / Ng + (acc["qo"].sum() / No - Mo ** 2) / No)
+    rec = {"config": name, "z_all_hits": float(z_all), "mean_time_gpu": float(Mg), "mean_time_oracle": float(Mo), "gpu_photons_per_seed": n_g, "oracle_photons_per_seed": n_o, "p_total": p_tot,
+           "p_per_seed": pvals, "chi2": chi2_sum, "dof": dof_sum, "gpu_hits": int(acc["ng"].sum()),
+           "oracle_hits": int(acc["no"].sum()), "doms_time_compared": int(sel.sum()), "doms_se_below_0.1pct": int(tight.sum()),
+           "max_rel_dt_tight": float(rel[tight].max()) if tight.any() else None,
+           "z_mean": float(zs.mean()) if len(zs) else None, "z_absmax": float(np.abs(zs).max()) if len(zs) else None}
+    print(json.dumps(rec))
+    try:
+        os.makedirs("gpurun_out", exist_ok=True)
+        with open(os.path.join("gpurun_out", "r03_stat_gate.jsonl"), "a") as f:
+            f.write(json.dumps(rec) + "\n")
+    except OSError:
+        pass
+    assert p_tot > 0.01, rec
+    assert sum(p < 0.01 for p in pvals) <= 1, rec
+    assert sel.sum() >= min_time_doms, rec
+    assert np.all(rel[tight] < 5e-3), rec
+    if len(zs):
+        assert abs(zs.mean()) < 4 / math.sqrt(len(zs)) and np.abs(zs).max() < 5.0, rec
+    assert abs(rec["z_all_hits"]) < 5.0, rec
+
+
+@pytest.mark.slow
+def test_stat_gate_c1_as_stated():
+    """C1 itself: 5160 DOMs of R = 0.1651 m, layered ice, the whole 1.96e9-photon muon on the GPU in the bench's launch
+    configuration; the oracle tracks photon_idx % 16 == 0 with other seeds (two independent
+    implementations agree on the observables)."""
+    geo, ice, src = W.geometry_full(), W.ice_layered(), W.sources_c1()
+    n_o = sum(-(-O.photon_count(e, ice.photons_per_GeV) // 16) for e in src.src[:, 7])
+    _stat_gate("C1", geo, ice, src, {"stride": 16}, n_o, 1, launch_photons_target=10 ** 8)
+
+
+@pytest.mark.slow
+def test_stat_gate_c0_big_as_stated():
+    """C0's geometry and ice (one string, R = 0.1651 m, homogeneous) with the axis toward the string: 1e8 photons on
+    the GPU, 1e7 in the oracle."""
+    geo, ice = W.geometry_single_string(), W.ice_homogeneous()
+    src = W.sources_c0(seed=0, n_photons=1.0e8, toward_string=True)
+    _stat_gate("C0-big", geo, ice, src, {"stride": 10}, 10 ** 7, 0)
+
+
+@pytest.mark.slow
+def test_stat_gate_c2_as_stated():
+    """C2 whole (1000 bundle events, real DOM radius) on the GPU; the oracle tracks photon_idx % 8 == 0."""
+    geo, ice, src = W.geometry_full(), W.ice_layered(), W.sources_c2()
+    n_o = sum(-(-O.photon_count(e, ice.photons_per_GeV) // 8) for e in src.src[:, 7])
+    _stat_gate("C2", geo, ice, src, {"stride": 8}, n_o, 0, launch_photons_target=3 * 10 ** 7)
+
+
 def test_identical_streams_per_dom_mean_time_bias():
     """R-15 first half: with IDENTICAL streams, per-DOM mean arrival times of DOMs with >= 100 hits agree
     to far better than 0.5 % (tests arithmetic bias, not statistics)."""
