@@ -1059,7 +1059,7 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
     P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
     for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x optional physics
-      P.acc_mode = (f & 2) ? 1u : 0u;  // (any of the optional-physics switches selects the same variant)
+      P.emit_on = (f & 2) ? 1u : 0u;  // (any of the switches of the flight-loop physics selects the same variant)
       if (launch_propagate(P, h->brute, (f & 1) != 0, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     }
     if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);

@@ -279,6 +279,23 @@ __device__ __noinline__ float absorb_distance(const LaunchParams& P, float phz, 
   }
 }
 
+// DOM acceptance (R-17), rare path: p(eta) in the arrival direction cosine eta = d_z of a photon that met a DOM on
+// flight k_hit.  Returns the weight of the hit (1 in the probabilistic mode, p in the weighted mode), or a negative
+// number if the photon makes no photoelectron.
+__device__ __noinline__ float dom_accepts(const LaunchParams& P, float dz, uint32_t pidx, uint32_t sid, uint32_t ev,
+                                          uint32_t k_hit) {
+  float pa = 0.0f;
+  for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
+  pa = fminf(fmaxf(pa, 0.0f), 1.0f);
+  if (P.spec_n != 0u) pa = fminf(1.0f, pa * P.spec_acc[spectrum_bin(P, pidx, sid, ev)]);  // R-21
+  if (P.acc_mode == 1u) {
+    uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | k_hit;
+    philox4x32_10(a0, a1, a2, a3, P.rk);
+    return (uniform_from_word(a0) < pa) ? 1.0f : -1.0f;
+  }
+  return (pa > 0.0f) ? pa : -1.0f;
+}
+
 // Fetch the next work item of the launch for a warp (lane 0 talks to the queues; rare: once per tile).
 // Returns the warp-uniform (t_next, t_end, s_cur, resume list not yet empty); t_next == t_end means no work is left.
 __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, bool use_resume) {
@@ -318,8 +335,8 @@ __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, b
   return r;
 }
 
-// kExt: the optional physics (DOM acceptance R-17, track-segment sources R-18, wavelength bins R-21, emission
-// smearing R-22) is compiled in.  kLoop: the inverse walk tables are coarser than the thinnest layer (pathological
+// kExt: the optional physics that touches the flight loop (track-segment sources R-18, wavelength bins R-21, emission
+// smearing R-22) is compiled in; the DOM acceptance (R-17) is in every variant, in the rare hit block.  kLoop: the inverse walk tables are coarser than the thinnest layer (pathological
 // ice, LaunchParams::walk_loop), so the layer found may be several layers short
 template <bool kBrute, bool kFates, bool kExt, bool kLoop>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
@@ -591,21 +608,12 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       }
       hit_mask = __ballot_sync(0xffffffffu, hit);
       float weight = 1.0f;
-      if (kExt && P.acc_mode != 0u && hit_mask) {
-        // ---- DOM acceptance (R-17): p(eta) in the arrival direction cosine eta = d_z ----
+      if (P.acc_mode != 0u && hit_mask) {
+        // ---- DOM acceptance (R-17): asked only here, where a lane of the warp has met a DOM (4e-5 of the photons
+        // in C1), behind a warp-uniform run-time switch: every kernel variant has it, and it costs the others nothing
         if (hit) {
-          float pa = 0.0f;
-          for (int c = (int)P.acc_n - 1; c >= 0; --c) pa = fmaf(pa, dz, P.acc_coef[c]);
-          pa = fminf(fmaxf(pa, 0.0f), 1.0f);
-          if (P.spec_n != 0u) pa = fminf(1.0f, pa * P.spec_acc[spectrum_bin(P, pidx, sid, ev)]);  // R-21
-          if (P.acc_mode == 1u) {
-            uint32_t a0 = pidx, a1 = sid, a2 = ev, a3 = 0x80000000u | (k - 1u);  // k was advanced: the hit flight is k - 1
-            philox4x32_10(a0, a1, a2, a3, P.rk);
-            rejected = !(uniform_from_word(a0) < pa);
-          } else {
-            weight = pa;
-            rejected = !(pa > 0.0f);
-          }
+          weight = dom_accepts(P, dz, pidx, sid, ev, k - 1u);  // k was advanced: the hit flight is k - 1
+          rejected = weight < 0.0f;
           hit = !rejected;
         }
         const unsigned rej_mask = __ballot_sync(0xffffffffu, rejected);
@@ -757,7 +765,8 @@ static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, c
 
 // the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use, coarse walk tables)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
-  const bool ext = P.acc_mode != 0u || P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u;
+  // (the DOM acceptance needs no variant of its own: it sits in the rare hit block of every variant)
+  const bool ext = P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u;
   const int v = (P.walk_loop ? 8 : 0) | (brute ? 4 : 0) | (fates ? 2 : 0) | (ext ? 1 : 0);
   switch (v) {
     case 0: return launch_prop_t<false, false, false, false>(P, grid, smem, st);
