@@ -15,7 +15,8 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpp.so")
+# (developer knob: PP_LIB names another build of the library, e.g. the tests' guard build -- never a fallback)
+LIB_PATH = os.environ.get("PP_LIB") or os.path.join(_HERE, "libpp.so")
 
 PP_OK = 0
 ERRORS = {-1: "PP_E_INVAL", -2: "PP_E_NOMEM", -3: "PP_E_CUDA", -4: "PP_E_OVERFLOW", -5: "PP_E_WOULDBLOCK",

@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpp.so")
 SOURCES = ["pp_kernels.cu", "pp_api.cpp", "pp_ipc.cpp", "pp_multi.cpp"]
-DEPS = SOURCES + ["pp_device.cuh", "pp_types.h", "pp_internal.h", os.path.join("..", "..", "include", "pp.h"),
+DEPS = SOURCES + ["pp_device.cuh", "pp_guard.cuh", "pp_types.h", "pp_internal.h", os.path.join("..", "..", "include", "pp.h"),
                   os.path.join("..", "..", "include", "pp_ipc.h"), os.path.join("..", "..", "include", "pp_multi.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -31,15 +31,16 @@ def nvcc() -> str:
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
+    """Builds libpp.so (or, for the tests, a variant of it: `out` elsewhere, with extra -D `defines`)."""
     deps = [os.path.join(CSRC, d) for d in DEPS]
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
-        return LIB
+    if not force and os.path.exists(out) and all(os.path.getmtime(out) >= os.path.getmtime(d) for d in deps):
+        return out
     extra = os.environ.get("PP_NVCC_EXTRA", "").split()  # e.g. -DPP_MIN_BLOCKS=4 (tuning experiments)
-    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
-        [os.path.join(CSRC, s) for s in SOURCES] + ["-lrt", "-lpthread"]
+    cmd = [nvcc()] + NVCC_FLAGS + extra + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + \
+        ["-o", out] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lrt", "-lpthread"]
     subprocess.check_call(cmd)
-    return LIB
+    return out
 
 
 if __name__ == "__main__":

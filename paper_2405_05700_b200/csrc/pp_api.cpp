@@ -33,15 +33,32 @@ using Clock = std::chrono::steady_clock;
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 
+#ifdef PP_GUARD
+// Test-only guard build (tests/test_gpu_guard.py; pp_guard.cuh): every piece of the DEVICE workspace is followed by a
+// zone of kGuardBytes filled with kGuardByte, which the host reads back and checks after every launch.
+constexpr uint64_t kGuardBytes = 256;
+constexpr unsigned char kGuardByte = 0xA5;
+std::atomic<uint64_t> g_guard_zone_checks{0};
+#endif
+
 struct Carver {  // hands out aligned pieces of one workspace
   unsigned char* base;
   uint64_t off = 0;
   explicit Carver(void* b) : base(static_cast<unsigned char*>(b)) {}
+#ifdef PP_GUARD
+  std::vector<unsigned char*>* zones = nullptr;  // where the guard zones of the pieces handed out are noted
+#endif
   template <class T>
   T* take(uint64_t count) {
     off = align_up(off, 256);
     T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
     off += count * sizeof(T);
+#ifdef PP_GUARD
+    if (zones) {
+      if (base) zones->push_back(base + off);
+      off += kGuardBytes;
+    }
+#endif
     return p;
   }
 };
@@ -157,6 +174,10 @@ struct pp_handle {
   bool wall_started = false;
   Clock::time_point wall_t0, wall_t1;
   double busy_end_ms = 0;
+
+#ifdef PP_GUARD
+  std::vector<unsigned char*> guard_zones;  // device addresses of the guard zones behind the workspace pieces
+#endif
 
   // error state
   std::atomic<int> sticky{PP_OK};
@@ -457,6 +478,10 @@ void fill_sizes(const pp_config& cfg, int n_sm, Sizes* s) {
 // Carve (or, with null base, just measure) the device workspace.
 uint64_t carve_device(pp_handle* h, void* base) {
   Carver c(base);
+#ifdef PP_GUARD
+  h->guard_zones.clear();
+  c.zones = &h->guard_zones;
+#endif
   const HostGeometry& g = h->hg;
   h->base.smem_image = c.take<uint4>(h->image_bytes / 16);
   h->base.dom_xyzw = c.take<float4>(g.dom_xyzw.size());
@@ -619,7 +644,23 @@ int push_hits(pp_handle* h, std::vector<pp_hit>&& v, bool may_block) {
 int finish_slot(pp_handle* h, Slot& s, bool may_block) {
   PP_CUDA(h, cudaEventSynchronize(s.ev_done));
   const Status hs = *s.h_status;
-  if (hs.error) return fail(h, PP_E_CUDA, "internal: resume list overflow");
+  if (hs.error) return fail(h, PP_E_CUDA, hs.error == 1u ? std::string("internal: resume list overflow")
+                                                          : "internal: guard check " + std::to_string(hs.error) + " failed in the kernel");
+#ifdef PP_GUARD
+  {
+    // every launch: the zones behind the workspace pieces must still hold their pattern (one small copy per zone; the
+    // guard build is not timed)
+    unsigned char z[kGuardBytes];
+    for (size_t q = 0; q < h->guard_zones.size(); ++q) {
+      PP_CUDA(h, cudaMemcpyAsync(z, h->guard_zones[q], kGuardBytes, cudaMemcpyDeviceToHost, s.stream));
+      PP_CUDA(h, cudaStreamSynchronize(s.stream));
+      for (uint64_t b = 0; b < kGuardBytes; ++b)
+        if (z[b] != kGuardByte)
+          return fail(h, PP_E_CUDA, "internal: guard zone " + std::to_string(q) + " behind a workspace piece was overwritten at byte " + std::to_string(b));
+      g_guard_zone_checks++;
+    }
+  }
+#endif
   float t0 = 0, t1 = 0;
   PP_CUDA(h, cudaEventElapsedTime(&t0, h->ev_base, s.ev_k0));
   PP_CUDA(h, cudaEventElapsedTime(&t1, h->ev_base, s.ev_k1));
@@ -1023,6 +1064,10 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
   }
   carve_device(h, h->dev_ws);
   carve_pinned(h, h->pin_ws);
+#ifdef PP_GUARD
+  for (unsigned char* z : h->guard_zones)
+    if (cudaMemset(z, kGuardByte, kGuardBytes) != cudaSuccess) return bail(PP_E_CUDA);
+#endif
   if (cfg->stream0 && cfg->stream1) {
     h->slot[0].stream = (cudaStream_t)cfg->stream0;
     h->slot[1].stream = (cudaStream_t)cfg->stream1;
@@ -1058,8 +1103,9 @@ int pp_create(const pp_geometry* geo, const pp_ice* ice, const pp_config* cfg, p
     P.resume_out = h->slot[0].d_resume[0]; P.resume_in = h->slot[0].d_resume[1]; P.resume_cap = (uint32_t)h->sz.resume_cap;
     P.ring = h->slot[0].d_ring; P.ring_cap = (uint32_t)h->sz.ring_cap; P.src = h->slot[0].d_src; P.cum = h->slot[0].d_cum;
     P.tile_src = h->slot[0].d_tile_src; P.cum_rel = h->slot[0].d_cum_rel;
-    for (int f = 0; f < 4; ++f) {  // every kernel variant this handle can launch: fates x optional physics
-      P.emit_on = (f & 2) ? 1u : 0u;  // (any of the switches of the flight-loop physics selects the same variant)
+    for (int f = 0; f < 6; ++f) {  // every kernel variant this handle can launch: fates x flight-loop physics
+      P.spec_n = (f >> 1) == 1 ? 1u : 0u;   // wavelength bins only
+      P.emit_on = (f >> 1) == 2 ? 1u : 0u;  // (any of the other switches selects the same, fullest variant)
       if (launch_propagate(P, h->brute, (f & 1) != 0, 1, h->smem, h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
     }
     if (cudaStreamSynchronize(h->slot[0].stream) != cudaSuccess) return bail(PP_E_CUDA);
@@ -1527,3 +1573,8 @@ int handle_launch_info(pp_handle* h, HandleLaunchInfo* out) {
 int handle_fail(pp_handle* h, int code, const char* msg) { return fail(h, code, msg ? msg : ""); }
 
 }  // namespace pp
+
+#ifdef PP_GUARD
+// guard build only: how many guard zones have been read back and found intact so far in this process
+extern "C" uint64_t pp_guard_zone_checks(void) { return g_guard_zone_checks.load(); }
+#endif

@@ -8,6 +8,7 @@
 #include "../../include/pp.h"
 #include "pp_internal.h"
 #include "pp_device.cuh"
+#include "pp_guard.cuh"
 
 #ifndef PP_MIN_BLOCKS
 #define PP_MIN_BLOCKS 1  // resident CTAs per SM the propagation kernel is compiled for (one CTA of 1024 threads)
@@ -318,6 +319,7 @@ __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, b
         a = P.g_begin + j * P.tile_photons;
         b = min(a + (unsigned long long)P.tile_photons, P.g_end);
         sh = __ldg(&P.tile_src[j]);
+        (void)PP_GUARD_CHECK(st, sh < P.n_src, PP_GUARD_TILE_SRC);
         if (*(volatile unsigned int*)&st->stop != 0u) {
           // the ring filled up while we were fetching: hand the whole tile to the next launch
           const unsigned o = atomicAdd(&st->n_resume_out, 1u);
@@ -335,10 +337,12 @@ __device__ __noinline__ uint4 fetch_work(const LaunchParams& P, unsigned lane, b
   return r;
 }
 
-// kExt: the optional physics that touches the flight loop (track-segment sources R-18, wavelength bins R-21, emission
-// smearing R-22) is compiled in; the DOM acceptance (R-17) is in every variant, in the rare hit block.  kLoop: the inverse walk tables are coarser than the thinnest layer (pathological
+// kExt: which of the optional physics that touches the flight loop is compiled in.  0: none.  1: wavelength bins
+// (R-21) only, switched on (no run-time test in the loop).  2: wavelength bins, track-segment sources (R-18) and
+// emission smearing (R-22), each behind its run-time switch.  The DOM acceptance (R-17) is in every variant, in the
+// rare hit block.  kLoop: the inverse walk tables are coarser than the thinnest layer (pathological
 // ice, LaunchParams::walk_loop), so the layer found may be several layers short
-template <bool kBrute, bool kFates, bool kExt, bool kLoop>
+template <bool kBrute, bool kFates, int kExt, bool kLoop>
 __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel(const __grid_constant__ LaunchParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // ---- stage the medium and the DOM lookup in shared memory (a4, a5): one verbatim copy of the host-built image ----
@@ -347,6 +351,10 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     const uint32_t n16 = P.smem_image_bytes >> 4;
     for (uint32_t i = threadIdx.x; i < n16; i += blockDim.x) dst[i] = __ldg(P.smem_image + i);
   }
+  // R-21: (1 / abs_scale, 1 / scat_scale) of the wavelength bins, where a lane can index them freely
+  __shared__ float2 s_spec[kExt != 0 ? PP_MAX_SPECTRUM_BINS : 1];
+  if (kExt != 0 && threadIdx.x < PP_MAX_SPECTRUM_BINS)
+    s_spec[threadIdx.x] = make_float2(P.spec_inv_a[threadIdx.x], P.spec_inv_b[threadIdx.x]);
   __syncthreads();
   // layer records at offset 0: coefficients (a, b, 1/b, a) of layer i, cumulative depths at boundary i
   auto walk_B = [&](int i) { return *reinterpret_cast<const float*>(smem_raw + (uint32_t)i * 32u + 16u); };
@@ -376,6 +384,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
   float Lh = 0, Ll = 0;  // path length, two-float
   float tau_a = 0;
   float sc_b = 1.0f;  // kExt only: 1 / scat_scale of the photon's wavelength bin (R-21)
+  const bool spectrum_on = kExt == 1 || (kExt == 2 && P.spec_n != 0u);  // (a compile-time constant unless kExt == 2)
   // k = flights started so far = index of the next Philox block; its top bit marks a DEAD lane (no register for a
   // flag; max_flights < 2^31 is checked at pp_create)
   uint32_t ev = 0, sid = 0, pidx = 0, k = kDeadBit, s_mine = 0;
@@ -391,8 +400,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
       ++s_cur;
     }
     if (t_next != t_end) {
-      uint32_t hi;
-      while ((hi = __ldg(&P.cum_rel[s_cur + 1])) <= t_next) ++s_cur;  // skips sources without photons
+      uint32_t hi = 0u;
+      while (PP_GUARD_CHECK(st, s_cur < P.n_src, PP_GUARD_SRC_INDEX) &&
+             (hi = __ldg(&P.cum_rel[s_cur + 1])) <= t_next) ++s_cur;  // skips sources without photons
       pbase = __ldg(&P.cum_rel[s_cur]);  // mod 2^32: right for the launch's first (split) source too
       run_end = min(t_end, hi);
       __syncwarp();
@@ -428,6 +438,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         Lh = 0.0f; Ll = 0.0f;
         ev = r2.x; sid = r2.y;
         pidx = r - pbase;
+        (void)PP_GUARD_CHECK(st, pidx < __ldg(&P.src[s_cur].n_photons), PP_GUARD_PHOTON_INDEX);
         k = 0; s_mine = s_cur;  // alive
       }
       t_next += min((uint32_t)__popc(need_mask), avail);
@@ -448,14 +459,14 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     // =========================== a7: emission (k = 0) or scatter (k > 0) ======================
     const float m_hg = hg_one_minus_cos(u_hg, P.hg_one_minus_g, P.hg_two_g, P.hg_one_minus_g2);
     const float m = (k == 0) ? P.one_minus_cos_c : m_hg;
-    if (kExt && P.has_segments != 0u && k == 0) {
+    if (kExt == 2 && P.has_segments != 0u && k == 0) {
       // R-18: a source with a length emits from a point uniform along it; u_hg is free on flight 0
       const float ell = segment_fraction(P, u_hg) * __ldg(&P.src[s_mine].length);
       const float nx_ = fmaf(dx, ell, phx); plx += fmaf(dx, ell, phx - nx_); phx = nx_;
       const float ny_ = fmaf(dy, ell, phy); ply += fmaf(dy, ell, phy - ny_); phy = ny_;
       const float nz_ = fmaf(dz, ell, phz); plz += fmaf(dz, ell, phz - nz_); phz = nz_;
     }
-    if (kExt && P.emit_on != 0u && k == 0) {
+    if (kExt == 2 && P.emit_on != 0u && k == 0) {
       // R-22: the axis the photon is emitted about = the source axis deflected by an HG(g_axis) polar angle
       uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0x20000000u;
       philox4x32_10(e0, e1, e2, e3, P.rk);
@@ -465,18 +476,20 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
     rotate(dx, dy, dz, m, u_az);
     // =========================== a3: absorption budget (once per photon) ======================
     float tau_new = neg_log_fast(u_abs);
-    if (kExt && P.spec_n != 0u && k == 0) {
+    if (spectrum_on && k == 0) {
       // R-21: the photon's wavelength bin from the spare bits of block 0.  Both optical-depth budgets are kept in
       // units of the unscaled ice table: tau_a is divided by abs_scale once, sc_b = 1 / scat_scale multiplies
       // every tau_s.
-      const uint32_t j = spectrum_bin_from_words(P, c0, c1, c2);
-      tau_new *= P.spec_inv_a[j];
-      sc_b = P.spec_inv_b[j];
+      // The bin's two scales come from shared memory: a per-lane index into the constant bank (where the tables
+      // arrive) is replayed once per distinct value in the warp, a shared-memory read is not.
+      const float2 sc = s_spec[spectrum_bin_from_words(P, c0, c1, c2)];
+      tau_new *= sc.x;
+      sc_b = sc.y;
     }
     tau_a = (k == 0) ? tau_new : tau_a;
     // =========================== a4: optical depth to the next scatter ========================
     float tau_s = neg_log_fast(u_dist);
-    if (kExt && P.spec_n != 0u) tau_s *= sc_b;
+    if (spectrum_on) tau_s *= sc_b;
     // =========================== a4: layer walk in vertical optical depth ======================
     // Along a straight ray the optical depth spent between two heights is (vertical optical depth)/|d_z|,
     // so the budgets are scaled by w = |d_z| once and the walk works in vertical metres.
@@ -628,9 +641,9 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         base = __shfl_sync(0xffffffffu, base, leader);
         if (hit) {
           const unsigned slot = base + __popc(hit_mask & lt);
-          if (slot < P.ring_cap) {
+          if (slot < P.ring_cap && PP_GUARD_CHECK(st, base + n_hit >= base, PP_GUARD_HIT_SLOT)) {
             double t0 = (double)__ldg(&P.src[s_mine].t);
-            if (kExt && P.has_segments != 0u) {
+            if (kExt == 2 && P.has_segments != 0u) {
               // R-18: emitted l / c after the source time; l is recomputed from block 0 instead of being carried
               uint32_t e0 = pidx, e1 = sid, e2 = ev, e3 = 0u;
               philox4x32_10(e0, e1, e2, e3, P.rk);
@@ -639,7 +652,7 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
             pp_hit h;
             h.event_id = ev; h.source_id = sid; h.photon_idx = pidx; h.dom_id = hit_dom;
             double inv_v = P.inv_v;
-            if (kExt && P.spec_n != 0u) inv_v = P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)];  // R-21
+            if (spectrum_on) inv_v = P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)];  // R-21
             h.time_ns = t0 + ((double)Lh + (double)Ll) * inv_v;
             h.weight = weight; h.n_scatter = k - 1;
             uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<pp_hit*>(P.ring) + slot);
@@ -674,12 +687,12 @@ __global__ void __launch_bounds__(kBlockThreads, PP_MIN_BLOCKS) propagate_kernel
         f.x = phx + plx; f.y = phy + ply; f.z = phz + plz;
         f.path_m = Lh + Ll;
         f.time_ns = (double)__ldg(&P.src[s_mine].t) + ((double)Lh + (double)Ll) *
-                    ((kExt && P.spec_n != 0u) ? P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)] : P.inv_v);
+                    (spectrum_on ? P.spec_inv_v[spectrum_bin(P, pidx, sid, ev)] : P.inv_v);
         f.n_flights = k;
         f.dom = (hit || rejected) ? (int32_t)hit_dom : -1;
         f.fate = hit ? 1u : (rejected ? 3u : (aborted ? 2u : 0u));
         f.photon_idx = pidx;
-        reinterpret_cast<pp_fate*>(P.fates)[g] = f;
+        if (PP_GUARD_CHECK(st, g < P.g_end, PP_GUARD_FATE_INDEX)) reinterpret_cast<pp_fate*>(P.fates)[g] = f;
       }
     }
     k |= done ? kDeadBit : 0u;  // (a dead lane stays dead whatever its stale state says)
@@ -739,7 +752,7 @@ cudaError_t launch_prologue(const SrcRec* d_src, uint32_t n_src, unsigned long l
 
 // Opt-in dynamic shared memory size of one kernel variant: raised when a handle needs more than any before it on
 // this device (the attribute is per device and per function; it is never lowered).
-template <bool B, bool F, bool A, bool L>
+template <bool B, bool F, int A, bool L>
 static cudaError_t ensure_smem(size_t smem) {
   static std::atomic<size_t> attr_smem[kMaxDevices];
   int dev = 0;
@@ -754,7 +767,7 @@ static cudaError_t ensure_smem(size_t smem) {
   return cudaSuccess;
 }
 
-template <bool B, bool F, bool A, bool L>
+template <bool B, bool F, int A, bool L>
 static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
   const cudaError_t e = ensure_smem<B, F, A, L>(smem);
   if (e != cudaSuccess) return e;
@@ -763,34 +776,33 @@ static cudaError_t launch_prop_t(const LaunchParams& P, int grid, size_t smem, c
   return cudaGetLastError();
 }
 
-// the kernel variant is picked by (brute-force DOM test, fate dump, optional physics in use, coarse walk tables)
+template <bool B, bool F, bool L>
+static cudaError_t launch_prop_ext(int ext, const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
+  switch (ext) {
+    case 0: return launch_prop_t<B, F, 0, L>(P, grid, smem, st);
+    case 1: return launch_prop_t<B, F, 1, L>(P, grid, smem, st);
+    default: return launch_prop_t<B, F, 2, L>(P, grid, smem, st);
+  }
+}
+template <bool B, bool F>
+static cudaError_t launch_prop_loop(bool loop, int ext, const LaunchParams& P, int grid, size_t smem, cudaStream_t st) {
+  return loop ? launch_prop_ext<B, F, true>(ext, P, grid, smem, st) : launch_prop_ext<B, F, false>(ext, P, grid, smem, st);
+}
+
+// the kernel variant is picked by (brute-force DOM test, fate dump, flight-loop physics in use, coarse walk tables)
 cudaError_t launch_propagate(const LaunchParams& P, bool brute, bool fates, int grid, size_t smem, cudaStream_t st) {
   // (the DOM acceptance needs no variant of its own: it sits in the rare hit block of every variant)
-  const bool ext = P.has_segments != 0u || P.spec_n != 0u || P.emit_on != 0u;
-  const int v = (P.walk_loop ? 8 : 0) | (brute ? 4 : 0) | (fates ? 2 : 0) | (ext ? 1 : 0);
-  switch (v) {
-    case 0: return launch_prop_t<false, false, false, false>(P, grid, smem, st);
-    case 1: return launch_prop_t<false, false, true, false>(P, grid, smem, st);
-    case 2: return launch_prop_t<false, true, false, false>(P, grid, smem, st);
-    case 3: return launch_prop_t<false, true, true, false>(P, grid, smem, st);
-    case 4: return launch_prop_t<true, false, false, false>(P, grid, smem, st);
-    case 5: return launch_prop_t<true, false, true, false>(P, grid, smem, st);
-    case 6: return launch_prop_t<true, true, false, false>(P, grid, smem, st);
-    case 7: return launch_prop_t<true, true, true, false>(P, grid, smem, st);
-    case 8: return launch_prop_t<false, false, false, true>(P, grid, smem, st);
-    case 9: return launch_prop_t<false, false, true, true>(P, grid, smem, st);
-    case 10: return launch_prop_t<false, true, false, true>(P, grid, smem, st);
-    case 11: return launch_prop_t<false, true, true, true>(P, grid, smem, st);
-    case 12: return launch_prop_t<true, false, false, true>(P, grid, smem, st);
-    case 13: return launch_prop_t<true, false, true, true>(P, grid, smem, st);
-    case 14: return launch_prop_t<true, true, false, true>(P, grid, smem, st);
-    default: return launch_prop_t<true, true, true, true>(P, grid, smem, st);
-  }
+  const int ext = (P.has_segments != 0u || P.emit_on != 0u) ? 2 : (P.spec_n != 0u ? 1 : 0);
+  const bool loop = P.walk_loop != 0u;
+  if (brute) return fates ? launch_prop_loop<true, true>(loop, ext, P, grid, smem, st)
+                          : launch_prop_loop<true, false>(loop, ext, P, grid, smem, st);
+  return fates ? launch_prop_loop<false, true>(loop, ext, P, grid, smem, st)
+               : launch_prop_loop<false, false>(loop, ext, P, grid, smem, st);
 }
 
 int propagate_warps_per_block() { return kBlockThreads / 32; }
 
-template <bool B, bool F, bool A, bool L>
+template <bool B, bool F, int A, bool L>
 static cudaError_t occupancy_t(size_t smem, int* n) {
   const cudaError_t e = ensure_smem<B, F, A, L>(smem);
   if (e != cudaSuccess) return e;
@@ -800,9 +812,9 @@ static cudaError_t occupancy_t(size_t smem, int* n) {
 cudaError_t propagate_occupancy(bool brute, bool fates, size_t smem, int* blocks_per_sm) {
   // all variants are compiled for the same launch bounds; the leanest and the fullest bracket the rest
   int a = 0, b = 0;
-  cudaError_t e = brute ? occupancy_t<true, true, true, true>(smem, &a) : occupancy_t<false, true, true, true>(smem, &a);
+  cudaError_t e = brute ? occupancy_t<true, true, 2, true>(smem, &a) : occupancy_t<false, true, 2, true>(smem, &a);
   if (e != cudaSuccess) return e;
-  e = brute ? occupancy_t<true, false, false, false>(smem, &b) : occupancy_t<false, false, false, false>(smem, &b);
+  e = brute ? occupancy_t<true, false, 0, false>(smem, &b) : occupancy_t<false, false, 0, false>(smem, &b);
   (void)fates;
   *blocks_per_sm = a < b ? a : b;
   return e;

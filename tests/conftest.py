@@ -24,6 +24,18 @@ def pytest_configure(config):
     from oracle import oracle as O
     O.build()
     build_echo_backend()
+    build_guard_library()
+
+
+GUARD_LIB = os.path.join(ROOT, "tests", "libpp_guard.so")
+
+
+def build_guard_library() -> str:
+    """tests/libpp_guard.so: the library compiled with -DPP_GUARD (guard zones behind every piece of the device
+    workspace, checked by the host after every launch; index checks inside the kernel: csrc/pp_guard.cuh).  Test
+    infrastructure standing in for compute-sanitizer; tests/test_gpu_guard.py runs against it in a process of its own."""
+    from paper_2405_05700_b200 import build as pp_build
+    return pp_build.build(out=GUARD_LIB, defines=("PP_GUARD",))
 
 
 ECHO_LIB = os.path.join(ROOT, "tests", "libpp_echo.so")
